@@ -1,0 +1,126 @@
+/*
+ * spin.h -- C ABI of libspin: checkerboard single-spin-flip Metropolis sweeps for O(n)
+ * lattice spin models on one B200 (sm_100a), plus the energy / magnetisation sums.
+ *
+ * What the calls compute (PAPER.md = the text of arXiv:1107.5463):
+ *   PAPER.md:31-35  Eq. (1)  H = -sum_<ij> J_ij s_i . s_j ; n = 1 Ising, 2 XY, 3 Heisenberg;
+ *                            square (d = 2) / simple-cubic (d = 3) lattice, nearest neighbours
+ *   PAPER.md:37-38  Eq. (2)  p_acc(s -> s') = min[1, exp(-beta dE)]                 (spin_sweep)
+ *   PAPER.md:42              checkerboard decomposition: all spins of one sub-lattice are
+ *                            updated concurrently, then the other; tabulated Boltzmann
+ *                            factors; a random number is drawn for every site      (spin_sweep)
+ *   PAPER.md:44              fp32 spins, fp64 aggregates (total energy)            (spin_measure)
+ *   PAPER.md:46, 52          disorder realisations side by side; multi-spin coding (n_replicas, BITPACK)
+ * Readings where the paper is silent (periodic boundaries, one sweep = colour 0 then colour 1,
+ * k = 1, Philox-4x32-10 keyed by (seed, sweep, colour, site), ...) are listed in DESIGN.md.
+ *
+ * Conventions
+ *   - Every call returns a spin_status; nothing throws or aborts across the ABI; outputs are
+ *     written only on SPIN_OK.  spin_last_error() gives a thread-local message.
+ *   - The CALLER owns device memory: spin_create() carves everything it needs out of the
+ *     device workspace passed in (size from spin_workspace_bytes()); the library allocates
+ *     device memory only transiently inside the get/set calls (staging of canonical arrays).
+ *   - "stream" arguments are cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - spin_sweep / spin_sweep_record only enqueue work; spin_measure and the get/set calls block.
+ *   - A handle is not thread-safe; different handles are independent.
+ *   - Sites: (x, y, z), lexicographic index i = x + Lx (y + Ly z); colour = (x + y + z) mod 2;
+ *     colour 0 is updated first.  Periodic boundaries in every direction.
+ */
+#ifndef SPIN_H
+#define SPIN_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct spin_system spin_system; /* opaque, host-side, owned by the library */
+
+typedef enum {
+    SPIN_OK = 0,
+    SPIN_ERR_INVALID_ARG = 1,         /* NULL pointer, odd dimension, beta < 0 or NaN, bad enum, ... */
+    SPIN_ERR_UNSUPPORTED = 2,         /* valid request the kernels do not cover (see spin_config)     */
+    SPIN_ERR_WORKSPACE_TOO_SMALL = 3,
+    SPIN_ERR_CUDA = 4,                /* a CUDA runtime call failed; message has cudaGetErrorString   */
+    SPIN_ERR_STATE = 5                /* sweep counter would pass 2^32 - 1                            */
+} spin_status;
+
+enum { SPIN_STORE_INT8 = 0,   /* n = 1: one byte per spin                                             */
+       SPIN_STORE_BITPACK = 1,/* n = 1: one bit per spin, 32 same-colour sites per word (multi-spin
+                                 coding); needs Lx % 64 == 0 and |J| = 1                 */
+       SPIN_STORE_FP32 = 2 }; /* n = 2, 3: fp32 unit vectors, one plane per component and colour      */
+enum { SPIN_J_UNIFORM = 0,        /* J[0] on every bond                                               */
+       SPIN_J_PER_DIRECTION = 1,  /* J[mu] on bonds in direction mu = x, y, z                         */
+       SPIN_J_BOND_PM1 = 2 };     /* one +-1 per bond and replica (Edwards-Anderson); n = 1 */
+enum { SPIN_INIT_HOT = 0,         /* iid uniform spins drawn from the seed                            */
+       SPIN_INIT_COLD = 1 };      /* all +1 (n = 1), (1, 0) (n = 2), (0, 0, 1) (n = 3)                */
+
+typedef struct {
+    int32_t dims[3];         /* Lx, Ly, Lz.  Lz == 1 -> d = 2.  Lx, Ly (and Lz if > 1) even, >= 2.      */
+    int32_t n;               /* 1 Ising, 2 XY, 3 Heisenberg                                             */
+    int32_t storage;         /* SPIN_STORE_*; INT8/BITPACK need n = 1, FP32 needs n >= 2                */
+    int32_t coupling_kind;   /* SPIN_J_*                                                                */
+    double  J[3];            /* UNIFORM: J[0]; PER_DIRECTION: Jx, Jy, Jz.  n = 1: each in {-1, 0, +1}   */
+    const int8_t *bonds;     /* BOND_PM1: HOST array [replica][mu][i] (mu < d) of +-1, the coupling of
+                                the bond leaving site i in direction +mu; NULL -> drawn iid +-1, p = 1/2,
+                                from the seed.  Read during spin_create only.                          */
+    int32_t n_replicas;      /* R >= 1 independent systems stored side by side            */
+    int32_t replica_streams; /* 0: all replicas see the same random numbers (needs distinct bonds or
+                                starts to be useful); 1: the replica index enters the Philox counter    */
+    int32_t init;            /* SPIN_INIT_*                                                             */
+    uint64_t seed;           /* Philox key                                                              */
+} spin_config;
+
+/* Bytes of device workspace spin_create() needs for this configuration. */
+spin_status spin_workspace_bytes(const spin_config *cfg, size_t *bytes);
+
+/* Build a system inside d_workspace (DEVICE pointer, 256-byte aligned, `bytes` long, owned by the
+ * caller and kept alive until spin_destroy): draws or uploads the bonds, initialises the spins,
+ * sweep counter = 0.  Work is enqueued on `stream` and synchronised before returning. */
+spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes, void *stream, spin_system **out);
+
+/* n_sweeps full sweeps (half-sweep of colour 0, then of colour 1) at inverse temperature
+ * beta >= 0, enqueued on `stream`; returns without synchronising.  sweep(b, a); sweep(b, c) is
+ * identical to sweep(b, a + c).  The sweep counter (the Philox sweep index) advances by n_sweeps. */
+spin_status spin_sweep(spin_system *s, double beta, int64_t n_sweeps, void *stream);
+
+/* E[r] = -sum over bonds J s.s (each bond once), M[r*n + a] = sum_i s_i^a (Eq. (1); double
+ * aggregates).  E, M are HOST pointers to R and R*n doubles.  n = 1: both are exact integers.
+ * Runs on `stream` and blocks until the result is on the host. */
+spin_status spin_measure(spin_system *s, double *E, double *M, void *stream);
+
+/* As spin_sweep, recording E and M after every sweep into DEVICE arrays d_E[n_sweeps][R] and
+ * d_M[n_sweeps][R][n] (doubles).  Enqueues only. */
+spin_status spin_sweep_record(spin_system *s, double beta, int64_t n_sweeps, double *d_E, double *d_M, void *stream);
+
+/* Canonical HOST layouts.  n = 1: int8 [replica][i] of +-1; n >= 2: float [replica][i][n].  Blocking. */
+spin_status spin_get_spins(spin_system *s, void *host, size_t bytes);
+spin_status spin_set_spins(spin_system *s, const void *host, size_t bytes);
+/* BOND_PM1 only: int8 [replica][mu][i] of +-1.  Blocking. */
+spin_status spin_get_bonds(spin_system *s, int8_t *host, size_t bytes);
+
+spin_status spin_get_sweep_count(const spin_system *s, uint64_t *t);
+spin_status spin_set_sweep_count(spin_system *s, uint64_t t);
+
+/* Number of kernel launches this handle has enqueued so far (bench.py's gpu_launches). */
+spin_status spin_get_launch_count(const spin_system *s, uint64_t *launches);
+
+/* Tuning knob for tests: multiply the default grid size by num/den and use `block` threads per CTA
+ * (0 = default).  Results never depend on it (the RNG is counter-based). */
+spin_status spin_set_launch_shape(spin_system *s, int32_t block, int32_t grid_num, int32_t grid_den);
+
+/* Frees the handle only; never the workspace. */
+spin_status spin_destroy(spin_system *s);
+
+/* Thread-local message of the last failing call on this thread ("" if none). */
+const char *spin_last_error(void);
+
+/* Library version string, e.g. "libspin 0.1 sm_100a". */
+const char *spin_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPIN_H */

@@ -1,0 +1,6 @@
+"""paper_1107_5463_b200 -- B200-native checkerboard Metropolis sweeps for O(n) lattice spin models
+(Weigel & Yavors'kii, arXiv:1107.5463): libspin.so (CUDA, C ABI in include/spin.h) and its thin binding."""
+from . import workloads  # noqa: F401
+from .binding import (  # noqa: F401
+    INIT_COLD, INIT_HOT, SpinError, SpinSystem, from_workload, lib, lib_path, make_config, workspace_bytes,
+)

@@ -1,0 +1,78 @@
+// common.cuh -- device-side building blocks shared by every libspin kernel (sm_100a).
+// Product code: shares nothing with oracle/.  The algorithm both follow is DESIGN.md "The contract".
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace spin {
+
+// ---------------------------------------------------------------------------------------------
+// Philox-4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11).  The ten round keys depend only on the seed,
+// so the host expands them once and they reach the kernels as __grid_constant__ parameters: the
+// XORs take them straight from the constant bank and a call is 20 IMAD.WIDE + 20 LOP3.
+struct PhiloxKeys {
+    uint32_t k0[10];
+    uint32_t k1[10];
+};
+
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              const PhiloxKeys &K, uint32_t out[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * (uint64_t)c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * (uint64_t)c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ K.k0[r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ K.k1[r];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// Counter layout of DESIGN.md: ctr = (unit, rho, t, tag), tag = colour + 16 domain + 256 call.
+enum : uint32_t { DOM_ISING_UPDATE = 0, DOM_INIT = 1, DOM_BONDS = 2, DOM_VECTOR_UPDATE = 3 };
+__host__ __device__ __forceinline__ uint32_t make_tag(uint32_t colour, uint32_t domain, uint32_t call) {
+    return colour + 16u * domain + 256u * call;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Division by a run-time constant fixed at handle creation: q = (n * mul) >> (32 + shift) for
+// n < 2^31 (round-up method).  Two instructions instead of ~20.
+struct FastDiv {
+    uint32_t mul;
+    uint32_t shift;
+    uint32_t div;
+};
+__device__ __forceinline__ uint32_t fdiv(uint32_t n, const FastDiv &d) {
+    return d.div == 1u ? n : (__umulhi(n, d.mul) >> d.shift);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Boltzmann thresholds for n = 1 ("pre-tabulation of the Boltzmann factors"):
+// T(dE) = floor(exp(-beta dE) 2^32), compared bit-serially, most significant digit first, against
+// the site's 32-bit uniform whose digit k is bit `lane` of Philox word k of the site's unit
+// (bit-plane contract).  digit[th][k] is the k-th digit of T(4 (th + 1)) spread to a full mask
+// (0 or ~0); always[th] = ~0 iff T = 2^32 (factor 1: every lane accepts).
+struct IsingTable {
+    uint32_t digit[3][32];
+    uint32_t always[3];
+    uint32_t T[13];       // low 32 bits of T(dE), dE = 0..12 (generic kernel)
+    uint32_t Talways;     // bit dE set iff T(dE) = 2^32
+};
+
+// Lattice geometry in the colour-compressed layout.  A colour-c site (x, y, z) has compressed
+// index j = (x >> 1) + RL (y + Ly z), RL = Lx / 2; all its neighbours are in the other colour's array:
+// same row at x >> 1 and at (x >> 1) -+ 1 (minus if x is even), rows y -+ 1 and planes z -+ 1 at x >> 1.
+struct Geometry {
+    int32_t Lx, Ly, Lz, d;
+    uint32_t RL;      // sites per row and colour = Lx / 2
+    uint32_t rows;    // Ly * Lz
+    uint32_t Nh;      // sites per colour = N / 2
+    uint32_t WX;      // 32-site words per row and colour = RL / 32 (fast kernels only)
+    uint32_t NW;      // words per colour = Nh / 32 (fast kernels only)
+    FastDiv divRL, divWX, divLy;
+};
+
+}  // namespace spin

@@ -1,0 +1,240 @@
+// ising_kernels.cuh -- n = 1 half-sweep kernels (Eq. (2), PAPER.md:42 checkerboard,
+// PAPER.md:46 / 52 replicas and multi-spin coding).  Three kernels share one decision rule:
+//   ising_generic_halfsweep  one thread per site, any even dims, any coupling kind  (reference shape)
+//   ising_bitpack_halfsweep  one thread per 32-site word, bitwise local field and acceptance
+//   ising_int8_halfsweep     one thread per 32 sites stored as bytes, SIMD-in-register byte arithmetic
+// All implement: flip iff dE <= 0 or U < T(dE), U the site's bit-plane uniform (common.cuh).
+#pragma once
+#include "common.cuh"
+
+namespace spin {
+
+struct IsingArgs {
+    Geometry g;
+    PhiloxKeys keys;
+    IsingTable tab;
+    void *s[2];          // per colour: int8 -> uint8_t [R][Nh] (0 = +1, 1 = -1); bitpack -> uint32_t [R][NW]
+    const void *bonds;   // bitpack: uint32_t [2][R][3][NW] (bit = 1: J = -1); generic: int8 [R][d][N] of +-1
+    uint32_t R, replica_streams, t, colour;
+    int32_t coupling_kind;  // 0 uniform, 1 per direction, 2 per bond
+    int32_t Jdir[3];        // generic kernel: coupling per direction in {-1, 0, +1}
+    uint32_t jneg;          // fast kernels: 1 iff the uniform coupling is -1
+};
+
+// ------------------------------------------------------------------ bit-serial U < T ---------
+// Lane masks of U < T(4 (th + 1)) for th < NT, for all 32 lanes of `unit`.  Digits are consumed most
+// significant first, four per Philox call, until every lane is decided for every threshold
+// (about log2(32) + 1.3 digits on average; a warp runs until its slowest thread is done).
+template <int NT>
+__device__ __forceinline__ void lt_masks_full(const IsingArgs &a, uint32_t unit, uint32_t rho, uint32_t lt[NT]) {
+    uint32_t eq[NT];
+#pragma unroll
+    for (int th = 0; th < NT; ++th) { lt[th] = a.tab.always[th]; eq[th] = ~a.tab.always[th]; }
+#pragma unroll
+    for (int call = 0; call < 8; ++call) {
+        uint32_t any = eq[0];
+#pragma unroll
+        for (int th = 1; th < NT; ++th) any |= eq[th];
+        if (any == 0u) break;
+        uint32_t w[4];
+        philox4x32_10(unit, rho, a.t, make_tag(a.colour, DOM_ISING_UPDATE, call), a.keys, w);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+#pragma unroll
+            for (int th = 0; th < NT; ++th) {
+                const uint32_t tb = a.tab.digit[th][4 * call + k];
+                lt[th] |= eq[th] & ~w[k] & tb;
+                eq[th] &= ~(w[k] ^ tb);
+            }
+        }
+    }
+}
+
+// The same comparison when every lane needs only ONE threshold: m[th] are disjoint lane masks
+// (lane in m[th] compares against T(4 (th + 1)); lanes in none are not compared).  Returns the
+// mask of lanes with U < their threshold.
+template <int NT>
+__device__ __forceinline__ uint32_t lt_mask_select(const IsingArgs &a, uint32_t unit, uint32_t rho, const uint32_t m[NT]) {
+    uint32_t lt = 0u, eq = 0u;
+#pragma unroll
+    for (int th = 0; th < NT; ++th) { lt |= m[th] & a.tab.always[th]; eq |= m[th] & ~a.tab.always[th]; }
+#pragma unroll
+    for (int call = 0; call < 8; ++call) {
+        if (eq == 0u) break;
+        uint32_t w[4];
+        philox4x32_10(unit, rho, a.t, make_tag(a.colour, DOM_ISING_UPDATE, call), a.keys, w);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int dg = 4 * call + k;
+            uint32_t tk = a.tab.digit[NT - 1][dg];
+#pragma unroll
+            for (int th = NT - 2; th >= 0; --th) tk = (m[th] & a.tab.digit[th][dg]) | (~m[th] & tk);
+            lt |= eq & ~w[k] & tk;
+            eq &= ~(w[k] ^ tk);
+        }
+    }
+    return lt;
+}
+
+__device__ __forceinline__ uint32_t maj3(uint32_t x, uint32_t y, uint32_t z) { return (x & y) | (z & (x | y)); }
+
+// ------------------------------------------------------------------ generic kernel -----------
+// One thread per (replica, site of the active colour).  Handles size-2 dimensions (the -mu and +mu
+// neighbour coincide and both bonds count), zero couplings and per-bond couplings.
+__global__ void __launch_bounds__(256) ising_generic_halfsweep(const __grid_constant__ IsingArgs a) {
+    const Geometry &g = a.g;
+    const uint32_t total = g.Nh * a.R;
+    const uint8_t *__restrict__ other_base = (const uint8_t *)a.s[1 - a.colour];
+    uint8_t *mine_base = (uint8_t *)a.s[a.colour];
+    const uint32_t N = 2u * g.Nh;
+    for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
+        const uint32_t r = idx / g.Nh, j = idx - r * g.Nh;
+        const uint32_t row = fdiv(j, g.divRL), xh = j - row * g.RL;
+        const uint32_t z = fdiv(row, g.divLy), y = row - z * (uint32_t)g.Ly;
+        const uint32_t p = (y + z + a.colour) & 1u;
+        const uint32_t x = 2u * xh + p;
+        const uint8_t *other = other_base + (size_t)r * g.Nh;
+        // neighbour coordinates (periodic)
+        const uint32_t xm = x == 0 ? g.Lx - 1 : x - 1, xp = x == (uint32_t)g.Lx - 1 ? 0 : x + 1;
+        const uint32_t ym = y == 0 ? g.Ly - 1 : y - 1, yp = y == (uint32_t)g.Ly - 1 ? 0 : y + 1;
+        const uint32_t zm = z == 0 ? g.Lz - 1 : z - 1, zp = z == (uint32_t)g.Lz - 1 ? 0 : z + 1;
+        const uint32_t rowbase = row * g.RL;
+        int nb[6];
+        uint32_t isite[6];  // lexicographic index of the site that owns the connecting forward bond
+        nb[0] = other[rowbase + (xm >> 1)];                         isite[0] = xm + g.Lx * row;
+        nb[1] = other[rowbase + (xp >> 1)];                         isite[1] = x + g.Lx * row;
+        nb[2] = other[(ym + g.Ly * z) * g.RL + xh];                 isite[2] = x + g.Lx * (ym + g.Ly * z);
+        nb[3] = other[(yp + g.Ly * z) * g.RL + xh];                 isite[3] = x + g.Lx * row;
+        if (g.d == 3) {
+            nb[4] = other[(y + g.Ly * zm) * g.RL + xh];             isite[4] = x + g.Lx * (y + g.Ly * zm);
+            nb[5] = other[(y + g.Ly * zp) * g.RL + xh];             isite[5] = x + g.Lx * row;
+        }
+        const int s = 1 - 2 * (int)mine_base[(size_t)r * g.Nh + j];
+        int h = 0;
+        const int8_t *bonds = (const int8_t *)a.bonds;
+        for (int k = 0; k < 2 * g.d; ++k) {
+            const int mu = k >> 1;
+            int J;
+            if (a.coupling_kind == 2) J = bonds[((size_t)r * g.d + mu) * N + isite[k]];
+            else J = a.Jdir[mu];
+            h += J * (1 - 2 * nb[k]);
+        }
+        const int dE = 2 * s * h;
+        bool flip = dE <= 0 || ((a.tab.Talways >> dE) & 1u);
+        if (!flip) {
+            const uint32_t T = a.tab.T[dE];
+            const uint32_t unit = j >> 5, lane = j & 31u;
+            const uint32_t rho = a.replica_streams ? r : 0u;
+            bool decided = false;
+            for (int call = 0; call < 8 && !decided; ++call) {
+                uint32_t w[4];
+                philox4x32_10(unit, rho, a.t, make_tag(a.colour, DOM_ISING_UPDATE, call), a.keys, w);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    if (decided) continue;
+                    const uint32_t ud = (w[k] >> lane) & 1u, td = (T >> (31 - (4 * call + k))) & 1u;
+                    if (ud != td) { decided = true; flip = ud < td; }
+                }
+            }
+        }
+        if (flip) mine_base[(size_t)r * g.Nh + j] = (uint8_t)(s > 0 ? 1 : 0);
+    }
+}
+
+// ------------------------------------------------------------------ bit-packed kernel --------
+// Word indices of the neighbours of 32-site word gi = w + WX (y + Ly z) of colour `colour`.
+struct WordNbrs {
+    uint32_t p, g_side, g_ym, g_yp, g_zm, g_zp;
+};
+template <int D>
+__device__ __forceinline__ WordNbrs word_neighbours(const Geometry &g, uint32_t colour, uint32_t gi) {
+    WordNbrs n;
+    const uint32_t WX = g.WX;
+    const uint32_t row = fdiv(gi, g.divWX), w = gi - row * WX;
+    const uint32_t z = fdiv(row, g.divLy), y = row - z * (uint32_t)g.Ly;
+    n.p = (y + z + colour) & 1u;
+    const uint32_t wside = n.p ? (w + 1 == WX ? 0 : w + 1) : (w == 0 ? WX - 1 : w - 1);
+    n.g_side = row * WX + wside;
+    n.g_ym = y == 0 ? gi + WX * (g.Ly - 1) : gi - WX;
+    n.g_yp = y == (uint32_t)g.Ly - 1 ? gi - WX * (g.Ly - 1) : gi + WX;
+    n.g_zm = gi;
+    n.g_zp = gi;
+    if (D == 3) {
+        const uint32_t plane = WX * g.Ly;
+        n.g_zm = z == 0 ? gi + plane * (g.Lz - 1) : gi - plane;
+        n.g_zp = z == (uint32_t)g.Lz - 1 ? gi - plane * (g.Lz - 1) : gi + plane;
+    }
+    return n;
+}
+
+// av[k] = lane mask of unsatisfied bonds (s_i ^ s_j ^ [J < 0]) of word gi of colour `colour`, replica r,
+// towards its 2 D neighbours; bit = 1 means spin -1 / coupling -1.  Returns the word's own spins.
+template <int D, bool BONDS>
+__device__ __forceinline__ uint32_t unsatisfied_bonds(const IsingArgs &a, uint32_t colour, uint32_t r, uint32_t gi,
+                                                      const WordNbrs &n, uint32_t av[6]) {
+    const uint32_t NW = a.g.NW;
+    const uint32_t *__restrict__ other = (const uint32_t *)a.s[1 - colour] + (size_t)r * NW;
+    const uint32_t raw = ((const uint32_t *)a.s[colour])[(size_t)r * NW + gi];
+    const uint32_t s = a.jneg ? ~raw : raw;
+    const uint32_t o = other[gi], os = other[n.g_side];
+    const uint32_t side = n.p ? ((o >> 1) | (os << 31)) : ((o << 1) | (os >> 31));
+    av[0] = s ^ o; av[1] = s ^ side; av[2] = s ^ other[n.g_ym]; av[3] = s ^ other[n.g_yp];
+    av[4] = 0u; av[5] = 0u;
+    if (D == 3) { av[4] = s ^ other[n.g_zm]; av[5] = s ^ other[n.g_zp]; }
+    if (BONDS) {
+        const uint32_t *__restrict__ bb = (const uint32_t *)a.bonds;
+        const uint32_t *__restrict__ bo = bb + ((size_t)(colour * a.R + r) * 3) * NW;        // own forward bonds
+        const uint32_t *__restrict__ bt = bb + ((size_t)((1 - colour) * a.R + r) * 3) * NW;  // other colour's
+        const uint32_t bx_own = bo[gi], bx_oth = bt[gi];
+        if (n.p) { av[0] ^= bx_oth; av[1] ^= bx_own; }
+        else { av[0] ^= bx_own; av[1] ^= (bx_oth << 1) | (bt[n.g_side] >> 31); }
+        av[2] ^= bt[(size_t)NW + n.g_ym];
+        av[3] ^= bo[(size_t)NW + gi];
+        if (D == 3) { av[4] ^= bt[2 * (size_t)NW + n.g_zm]; av[5] ^= bo[2 * (size_t)NW + gi]; }
+    }
+    return raw;
+}
+
+// One thread per 32-site word of the active colour; loops over the replicas.  dE = 2q - 4 n_u with n_u
+// the number of unsatisfied bonds, counted bit-sliced with full adders.  SHARED: all replicas see
+// the same random numbers (R > 1, replica_streams = 0), so the masks are built once per word and
+// reused R times; otherwise each lane is compared against the one threshold it needs.
+template <int D, bool BONDS, bool SHARED>
+__global__ void __launch_bounds__(256) ising_bitpack_halfsweep(const __grid_constant__ IsingArgs a) {
+    constexpr int NT = D;  // thresholds: dE = 4, 8 (2D) and 12 (3D)
+    const uint32_t NW = a.g.NW;
+    uint32_t *mine_base = (uint32_t *)a.s[a.colour];
+    for (uint32_t gi = blockIdx.x * blockDim.x + threadIdx.x; gi < NW; gi += gridDim.x * blockDim.x) {
+        const WordNbrs n = word_neighbours<D>(a.g, a.colour, gi);
+        uint32_t ltf[NT];
+        if (SHARED) lt_masks_full<NT>(a, gi, 0u, ltf);
+        for (uint32_t r = 0; r < a.R; ++r) {
+            uint32_t av[6];
+            const uint32_t raw = unsatisfied_bonds<D, BONDS>(a, a.colour, r, gi, n, av);
+            uint32_t flip;
+            if (D == 2) {
+                const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
+                const uint32_t ge2 = c1 | (s1 & av[3]), ge1 = av[0] | av[1] | av[2] | av[3];
+                if (SHARED) flip = ge2 | (ge1 & ltf[0]) | ltf[1];
+                else {
+                    const uint32_t m[2] = {ge1 & ~ge2, ~ge1};
+                    flip = ge2 | lt_mask_select<2>(a, gi, a.replica_streams ? r : 0u, m);
+                }
+            } else {
+                const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
+                const uint32_t s2 = av[3] ^ av[4] ^ av[5], c2 = maj3(av[3], av[4], av[5]);
+                const uint32_t b0 = s1 ^ s2, c3 = s1 & s2;
+                const uint32_t b1 = c1 ^ c2 ^ c3, b2 = maj3(c1, c2, c3);
+                const uint32_t ge3 = b2 | (b1 & b0);
+                if (SHARED) flip = ge3 | ((b1 | b2) & ltf[0]) | ((b0 | b1 | b2) & ltf[1]) | ltf[2];
+                else {
+                    const uint32_t m[3] = {b1 & ~b0 & ~b2, b0 & ~b1 & ~b2, ~(b0 | b1 | b2)};
+                    flip = ge3 | lt_mask_select<3>(a, gi, a.replica_streams ? r : 0u, m);
+                }
+            }
+            mine_base[(size_t)r * NW + gi] = raw ^ flip;
+        }
+    }
+}
+
+}  // namespace spin

@@ -1,0 +1,161 @@
+// setup_kernels.cuh -- initial states, bond tables and conversion between the canonical (lexicographic)
+// layouts of the ABI and the colour-split device layouts.  Not on the timed path.
+// Random draws follow DESIGN.md "The contract":
+//   hot start n = 1 : s_i = -1 iff bit (i & 31) of word ((i >> 5) & 3) of rand(i >> 7, r, 0, INIT)
+//   hot start n >= 2: direction(w0, w1) of rand(i, r, 0, INIT)
+//   bonds           : J[r][mu][i] = -1 iff bit (i & 31) of word mu of rand(i >> 5, r, 0, BONDS)
+#pragma once
+#include "ising_kernels.cuh"
+#include "vector_kernels.cuh"
+
+namespace spin {
+
+struct SetupArgs {
+    Geometry g;
+    PhiloxKeys keys;
+    uint32_t R;
+    int32_t bitpack;  // n = 1 only
+    int32_t nc;       // 1, 2, 3
+};
+
+// (colour c, compressed index j) -> lexicographic site index
+__device__ __forceinline__ uint32_t lex_index(const Geometry &g, uint32_t c, uint32_t j) {
+    const uint32_t row = fdiv(j, g.divRL), xh = j - row * g.RL;
+    const uint32_t z = fdiv(row, g.divLy), y = row - z * (uint32_t)g.Ly;
+    const uint32_t p = (y + z + c) & 1u;
+    return 2u * xh + p + (uint32_t)g.Lx * row;
+}
+
+// mode 0: cold, 1: hot (from seed), 2: from canonical int8 [R][N] of +-1.
+// idx runs over (colour, replica, j); with bit-packing a warp covers exactly one word (Nh % 32 == 0).
+__global__ void __launch_bounds__(256) ising_fill(const __grid_constant__ SetupArgs a, int mode, const int8_t *canon,
+                                                  void *s0, void *s1) {
+    const Geometry &g = a.g;
+    const uint32_t per_colour = a.R * g.Nh, total = 2u * per_colour, N = 2u * g.Nh;
+    for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
+        const uint32_t c = idx / per_colour, rem = idx - c * per_colour;
+        const uint32_t r = rem / g.Nh, j = rem - r * g.Nh;
+        const uint32_t i = lex_index(g, c, j);
+        uint32_t bit = 0u;
+        if (mode == 1) {
+            uint32_t w[4];
+            philox4x32_10(i >> 7, r, 0u, make_tag(0u, DOM_INIT, 0u), a.keys, w);
+            bit = (w[(i >> 5) & 3u] >> (i & 31u)) & 1u;
+        } else if (mode == 2) {
+            bit = canon[(size_t)r * N + i] < 0 ? 1u : 0u;
+        }
+        void *dst = c ? s1 : s0;
+        if (a.bitpack) {
+            const uint32_t word = __ballot_sync(0xFFFFFFFFu, bit);
+            if ((threadIdx.x & 31) == 0) ((uint32_t *)dst)[(size_t)r * g.NW + (j >> 5)] = word;
+        } else {
+            ((uint8_t *)dst)[(size_t)r * g.Nh + j] = (uint8_t)bit;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) ising_to_canonical(const __grid_constant__ SetupArgs a, const void *s0, const void *s1,
+                                                          int8_t *canon) {
+    const Geometry &g = a.g;
+    const uint32_t per_colour = a.R * g.Nh, total = 2u * per_colour, N = 2u * g.Nh;
+    for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
+        const uint32_t c = idx / per_colour, rem = idx - c * per_colour;
+        const uint32_t r = rem / g.Nh, j = rem - r * g.Nh;
+        const uint32_t i = lex_index(g, c, j);
+        const void *src = c ? s1 : s0;
+        uint32_t bit;
+        if (a.bitpack) bit = (((const uint32_t *)src)[(size_t)r * g.NW + (j >> 5)] >> (j & 31u)) & 1u;
+        else bit = ((const uint8_t *)src)[(size_t)r * g.Nh + j];
+        canon[(size_t)r * N + i] = bit ? (int8_t)-1 : (int8_t)1;
+    }
+}
+
+// mode 0: cold, 1: hot, 2: from canonical float [R][N][nc]
+template <int NC>
+__global__ void __launch_bounds__(256) vector_fill(const __grid_constant__ SetupArgs a, int mode, const float *canon,
+                                                   float *s0, float *s1) {
+    const Geometry &g = a.g;
+    const uint32_t per_colour = a.R * g.Nh, total = 2u * per_colour, N = 2u * g.Nh;
+    for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
+        const uint32_t c = idx / per_colour, rem = idx - c * per_colour;
+        const uint32_t r = rem / g.Nh, j = rem - r * g.Nh;
+        const uint32_t i = lex_index(g, c, j);
+        float v[3] = {0.0f, 0.0f, 0.0f};
+        if (mode == 0) {
+            if (NC == 3) v[2] = 1.0f; else v[0] = 1.0f;
+        } else if (mode == 1) {
+            uint32_t w[4];
+            philox4x32_10(i, r, 0u, make_tag(0u, DOM_INIT, 0u), a.keys, w);
+            if (NC == 3) direction3(w[0], w[1], v); else direction2(w[0], v);
+        } else {
+#pragma unroll
+            for (int k = 0; k < NC; ++k) v[k] = canon[((size_t)r * N + i) * NC + k];
+        }
+        float *dst = (c ? s1 : s0) + (size_t)r * NC * g.Nh;
+#pragma unroll
+        for (int k = 0; k < NC; ++k) dst[(size_t)k * g.Nh + j] = v[k];
+    }
+}
+
+template <int NC>
+__global__ void __launch_bounds__(256) vector_to_canonical(const __grid_constant__ SetupArgs a, const float *s0, const float *s1,
+                                                           float *canon) {
+    const Geometry &g = a.g;
+    const uint32_t per_colour = a.R * g.Nh, total = 2u * per_colour, N = 2u * g.Nh;
+    for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
+        const uint32_t c = idx / per_colour, rem = idx - c * per_colour;
+        const uint32_t r = rem / g.Nh, j = rem - r * g.Nh;
+        const uint32_t i = lex_index(g, c, j);
+        const float *src = (c ? s1 : s0) + (size_t)r * NC * g.Nh;
+#pragma unroll
+        for (int k = 0; k < NC; ++k) canon[((size_t)r * N + i) * NC + k] = src[(size_t)k * g.Nh + j];
+    }
+}
+
+// Canonical int8 bonds [R][d][N] drawn from the seed (generic kernels keep this layout).
+__global__ void __launch_bounds__(256) bonds_draw_canonical(const __grid_constant__ SetupArgs a, int8_t *canon) {
+    const Geometry &g = a.g;
+    const uint32_t N = 2u * g.Nh, total = a.R * N;
+    for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
+        const uint32_t r = idx / N, i = idx - r * N;
+        uint32_t w[4];
+        philox4x32_10(i >> 5, r, 0u, make_tag(0u, DOM_BONDS, 0u), a.keys, w);
+        for (int mu = 0; mu < g.d; ++mu)
+            canon[((size_t)r * g.d + mu) * N + i] = ((w[mu] >> (i & 31u)) & 1u) ? (int8_t)-1 : (int8_t)1;
+    }
+}
+
+// Bit planes bb[colour][r][3][NW] (bit = 1: J = -1) from the seed (canon == NULL) or a canonical array.
+__global__ void __launch_bounds__(256) bonds_pack(const __grid_constant__ SetupArgs a, const int8_t *canon, uint32_t *bb) {
+    const Geometry &g = a.g;
+    const uint32_t per_colour = a.R * g.Nh, total = 2u * per_colour, N = 2u * g.Nh;
+    for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
+        const uint32_t c = idx / per_colour, rem = idx - c * per_colour;
+        const uint32_t r = rem / g.Nh, j = rem - r * g.Nh;
+        const uint32_t i = lex_index(g, c, j);
+        uint32_t w[4] = {0u, 0u, 0u, 0u};
+        if (canon == nullptr) philox4x32_10(i >> 5, r, 0u, make_tag(0u, DOM_BONDS, 0u), a.keys, w);
+        for (int mu = 0; mu < 3; ++mu) {
+            uint32_t bit = 0u;
+            if (mu < g.d) bit = canon ? (canon[((size_t)r * g.d + mu) * N + i] < 0 ? 1u : 0u) : ((w[mu] >> (i & 31u)) & 1u);
+            const uint32_t word = __ballot_sync(0xFFFFFFFFu, bit);
+            if ((threadIdx.x & 31) == 0) bb[((size_t)(c * a.R + r) * 3 + mu) * g.NW + (j >> 5)] = word;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) bonds_unpack(const __grid_constant__ SetupArgs a, const uint32_t *bb, int8_t *canon) {
+    const Geometry &g = a.g;
+    const uint32_t per_colour = a.R * g.Nh, total = 2u * per_colour, N = 2u * g.Nh;
+    for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
+        const uint32_t c = idx / per_colour, rem = idx - c * per_colour;
+        const uint32_t r = rem / g.Nh, j = rem - r * g.Nh;
+        const uint32_t i = lex_index(g, c, j);
+        for (int mu = 0; mu < g.d; ++mu) {
+            const uint32_t bit = (bb[((size_t)(c * a.R + r) * 3 + mu) * g.NW + (j >> 5)] >> (j & 31u)) & 1u;
+            canon[((size_t)r * g.d + mu) * N + i] = bit ? (int8_t)-1 : (int8_t)1;
+        }
+    }
+}
+
+}  // namespace spin

@@ -1,0 +1,561 @@
+// spin_api.cu -- host side of libspin: the C ABI of include/spin.h (argument checks, workspace carving,
+// Boltzmann table, kernel selection and launches).  No torch types, no CPU fallback: every step of the
+// sweep and of the measurement runs in the kernels of this directory.
+#include "../../include/spin.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "ising_int8_kernel.cuh"
+#include "ising_kernels.cuh"
+#include "measure_kernels.cuh"
+#include "setup_kernels.cuh"
+#include "vector_kernels.cuh"
+
+using namespace spin;
+
+// ------------------------------------------------------------------------------- errors ------
+static thread_local char g_err[512] = "";
+
+static spin_status fail(spin_status st, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return st;
+}
+
+#define CUDA_TRY(expr)                                                                                    \
+    do {                                                                                                  \
+        cudaError_t e_ = (expr);                                                                          \
+        if (e_ != cudaSuccess) return fail(SPIN_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_));       \
+    } while (0)
+
+// ------------------------------------------------------------------------------- handle ------
+enum Path { PATH_ISING_GENERIC, PATH_ISING_INT8, PATH_ISING_BITPACK, PATH_VECTOR };
+
+struct Layout {
+    size_t off_s[2], bytes_s;   // one colour array
+    size_t off_bonds, bytes_bonds;
+    size_t off_acc, bytes_acc;  // n = 1: int64 [R][2]; n >= 2: double [R][mblocks][1 + n]
+    size_t off_res, bytes_res;  // double [R] E then [R][n] M
+    size_t total;
+};
+
+struct spin_system {
+    spin_config cfg;
+    Geometry g;
+    PhiloxKeys keys;
+    Path path;
+    int d, n;
+    uint32_t R;
+    uint64_t N;
+    Layout lay;
+    char *ws;
+    uint64_t t;          // sweeps done = Philox sweep index of the next sweep
+    uint64_t launches;
+    int sm_count;
+    int block;           // threads per CTA
+    int grid_num, grid_den;
+    uint32_t mblocks;    // CTAs (per replica) of the measurement kernels
+    double table_beta;   // beta the cached table was built for (NaN = none)
+    IsingTable tab;
+};
+
+static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
+
+static FastDiv make_fastdiv(uint32_t d) {
+    FastDiv f;
+    f.div = d;
+    if (d <= 1) { f.mul = 0; f.shift = 0; return f; }
+    uint32_t l = 0;
+    while ((1ull << l) < d) ++l;                       // l = ceil(log2 d) >= 1
+    const unsigned __int128 one = 1;
+    const unsigned __int128 num = one << (31 + l);
+    f.mul = (uint32_t)((num + d - 1) / d);             // ceil(2^(31+l) / d) <= 2^32 - 1 for d not a power of two
+    if (((uint64_t)d & ((uint64_t)d - 1)) == 0) f.mul = 0x80000000u;  // power of two: exact
+    f.shift = l - 1;
+    return f;
+}
+
+struct Derived {
+    int d;
+    uint64_t N;
+    Path path;
+};
+
+static spin_status derive(const spin_config *c, Derived *out) {
+    if (!c) return fail(SPIN_ERR_INVALID_ARG, "config is NULL");
+    const int32_t *L = c->dims;
+    if (L[0] < 2 || L[1] < 2 || L[2] < 1) return fail(SPIN_ERR_INVALID_ARG, "dims must be >= 2 (Lz >= 1)");
+    if ((L[0] & 1) || (L[1] & 1) || (L[2] > 1 && (L[2] & 1)))
+        return fail(SPIN_ERR_INVALID_ARG, "every lattice dimension must be even (checkerboard + periodic)");
+    if (c->n < 1 || c->n > 3) return fail(SPIN_ERR_INVALID_ARG, "n must be 1, 2 or 3");
+    if (c->n_replicas < 1) return fail(SPIN_ERR_INVALID_ARG, "n_replicas must be >= 1");
+    if (c->coupling_kind < SPIN_J_UNIFORM || c->coupling_kind > SPIN_J_BOND_PM1)
+        return fail(SPIN_ERR_INVALID_ARG, "bad coupling_kind");
+    if (c->init != SPIN_INIT_HOT && c->init != SPIN_INIT_COLD) return fail(SPIN_ERR_INVALID_ARG, "bad init");
+    if (c->storage < SPIN_STORE_INT8 || c->storage > SPIN_STORE_FP32) return fail(SPIN_ERR_INVALID_ARG, "bad storage");
+    if (c->n == 1 && c->storage == SPIN_STORE_FP32) return fail(SPIN_ERR_INVALID_ARG, "n = 1 needs INT8 or BITPACK storage");
+    if (c->n > 1 && c->storage != SPIN_STORE_FP32) return fail(SPIN_ERR_INVALID_ARG, "n >= 2 needs FP32 storage");
+    out->d = L[2] == 1 ? 2 : 3;
+    out->N = (uint64_t)L[0] * (uint64_t)L[1] * (uint64_t)L[2];
+    if (out->N * (uint64_t)c->n_replicas >= (1ull << 31))
+        return fail(SPIN_ERR_UNSUPPORTED, "N * n_replicas must stay below 2^31");
+    const int used = c->coupling_kind == SPIN_J_UNIFORM ? 1 : (c->coupling_kind == SPIN_J_PER_DIRECTION ? out->d : 0);
+    for (int mu = 0; mu < used; ++mu)
+        if (!std::isfinite(c->J[mu])) return fail(SPIN_ERR_INVALID_ARG, "J must be finite");
+    if (c->n == 1) {
+        for (int mu = 0; mu < used; ++mu)
+            if (!(c->J[mu] == -1.0 || c->J[mu] == 0.0 || c->J[mu] == 1.0))
+                return fail(SPIN_ERR_UNSUPPORTED, "n = 1 supports couplings in {-1, 0, +1} only (integer table)");
+        const bool unit_uniform = c->coupling_kind == SPIN_J_UNIFORM && c->J[0] != 0.0;
+        if (c->storage == SPIN_STORE_BITPACK) {
+            if (L[0] % 64) return fail(SPIN_ERR_UNSUPPORTED, "BITPACK storage needs Lx %% 64 == 0");
+            if (!(unit_uniform || c->coupling_kind == SPIN_J_BOND_PM1))
+                return fail(SPIN_ERR_UNSUPPORTED, "BITPACK storage needs uniform J = +-1 or per-bond +-1 couplings");
+            out->path = PATH_ISING_BITPACK;
+        } else {
+            out->path = (L[0] % 64 == 0 && unit_uniform) ? PATH_ISING_INT8 : PATH_ISING_GENERIC;
+        }
+    } else {
+        if (c->coupling_kind == SPIN_J_BOND_PM1) return fail(SPIN_ERR_UNSUPPORTED, "per-bond couplings are n = 1 only");
+        out->path = PATH_VECTOR;
+    }
+    return SPIN_OK;
+}
+
+static uint32_t measure_blocks(uint64_t work_items) {
+    uint64_t b = (work_items + 255) / 256;
+    if (b > 592) b = 592;  // 4 CTAs per SM on 148 SMs
+    if (b < 1) b = 1;
+    return (uint32_t)b;
+}
+
+static void make_layout(const spin_config *c, const Derived &dv, Layout *l, uint32_t *mblocks) {
+    const uint64_t Nh = dv.N / 2, R = (uint64_t)c->n_replicas;
+    size_t off = 0;
+    if (dv.path == PATH_ISING_BITPACK) l->bytes_s = (size_t)(R * Nh / 8);
+    else if (dv.path == PATH_VECTOR) l->bytes_s = (size_t)(R * Nh * c->n * sizeof(float));
+    else l->bytes_s = (size_t)(R * Nh);
+    for (int k = 0; k < 2; ++k) { l->off_s[k] = off; off += align_up(l->bytes_s); }
+    l->bytes_bonds = 0;
+    if (c->coupling_kind == SPIN_J_BOND_PM1)
+        l->bytes_bonds = dv.path == PATH_ISING_BITPACK ? (size_t)(2 * R * 3 * (Nh / 32) * 4) : (size_t)(R * dv.d * dv.N);
+    l->off_bonds = off; off += align_up(l->bytes_bonds);
+    *mblocks = measure_blocks(dv.path == PATH_ISING_BITPACK ? Nh / 32 : Nh);
+    l->bytes_acc = c->n == 1 ? (size_t)(R * 2 * sizeof(long long)) : (size_t)(R * *mblocks * (1 + c->n) * sizeof(double));
+    l->off_acc = off; off += align_up(l->bytes_acc);
+    l->bytes_res = (size_t)(R * (1 + c->n) * sizeof(double));
+    l->off_res = off; off += align_up(l->bytes_res);
+    l->total = off;
+}
+
+static SetupArgs setup_args(const spin_system *s) {
+    SetupArgs a;
+    a.g = s->g; a.keys = s->keys; a.R = s->R;
+    a.bitpack = s->path == PATH_ISING_BITPACK;
+    a.nc = s->n;
+    return a;
+}
+
+static int grid_for(const spin_system *s, uint64_t work_items) {
+    uint64_t need = (work_items + s->block - 1) / s->block;
+    uint64_t cap = (uint64_t)s->sm_count * (2048 / s->block) * (uint64_t)s->grid_num / (uint64_t)s->grid_den;
+    if (cap < 1) cap = 1;
+    if (need > cap) need = cap;
+    if (need < 1) need = 1;
+    return (int)need;
+}
+
+// ------------------------------------------------------------------- Boltzmann table ---------
+// T(dE) = floor(exp(-beta dE) 2^32), 0 <= T <= 2^32, in double (R-4, R-5).
+static void build_table(double beta, IsingTable *tab) {
+    std::memset(tab, 0, sizeof *tab);
+    for (int dE = 0; dE <= 12; ++dE) {
+        const double scaled = std::ldexp(std::exp(-beta * (double)dE), 32);
+        uint64_t T;
+        if (!(scaled < 4294967296.0)) T = 4294967296ull;
+        else if (!(scaled > 0.0)) T = 0ull;
+        else T = (uint64_t)std::floor(scaled);
+        if (T >= 4294967296ull) { tab->Talways |= 1u << dE; tab->T[dE] = 0xFFFFFFFFu; }
+        else tab->T[dE] = (uint32_t)T;
+    }
+    for (int th = 0; th < 3; ++th) {
+        const int dE = 4 * (th + 1);
+        tab->always[th] = ((tab->Talways >> dE) & 1u) ? 0xFFFFFFFFu : 0u;
+        for (int k = 0; k < 32; ++k) tab->digit[th][k] = ((tab->T[dE] >> (31 - k)) & 1u) ? 0xFFFFFFFFu : 0u;
+    }
+}
+
+static IsingArgs ising_args(const spin_system *s) {
+    IsingArgs a;
+    a.g = s->g; a.keys = s->keys; a.tab = s->tab;
+    a.s[0] = s->ws + s->lay.off_s[0];
+    a.s[1] = s->ws + s->lay.off_s[1];
+    a.bonds = s->lay.bytes_bonds ? s->ws + s->lay.off_bonds : nullptr;
+    a.R = s->R; a.replica_streams = s->cfg.replica_streams ? 1u : 0u;
+    a.t = (uint32_t)s->t; a.colour = 0;
+    a.coupling_kind = s->cfg.coupling_kind;
+    for (int mu = 0; mu < 3; ++mu)
+        a.Jdir[mu] = s->cfg.coupling_kind == SPIN_J_UNIFORM ? (int)s->cfg.J[0]
+                   : (s->cfg.coupling_kind == SPIN_J_PER_DIRECTION ? (mu < s->d ? (int)s->cfg.J[mu] : 0) : 0);
+    a.jneg = (s->cfg.coupling_kind == SPIN_J_UNIFORM && s->cfg.J[0] < 0.0) ? 1u : 0u;
+    return a;
+}
+
+static VectorArgs vector_args(const spin_system *s, double beta) {
+    VectorArgs a;
+    a.g = s->g; a.keys = s->keys;
+    a.s[0] = (float *)(s->ws + s->lay.off_s[0]);
+    a.s[1] = (float *)(s->ws + s->lay.off_s[1]);
+    a.R = s->R; a.replica_streams = s->cfg.replica_streams ? 1u : 0u;
+    a.t = (uint32_t)s->t; a.colour = 0;
+    for (int mu = 0; mu < 3; ++mu)
+        a.Jdir[mu] = s->cfg.coupling_kind == SPIN_J_UNIFORM ? (float)s->cfg.J[0] : (mu < s->d ? (float)s->cfg.J[mu] : 0.0f);
+    a.beta = (float)beta;
+    return a;
+}
+
+// ----------------------------------------------------------------------------- launches ------
+static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cudaStream_t st) {
+    const bool bonds = s->cfg.coupling_kind == SPIN_J_BOND_PM1;
+    const bool shared = s->R > 1 && !s->cfg.replica_streams;
+    const int B = s->block;
+    if (s->path == PATH_ISING_GENERIC) {
+        ising_generic_halfsweep<<<grid_for(s, (uint64_t)s->g.Nh * s->R), B, 0, st>>>(a);
+    } else if (s->path == PATH_ISING_INT8) {
+        const int G = grid_for(s, s->g.NW);
+        if (s->d == 2) ising_int8_halfsweep<2><<<G, B, 0, st>>>(a);
+        else ising_int8_halfsweep<3><<<G, B, 0, st>>>(a);
+    } else {
+        const int G = grid_for(s, s->g.NW);
+#define BP(D_, BONDS_, SH_) ising_bitpack_halfsweep<D_, BONDS_, SH_><<<G, B, 0, st>>>(a)
+        if (s->d == 2) {
+            if (bonds) { if (shared) BP(2, true, true); else BP(2, true, false); }
+            else { if (shared) BP(2, false, true); else BP(2, false, false); }
+        } else {
+            if (bonds) { if (shared) BP(3, true, true); else BP(3, true, false); }
+            else { if (shared) BP(3, false, true); else BP(3, false, false); }
+        }
+#undef BP
+    }
+    s->launches += 1;
+    CUDA_TRY(cudaGetLastError());
+    return SPIN_OK;
+}
+
+static spin_status enqueue_sweep(spin_system *s, double beta, cudaStream_t st) {
+    if (s->n == 1) {
+        IsingArgs a = ising_args(s);
+        for (uint32_t colour = 0; colour < 2; ++colour) {
+            a.colour = colour;
+            spin_status rc = launch_halfsweep_ising(s, a, st);
+            if (rc != SPIN_OK) return rc;
+        }
+    } else {
+        VectorArgs a = vector_args(s, beta);
+        const int G = grid_for(s, (uint64_t)s->g.Nh * s->R);
+        for (uint32_t colour = 0; colour < 2; ++colour) {
+            a.colour = colour;
+            if (s->n == 2) vector_halfsweep<2><<<G, s->block, 0, st>>>(a);
+            else vector_halfsweep<3><<<G, s->block, 0, st>>>(a);
+            s->launches += 1;
+            CUDA_TRY(cudaGetLastError());
+        }
+    }
+    s->t += 1;
+    return SPIN_OK;
+}
+
+// E, M of every replica into device doubles dE[R], dM[R][n]
+static spin_status enqueue_measure(spin_system *s, double *dE, double *dM, cudaStream_t st) {
+    const dim3 grid(s->mblocks, s->R);
+    if (s->n == 1) {
+        IsingArgs a = ising_args(s);
+        long long *acc = (long long *)(s->ws + s->lay.off_acc);
+        const bool bonds = s->cfg.coupling_kind == SPIN_J_BOND_PM1;
+        if (s->path == PATH_ISING_BITPACK) {
+            if (s->d == 2) { if (bonds) ising_bitpack_measure<2, true><<<grid, 256, 0, st>>>(a, acc); else ising_bitpack_measure<2, false><<<grid, 256, 0, st>>>(a, acc); }
+            else { if (bonds) ising_bitpack_measure<3, true><<<grid, 256, 0, st>>>(a, acc); else ising_bitpack_measure<3, false><<<grid, 256, 0, st>>>(a, acc); }
+        } else {
+            ising_generic_measure<<<grid, 256, 0, st>>>(a, acc);
+        }
+        CUDA_TRY(cudaGetLastError());
+        ising_measure_finalize<<<(s->R + 63) / 64, 64, 0, st>>>(acc, s->R, dE, dM);
+    } else {
+        VectorArgs a = vector_args(s, 0.0);
+        double *part = (double *)(s->ws + s->lay.off_acc);
+        if (s->n == 2) vector_measure<2><<<grid, 256, 0, st>>>(a, part);
+        else vector_measure<3><<<grid, 256, 0, st>>>(a, part);
+        CUDA_TRY(cudaGetLastError());
+        vector_measure_finalize<<<s->R, 256, 0, st>>>(part, s->mblocks, s->n, dE, dM);
+    }
+    s->launches += 2;
+    CUDA_TRY(cudaGetLastError());
+    return SPIN_OK;
+}
+
+static spin_status check_sweep_args(spin_system *s, double beta, int64_t n_sweeps) {
+    if (!s) return fail(SPIN_ERR_INVALID_ARG, "handle is NULL");
+    if (!(beta >= 0.0) || !std::isfinite(beta)) return fail(SPIN_ERR_INVALID_ARG, "beta must be finite and >= 0");
+    if (n_sweeps < 0) return fail(SPIN_ERR_INVALID_ARG, "n_sweeps must be >= 0");
+    if (s->t + (uint64_t)n_sweeps > 0x100000000ull) return fail(SPIN_ERR_STATE, "sweep counter would pass 2^32");
+    if (s->n == 1 && !(beta == s->table_beta)) { build_table(beta, &s->tab); s->table_beta = beta; }
+    return SPIN_OK;
+}
+
+// ------------------------------------------------------------------------------ C ABI --------
+extern "C" {
+
+const char *spin_last_error(void) { return g_err; }
+const char *spin_version(void) { return "libspin 0.1 sm_100a"; }
+
+spin_status spin_workspace_bytes(const spin_config *cfg, size_t *bytes) {
+    if (!bytes) return fail(SPIN_ERR_INVALID_ARG, "bytes is NULL");
+    Derived dv;
+    spin_status rc = derive(cfg, &dv);
+    if (rc != SPIN_OK) return rc;
+    Layout l;
+    uint32_t mb;
+    make_layout(cfg, dv, &l, &mb);
+    *bytes = l.total;
+    return SPIN_OK;
+}
+
+spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes, void *stream, spin_system **out) {
+    if (!out) return fail(SPIN_ERR_INVALID_ARG, "out is NULL");
+    Derived dv;
+    spin_status rc = derive(cfg, &dv);
+    if (rc != SPIN_OK) return rc;
+    if (!d_workspace) return fail(SPIN_ERR_INVALID_ARG, "d_workspace is NULL");
+    if (((uintptr_t)d_workspace & 255) != 0) return fail(SPIN_ERR_INVALID_ARG, "d_workspace must be 256-byte aligned");
+    if (cfg->coupling_kind == SPIN_J_BOND_PM1 && cfg->bonds) {
+        const size_t nb = (size_t)cfg->n_replicas * dv.d * dv.N;
+        for (size_t k = 0; k < nb; ++k)
+            if (cfg->bonds[k] != 1 && cfg->bonds[k] != -1) return fail(SPIN_ERR_INVALID_ARG, "bonds must be +-1");
+    }
+    spin_system *s = new (std::nothrow) spin_system();
+    if (!s) return fail(SPIN_ERR_INVALID_ARG, "out of host memory");
+    s->cfg = *cfg;
+    s->cfg.bonds = nullptr;  // host array is read here only
+    s->d = dv.d; s->n = cfg->n; s->R = (uint32_t)cfg->n_replicas; s->N = dv.N; s->path = dv.path;
+    make_layout(cfg, dv, &s->lay, &s->mblocks);
+    if (bytes < s->lay.total) {
+        const size_t need = s->lay.total;
+        delete s;
+        return fail(SPIN_ERR_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, %zu needed", bytes, need);
+    }
+    s->ws = (char *)d_workspace;
+    s->t = 0; s->launches = 0;
+    s->block = 256; s->grid_num = 1; s->grid_den = 1;
+    s->table_beta = std::nan("");
+    Geometry &g = s->g;
+    g.Lx = cfg->dims[0]; g.Ly = cfg->dims[1]; g.Lz = cfg->dims[2]; g.d = dv.d;
+    g.RL = (uint32_t)(g.Lx / 2); g.rows = (uint32_t)(g.Ly * g.Lz); g.Nh = (uint32_t)(dv.N / 2);
+    g.WX = g.RL / 32; g.NW = g.Nh / 32;
+    g.divRL = make_fastdiv(g.RL); g.divWX = make_fastdiv(g.WX ? g.WX : 1); g.divLy = make_fastdiv((uint32_t)g.Ly);
+    for (int r = 0; r < 10; ++r) {
+        s->keys.k0[r] = (uint32_t)(cfg->seed & 0xFFFFFFFFull) + (uint32_t)r * 0x9E3779B9u;
+        s->keys.k1[r] = (uint32_t)(cfg->seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e;
+    int dev = 0;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess ||
+        (e = cudaDeviceGetAttribute(&s->sm_count, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) {
+        delete s;
+        return fail(SPIN_ERR_CUDA, "no usable CUDA device: %s", cudaGetErrorString(e));
+    }
+#define CREATE_TRY(expr)                                                                              \
+    do {                                                                                              \
+        cudaError_t e2_ = (expr);                                                                     \
+        if (e2_ != cudaSuccess) {                                                                     \
+            if (staging) cudaFree(staging);                                                           \
+            delete s;                                                                                 \
+            return fail(SPIN_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e2_));                     \
+        }                                                                                             \
+    } while (0)
+    void *staging = nullptr;
+    const SetupArgs sa = setup_args(s);
+    const int B = 256;
+    const int G = grid_for(s, 2ull * s->R * g.Nh);
+    CREATE_TRY(cudaMemsetAsync(s->ws + s->lay.off_acc, 0, s->lay.bytes_acc, st));
+    if (cfg->coupling_kind == SPIN_J_BOND_PM1) {
+        const size_t nb = (size_t)s->R * s->d * s->N;
+        if (s->path == PATH_ISING_BITPACK) {
+            if (cfg->bonds) {
+                CREATE_TRY(cudaMalloc(&staging, nb));
+                CREATE_TRY(cudaMemcpyAsync(staging, cfg->bonds, nb, cudaMemcpyHostToDevice, st));
+            }
+            bonds_pack<<<G, B, 0, st>>>(sa, (const int8_t *)staging, (uint32_t *)(s->ws + s->lay.off_bonds));
+        } else if (cfg->bonds) {
+            CREATE_TRY(cudaMemcpyAsync(s->ws + s->lay.off_bonds, cfg->bonds, nb, cudaMemcpyHostToDevice, st));
+        } else {
+            bonds_draw_canonical<<<grid_for(s, (uint64_t)s->R * s->N), B, 0, st>>>(sa, (int8_t *)(s->ws + s->lay.off_bonds));
+        }
+        CREATE_TRY(cudaGetLastError());
+    }
+    const int mode = cfg->init == SPIN_INIT_HOT ? 1 : 0;
+    if (s->n == 1) ising_fill<<<G, B, 0, st>>>(sa, mode, nullptr, s->ws + s->lay.off_s[0], s->ws + s->lay.off_s[1]);
+    else if (s->n == 2) vector_fill<2><<<G, B, 0, st>>>(sa, mode, nullptr, (float *)(s->ws + s->lay.off_s[0]), (float *)(s->ws + s->lay.off_s[1]));
+    else vector_fill<3><<<G, B, 0, st>>>(sa, mode, nullptr, (float *)(s->ws + s->lay.off_s[0]), (float *)(s->ws + s->lay.off_s[1]));
+    CREATE_TRY(cudaGetLastError());
+    CREATE_TRY(cudaStreamSynchronize(st));
+    if (staging) cudaFree(staging);
+#undef CREATE_TRY
+    *out = s;
+    return SPIN_OK;
+}
+
+spin_status spin_destroy(spin_system *s) {
+    delete s;
+    return SPIN_OK;
+}
+
+spin_status spin_sweep(spin_system *s, double beta, int64_t n_sweeps, void *stream) {
+    spin_status rc = check_sweep_args(s, beta, n_sweeps);
+    if (rc != SPIN_OK) return rc;
+    for (int64_t k = 0; k < n_sweeps; ++k) {
+        rc = enqueue_sweep(s, beta, (cudaStream_t)stream);
+        if (rc != SPIN_OK) return rc;
+    }
+    return SPIN_OK;
+}
+
+spin_status spin_sweep_record(spin_system *s, double beta, int64_t n_sweeps, double *d_E, double *d_M, void *stream) {
+    spin_status rc = check_sweep_args(s, beta, n_sweeps);
+    if (rc != SPIN_OK) return rc;
+    if (!d_E || !d_M) return fail(SPIN_ERR_INVALID_ARG, "d_E / d_M is NULL");
+    for (int64_t k = 0; k < n_sweeps; ++k) {
+        rc = enqueue_sweep(s, beta, (cudaStream_t)stream);
+        if (rc != SPIN_OK) return rc;
+        rc = enqueue_measure(s, d_E + (size_t)k * s->R, d_M + (size_t)k * s->R * s->n, (cudaStream_t)stream);
+        if (rc != SPIN_OK) return rc;
+    }
+    return SPIN_OK;
+}
+
+spin_status spin_measure(spin_system *s, double *E, double *M, void *stream) {
+    if (!s || !E || !M) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    double *res = (double *)(s->ws + s->lay.off_res);
+    spin_status rc = enqueue_measure(s, res, res + s->R, st);
+    if (rc != SPIN_OK) return rc;
+    // small result: stage through a local buffer so outputs are written only on success
+    const size_t nE = s->R, nM = (size_t)s->R * s->n;
+    double *tmp = new (std::nothrow) double[nE + nM];
+    if (!tmp) return fail(SPIN_ERR_INVALID_ARG, "out of host memory");
+    cudaError_t e = cudaMemcpyAsync(tmp, res, (nE + nM) * sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { delete[] tmp; return fail(SPIN_ERR_CUDA, "measure copy: %s", cudaGetErrorString(e)); }
+    std::memcpy(E, tmp, nE * sizeof(double));
+    std::memcpy(M, tmp + nE, nM * sizeof(double));
+    delete[] tmp;
+    return SPIN_OK;
+}
+
+static size_t canonical_spin_bytes(const spin_system *s) {
+    return s->n == 1 ? (size_t)s->R * s->N : (size_t)s->R * s->N * s->n * sizeof(float);
+}
+
+spin_status spin_get_spins(spin_system *s, void *host, size_t bytes) {
+    if (!s || !host) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    const size_t need = canonical_spin_bytes(s);
+    if (bytes != need) return fail(SPIN_ERR_INVALID_ARG, "spins need exactly %zu bytes, got %zu", need, bytes);
+    void *staging = nullptr;
+    CUDA_TRY(cudaDeviceSynchronize());
+    CUDA_TRY(cudaMalloc(&staging, need));
+    const SetupArgs sa = setup_args(s);
+    const int G = grid_for(s, 2ull * s->R * s->g.Nh);
+    void *s0 = s->ws + s->lay.off_s[0], *s1 = s->ws + s->lay.off_s[1];
+    if (s->n == 1) ising_to_canonical<<<G, 256>>>(sa, s0, s1, (int8_t *)staging);
+    else if (s->n == 2) vector_to_canonical<2><<<G, 256>>>(sa, (const float *)s0, (const float *)s1, (float *)staging);
+    else vector_to_canonical<3><<<G, 256>>>(sa, (const float *)s0, (const float *)s1, (float *)staging);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpy(host, staging, need, cudaMemcpyDeviceToHost);
+    cudaFree(staging);
+    if (e != cudaSuccess) return fail(SPIN_ERR_CUDA, "get_spins: %s", cudaGetErrorString(e));
+    return SPIN_OK;
+}
+
+spin_status spin_set_spins(spin_system *s, const void *host, size_t bytes) {
+    if (!s || !host) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    const size_t need = canonical_spin_bytes(s);
+    if (bytes != need) return fail(SPIN_ERR_INVALID_ARG, "spins need exactly %zu bytes, got %zu", need, bytes);
+    if (s->n == 1) {
+        const int8_t *p = (const int8_t *)host;
+        for (size_t k = 0; k < need; ++k)
+            if (p[k] != 1 && p[k] != -1) return fail(SPIN_ERR_INVALID_ARG, "Ising spins must be +-1");
+    }
+    void *staging = nullptr;
+    CUDA_TRY(cudaDeviceSynchronize());
+    CUDA_TRY(cudaMalloc(&staging, need));
+    cudaError_t e = cudaMemcpy(staging, host, need, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        const SetupArgs sa = setup_args(s);
+        const int G = grid_for(s, 2ull * s->R * s->g.Nh);
+        void *s0 = s->ws + s->lay.off_s[0], *s1 = s->ws + s->lay.off_s[1];
+        if (s->n == 1) ising_fill<<<G, 256>>>(sa, 2, (const int8_t *)staging, s0, s1);
+        else if (s->n == 2) vector_fill<2><<<G, 256>>>(sa, 2, (const float *)staging, (float *)s0, (float *)s1);
+        else vector_fill<3><<<G, 256>>>(sa, 2, (const float *)staging, (float *)s0, (float *)s1);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    }
+    cudaFree(staging);
+    if (e != cudaSuccess) return fail(SPIN_ERR_CUDA, "set_spins: %s", cudaGetErrorString(e));
+    return SPIN_OK;
+}
+
+spin_status spin_get_bonds(spin_system *s, int8_t *host, size_t bytes) {
+    if (!s || !host) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    if (s->cfg.coupling_kind != SPIN_J_BOND_PM1) return fail(SPIN_ERR_INVALID_ARG, "system has no per-bond couplings");
+    const size_t need = (size_t)s->R * s->d * s->N;
+    if (bytes != need) return fail(SPIN_ERR_INVALID_ARG, "bonds need exactly %zu bytes, got %zu", need, bytes);
+    CUDA_TRY(cudaDeviceSynchronize());
+    if (s->path != PATH_ISING_BITPACK) {
+        CUDA_TRY(cudaMemcpy(host, s->ws + s->lay.off_bonds, need, cudaMemcpyDeviceToHost));
+        return SPIN_OK;
+    }
+    void *staging = nullptr;
+    CUDA_TRY(cudaMalloc(&staging, need));
+    bonds_unpack<<<grid_for(s, 2ull * s->R * s->g.Nh), 256>>>(setup_args(s), (const uint32_t *)(s->ws + s->lay.off_bonds), (int8_t *)staging);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpy(host, staging, need, cudaMemcpyDeviceToHost);
+    cudaFree(staging);
+    if (e != cudaSuccess) return fail(SPIN_ERR_CUDA, "get_bonds: %s", cudaGetErrorString(e));
+    return SPIN_OK;
+}
+
+spin_status spin_get_sweep_count(const spin_system *s, uint64_t *t) {
+    if (!s || !t) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    *t = s->t;
+    return SPIN_OK;
+}
+
+spin_status spin_set_sweep_count(spin_system *s, uint64_t t) {
+    if (!s) return fail(SPIN_ERR_INVALID_ARG, "handle is NULL");
+    if (t > 0x100000000ull) return fail(SPIN_ERR_INVALID_ARG, "sweep counter is 32 bits wide");
+    s->t = t;
+    return SPIN_OK;
+}
+
+spin_status spin_get_launch_count(const spin_system *s, uint64_t *launches) {
+    if (!s || !launches) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    *launches = s->launches;
+    return SPIN_OK;
+}
+
+spin_status spin_set_launch_shape(spin_system *s, int32_t block, int32_t grid_num, int32_t grid_den) {
+    if (!s) return fail(SPIN_ERR_INVALID_ARG, "handle is NULL");
+    if (block == 0) block = 256;
+    if (block != 64 && block != 128 && block != 256) return fail(SPIN_ERR_INVALID_ARG, "block must be 64, 128 or 256");
+    if (grid_num < 1 || grid_den < 1) return fail(SPIN_ERR_INVALID_ARG, "grid_num / grid_den must be >= 1");
+    s->block = block; s->grid_num = grid_num; s->grid_den = grid_den;
+    return SPIN_OK;
+}
+
+}  // extern "C"

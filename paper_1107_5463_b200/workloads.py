@@ -1,0 +1,57 @@
+"""The BASELINE.json workloads as plain data (dims, model, storage, beta, sweeps, seed).
+
+Holds none of the method's arithmetic: the tests, bench.py and the oracle harness all read the same
+recipes from here and build their own systems from them.  Every input is synthetic and seeded
+(hot start and bonds are drawn from the seed by each implementation's own Philox).
+"""
+SEED = 11075463
+
+# name -> recipe.  `storage` values name the C-ABI enums (binding.STORE_*).
+WORKLOADS = {
+    # config 1: 2D Ising L = 64, 1000 sweeps, E and M recorded every sweep
+    "ising2d_L64_int8": dict(dims=(64, 64, 1), n=1, storage="int8", coupling="uniform", J=(1.0, 1.0, 1.0),
+                             beta=0.4406868, sweeps=1000, replicas=1, replica_streams=0, record=True),
+    # config 2: 2D Ising L = 16384, 1000 sweeps, int8 and bit-packed
+    "ising2d_L16384_int8": dict(dims=(16384, 16384, 1), n=1, storage="int8", coupling="uniform", J=(1.0, 1.0, 1.0),
+                                beta=0.4406868, sweeps=1000, replicas=1, replica_streams=0, record=False),
+    "ising2d_L16384_bitpack": dict(dims=(16384, 16384, 1), n=1, storage="bitpack", coupling="uniform",
+                                   J=(1.0, 1.0, 1.0), beta=0.4406868, sweeps=1000, replicas=1, replica_streams=0,
+                                   record=False),
+    # config 3: 3D Ising L = 512, 500 sweeps, multi-spin coded
+    "ising3d_L512_bitpack": dict(dims=(512, 512, 512), n=1, storage="bitpack", coupling="uniform", J=(1.0, 1.0, 1.0),
+                                 beta=0.2216546, sweeps=500, replicas=1, replica_streams=0, record=False),
+    # config 4: 3D +-J Edwards-Anderson L = 256, 16 disorder realisations side by side, shared update stream
+    "ea3d_L256_R16_bitpack": dict(dims=(256, 256, 256), n=1, storage="bitpack", coupling="bond_pm1",
+                                  J=(1.0, 1.0, 1.0), beta=1.0 / 1.1, sweeps=1000, replicas=16, replica_streams=0,
+                                  record=False),
+    # config 5: 3D Heisenberg L = 256, 500 sweeps
+    "heisenberg3d_L256_fp32": dict(dims=(256, 256, 256), n=3, storage="fp32", coupling="uniform", J=(1.0, 1.0, 1.0),
+                                   beta=0.693, sweeps=500, replicas=1, replica_streams=0, record=False),
+    # extra: 3D XY (named by north_star, absent from the configs)
+    "xy3d_L256_fp32": dict(dims=(256, 256, 256), n=2, storage="fp32", coupling="uniform", J=(1.0, 1.0, 1.0),
+                           beta=0.4542, sweeps=500, replicas=1, replica_streams=0, record=False),
+}
+
+# Algorithmic bytes moved per attempted update: read the target colour, read the
+# other colour once, write the target colour; +-J adds each bond word once per end point and sweep.
+BYTES_PER_UPDATE = {
+    "ising2d_L64_int8": 3.0,
+    "ising2d_L16384_int8": 3.0,
+    "ising2d_L16384_bitpack": 0.375,
+    "ising3d_L512_bitpack": 0.375,
+    "ea3d_L256_R16_bitpack": 1.125,
+    "heisenberg3d_L256_fp32": 36.0,
+    "xy3d_L256_fp32": 24.0,
+}
+
+
+def n_sites(name):
+    d = WORKLOADS[name]["dims"]
+    return d[0] * d[1] * d[2]
+
+
+def scaled(name, dims):
+    """The same recipe on a smaller lattice (parity tests)."""
+    w = dict(WORKLOADS[name])
+    w["dims"] = tuple(dims)
+    return w

@@ -1,0 +1,267 @@
+"""GPU <-> oracle parity through the C ABI (include/spin.h), run with -m gpu on the B200.
+
+Bar (BASELINE.json north_star): Ising and +-J spins bit-exact after every sweep, E and M equal as integers;
+XY / Heisenberg per-sweep energy within 1e-5 relative over the first 10 sweeps, fewer than 1e-6 of the
+acceptance decisions differing.  The oracle (oracle/) is the plain CPU restatement of PAPER.md:31-46.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+SEED = 11075463
+BETA_2D = 0.4406868
+BETA_3D = 0.2216546
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1107_5463_b200 as pkg
+
+    pkg.lib()
+    return pkg
+
+
+def _oracle_kind(oracle, coupling):
+    return {"uniform": oracle.J_UNIFORM, "per_direction": oracle.J_PER_DIRECTION, "bond_pm1": oracle.J_BOND_PM1}[coupling]
+
+
+def _pair(P, oracle, dims, n=1, storage="int8", coupling="uniform", J=(1.0, 1.0, 1.0), replicas=1, replica_streams=0,
+          seed=SEED, init=0):
+    G = P.SpinSystem(dims, n=n, storage=storage, coupling=coupling, J=J, replicas=replicas,
+                     replica_streams=replica_streams, seed=seed, init=init)
+    O = oracle.System(dims, n=n, coupling_kind=_oracle_kind(oracle, coupling), J=J, n_replicas=replicas,
+                      replica_streams=replica_streams, seed=seed, init=init)
+    return G, O
+
+
+def _assert_ising_equal(G, O, tag):
+    gs, os_ = G.get_spins(), O.get_spins()
+    assert gs.shape == os_.shape
+    bad = int(np.count_nonzero(gs != os_))
+    assert bad == 0, "%s: %d spins differ" % (tag, bad)
+    Eg, Mg = G.measure()
+    Eo, Mo = O.measure()
+    assert np.array_equal(Eg, Eo), (tag, Eg, Eo)
+    assert np.array_equal(Mg, Mo), (tag, Mg, Mo)
+
+
+ISING_CASES = [
+    # dims, storage, beta, sweeps  -- generic kernel (odd shapes, size-2 dimensions)
+    ((4, 4, 1), "int8", BETA_2D, 6),
+    ((8, 6, 1), "int8", BETA_2D, 6),
+    ((66, 2, 1), "int8", BETA_2D, 6),
+    ((4, 2, 2), "int8", BETA_3D, 6),
+    ((6, 4, 8), "int8", BETA_3D, 6),
+    ((2, 2, 2), "int8", BETA_3D, 6),
+    # fast int8 kernel (Lx % 64 == 0): several units per row, ragged grids, 2D and 3D
+    ((64, 4, 1), "int8", BETA_2D, 8),
+    ((128, 6, 1), "int8", BETA_2D, 8),
+    ((192, 10, 1), "int8", BETA_2D, 5),
+    ((64, 2, 2), "int8", BETA_3D, 8),
+    ((128, 6, 4), "int8", BETA_3D, 6),
+    ((192, 10, 6), "int8", BETA_3D, 4),
+    # bit-packed multi-spin coding
+    ((64, 4, 1), "bitpack", BETA_2D, 8),
+    ((128, 6, 1), "bitpack", BETA_2D, 8),
+    ((192, 10, 1), "bitpack", BETA_2D, 5),
+    ((64, 2, 2), "bitpack", BETA_3D, 8),
+    ((128, 6, 4), "bitpack", BETA_3D, 6),
+    ((192, 10, 6), "bitpack", BETA_3D, 4),
+]
+
+
+@pytest.mark.parametrize("dims,storage,beta,sweeps", ISING_CASES)
+def test_ising_bit_exact_every_sweep(P, oracle, dims, storage, beta, sweeps):
+    G, O = _pair(P, oracle, dims, storage=storage)
+    _assert_ising_equal(G, O, "initial state %s" % (dims,))
+    for t in range(sweeps):
+        G.sweep(beta, 1)
+        O.sweep(beta, 1)
+        _assert_ising_equal(G, O, "%s %s sweep %d" % (dims, storage, t))
+
+
+@pytest.mark.parametrize("storage", ["int8", "bitpack"])
+def test_config1_L64_1000_sweeps_recorded(P, oracle, storage):
+    """BASELINE config 1: 64 x 64 at beta_c, 1000 sweeps, E and M after every sweep (bit-exact)."""
+    import torch
+
+    G, O = _pair(P, oracle, (64, 64, 1), storage=storage)
+    dE, dM = G.sweep_record(BETA_2D, 1000)
+    torch.cuda.synchronize()
+    Eg, Mg = dE.cpu().numpy()[:, 0], dM.cpu().numpy()[:, 0, 0]
+    Eo, Mo = np.zeros(1000), np.zeros(1000)
+    for t in range(1000):
+        O.sweep(BETA_2D, 1)
+        e, m = O.measure()
+        Eo[t], Mo[t] = e[0], m[0, 0]
+    assert np.array_equal(Eg, Eo)
+    assert np.array_equal(Mg, Mo)
+    _assert_ising_equal(G, O, "config 1 after 1000 sweeps")
+    assert G.sweep_counter == 1000
+
+
+@pytest.mark.parametrize("dims,storage", [((64, 16, 1), "int8"), ((64, 16, 1), "bitpack"), ((64, 8, 4), "bitpack"),
+                                          ((12, 8, 1), "int8")])
+def test_antiferromagnet(P, oracle, dims, storage):
+    G, O = _pair(P, oracle, dims, storage=storage, J=(-1.0, -1.0, -1.0))
+    for t in range(5):
+        G.sweep(0.5, 1)
+        O.sweep(0.5, 1)
+        _assert_ising_equal(G, O, "J = -1 %s %s sweep %d" % (dims, storage, t))
+
+
+@pytest.mark.parametrize("beta", [0.0, 50.0, 0.1, 1.0 / 1.1])
+@pytest.mark.parametrize("storage,dims", [("int8", (64, 8, 1)), ("bitpack", (64, 8, 4)), ("int8", (10, 8, 1))])
+def test_extreme_betas(P, oracle, beta, storage, dims):
+    """beta = 0: T = 2^32 (33 bits) -> every spin flips; beta = 50: T = 0."""
+    G, O = _pair(P, oracle, dims, storage=storage)
+    for t in range(3):
+        G.sweep(beta, 1)
+        O.sweep(beta, 1)
+        _assert_ising_equal(G, O, "beta %g sweep %d" % (beta, t))
+
+
+def test_per_direction_couplings_generic(P, oracle):
+    for J in [(1.0, 0.0, 0.0), (1.0, -1.0, 0.0), (0.0, 1.0, 1.0)]:
+        G, O = _pair(P, oracle, (8, 6, 4), coupling="per_direction", J=J)
+        for t in range(4):
+            G.sweep(0.7, 1)
+            O.sweep(0.7, 1)
+            _assert_ising_equal(G, O, "J = %s sweep %d" % (J, t))
+
+
+@pytest.mark.parametrize("dims,storage,R,streams", [
+    ((64, 6, 4), "bitpack", 16, 0),   # config 4 shape: 16 realisations, shared update stream
+    ((128, 4, 6), "bitpack", 3, 1),
+    ((64, 8, 1), "bitpack", 5, 0),
+    ((64, 8, 1), "bitpack", 2, 1),
+    ((8, 6, 4), "int8", 3, 0),        # generic kernel with int8 bonds
+    ((64, 4, 1), "int8", 2, 1),
+])
+def test_pm_j_spin_glass_bit_exact(P, oracle, dims, storage, R, streams):
+    G, O = _pair(P, oracle, dims, storage=storage, coupling="bond_pm1", replicas=R, replica_streams=streams)
+    assert np.array_equal(G.get_bonds(), O.get_bonds())
+    _assert_ising_equal(G, O, "+-J initial")
+    beta = 1.0 / 1.1
+    for t in range(6):
+        G.sweep(beta, 1)
+        O.sweep(beta, 1)
+        _assert_ising_equal(G, O, "+-J %s %s R=%d sweep %d" % (dims, storage, R, t))
+
+
+def test_pm_j_user_bonds_and_replica_streams_uniform(P, oracle):
+    rng = np.random.default_rng(5)
+    dims, R = (64, 4, 2), 4
+    N = dims[0] * dims[1] * dims[2]
+    bonds = (1 - 2 * rng.integers(0, 2, size=(R, 3, N))).astype(np.int8)
+    for storage in ("bitpack", "int8"):
+        G = P.SpinSystem(dims, storage=storage, coupling="bond_pm1", bonds=bonds, replicas=R, seed=3)
+        O = oracle.System(dims, coupling_kind=oracle.J_BOND_PM1, bonds=bonds, n_replicas=R, seed=3)
+        assert np.array_equal(G.get_bonds(), bonds)
+        for t in range(4):
+            G.sweep(0.8, 1)
+            O.sweep(0.8, 1)
+            _assert_ising_equal(G, O, "user bonds %s sweep %d" % (storage, t))
+    # uniform couplings, several replicas with their own streams (int8 fast + bitpack)
+    for storage in ("bitpack", "int8"):
+        G, O = _pair(P, oracle, (64, 6, 1), storage=storage, replicas=3, replica_streams=1)
+        for t in range(4):
+            G.sweep(BETA_2D, 1)
+            O.sweep(BETA_2D, 1)
+            _assert_ising_equal(G, O, "replica streams %s sweep %d" % (storage, t))
+
+
+@pytest.mark.parametrize("storage,dims", [("int8", (128, 10, 1)), ("bitpack", (128, 10, 6)), ("int8", (10, 6, 4))])
+def test_launch_shape_and_call_splitting_do_not_matter(P, oracle, storage, dims):
+    beta = 0.3
+    A = P.SpinSystem(dims, storage=storage, seed=SEED)
+    B = P.SpinSystem(dims, storage=storage, seed=SEED)
+    B.set_launch_shape(64, 1, 37)
+    A.sweep(beta, 10)
+    for _ in range(10):
+        B.sweep(beta, 1)
+    assert np.array_equal(A.get_spins(), B.get_spins())
+    O = oracle.System(dims, seed=SEED)
+    O.sweep(beta, 10)
+    assert np.array_equal(A.get_spins(), O.get_spins())
+    # checkpoint / resume: state = spins + sweep counter
+    C2 = P.SpinSystem(dims, storage=storage, seed=SEED, init=P.INIT_COLD)
+    C2.set_spins(A.get_spins())
+    C2.sweep_counter = A.sweep_counter
+    A.sweep(beta, 3)
+    C2.sweep(beta, 3)
+    assert np.array_equal(A.get_spins(), C2.get_spins())
+
+
+@pytest.mark.parametrize("n,dims,beta", [(3, (16, 16, 16), 0.693), (2, (16, 16, 16), 0.4542), (3, (32, 32, 1), 0.693),
+                                         (2, (32, 32, 1), 1.1), (3, (6, 4, 2), 0.693), (2, (4, 2, 2), 0.5)])
+def test_vector_models_within_tolerance(P, oracle, n, dims, beta):
+    G, O = _pair(P, oracle, dims, n=n, storage="fp32")
+    N = dims[0] * dims[1] * dims[2]
+    g0, o0 = G.get_spins(), O.get_spins()
+    assert np.max(np.abs(g0 - o0)) <= 2.4e-7, "hot start differs by more than 2 ulp"
+    mismatched_sites = 0
+    for t in range(10):
+        G.sweep(beta, 1)
+        O.sweep(beta, 1)
+        Eg, Mg = G.measure()
+        Eo, Mo = O.measure()
+        assert abs(Eg[0] - Eo[0]) <= 1e-5 * abs(Eo[0]), (t, Eg, Eo)
+        assert np.max(np.abs(Mg - Mo)) <= 1e-5 * N
+        # a differing acceptance decision leaves a spin that differs by O(1), not by rounding
+        diff = np.max(np.abs(G.get_spins() - O.get_spins()), axis=2)
+        mismatched_sites += int(np.count_nonzero(diff > 1e-4))
+    assert mismatched_sites <= max(0, int(1e-6 * 10 * N)), mismatched_sites
+    norm = np.linalg.norm(G.get_spins(), axis=2)
+    assert np.max(np.abs(norm - 1.0)) < 4e-7
+
+
+def test_vector_per_direction_and_replicas(P, oracle):
+    G, O = _pair(P, oracle, (16, 8, 4), n=3, storage="fp32", coupling="per_direction", J=(1.0, 0.0, 0.5), replicas=3,
+                 replica_streams=1)
+    for t in range(5):
+        G.sweep(1.0, 1)
+        O.sweep(1.0, 1)
+        Eg, Mg = G.measure()
+        Eo, Mo = O.measure()
+        assert np.allclose(Eg, Eo, rtol=1e-5, atol=1e-4)
+        assert np.allclose(Mg, Mo, rtol=1e-5, atol=1e-3)
+
+
+def test_measure_matches_oracle_on_identical_spins(P, oracle):
+    """E and M of the SAME configuration (set_spins from the oracle's state): fp64 sums, 1e-12 relative."""
+    for n, dims in [(3, (8, 6, 4)), (2, (12, 10, 1))]:
+        O = oracle.System(dims, n=n, seed=7)
+        O.sweep(0.6, 3)
+        G = P.SpinSystem(dims, n=n, storage="fp32", seed=1)
+        G.set_spins(O.get_spins())
+        assert np.array_equal(G.get_spins(), O.get_spins())
+        Eg, Mg = G.measure()
+        Eo, Mo = O.measure()
+        assert np.allclose(Eg, Eo, rtol=1e-12, atol=1e-9)
+        assert np.allclose(Mg, Mo, rtol=1e-12, atol=1e-9)
+
+
+def test_error_paths(P):
+    with pytest.raises(P.SpinError) as e:
+        P.SpinSystem((64, 64, 1), storage="bitpack", coupling="per_direction", J=(1.0, 0.0, 0.0))
+    assert e.value.status == 2
+    with pytest.raises(P.SpinError):
+        P.SpinSystem((32, 32, 1), storage="bitpack")
+    S = P.SpinSystem((64, 4, 1))
+    with pytest.raises(P.SpinError):
+        S.sweep(-1.0, 1)
+    with pytest.raises(P.SpinError):
+        S.sweep(float("nan"), 1)
+    with pytest.raises(P.SpinError):
+        S.set_spins(np.zeros((1, 256), dtype=np.int8))
+    S.sweep_counter = 2 ** 32 - 1
+    S.sweep(0.4, 1)
+    with pytest.raises(P.SpinError) as e:
+        S.sweep(0.4, 1)
+    assert e.value.status == 5
