@@ -1,0 +1,367 @@
+#!/usr/bin/env python
+"""bench.py -- spin flips/ns of the checkerboard Metropolis hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl graft|reference] [--workload NAME]
+
+One STEP = `--sweeps-per-step` full sweeps (colour 0 then colour 1) of the workload followed by
+one energy / magnetisation measurement -- every row of SURVEY.md section 8(a).  Default workload:
+BASELINE.json configs[1], the 2D Ising lattice L = 16384 with int8 spins (the configuration the
+">= 70 % of the HBM roofline" target is quoted on).  Prints ONE JSON line.
+
+  value         attempted spin updates per ns, whole job, state resident in HBM, CUDA-event timed
+  e2e           the same through the C ABI with HOST buffers: every step uploads the spin configuration
+                (spin_set_spins from pinned host memory), sweeps, and reads E, M back (spin_measure)
+  roofline      dominant kernel (the half-sweep): algorithmic bytes per launch / mean launch duration
+  cpu_baseline  the oracle (oracle/, plain single-threaded C++) on this box's host cores, bounded sample
+  per_model     flips/ns and roofline fraction of the other BASELINE.json workloads (short runs)
+
+--impl reference times the oracle itself (the CPU arm of the driver's ratio).
+N > 1 (torchrun): every rank runs its own independent lattice (weak scaling, no data-path collective).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "spin flips/ns (device-timed) and achieved HBM GB/s vs B200 peak, per model"
+UNIT = "flips/ns"
+DEFAULT_WORKLOAD = "ising2d_L16384_int8"
+# per-model legs of the default run: (workload, sweeps timed)
+PER_MODEL = [("ising2d_L64_int8", 200), ("ising2d_L16384_bitpack", 40), ("ising3d_L512_bitpack", 40),
+             ("ea3d_L256_R16_bitpack", 40), ("heisenberg3d_L256_fp32", 20), ("xy3d_L256_fp32", 20)]
+DTYPE = {"int8": "u8", "bitpack": "u32 (bit-packed, 32 spins per word)", "fp32": "f32"}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.thread = [], None, None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.QUERY,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, power = [], None, set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [r for (t, r) in self.rows if t0 - 0.05 <= t <= t1 + 0.15] or [r for (_, r) in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx = float(f[1]); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm), "power_w_max": max(power) if power else None}
+
+
+def time_sweeps(S, beta, sweeps, warm=3):
+    """ms per half-sweep launch and flips/ns of `sweeps` sweeps of system S (state resident, CUDA events)."""
+    import torch
+
+    S.sweep(beta, warm)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    S.sweep(beta, sweeps)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    return ms / (2 * sweeps), S.N * S.R * sweeps / (ms * 1e6)
+
+
+def run_per_model(P, peak):
+    import torch
+
+    out = {}
+    for name, sweeps in PER_MODEL:
+        w = P.workloads.WORKLOADS[name]
+        S = P.from_workload(w, P.workloads.SEED)
+        if w["record"]:
+            # config 1: E and M after every sweep (spin_sweep_record)
+            S.sweep_record(w["beta"], 3)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            S.sweep_record(w["beta"], sweeps)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            out[name] = {"flips_per_ns": S.N * S.R * sweeps / (ms * 1e6), "us_per_sweep_recorded": 1e3 * ms / sweeps,
+                         "note": "launch-bound; E and M recorded every sweep"}
+        else:
+            ms_launch, fpn = time_sweeps(S, w["beta"], sweeps)
+            bpu = P.workloads.BYTES_PER_UPDATE[name]
+            out[name] = {"flips_per_ns": fpn, "ms_per_halfsweep": ms_launch, "algorithmic_GBps": fpn * bpu,
+                         "hbm_frac": fpn * bpu / peak, "bytes_per_update": bpu}
+            if w["storage"] == "bitpack":
+                out[name]["note"] = "state is L2-resident or nearly so; bound by integer issue, not HBM"
+        S.close()
+        del S
+        torch.cuda.empty_cache()
+    return out
+
+
+def oracle_sample(w):
+    """The bounded sample of workload w the oracle is timed on: the same recipe on a strip of the lattice."""
+    dims = list(w["dims"])
+    if dims[2] == 1:
+        dims[1] = min(dims[1], 1024)
+        what = "%d x %d strip of the %d x %d lattice" % (dims[0], dims[1], w["dims"][0], w["dims"][1])
+    else:
+        dims[2] = min(dims[2], 16)
+        what = "%d x %d x %d slab of the %d^3 lattice" % (dims[0], dims[1], dims[2], w["dims"][0])
+    return tuple(dims), what
+
+
+def make_oracle_system(w, dims, seed):
+    import oracle
+
+    kinds = {"uniform": oracle.J_UNIFORM, "per_direction": oracle.J_PER_DIRECTION, "bond_pm1": oracle.J_BOND_PM1}
+    return oracle.System(dims, n=w["n"], coupling_kind=kinds[w["coupling"]], J=w["J"], n_replicas=w["replicas"],
+                         replica_streams=w["replica_streams"], seed=seed)
+
+
+def cpu_baseline(P, name, budget_s=15.0):
+    """The oracle as it stands, single thread, on a bounded sample (about `budget_s` seconds of CPU work)."""
+    w = P.workloads.WORKLOADS[name]
+    dims, what = oracle_sample(w)
+    O = make_oracle_system(w, dims, P.workloads.SEED)
+    updates_per_sweep = dims[0] * dims[1] * dims[2] * w["replicas"]
+    t0 = time.perf_counter()
+    sweeps = 0
+    while True:
+        O.sweep(w["beta"], 1)
+        sweeps += 1
+        el = time.perf_counter() - t0
+        if el > budget_s or sweeps >= 1000:
+            break
+    O.measure()
+    el = time.perf_counter() - t0
+    return {"value": updates_per_sweep * sweeps / (el * 1e9), "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "%d sweeps + 1 E/M measurement of a %s, %.1f s" % (sweeps, what, el),
+            "ns_per_update": el * 1e9 / (updates_per_sweep * sweeps), "host_cores_present": os.cpu_count()}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same metric and config; rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1107_5463_b200 import workloads as WL
+
+    w = WL.WORKLOADS[args.workload]
+    dims, what = oracle_sample(w)
+    O = make_oracle_system(w, dims, WL.SEED)
+    updates = dims[0] * dims[1] * dims[2] * w["replicas"]
+    for _ in range(args.warmup):
+        O.sweep(w["beta"], 1)
+        O.measure()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        O.sweep(w["beta"], 1)
+        O.measure()
+    el = time.perf_counter() - t0
+    value = updates * args.steps / (el * 1e9)
+    sample = "each step: 1 sweep + 1 E/M measurement of a %s" % what
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": DTYPE[w["storage"]], "data": "synthetic",
+            "config": {"workload": args.workload, "dims": list(w["dims"]), "beta": w["beta"], "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_graft(args):
+    import numpy as np
+    import torch
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = "cuda:%d" % local_rank
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    import paper_1107_5463_b200 as P
+
+    P.lib()
+    peak, peak_src = measured_peaks()
+    w = P.workloads.WORKLOADS[args.workload]
+    S = P.from_workload(w, P.workloads.SEED + rank, device=dev)  # every rank: its own independent lattice
+    beta, SPS = w["beta"], args.sweeps_per_step
+    updates_per_step = S.N * S.R * SPS
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ---- device-resident arm -------------------------------------------------------------------
+    for _ in range(args.warmup):
+        S.sweep(beta, SPS)
+        S.measure()
+    sweep_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = S.launch_count
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    barrier()
+    t_wall0 = time.time()
+    e0.record()
+    for k in range(args.steps):
+        sweep_ev[k][0].record()
+        S.sweep(beta, SPS)
+        sweep_ev[k][1].record()
+        E, M = S.measure()
+    e1.record()
+    barrier()
+    t_wall1 = time.time()
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+    launches = S.launch_count - launches0
+    ms_total = max_over_ranks(e0.elapsed_time(e1))
+    ms_sweeps = sum(a.elapsed_time(b) for a, b in sweep_ev)
+    value = world * updates_per_step * args.steps / (ms_total * 1e6)
+    ms_launch = ms_sweeps / (args.steps * SPS * 2)
+    bpu = P.workloads.BYTES_PER_UPDATE[args.workload]
+    bytes_per_launch = bpu * S.N * S.R / 2
+    achieved = bytes_per_launch / (ms_launch * 1e6)  # GB/s
+
+    # ---- end-to-end arm: host buffers through the C ABI ------------------------------------------
+    host = torch.from_numpy(S.get_spins()).pin_memory()
+    host_np = host.numpy()
+    for _ in range(2):
+        S.set_spins(host_np)
+        S.sweep(beta, SPS)
+        S.measure()
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    f0.record()
+    for k in range(args.steps):
+        S.set_spins(host_np)
+        S.sweep(beta, SPS)
+        E, M = S.measure()
+    f1.record()
+    barrier()
+    ms_e2e = max_over_ranks(f0.elapsed_time(f1))
+    e2e = {"value": world * updates_per_step * args.steps / (ms_e2e * 1e6), "unit": UNIT,
+           "h2d_bytes_per_step": int(host_np.nbytes), "d2h_bytes_per_step": int(8 * S.R * (1 + S.n)),
+           "ms_per_step": ms_e2e / args.steps,
+           "what": "spin_set_spins(pinned host array) + spin_sweep + spin_measure(host E, M) per step"}
+    S.close()
+    del S, host, host_np
+    torch.cuda.empty_cache()
+
+    if rank != 0:
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": DTYPE[w["storage"]], "data": "synthetic",
+        "config": {"workload": args.workload, "dims": list(w["dims"]), "n": w["n"], "beta": beta,
+                   "storage": w["storage"], "replicas": w["replicas"], "sweeps_per_step": SPS,
+                   "step": "%d sweeps + 1 E/M measurement" % SPS, "seed": P.workloads.SEED,
+                   "l2": "state (%.0f MB) larger than L2 (126 MB); no flush needed" % (w["dims"][0] * w["dims"][1] * w["dims"][2] * w["replicas"] / 1e6)
+                   if w["storage"] != "bitpack" else "bit-packed state is L2-resident by design (33.5 MB); not flushed",
+                   "parallelism": "independent lattice per GPU (weak scaling, no collective)" if world > 1 else "1 GPU"},
+        "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": "half-sweep of %s" % args.workload, "achieved": achieved, "peak": peak,
+                     "unit": "GB/s", "frac": achieved / peak, "traffic": TRAFFIC.get(args.workload),
+                     "peak_source": peak_src, "bytes_per_launch": bytes_per_launch, "ms_per_launch": ms_launch,
+                     "bytes_per_update": bpu, "frac_of_nominal_8000": achieved / 8000.0},
+    }
+    if not args.no_per_model and world == 1:
+        line["per_model"] = run_per_model(P, peak)
+    if not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(P, args.workload)
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
+TRAFFIC = {}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="graft", choices=["graft", "reference"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
+    ap.add_argument("--sweeps-per-step", type=int, default=100)
+    ap.add_argument("--no-per-model", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "graft":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_graft(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -54,6 +54,16 @@ __global__ void __launch_bounds__(256) ising_fill(const __grid_constant__ SetupA
     }
 }
 
+// *bad = 1 if any byte of canon[0 .. n) is not +1 or -1
+__global__ void __launch_bounds__(256) ising_validate_canonical(const int8_t *canon, size_t n, int *bad) {
+    int local = 0;
+    for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (size_t)gridDim.x * blockDim.x) {
+        const int v = canon[k];
+        local |= (v != 1 && v != -1);
+    }
+    if (local) *bad = 1;
+}
+
 __global__ void __launch_bounds__(256) ising_to_canonical(const __grid_constant__ SetupArgs a, const void *s0, const void *s1,
                                                           int8_t *canon) {
     const Geometry &g = a.g;

@@ -486,15 +486,25 @@ spin_status spin_set_spins(spin_system *s, const void *host, size_t bytes) {
     if (!s || !host) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
     const size_t need = canonical_spin_bytes(s);
     if (bytes != need) return fail(SPIN_ERR_INVALID_ARG, "spins need exactly %zu bytes, got %zu", need, bytes);
-    if (s->n == 1) {
-        const int8_t *p = (const int8_t *)host;
-        for (size_t k = 0; k < need; ++k)
-            if (p[k] != 1 && p[k] != -1) return fail(SPIN_ERR_INVALID_ARG, "Ising spins must be +-1");
-    }
-    void *staging = nullptr;
+    char *staging = nullptr;
     CUDA_TRY(cudaDeviceSynchronize());
-    CUDA_TRY(cudaMalloc(&staging, need));
+    CUDA_TRY(cudaMalloc((void **)&staging, need + 256));
+    int *d_bad = (int *)(staging + need + (256 - need % 256) % 256);  // 4 aligned bytes after the spins
+    int bad = 0;
     cudaError_t e = cudaMemcpy(staging, host, need, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && s->n == 1) {
+        // Ising spins must be +-1: checked on the device before anything is overwritten
+        e = cudaMemset(d_bad, 0, sizeof(int));
+        if (e == cudaSuccess) {
+            ising_validate_canonical<<<grid_for(s, need / 16 + 1), 256>>>((const int8_t *)staging, need, d_bad);
+            e = cudaGetLastError();
+        }
+        if (e == cudaSuccess) e = cudaMemcpy(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost);
+    }
+    if (e == cudaSuccess && bad) {
+        cudaFree(staging);
+        return fail(SPIN_ERR_INVALID_ARG, "Ising spins must be +-1");
+    }
     if (e == cudaSuccess) {
         const SetupArgs sa = setup_args(s);
         const int G = grid_for(s, 2ull * s->R * s->g.Nh);
