@@ -111,6 +111,10 @@ spin_status spin_get_launch_count(const spin_system *s, uint64_t *launches);
  * (0 = default).  Results never depend on it (the RNG is counter-based). */
 spin_status spin_set_launch_shape(spin_system *s, int32_t block, int32_t grid_num, int32_t grid_den);
 
+/* Tuning knob of the int8 Ising kernel: rows of one unit column a thread sweeps before moving on
+ * (1, 2, 4, 8 or 16; 0 = default).  Results never depend on it. */
+spin_status spin_set_strip_rows(spin_system *s, int32_t rows);
+
 /* Frees the handle only; never the workspace. */
 spin_status spin_destroy(spin_system *s);
 

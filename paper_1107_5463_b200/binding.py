@@ -23,7 +23,7 @@ _COUPLING = {"uniform": J_UNIFORM, "per_direction": J_PER_DIRECTION, "bond_pm1":
 SYMBOLS = [
     "spin_workspace_bytes", "spin_create", "spin_sweep", "spin_measure", "spin_sweep_record", "spin_get_spins",
     "spin_set_spins", "spin_get_bonds", "spin_get_sweep_count", "spin_set_sweep_count", "spin_get_launch_count",
-    "spin_set_launch_shape", "spin_destroy", "spin_last_error", "spin_version",
+    "spin_set_launch_shape", "spin_set_strip_rows", "spin_destroy", "spin_last_error", "spin_version",
 ]
 
 
@@ -73,6 +73,7 @@ def lib():
         L.spin_set_sweep_count.argtypes = [vp, C.c_uint64]
         L.spin_get_launch_count.argtypes = [vp, C.POINTER(C.c_uint64)]
         L.spin_set_launch_shape.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32]
+        L.spin_set_strip_rows.argtypes = [vp, C.c_int32]
         L.spin_destroy.argtypes = [vp]
         for name in SYMBOLS:
             getattr(L, name).restype = C.c_int
@@ -222,6 +223,10 @@ class SpinSystem:
 
     def set_launch_shape(self, block=0, grid_num=1, grid_den=1):
         _check(lib().spin_set_launch_shape(self._h, int(block), int(grid_num), int(grid_den)))
+
+
+    def set_strip_rows(self, rows=0):
+        _check(lib().spin_set_strip_rows(self._h, int(rows)))
 
 
 def from_workload(w, seed, **over):

@@ -1,98 +1,121 @@
 // ising_int8_kernel.cuh -- n = 1, one byte per spin (0 = +1, 1 = -1), uniform coupling +-1, Lx % 64 == 0.
-// One thread per 32-site unit: two 128-bit loads per neighbour row, byte-parallel arithmetic on
-// 32-bit registers (4 sites each), acceptance masks from the bit-serial comparison expanded from
-// bits to bytes, two 128-bit stores.  PAPER.md:37-38 (Eq. (2)), PAPER.md:42 (checkerboard, table).
+// PAPER.md:37-38 (Eq. (2)), PAPER.md:42 (checkerboard, pre-tabulated Boltzmann factors).
+//
+// Layout: a unit = 32 consecutive same-colour sites of a row = 32 consecutive bytes;
+// inside a unit, site sigma (0..31, position along x) sits at byte 4 (sigma & 7) + (sigma >> 3).  With that
+// order the eight 32-bit words w0..w7 of a unit pack into the lane mask of the unit (bit sigma = spin of site
+// sigma) by m = w0 + 2 w1 + 4 w2 + ... + 128 w7 -- seven IMADs on the FMA pipe and no ALU-pipe work -- and
+// unpack by w_k = (m >> k) & 0x01010101.  Everything between load and store is the bit-sliced logic of the
+// multi-spin-coded kernel, 32 sites per instruction.
+//
+// Work decomposition: one thread owns unit column w over K consecutive rows (a "strip") and rolls the other
+// colour's rows through registers, so each neighbour row is loaded and packed (K + 2) / K times instead of 3.
 #pragma once
 #include "ising_kernels.cuh"
 
 namespace spin {
 
-__device__ __forceinline__ void load32(const uint8_t *p, uint32_t v[8]) {
+// byte offset of site sigma inside its 32-byte unit (int8 fast layout)
+__host__ __device__ __forceinline__ uint32_t int8_byte_of_lane(uint32_t sigma) { return 4u * (sigma & 7u) + (sigma >> 3); }
+
+// lane mask of the 32-byte unit at p (bytes are exactly 0 or 1)
+__device__ __forceinline__ uint32_t int8_pack_unit(const uint8_t *p) {
     const uint4 lo = __ldg((const uint4 *)p), hi = __ldg((const uint4 *)p + 1);
-    v[0] = lo.x; v[1] = lo.y; v[2] = lo.z; v[3] = lo.w;
-    v[4] = hi.x; v[5] = hi.y; v[6] = hi.z; v[7] = hi.w;
+    uint32_t m = lo.x;
+    m = lo.y * 2u + m;
+    m = lo.z * 4u + m;
+    m = lo.w * 8u + m;
+    m = hi.x * 16u + m;
+    m = hi.y * 32u + m;
+    m = hi.z * 64u + m;
+    m = hi.w * 128u + m;
+    return m;
 }
 
-// lanes 4k .. 4k+3 of mask m as bit 0 of the four bytes of the result (other bits are junk)
-__device__ __forceinline__ uint32_t expand4(uint32_t m, int k) {
-    return ((m >> (4 * k)) & 0xFu) * 0x00204081u;
+__device__ __forceinline__ void int8_store_unit(uint8_t *p, uint32_t m) {
+    const uint32_t c = 0x01010101u;
+    uint4 *dst = (uint4 *)p;
+    dst[0] = make_uint4(m & c, (m >> 1) & c, (m >> 2) & c, (m >> 3) & c);
+    dst[1] = make_uint4((m >> 4) & c, (m >> 5) & c, (m >> 6) & c, (m >> 7) & c);
 }
 
+// Lane mask of the x-neighbour that is not at the same compressed index: p = 1 -> site xh + 1, p = 0 -> xh - 1
+// (periodic along the row).  o = this unit of the other colour, rowp = start of that row, w = unit in row.
+__device__ __forceinline__ uint32_t int8_side_mask(const uint8_t *rowp, uint32_t o, uint32_t p, uint32_t w, uint32_t WX) {
+    if (p) {
+        const uint32_t wn = w + 1u == WX ? 0u : w + 1u;
+        return (o >> 1) | ((uint32_t)__ldg(rowp + 32u * wn) << 31);       // lane 0 of the next unit: byte 0
+    }
+    const uint32_t wn = w == 0u ? WX - 1u : w - 1u;
+    return (o << 1) | (uint32_t)__ldg(rowp + 32u * wn + 31u);              // lane 31 of the previous unit: byte 31
+}
+
+// flip mask of one unit from its unsatisfied-bond masks av[0 .. 2 D): flip iff dE <= 0 or U < T(dE)
 template <int D>
+__device__ __forceinline__ uint32_t ising_flip_mask(const IsingArgs &a, uint32_t unit, uint32_t rho, const uint32_t av[6]) {
+    if (D == 2) {
+        const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
+        const uint32_t ge2 = c1 | (s1 & av[3]), ge1 = av[0] | av[1] | av[2] | av[3];
+        const uint32_t m[2] = {ge1 & ~ge2, ~ge1};
+        return ge2 | lt_mask_select<2>(a, unit, rho, m);
+    }
+    const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
+    const uint32_t s2 = av[3] ^ av[4] ^ av[5], c2 = maj3(av[3], av[4], av[5]);
+    const uint32_t b0 = s1 ^ s2, c3 = s1 & s2;
+    const uint32_t b1 = c1 ^ c2 ^ c3, b2 = maj3(c1, c2, c3);
+    const uint32_t ge3 = b2 | (b1 & b0);
+    const uint32_t m[3] = {b1 & ~b0 & ~b2, b0 & ~b1 & ~b2, ~(b0 | b1 | b2)};
+    return ge3 | lt_mask_select<3>(a, unit, rho, m);
+}
+
+// One thread per (replica, z, strip of K rows, unit column w); w is the fastest index, so a warp reads
+// 1 KB of consecutive bytes per row.
+template <int D, int K>
 __global__ void __launch_bounds__(256) ising_int8_halfsweep(const __grid_constant__ IsingArgs a) {
     const Geometry &g = a.g;
-    constexpr int NT = D;
-    const uint32_t NW = g.NW, WX = g.WX;
-    const uint8_t *__restrict__ other_base = (const uint8_t *)a.s[1 - a.colour];
-    uint8_t *mine_base = (uint8_t *)a.s[a.colour];
-    const uint32_t jmask = a.jneg ? 0x01010101u : 0u;
-    for (uint32_t gi = blockIdx.x * blockDim.x + threadIdx.x; gi < NW; gi += gridDim.x * blockDim.x) {
-        const uint32_t row = fdiv(gi, g.divWX), w = gi - row * WX;
-        const uint32_t z = fdiv(row, g.divLy), y = row - z * (uint32_t)g.Ly;
-        const uint32_t p = (y + z + a.colour) & 1u;
-        // byte index of the one neighbour outside this unit's own 32 bytes of the other colour's row
-        const uint32_t xh0 = 32u * w;
-        const uint32_t xs = p ? (xh0 + 32u == g.RL ? 0u : xh0 + 32u) : (xh0 == 0u ? g.RL - 1u : xh0 - 1u);
-        const size_t b_side = (size_t)row * g.RL + xs;
-        const size_t b_c = (size_t)gi * 32u;
-        const size_t rowbytes = g.RL;
-        const size_t b_ym = y == 0 ? b_c + rowbytes * (g.Ly - 1) : b_c - rowbytes;
-        const size_t b_yp = y == (uint32_t)g.Ly - 1 ? b_c - rowbytes * (g.Ly - 1) : b_c + rowbytes;
-        size_t b_zm = b_c, b_zp = b_c;
-        if (D == 3) {
-            const size_t plane = rowbytes * g.Ly;
-            b_zm = z == 0 ? b_c + plane * (g.Lz - 1) : b_c - plane;
-            b_zp = z == (uint32_t)g.Lz - 1 ? b_c - plane * (g.Lz - 1) : b_c + plane;
-        }
-        uint32_t lt[NT];
-        for (uint32_t r = 0; r < a.R; ++r) {
-            const uint8_t *__restrict__ other = other_base + (size_t)r * g.Nh;
-            uint8_t *mine = mine_base + (size_t)r * g.Nh;
-            uint32_t s[8], o[8], nu[8];
-            load32(mine + b_c, s);
-            load32(other + b_c, o);
-            const uint32_t sb = other[b_side];
-            {
-                uint32_t u[8], v[8];
-                load32(other + b_ym, u);
-                load32(other + b_yp, v);
+    const uint32_t WX = g.WX, Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz;
+    const uint32_t nstrip = (Ly + K - 1) / K;
+    const uint32_t per_replica = WX * nstrip * Lz;
+    const uint32_t item = blockIdx.x * blockDim.x + threadIdx.x;
+    if (item >= per_replica * a.R) return;
+    const uint32_t r = item / per_replica, it = item - r * per_replica;
+    const uint32_t sz = fdiv(it, g.divWX), w = it - sz * WX;      // sz = strip + nstrip * z
+    const uint32_t z = sz / nstrip, y0 = (sz - z * nstrip) * K;
+    const uint32_t kend = min((uint32_t)K, Ly - y0);
+    const uint8_t *__restrict__ other = (const uint8_t *)a.s[1 - a.colour] + (size_t)r * g.Nh;
+    uint8_t *mine = (uint8_t *)a.s[a.colour] + (size_t)r * g.Nh;
+    const uint32_t rho = a.replica_streams ? r : 0u;
+    const uint32_t jflip = a.jneg ? 0xFFFFFFFFu : 0u;
+    const size_t rowbytes = g.RL, plane = rowbytes * Ly;
+    const size_t zoff = (size_t)z * plane;
+    const size_t zm_off = (D == 3) ? (size_t)(z == 0 ? Lz - 1 : z - 1) * plane : 0;
+    const size_t zp_off = (D == 3) ? (size_t)(z == Lz - 1 ? 0 : z + 1) * plane : 0;
+    const uint32_t ym0 = y0 == 0 ? Ly - 1 : y0 - 1;
+    uint32_t o_prev = int8_pack_unit(other + zoff + ym0 * rowbytes + 32u * w);
+    uint32_t o_cur = int8_pack_unit(other + zoff + y0 * rowbytes + 32u * w);
+    uint32_t p = (y0 + z + a.colour) & 1u;
 #pragma unroll
-                for (int k = 0; k < 8; ++k) {
-                    // the neighbour at (x >> 1) -+ 1: this row shifted by one byte
-                    const uint32_t sd = p ? __byte_perm(o[k], k < 7 ? o[k + 1] : sb, 0x4321)
-                                          : __byte_perm(k ? o[k - 1] : (sb << 24), o[k], 0x6543);
-                    const uint32_t sj = s[k] ^ jmask;
-                    nu[k] = (sj ^ o[k]) + (sj ^ sd) + (sj ^ u[k]) + (sj ^ v[k]);
-                }
-            }
+    for (int k = 0; k < K; ++k) {
+        if ((uint32_t)k < kend) {
+            const uint32_t y = y0 + k;
+            const uint32_t yp = y + 1 == Ly ? 0u : y + 1;
+            const size_t off = y * rowbytes + 32u * w;
+            const uint32_t o_next = int8_pack_unit(other + zoff + yp * rowbytes + 32u * w);
+            const uint32_t raw = int8_pack_unit(mine + zoff + off);
+            const uint32_t side = int8_side_mask(other + zoff + y * rowbytes, o_cur, p, w, WX);
+            const uint32_t s = raw ^ jflip;
+            uint32_t av[6];
+            av[0] = s ^ o_cur; av[1] = s ^ side; av[2] = s ^ o_prev; av[3] = s ^ o_next;
             if (D == 3) {
-                uint32_t u[8], v[8];
-                load32(other + b_zm, u);
-                load32(other + b_zp, v);
-#pragma unroll
-                for (int k = 0; k < 8; ++k) {
-                    const uint32_t sj = s[k] ^ jmask;
-                    nu[k] += (sj ^ u[k]) + (sj ^ v[k]);
-                }
+                av[4] = s ^ int8_pack_unit(other + zm_off + off);
+                av[5] = s ^ int8_pack_unit(other + zp_off + off);
             }
-            if (r == 0 || a.replica_streams) lt_masks_full<NT>(a, gi, a.replica_streams ? r : 0u, lt);
-            // flip = [n_u >= q/2] | [n_u >= q/2 - 1] & lt4 | ... | lt_{2q}, evaluated on the bits of n_u
-#pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                const uint32_t x = nu[k], x1 = x >> 1, x2 = x >> 2;
-                uint32_t f;
-                if (D == 2) {
-                    // n_u in 0..4: flip = (n_u >= 2) | (n_u odd & lt4) | lt8
-                    f = x1 | x2 | (x & expand4(lt[0], k)) | expand4(lt[1], k);
-                } else {
-                    // n_u in 0..6 = (x2 x1 x0): flip = x2 | x1 & (x0 | lt4) | x0 & lt8 | lt12
-                    f = x2 | (x1 & (x | expand4(lt[0], k))) | (x & expand4(lt[1], k)) | expand4(lt[2], k);
-                }
-                s[k] ^= f & 0x01010101u;
-            }
-            uint4 *dst = (uint4 *)(mine + b_c);
-            dst[0] = make_uint4(s[0], s[1], s[2], s[3]);
-            dst[1] = make_uint4(s[4], s[5], s[6], s[7]);
+            const uint32_t unit = (y + Ly * z) * WX + w;
+            const uint32_t flip = ising_flip_mask<D>(a, unit, rho, av);
+            int8_store_unit(mine + zoff + off, raw ^ flip);
+            o_prev = o_cur;
+            o_cur = o_next;
+            p ^= 1u;
         }
     }
 }

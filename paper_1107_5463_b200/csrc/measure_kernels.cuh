@@ -5,6 +5,7 @@
 //   n = 1 : exact int64 sums (warp shuffle -> shared -> one 64-bit atomic per CTA and quantity)
 //   n >= 2: fp64 per-CTA partials, summed in a fixed order by the finalize kernel (deterministic)
 #pragma once
+#include "ising_int8_kernel.cuh"
 #include "ising_kernels.cuh"
 #include "vector_kernels.cuh"
 
@@ -88,6 +89,38 @@ __global__ void __launch_bounds__(256) ising_bitpack_measure(const __grid_consta
         if (D == 3) unsat += __popc(av[4]) + __popc(av[5]);
         e += 2 * unsat - 2 * D * 32;
         m += 64 - 2 * (__popc(raw) + __popc(s0[gi]));
+    }
+    e = block_sum(e, sm);
+    m = block_sum(m, sm);
+    if (threadIdx.x == 0) {
+        atomicAdd((unsigned long long *)&acc[2 * r], (unsigned long long)e);
+        atomicAdd((unsigned long long *)&acc[2 * r + 1], (unsigned long long)m);
+    }
+}
+
+// int8 fast layout (uniform J = +-1): units packed to lane masks, then as the bit-packed kernel.  grid = (blocks, R).
+template <int D>
+__global__ void __launch_bounds__(256) ising_int8_measure(const __grid_constant__ IsingArgs a, long long *acc) {
+    __shared__ long long sm[32];
+    const Geometry &g = a.g;
+    const uint32_t r = blockIdx.y, NW = g.NW;
+    const uint8_t *__restrict__ s0 = (const uint8_t *)a.s[0] + (size_t)r * g.Nh;
+    const uint8_t *__restrict__ s1 = (const uint8_t *)a.s[1] + (size_t)r * g.Nh;
+    const uint32_t jflip = a.jneg ? 0xFFFFFFFFu : 0u;
+    long long e = 0, m = 0;
+    for (uint32_t gi = blockIdx.x * blockDim.x + threadIdx.x; gi < NW; gi += gridDim.x * blockDim.x) {
+        const WordNbrs n = word_neighbours<D>(g, 1u, gi);
+        const uint32_t row = fdiv(gi, g.divWX), w = gi - row * g.WX;
+        const uint32_t raw = int8_pack_unit(s1 + 32u * (size_t)gi);
+        const uint32_t o = int8_pack_unit(s0 + 32u * (size_t)gi);
+        const uint32_t side = int8_side_mask(s0 + (size_t)row * g.RL, o, n.p, w, g.WX);
+        const uint32_t s = raw ^ jflip;
+        int unsat = __popc(s ^ o) + __popc(s ^ side) + __popc(s ^ int8_pack_unit(s0 + 32u * (size_t)n.g_ym)) +
+                    __popc(s ^ int8_pack_unit(s0 + 32u * (size_t)n.g_yp));
+        if (D == 3)
+            unsat += __popc(s ^ int8_pack_unit(s0 + 32u * (size_t)n.g_zm)) + __popc(s ^ int8_pack_unit(s0 + 32u * (size_t)n.g_zp));
+        e += 2 * unsat - 2 * D * 32;
+        m += 64 - 2 * (__popc(raw) + __popc(o));
     }
     e = block_sum(e, sm);
     m = block_sum(m, sm);

@@ -15,8 +15,14 @@ struct SetupArgs {
     PhiloxKeys keys;
     uint32_t R;
     int32_t bitpack;  // n = 1 only
+    int32_t int8perm; // n = 1, int8 fast layout: site sigma of a unit at byte 4 (sigma & 7) + (sigma >> 3)
     int32_t nc;       // 1, 2, 3
 };
+
+// byte index of compressed site j in an int8 colour array
+__device__ __forceinline__ uint32_t int8_byte_index(const SetupArgs &a, uint32_t j) {
+    return a.int8perm ? ((j & ~31u) | (4u * (j & 7u) + ((j >> 3) & 3u))) : j;
+}
 
 // (colour c, compressed index j) -> lexicographic site index
 __device__ __forceinline__ uint32_t lex_index(const Geometry &g, uint32_t c, uint32_t j) {
@@ -49,7 +55,7 @@ __global__ void __launch_bounds__(256) ising_fill(const __grid_constant__ SetupA
             const uint32_t word = __ballot_sync(0xFFFFFFFFu, bit);
             if ((threadIdx.x & 31) == 0) ((uint32_t *)dst)[(size_t)r * g.NW + (j >> 5)] = word;
         } else {
-            ((uint8_t *)dst)[(size_t)r * g.Nh + j] = (uint8_t)bit;
+            ((uint8_t *)dst)[(size_t)r * g.Nh + int8_byte_index(a, j)] = (uint8_t)bit;
         }
     }
 }
@@ -75,7 +81,7 @@ __global__ void __launch_bounds__(256) ising_to_canonical(const __grid_constant_
         const void *src = c ? s1 : s0;
         uint32_t bit;
         if (a.bitpack) bit = (((const uint32_t *)src)[(size_t)r * g.NW + (j >> 5)] >> (j & 31u)) & 1u;
-        else bit = ((const uint8_t *)src)[(size_t)r * g.Nh + j];
+        else bit = ((const uint8_t *)src)[(size_t)r * g.Nh + int8_byte_index(a, j)];
         canon[(size_t)r * N + i] = bit ? (int8_t)-1 : (int8_t)1;
     }
 }

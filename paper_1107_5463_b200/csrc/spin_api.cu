@@ -59,6 +59,7 @@ struct spin_system {
     uint64_t launches;
     int sm_count;
     int block;           // threads per CTA
+    int strip_rows;      // int8 fast kernel: rows per thread (1, 2, 4, 8, 16)
     int grid_num, grid_den;
     uint32_t mblocks;    // CTAs (per replica) of the measurement kernels
     double table_beta;   // beta the cached table was built for (NaN = none)
@@ -146,7 +147,7 @@ static void make_layout(const spin_config *c, const Derived &dv, Layout *l, uint
     if (c->coupling_kind == SPIN_J_BOND_PM1)
         l->bytes_bonds = dv.path == PATH_ISING_BITPACK ? (size_t)(2 * R * 3 * (Nh / 32) * 4) : (size_t)(R * dv.d * dv.N);
     l->off_bonds = off; off += align_up(l->bytes_bonds);
-    *mblocks = measure_blocks(dv.path == PATH_ISING_BITPACK ? Nh / 32 : Nh);
+    *mblocks = measure_blocks(dv.path == PATH_ISING_BITPACK || dv.path == PATH_ISING_INT8 ? Nh / 32 : Nh);
     l->bytes_acc = c->n == 1 ? (size_t)(R * 2 * sizeof(long long)) : (size_t)(R * *mblocks * (1 + c->n) * sizeof(double));
     l->off_acc = off; off += align_up(l->bytes_acc);
     l->bytes_res = (size_t)(R * (1 + c->n) * sizeof(double));
@@ -158,6 +159,7 @@ static SetupArgs setup_args(const spin_system *s) {
     SetupArgs a;
     a.g = s->g; a.keys = s->keys; a.R = s->R;
     a.bitpack = s->path == PATH_ISING_BITPACK;
+    a.int8perm = s->path == PATH_ISING_INT8;
     a.nc = s->n;
     return a;
 }
@@ -228,9 +230,14 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
     if (s->path == PATH_ISING_GENERIC) {
         ising_generic_halfsweep<<<grid_for(s, (uint64_t)s->g.Nh * s->R), B, 0, st>>>(a);
     } else if (s->path == PATH_ISING_INT8) {
-        const int G = grid_for(s, s->g.NW);
-        if (s->d == 2) ising_int8_halfsweep<2><<<G, B, 0, st>>>(a);
-        else ising_int8_halfsweep<3><<<G, B, 0, st>>>(a);
+        // one thread per (replica, z, strip of K rows, unit column)
+        const int K = s->strip_rows;
+        const uint64_t items = (uint64_t)s->g.WX * ((s->g.Ly + K - 1) / K) * s->g.Lz * s->R;
+        const int G = (int)((items + B - 1) / B);
+#define I8(D_, K_) ising_int8_halfsweep<D_, K_><<<G, B, 0, st>>>(a)
+        if (s->d == 2) { if (K == 1) I8(2, 1); else if (K == 2) I8(2, 2); else if (K == 4) I8(2, 4); else if (K == 8) I8(2, 8); else I8(2, 16); }
+        else { if (K == 1) I8(3, 1); else if (K == 2) I8(3, 2); else if (K == 4) I8(3, 4); else if (K == 8) I8(3, 8); else I8(3, 16); }
+#undef I8
     } else {
         const int G = grid_for(s, s->g.NW);
 #define BP(D_, BONDS_, SH_) ising_bitpack_halfsweep<D_, BONDS_, SH_><<<G, B, 0, st>>>(a)
@@ -281,6 +288,9 @@ static spin_status enqueue_measure(spin_system *s, double *dE, double *dM, cudaS
         if (s->path == PATH_ISING_BITPACK) {
             if (s->d == 2) { if (bonds) ising_bitpack_measure<2, true><<<grid, 256, 0, st>>>(a, acc); else ising_bitpack_measure<2, false><<<grid, 256, 0, st>>>(a, acc); }
             else { if (bonds) ising_bitpack_measure<3, true><<<grid, 256, 0, st>>>(a, acc); else ising_bitpack_measure<3, false><<<grid, 256, 0, st>>>(a, acc); }
+        } else if (s->path == PATH_ISING_INT8) {
+            if (s->d == 2) ising_int8_measure<2><<<grid, 256, 0, st>>>(a, acc);
+            else ising_int8_measure<3><<<grid, 256, 0, st>>>(a, acc);
         } else {
             ising_generic_measure<<<grid, 256, 0, st>>>(a, acc);
         }
@@ -351,7 +361,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
     }
     s->ws = (char *)d_workspace;
     s->t = 0; s->launches = 0;
-    s->block = 256; s->grid_num = 1; s->grid_den = 1;
+    s->block = dv.path == PATH_ISING_INT8 ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4;
     s->table_beta = std::nan("");
     Geometry &g = s->g;
     g.Lx = cfg->dims[0]; g.Ly = cfg->dims[1]; g.Lz = cfg->dims[2]; g.d = dv.d;
@@ -561,10 +571,19 @@ spin_status spin_get_launch_count(const spin_system *s, uint64_t *launches) {
 
 spin_status spin_set_launch_shape(spin_system *s, int32_t block, int32_t grid_num, int32_t grid_den) {
     if (!s) return fail(SPIN_ERR_INVALID_ARG, "handle is NULL");
-    if (block == 0) block = 256;
+    if (block == 0) block = s->path == PATH_ISING_INT8 ? 128 : 256;
     if (block != 64 && block != 128 && block != 256) return fail(SPIN_ERR_INVALID_ARG, "block must be 64, 128 or 256");
     if (grid_num < 1 || grid_den < 1) return fail(SPIN_ERR_INVALID_ARG, "grid_num / grid_den must be >= 1");
     s->block = block; s->grid_num = grid_num; s->grid_den = grid_den;
+    return SPIN_OK;
+}
+
+spin_status spin_set_strip_rows(spin_system *s, int32_t rows) {
+    if (!s) return fail(SPIN_ERR_INVALID_ARG, "handle is NULL");
+    if (rows == 0) rows = 4;
+    if (rows != 1 && rows != 2 && rows != 4 && rows != 8 && rows != 16)
+        return fail(SPIN_ERR_INVALID_ARG, "strip rows must be 1, 2, 4, 8 or 16");
+    s->strip_rows = rows;
     return SPIN_OK;
 }
 

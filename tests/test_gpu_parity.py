@@ -198,6 +198,28 @@ def test_launch_shape_and_call_splitting_do_not_matter(P, oracle, storage, dims)
     assert np.array_equal(A.get_spins(), C2.get_spins())
 
 
+@pytest.mark.parametrize("dims,J", [((128, 10, 1), 1.0), ((192, 6, 4), 1.0), ((64, 22, 1), -1.0), ((2048, 34, 1), 1.0)])
+def test_int8_strip_rows_do_not_matter(P, oracle, dims, J):
+    """The int8 kernel's rows-per-thread knob (register-rolled neighbour rows, ragged last strip, warps that
+    straddle rows and warps inside one row) never changes a spin: every K against the oracle."""
+    beta = BETA_2D if dims[2] == 1 else BETA_3D
+    O = oracle.System(dims, J=(J, J, J), seed=SEED)
+    O.sweep(beta, 3)
+    want = O.get_spins()
+    Eo, Mo = O.measure()
+    for rows in (1, 2, 4, 8, 16):
+        for block in (64, 256):
+            G = P.SpinSystem(dims, storage="int8", J=(J, J, J), seed=SEED)
+            G.set_strip_rows(rows)
+            G.set_launch_shape(block, 1, 1)
+            G.sweep(beta, 3)
+            assert np.array_equal(G.get_spins(), want), (rows, block)
+            Eg, Mg = G.measure()
+            assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    with pytest.raises(P.SpinError):
+        G.set_strip_rows(3)
+
+
 @pytest.mark.parametrize("n,dims,beta", [(3, (16, 16, 16), 0.693), (2, (16, 16, 16), 0.4542), (3, (32, 32, 1), 0.693),
                                          (2, (32, 32, 1), 1.1), (3, (6, 4, 2), 0.693), (2, (4, 2, 2), 0.5)])
 def test_vector_models_within_tolerance(P, oracle, n, dims, beta):
