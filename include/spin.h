@@ -115,6 +115,11 @@ spin_status spin_set_launch_shape(spin_system *s, int32_t block, int32_t grid_nu
  * (1, 2, 4, 8 or 16; 0 = default).  Results never depend on it. */
 spin_status spin_set_strip_rows(spin_system *s, int32_t rows);
 
+/* Test knob: value 1 selects the plain kernels (one launch per half-sweep, one thread per site for n >= 2,
+ * no resident small-lattice kernel), 0 (default) the tuned ones.  Results never depend on it bit for bit. */
+enum { SPIN_OPT_PLAIN_KERNELS = 0 };
+spin_status spin_set_option(spin_system *s, int32_t option, int64_t value);
+
 /* Frees the handle only; never the workspace. */
 spin_status spin_destroy(spin_system *s);
 

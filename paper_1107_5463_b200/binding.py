@@ -14,6 +14,7 @@ from . import build as _build
 STORE_INT8, STORE_BITPACK, STORE_FP32 = 0, 1, 2
 J_UNIFORM, J_PER_DIRECTION, J_BOND_PM1 = 0, 1, 2
 INIT_HOT, INIT_COLD = 0, 1
+OPT_PLAIN_KERNELS = 0
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE_TOO_SMALL, ERR_CUDA, ERR_STATE = range(6)
 
 _STORAGE = {"int8": STORE_INT8, "bitpack": STORE_BITPACK, "fp32": STORE_FP32}
@@ -23,7 +24,7 @@ _COUPLING = {"uniform": J_UNIFORM, "per_direction": J_PER_DIRECTION, "bond_pm1":
 SYMBOLS = [
     "spin_workspace_bytes", "spin_create", "spin_sweep", "spin_measure", "spin_sweep_record", "spin_get_spins",
     "spin_set_spins", "spin_get_bonds", "spin_get_sweep_count", "spin_set_sweep_count", "spin_get_launch_count",
-    "spin_set_launch_shape", "spin_set_strip_rows", "spin_destroy", "spin_last_error", "spin_version",
+    "spin_set_launch_shape", "spin_set_strip_rows", "spin_set_option", "spin_destroy", "spin_last_error", "spin_version",
 ]
 
 
@@ -74,6 +75,7 @@ def lib():
         L.spin_get_launch_count.argtypes = [vp, C.POINTER(C.c_uint64)]
         L.spin_set_launch_shape.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32]
         L.spin_set_strip_rows.argtypes = [vp, C.c_int32]
+        L.spin_set_option.argtypes = [vp, C.c_int32, C.c_int64]
         L.spin_destroy.argtypes = [vp]
         for name in SYMBOLS:
             getattr(L, name).restype = C.c_int
@@ -224,9 +226,11 @@ class SpinSystem:
     def set_launch_shape(self, block=0, grid_num=1, grid_den=1):
         _check(lib().spin_set_launch_shape(self._h, int(block), int(grid_num), int(grid_den)))
 
-
     def set_strip_rows(self, rows=0):
         _check(lib().spin_set_strip_rows(self._h, int(rows)))
+
+    def set_option(self, option, value):
+        _check(lib().spin_set_option(self._h, int(option), int(value)))
 
 
 def from_workload(w, seed, **over):

@@ -73,6 +73,7 @@ struct Geometry {
     uint32_t WX;      // 32-site words per row and colour = RL / 32 (fast kernels only)
     uint32_t NW;      // words per colour = Nh / 32 (fast kernels only)
     FastDiv divRL, divWX, divLy;
+    FastDiv divQX;    // by RL / 4 (quads of 4 sites per row and colour; strip kernel of the n >= 2 models)
 };
 
 }  // namespace spin

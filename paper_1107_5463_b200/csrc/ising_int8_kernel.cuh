@@ -52,12 +52,13 @@ __device__ __forceinline__ uint32_t int8_side_mask(const uint8_t *rowp, uint32_t
 
 // flip mask of one unit from its unsatisfied-bond masks av[0 .. 2 D): flip iff dE <= 0 or U < T(dE)
 template <int D>
-__device__ __forceinline__ uint32_t ising_flip_mask(const IsingArgs &a, uint32_t unit, uint32_t rho, const uint32_t av[6]) {
+__device__ __forceinline__ uint32_t ising_flip_mask(const IsingArgs &a, uint32_t t, uint32_t colour, uint32_t unit, uint32_t rho,
+                                                    const uint32_t av[6]) {
     if (D == 2) {
         const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
         const uint32_t ge2 = c1 | (s1 & av[3]), ge1 = av[0] | av[1] | av[2] | av[3];
         const uint32_t m[2] = {ge1 & ~ge2, ~ge1};
-        return ge2 | lt_mask_select<2>(a, unit, rho, m);
+        return ge2 | lt_mask_select<2>(a, t, colour, unit, rho, m);
     }
     const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
     const uint32_t s2 = av[3] ^ av[4] ^ av[5], c2 = maj3(av[3], av[4], av[5]);
@@ -65,7 +66,7 @@ __device__ __forceinline__ uint32_t ising_flip_mask(const IsingArgs &a, uint32_t
     const uint32_t b1 = c1 ^ c2 ^ c3, b2 = maj3(c1, c2, c3);
     const uint32_t ge3 = b2 | (b1 & b0);
     const uint32_t m[3] = {b1 & ~b0 & ~b2, b0 & ~b1 & ~b2, ~(b0 | b1 | b2)};
-    return ge3 | lt_mask_select<3>(a, unit, rho, m);
+    return ge3 | lt_mask_select<3>(a, t, colour, unit, rho, m);
 }
 
 // One thread per (replica, z, strip of K rows, unit column w); w is the fastest index, so a warp reads
@@ -111,7 +112,7 @@ __global__ void __launch_bounds__(256) ising_int8_halfsweep(const __grid_constan
                 av[5] = s ^ int8_pack_unit(other + zp_off + off);
             }
             const uint32_t unit = (y + Ly * z) * WX + w;
-            const uint32_t flip = ising_flip_mask<D>(a, unit, rho, av);
+            const uint32_t flip = ising_flip_mask<D>(a, a.t, a.colour, unit, rho, av);
             int8_store_unit(mine + zoff + off, raw ^ flip);
             o_prev = o_cur;
             o_cur = o_next;

@@ -26,7 +26,8 @@ struct IsingArgs {
 // significant first, four per Philox call, until every lane is decided for every threshold
 // (about log2(32) + 1.3 digits on average; a warp runs until its slowest thread is done).
 template <int NT>
-__device__ __forceinline__ void lt_masks_full(const IsingArgs &a, uint32_t unit, uint32_t rho, uint32_t lt[NT]) {
+__device__ __forceinline__ void lt_masks_full(const IsingArgs &a, uint32_t t, uint32_t colour, uint32_t unit, uint32_t rho,
+                                              uint32_t lt[NT]) {
     uint32_t eq[NT];
 #pragma unroll
     for (int th = 0; th < NT; ++th) { lt[th] = a.tab.always[th]; eq[th] = ~a.tab.always[th]; }
@@ -37,7 +38,7 @@ __device__ __forceinline__ void lt_masks_full(const IsingArgs &a, uint32_t unit,
         for (int th = 1; th < NT; ++th) any |= eq[th];
         if (any == 0u) break;
         uint32_t w[4];
-        philox4x32_10(unit, rho, a.t, make_tag(a.colour, DOM_ISING_UPDATE, call), a.keys, w);
+        philox4x32_10(unit, rho, t, make_tag(colour, DOM_ISING_UPDATE, call), a.keys, w);
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
 #pragma unroll
@@ -54,7 +55,8 @@ __device__ __forceinline__ void lt_masks_full(const IsingArgs &a, uint32_t unit,
 // (lane in m[th] compares against T(4 (th + 1)); lanes in none are not compared).  Returns the
 // mask of lanes with U < their threshold.
 template <int NT>
-__device__ __forceinline__ uint32_t lt_mask_select(const IsingArgs &a, uint32_t unit, uint32_t rho, const uint32_t m[NT]) {
+__device__ __forceinline__ uint32_t lt_mask_select(const IsingArgs &a, uint32_t t, uint32_t colour, uint32_t unit, uint32_t rho,
+                                                   const uint32_t m[NT]) {
     uint32_t lt = 0u, eq = 0u;
 #pragma unroll
     for (int th = 0; th < NT; ++th) { lt |= m[th] & a.tab.always[th]; eq |= m[th] & ~a.tab.always[th]; }
@@ -62,7 +64,7 @@ __device__ __forceinline__ uint32_t lt_mask_select(const IsingArgs &a, uint32_t 
     for (int call = 0; call < 8; ++call) {
         if (eq == 0u) break;
         uint32_t w[4];
-        philox4x32_10(unit, rho, a.t, make_tag(a.colour, DOM_ISING_UPDATE, call), a.keys, w);
+        philox4x32_10(unit, rho, t, make_tag(colour, DOM_ISING_UPDATE, call), a.keys, w);
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             const int dg = 4 * call + k;
@@ -207,7 +209,7 @@ __global__ void __launch_bounds__(256) ising_bitpack_halfsweep(const __grid_cons
     for (uint32_t gi = blockIdx.x * blockDim.x + threadIdx.x; gi < NW; gi += gridDim.x * blockDim.x) {
         const WordNbrs n = word_neighbours<D>(a.g, a.colour, gi);
         uint32_t ltf[NT];
-        if (SHARED) lt_masks_full<NT>(a, gi, 0u, ltf);
+        if (SHARED) lt_masks_full<NT>(a, a.t, a.colour, gi, 0u, ltf);
         for (uint32_t r = 0; r < a.R; ++r) {
             uint32_t av[6];
             const uint32_t raw = unsatisfied_bonds<D, BONDS>(a, a.colour, r, gi, n, av);
@@ -218,7 +220,7 @@ __global__ void __launch_bounds__(256) ising_bitpack_halfsweep(const __grid_cons
                 if (SHARED) flip = ge2 | (ge1 & ltf[0]) | ltf[1];
                 else {
                     const uint32_t m[2] = {ge1 & ~ge2, ~ge1};
-                    flip = ge2 | lt_mask_select<2>(a, gi, a.replica_streams ? r : 0u, m);
+                    flip = ge2 | lt_mask_select<2>(a, a.t, a.colour, gi, a.replica_streams ? r : 0u, m);
                 }
             } else {
                 const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
@@ -229,7 +231,7 @@ __global__ void __launch_bounds__(256) ising_bitpack_halfsweep(const __grid_cons
                 if (SHARED) flip = ge3 | ((b1 | b2) & ltf[0]) | ((b0 | b1 | b2) & ltf[1]) | ltf[2];
                 else {
                     const uint32_t m[3] = {b1 & ~b0 & ~b2, b0 & ~b1 & ~b2, ~(b0 | b1 | b2)};
-                    flip = ge3 | lt_mask_select<3>(a, gi, a.replica_streams ? r : 0u, m);
+                    flip = ge3 | lt_mask_select<3>(a, a.t, a.colour, gi, a.replica_streams ? r : 0u, m);
                 }
             }
             mine_base[(size_t)r * NW + gi] = raw ^ flip;

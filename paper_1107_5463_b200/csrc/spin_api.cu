@@ -59,7 +59,8 @@ struct spin_system {
     uint64_t launches;
     int sm_count;
     int block;           // threads per CTA
-    int strip_rows;      // int8 fast kernel: rows per thread (1, 2, 4, 8, 16)
+    int strip_rows;      // strip kernels: rows per thread (1, 2, 4, 8, 16)
+    int vector_generic;  // n >= 2: force the one-thread-per-site kernel (test knob)
     int grid_num, grid_den;
     uint32_t mblocks;    // CTAs (per replica) of the measurement kernels
     double table_beta;   // beta the cached table was built for (NaN = none)
@@ -255,6 +256,35 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
     return SPIN_OK;
 }
 
+// n >= 2: the strip kernel (128-bit accesses, K rows per thread) when a row holds whole quads of 4 sites,
+// the one-thread-per-site kernel otherwise.
+static spin_status launch_halfsweep_vector(spin_system *s, const VectorArgs &a, cudaStream_t st) {
+    const Geometry &g = s->g;
+    if (g.RL % 4 == 0 && !s->vector_generic) {
+        bool unitj = true;
+        for (int mu = 0; mu < s->d; ++mu) unitj = unitj && a.Jdir[mu] == 1.0f;
+        const int K = s->strip_rows >= 4 ? 4 : s->strip_rows;
+        const int B = s->block > 128 ? 128 : s->block;
+        const uint64_t items = (uint64_t)(g.RL / 4) * ((g.Ly + K - 1) / K) * g.Lz * s->R;
+        const int G = (int)((items + B - 1) / B);
+#define VS4(NC_, D_, U_, K_) vector_strip_halfsweep<NC_, D_, U_, K_><<<G, B, 0, st>>>(a)
+#define VS3(NC_, D_, U_) do { if (K == 1) VS4(NC_, D_, U_, 1); else if (K == 2) VS4(NC_, D_, U_, 2); else VS4(NC_, D_, U_, 4); } while (0)
+#define VS2(NC_, D_) do { if (unitj) VS3(NC_, D_, true); else VS3(NC_, D_, false); } while (0)
+        if (s->n == 2) { if (s->d == 2) VS2(2, 2); else VS2(2, 3); }
+        else { if (s->d == 2) VS2(3, 2); else VS2(3, 3); }
+#undef VS2
+#undef VS3
+#undef VS4
+    } else {
+        const int G = grid_for(s, (uint64_t)g.Nh * s->R);
+        if (s->n == 2) vector_halfsweep<2><<<G, s->block, 0, st>>>(a);
+        else vector_halfsweep<3><<<G, s->block, 0, st>>>(a);
+    }
+    s->launches += 1;
+    CUDA_TRY(cudaGetLastError());
+    return SPIN_OK;
+}
+
 static spin_status enqueue_sweep(spin_system *s, double beta, cudaStream_t st) {
     if (s->n == 1) {
         IsingArgs a = ising_args(s);
@@ -265,13 +295,10 @@ static spin_status enqueue_sweep(spin_system *s, double beta, cudaStream_t st) {
         }
     } else {
         VectorArgs a = vector_args(s, beta);
-        const int G = grid_for(s, (uint64_t)s->g.Nh * s->R);
         for (uint32_t colour = 0; colour < 2; ++colour) {
             a.colour = colour;
-            if (s->n == 2) vector_halfsweep<2><<<G, s->block, 0, st>>>(a);
-            else vector_halfsweep<3><<<G, s->block, 0, st>>>(a);
-            s->launches += 1;
-            CUDA_TRY(cudaGetLastError());
+            spin_status rc = launch_halfsweep_vector(s, a, st);
+            if (rc != SPIN_OK) return rc;
         }
     }
     s->t += 1;
@@ -361,13 +388,14 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
     }
     s->ws = (char *)d_workspace;
     s->t = 0; s->launches = 0;
-    s->block = dv.path == PATH_ISING_INT8 ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4;
+    s->block = dv.path == PATH_ISING_INT8 ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->vector_generic = 0;
     s->table_beta = std::nan("");
     Geometry &g = s->g;
     g.Lx = cfg->dims[0]; g.Ly = cfg->dims[1]; g.Lz = cfg->dims[2]; g.d = dv.d;
     g.RL = (uint32_t)(g.Lx / 2); g.rows = (uint32_t)(g.Ly * g.Lz); g.Nh = (uint32_t)(dv.N / 2);
     g.WX = g.RL / 32; g.NW = g.Nh / 32;
     g.divRL = make_fastdiv(g.RL); g.divWX = make_fastdiv(g.WX ? g.WX : 1); g.divLy = make_fastdiv((uint32_t)g.Ly);
+    g.divQX = make_fastdiv(g.RL / 4 ? g.RL / 4 : 1);
     for (int r = 0; r < 10; ++r) {
         s->keys.k0[r] = (uint32_t)(cfg->seed & 0xFFFFFFFFull) + (uint32_t)r * 0x9E3779B9u;
         s->keys.k1[r] = (uint32_t)(cfg->seed >> 32) + (uint32_t)r * 0xBB67AE85u;
@@ -585,6 +613,16 @@ spin_status spin_set_strip_rows(spin_system *s, int32_t rows) {
         return fail(SPIN_ERR_INVALID_ARG, "strip rows must be 1, 2, 4, 8 or 16");
     s->strip_rows = rows;
     return SPIN_OK;
+}
+
+spin_status spin_set_option(spin_system *s, int32_t option, int64_t value) {
+    if (!s) return fail(SPIN_ERR_INVALID_ARG, "handle is NULL");
+    if (option == SPIN_OPT_PLAIN_KERNELS) {
+        if (value != 0 && value != 1) return fail(SPIN_ERR_INVALID_ARG, "SPIN_OPT_PLAIN_KERNELS takes 0 or 1");
+        s->vector_generic = (int)value;
+        return SPIN_OK;
+    }
+    return fail(SPIN_ERR_INVALID_ARG, "unknown option %d", (int)option);
 }
 
 }  // extern "C"

@@ -100,4 +100,127 @@ __global__ void __launch_bounds__(256) vector_halfsweep(const __grid_constant__ 
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Strip kernel (Lx % 8 == 0): one thread owns a quad of 4 consecutive same-colour sites (one 128-bit word per
+// component plane) and walks K consecutive rows y, rolling the other colour's rows y-1, y, y+1 through
+// registers: every access is a coalesced 128-bit load or store, each other-colour row is loaded (K + 2) / K
+// times, and the index arithmetic is paid once per strip.  Same arithmetic, in the same order, as
+// vector_halfsweep: the result is bit-identical to it for any K and launch shape.
+//   UNITJ: every coupling in use is exactly +1, so J * s is s (exact) and the products are skipped.
+template <int NC>
+struct Quad {
+    float4 c[NC];
+};
+
+template <int NC>
+__device__ __forceinline__ Quad<NC> load_quad(const float *__restrict__ base, uint32_t Nh, uint32_t off) {
+    Quad<NC> q;
+#pragma unroll
+    for (int c = 0; c < NC; ++c) q.c[c] = __ldg((const float4 *)(base + (size_t)c * Nh + off));
+    return q;
+}
+
+__device__ __forceinline__ float lane_of(const float4 &v, int i) { return i == 0 ? v.x : (i == 1 ? v.y : (i == 2 ? v.z : v.w)); }
+
+template <bool UNITJ>
+__device__ __forceinline__ float add_nb(float h, float J, float s) {
+    return UNITJ ? __fadd_rn(h, s) : __fadd_rn(h, __fmul_rn(J, s));
+}
+
+template <int NC, int D, bool UNITJ, int K>
+__global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_constant__ VectorArgs a) {
+    const Geometry &g = a.g;
+    const uint32_t RL = g.RL, QX = RL >> 2, Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz, Nh = g.Nh;
+    const uint32_t nstrip = (Ly + K - 1) / K;
+    const uint32_t per_replica = QX * nstrip * Lz;
+    const uint32_t item = blockIdx.x * blockDim.x + threadIdx.x;
+    if (item >= per_replica * a.R) return;
+    const uint32_t r = item / per_replica, it = item - r * per_replica;
+    const uint32_t sz = fdiv(it, g.divQX), q = it - sz * QX;       // sz = strip + nstrip * z
+    const uint32_t z = sz / nstrip, y0 = (sz - z * nstrip) * K;
+    const uint32_t kend = min((uint32_t)K, Ly - y0);
+    const float *__restrict__ other = a.s[1 - a.colour] + (size_t)r * NC * Nh;
+    float *mine = a.s[a.colour] + (size_t)r * NC * Nh;
+    const uint32_t rho = a.replica_streams ? r : 0u;
+    const uint32_t tag = make_tag(a.colour, DOM_VECTOR_UPDATE, 0);
+    const uint32_t plane = RL * Ly, zoff = z * plane;
+    const uint32_t zm_off = (D == 3) ? (z == 0 ? Lz - 1 : z - 1) * plane : 0u;
+    const uint32_t zp_off = (D == 3) ? (z == Lz - 1 ? 0u : z + 1) * plane : 0u;
+    const uint32_t x4 = 4u * q;
+    // position, inside a row, of the one x-neighbour outside this quad: p = 1 -> first site of the next quad,
+    // p = 0 -> last site of the previous quad (periodic)
+    const uint32_t side_p1 = q + 1 == QX ? 0u : x4 + 4u, side_p0 = q == 0 ? RL - 1u : x4 - 1u;
+    const float Jx = a.Jdir[0], Jy = a.Jdir[1], Jz = a.Jdir[2];
+    const uint32_t ym0 = y0 == 0 ? Ly - 1 : y0 - 1;
+    Quad<NC> o_prev = load_quad<NC>(other, Nh, zoff + ym0 * RL + x4);
+    Quad<NC> o_cur = load_quad<NC>(other, Nh, zoff + y0 * RL + x4);
+    uint32_t p = (y0 + z + a.colour) & 1u;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        if ((uint32_t)k < kend) {
+            const uint32_t y = y0 + k;
+            const uint32_t yp = y + 1 == Ly ? 0u : y + 1;
+            const uint32_t row = zoff + y * RL, off = row + x4;
+            const Quad<NC> o_next = load_quad<NC>(other, Nh, zoff + yp * RL + x4);
+            Quad<NC> own;
+#pragma unroll
+            for (int c = 0; c < NC; ++c) own.c[c] = *(const float4 *)(mine + (size_t)c * Nh + off);
+            Quad<NC> o_zm, o_zp;
+            if (D == 3) {
+                o_zm = load_quad<NC>(other, Nh, zm_off + y * RL + x4);
+                o_zp = load_quad<NC>(other, Nh, zp_off + y * RL + x4);
+            }
+            float side[NC];
+#pragma unroll
+            for (int c = 0; c < NC; ++c) side[c] = __ldg(other + (size_t)c * Nh + row + (p ? side_p1 : side_p0));
+            // local field, order -x, +x, -y, +y, -z, +z, every product and sum rounded separately
+            float h[4][NC];
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+                const float4 o = o_cur.c[c];
+                float xm[4], xp[4];
+                if (p) { xm[0] = o.x; xm[1] = o.y; xm[2] = o.z; xm[3] = o.w; xp[0] = o.y; xp[1] = o.z; xp[2] = o.w; xp[3] = side[c]; }
+                else { xm[0] = side[c]; xm[1] = o.x; xm[2] = o.y; xm[3] = o.z; xp[0] = o.x; xp[1] = o.y; xp[2] = o.z; xp[3] = o.w; }
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    float v = UNITJ ? xm[i] : __fadd_rn(0.0f, __fmul_rn(Jx, xm[i]));
+                    v = add_nb<UNITJ>(v, Jx, xp[i]);
+                    v = add_nb<UNITJ>(v, Jy, lane_of(o_prev.c[c], i));
+                    v = add_nb<UNITJ>(v, Jy, lane_of(o_next.c[c], i));
+                    if (D == 3) {
+                        v = add_nb<UNITJ>(v, Jz, lane_of(o_zm.c[c], i));
+                        v = add_nb<UNITJ>(v, Jz, lane_of(o_zp.c[c], i));
+                    }
+                    h[i][c] = v;
+                }
+            }
+            float res[NC][4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                uint32_t w[4];
+                philox4x32_10(off + i, rho, a.t, tag, a.keys, w);
+                float sn[NC], so[NC];
+                uint32_t wacc;
+                if (NC == 3) { direction3(w[0], w[1], sn); wacc = w[2]; }
+                else { direction2(w[0], sn); wacc = w[1]; }
+#pragma unroll
+                for (int c = 0; c < NC; ++c) so[c] = lane_of(own.c[c], i);
+                float acc = __fmul_rn(__fsub_rn(sn[0], so[0]), h[i][0]);
+#pragma unroll
+                for (int c = 1; c < NC; ++c) acc = __fadd_rn(acc, __fmul_rn(__fsub_rn(sn[c], so[c]), h[i][c]));
+                const float dE = -acc;
+                const bool accept = dE <= 0.0f || u24(wacc) < expf(__fmul_rn(-a.beta, dE));
+#pragma unroll
+                for (int c = 0; c < NC; ++c) res[c][i] = accept ? sn[c] : so[c];
+            }
+#pragma unroll
+            for (int c = 0; c < NC; ++c)
+                *(float4 *)(mine + (size_t)c * Nh + off) = make_float4(res[c][0], res[c][1], res[c][2], res[c][3]);
+            o_prev = o_cur;
+            o_cur = o_next;
+            p ^= 1u;
+        }
+    }
+}
+
 }  // namespace spin
