@@ -1,0 +1,114 @@
+// ising_resident_kernel.cuh -- n = 1, uniform coupling +-1, small lattices: ONE CTA keeps the whole system
+// bit-packed in shared memory and runs all n_sweeps sweeps of a spin_sweep / spin_sweep_record call in a single
+// launch (the paper keeps a tile in shared memory for k updates; here the "tile" is the entire
+// lattice, so the dynamics is the plain k = 1 checkerboard sweep, bit for bit the same as the one-launch-per-
+// half-sweep kernels).  BASELINE.json config 1 (64 x 64, E and M after every sweep) is launch-bound otherwise:
+// two half-sweep launches plus two measurement launches per sweep.
+//
+// Work decomposition: thread i owns 32-site word i of BOTH colours (words = R * NW <= 1024); its two words live
+// in registers, a copy in shared memory serves the neighbours.  One __syncthreads per half-sweep.  E and M
+// are taken from the masks the colour-1 half-sweep has already formed: every bond joins the two
+// colours, so E = 2 (#unsatisfied bonds of colour-1 sites) - #bonds and M = N - 2 popcount.
+#pragma once
+#include "ising_int8_kernel.cuh"
+#include "ising_kernels.cuh"
+
+namespace spin {
+
+constexpr int RESIDENT_MAX_WORDS = 1024;
+
+// unsatisfied-bond masks of word gi (replica base rb) of colour `colour` against shared copy `oth` of the other colour
+template <int D>
+__device__ __forceinline__ void resident_bonds(const uint32_t *oth, uint32_t rb, uint32_t gi, const WordNbrs &n, uint32_t s,
+                                               uint32_t av[6]) {
+    const uint32_t o = oth[rb + gi], os = oth[rb + n.g_side];
+    const uint32_t side = n.p ? ((o >> 1) | (os << 31)) : ((o << 1) | (os >> 31));
+    av[0] = s ^ o; av[1] = s ^ side; av[2] = s ^ oth[rb + n.g_ym]; av[3] = s ^ oth[rb + n.g_yp];
+    av[4] = 0u; av[5] = 0u;
+    if (D == 3) { av[4] = s ^ oth[rb + n.g_zm]; av[5] = s ^ oth[rb + n.g_zp]; }
+}
+
+// INT8: the global arrays are the int8 fast layout (ising_int8_kernel.cuh), else bit-packed words.
+// d_E / d_M: NULL, or device arrays [n_sweeps][R] that receive E and M after every sweep.
+template <int D, bool INT8>
+__global__ void __launch_bounds__(RESIDENT_MAX_WORDS) ising_resident_sweeps(const __grid_constant__ IsingArgs a, uint32_t n_sweeps,
+                                                                             double *d_E, double *d_M) {
+    __shared__ uint32_t sp[2][RESIDENT_MAX_WORDS];
+    __shared__ int acc[2][2][32];   // [sweep parity][unsatisfied, minus spins][replica slot]; R <= 32 when recording
+    const uint32_t NW = a.g.NW, words = NW * a.R;
+    const uint32_t i = threadIdx.x;
+    const bool live = i < words;
+    const uint32_t r = live ? i / NW : 0u, gi = live ? i - r * NW : 0u, rb = r * NW;
+    const uint32_t rho = a.replica_streams ? r : 0u;
+    const uint32_t jflip = a.jneg ? 0xFFFFFFFFu : 0u;
+    WordNbrs nb[2];
+    nb[0] = word_neighbours<D>(a.g, 0u, gi);
+    nb[1] = word_neighbours<D>(a.g, 1u, gi);
+    uint32_t w[2] = {0u, 0u};
+    if (live) {
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            if (INT8) w[c] = int8_pack_unit((const uint8_t *)a.s[c] + (size_t)r * a.g.Nh + 32u * gi);
+            else w[c] = ((const uint32_t *)a.s[c])[i];
+            sp[c][i] = w[c];
+        }
+    }
+    if (i < 32) { acc[0][0][i] = 0; acc[0][1][i] = 0; acc[1][0][i] = 0; acc[1][1][i] = 0; }
+    __syncthreads();
+    const bool record = d_E != nullptr;
+    const bool warp_one_replica = (NW % 32u) == 0u;   // then all live lanes of a warp share r
+    for (uint32_t k = 0; k < n_sweeps; ++k) {
+        const uint32_t t = a.t + k;
+        int unsat = 0;
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            if (live) {
+                uint32_t av[6];
+                resident_bonds<D>(sp[1 - c], rb, gi, nb[c], w[c] ^ jflip, av);
+                const uint32_t flip = ising_flip_mask<D>(a, t, (uint32_t)c, gi, rho, av);
+                w[c] ^= flip;
+                sp[c][i] = w[c];
+                if (c == 1 && record) {
+                    // after the flip the bond masks of the flipped lanes are inverted
+                    unsat = __popc(av[0] ^ flip) + __popc(av[1] ^ flip) + __popc(av[2] ^ flip) + __popc(av[3] ^ flip);
+                    if (D == 3) unsat += __popc(av[4] ^ flip) + __popc(av[5] ^ flip);
+                }
+            }
+            if (c == 1 && record) {
+                int minus = __popc(w[0]) + __popc(w[1]);
+                const uint32_t par = k & 1u;
+                if (warp_one_replica) {
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) {
+                        unsat += __shfl_down_sync(0xFFFFFFFFu, unsat, o);
+                        minus += __shfl_down_sync(0xFFFFFFFFu, minus, o);
+                    }
+                    if ((i & 31u) == 0u && live) { atomicAdd(&acc[par][0][r], unsat); atomicAdd(&acc[par][1][r], minus); }
+                } else if (live) {
+                    atomicAdd(&acc[par][0][r], unsat);
+                    atomicAdd(&acc[par][1][r], minus);
+                }
+            }
+            __syncthreads();
+        }
+        if (record && i < a.R) {
+            // sums of sweep k are complete (barrier above); slot `par` is not touched again before the barrier
+            // that ends colour 0 of sweep k + 2, which this thread must reach first
+            const uint32_t par = k & 1u;
+            const long long nbonds = (long long)D * 64ll * NW;   // d N bonds, N = 64 NW sites
+            d_E[(size_t)k * a.R + i] = (double)(2ll * acc[par][0][i] - nbonds);
+            d_M[(size_t)k * a.R + i] = (double)(64ll * NW - 2ll * acc[par][1][i]);
+            acc[par][0][i] = 0;
+            acc[par][1][i] = 0;
+        }
+    }
+    if (live) {
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            if (INT8) int8_store_unit((uint8_t *)a.s[c] + (size_t)r * a.g.Nh + 32u * gi, w[c]);
+            else ((uint32_t *)a.s[c])[i] = w[c];
+        }
+    }
+}
+
+}  // namespace spin

@@ -11,6 +11,7 @@
 
 #include "ising_int8_kernel.cuh"
 #include "ising_kernels.cuh"
+#include "ising_resident_kernel.cuh"
 #include "measure_kernels.cuh"
 #include "setup_kernels.cuh"
 #include "vector_kernels.cuh"
@@ -336,6 +337,33 @@ static spin_status enqueue_measure(spin_system *s, double *dE, double *dM, cudaS
     return SPIN_OK;
 }
 
+// Small uniform-coupling Ising systems (at most RESIDENT_MAX_WORDS 32-site words per colour over all replicas):
+// all n_sweeps sweeps, and the per-sweep E and M if asked for, in ONE launch of the shared-memory-resident kernel.
+static bool resident_ok(const spin_system *s, bool record) {
+    if (s->vector_generic || s->n != 1) return false;
+    if (!(s->path == PATH_ISING_INT8 || s->path == PATH_ISING_BITPACK)) return false;
+    if (s->cfg.coupling_kind != SPIN_J_UNIFORM) return false;
+    if ((uint64_t)s->g.NW * s->R > (uint64_t)RESIDENT_MAX_WORDS) return false;
+    return !record || s->R <= 32;
+}
+
+static spin_status enqueue_resident(spin_system *s, int64_t n_sweeps, double *d_E, double *d_M, cudaStream_t st) {
+    const int words = (int)(s->g.NW * s->R), B = (words + 31) / 32 * 32;
+    while (n_sweeps > 0) {
+        const uint32_t chunk = (uint32_t)(n_sweeps > (1 << 20) ? (1 << 20) : n_sweeps);
+        const IsingArgs a = ising_args(s);
+        const bool i8 = s->path == PATH_ISING_INT8;
+        if (s->d == 2) { if (i8) ising_resident_sweeps<2, true><<<1, B, 0, st>>>(a, chunk, d_E, d_M); else ising_resident_sweeps<2, false><<<1, B, 0, st>>>(a, chunk, d_E, d_M); }
+        else { if (i8) ising_resident_sweeps<3, true><<<1, B, 0, st>>>(a, chunk, d_E, d_M); else ising_resident_sweeps<3, false><<<1, B, 0, st>>>(a, chunk, d_E, d_M); }
+        CUDA_TRY(cudaGetLastError());
+        s->launches += 1;
+        s->t += chunk;
+        n_sweeps -= chunk;
+        if (d_E) { d_E += (size_t)chunk * s->R; d_M += (size_t)chunk * s->R; }
+    }
+    return SPIN_OK;
+}
+
 static spin_status check_sweep_args(spin_system *s, double beta, int64_t n_sweeps) {
     if (!s) return fail(SPIN_ERR_INVALID_ARG, "handle is NULL");
     if (!(beta >= 0.0) || !std::isfinite(beta)) return fail(SPIN_ERR_INVALID_ARG, "beta must be finite and >= 0");
@@ -457,6 +485,7 @@ spin_status spin_destroy(spin_system *s) {
 spin_status spin_sweep(spin_system *s, double beta, int64_t n_sweeps, void *stream) {
     spin_status rc = check_sweep_args(s, beta, n_sweeps);
     if (rc != SPIN_OK) return rc;
+    if (resident_ok(s, false)) return enqueue_resident(s, n_sweeps, nullptr, nullptr, (cudaStream_t)stream);
     for (int64_t k = 0; k < n_sweeps; ++k) {
         rc = enqueue_sweep(s, beta, (cudaStream_t)stream);
         if (rc != SPIN_OK) return rc;
@@ -468,6 +497,7 @@ spin_status spin_sweep_record(spin_system *s, double beta, int64_t n_sweeps, dou
     spin_status rc = check_sweep_args(s, beta, n_sweeps);
     if (rc != SPIN_OK) return rc;
     if (!d_E || !d_M) return fail(SPIN_ERR_INVALID_ARG, "d_E / d_M is NULL");
+    if (resident_ok(s, true)) return enqueue_resident(s, n_sweeps, d_E, d_M, (cudaStream_t)stream);
     for (int64_t k = 0; k < n_sweeps; ++k) {
         rc = enqueue_sweep(s, beta, (cudaStream_t)stream);
         if (rc != SPIN_OK) return rc;

@@ -21,13 +21,15 @@ struct VectorArgs {
 };
 
 __device__ __forceinline__ float u24(uint32_t w) { return (float)(w >> 8) * 5.9604644775390625e-08f; }
+// 2 u24(w): the product by 2 is exact, so one multiplication by 2^-23 gives the same float
+__device__ __forceinline__ float two_u24(uint32_t w) { return (float)(w >> 8) * 1.1920928955078125e-07f; }
 
 __device__ __forceinline__ void direction3(uint32_t w0, uint32_t w1, float out[3]) {
-    const float z = __fsub_rn(__fmul_rn(2.0f, u24(w0)), 1.0f);
+    const float z = __fsub_rn(two_u24(w0), 1.0f);  // exact: (k - 2^23) 2^-23 with k < 2^24
     const float om = fmaxf(__fsub_rn(1.0f, __fmul_rn(z, z)), 0.0f);
     const float rho = __fsqrt_rn(om);
     float sn, cs;
-    sincospif(__fmul_rn(2.0f, u24(w1)), &sn, &cs);
+    sincospif(two_u24(w1), &sn, &cs);
     out[0] = __fmul_rn(rho, cs);
     out[1] = __fmul_rn(rho, sn);
     out[2] = z;
@@ -35,7 +37,7 @@ __device__ __forceinline__ void direction3(uint32_t w0, uint32_t w1, float out[3
 
 __device__ __forceinline__ void direction2(uint32_t w0, float out[2]) {
     float sn, cs;
-    sincospif(__fmul_rn(2.0f, u24(w0)), &sn, &cs);
+    sincospif(two_u24(w0), &sn, &cs);
     out[0] = cs;
     out[1] = sn;
 }
@@ -177,14 +179,14 @@ __global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_const
             float h[4][NC];
 #pragma unroll
             for (int c = 0; c < NC; ++c) {
+                // the two x-neighbours are o (same compressed index) and sh (index + 1 if p, index - 1 if not); the
+                // first sum J x(-x) + J x(+x) is commutative, so which of the two is "-x" does not matter
                 const float4 o = o_cur.c[c];
-                float xm[4], xp[4];
-                if (p) { xm[0] = o.x; xm[1] = o.y; xm[2] = o.z; xm[3] = o.w; xp[0] = o.y; xp[1] = o.z; xp[2] = o.w; xp[3] = side[c]; }
-                else { xm[0] = side[c]; xm[1] = o.x; xm[2] = o.y; xm[3] = o.z; xp[0] = o.x; xp[1] = o.y; xp[2] = o.z; xp[3] = o.w; }
+                const float4 sh = p ? make_float4(o.y, o.z, o.w, side[c]) : make_float4(side[c], o.x, o.y, o.z);
 #pragma unroll
                 for (int i = 0; i < 4; ++i) {
-                    float v = UNITJ ? xm[i] : __fadd_rn(0.0f, __fmul_rn(Jx, xm[i]));
-                    v = add_nb<UNITJ>(v, Jx, xp[i]);
+                    float v = UNITJ ? __fadd_rn(lane_of(o, i), lane_of(sh, i))
+                                    : __fadd_rn(__fmul_rn(Jx, lane_of(o, i)), __fmul_rn(Jx, lane_of(sh, i)));
                     v = add_nb<UNITJ>(v, Jy, lane_of(o_prev.c[c], i));
                     v = add_nb<UNITJ>(v, Jy, lane_of(o_next.c[c], i));
                     if (D == 3) {

@@ -26,13 +26,33 @@ def P():
     return pkg
 
 
+_PLAIN = False
+
+
+@pytest.fixture(autouse=True, params=["tuned", "plain"])
+def kernels(request):
+    """Every test runs twice: with the tuned kernels (strip kernels, the shared-memory-resident small-lattice kernel)
+    and with the plain ones (SPIN_OPT_PLAIN_KERNELS: one launch per half-sweep, one thread per site for n >= 2)."""
+    global _PLAIN
+    _PLAIN = request.param == "plain"
+    yield request.param
+    _PLAIN = False
+
+
+def _system(P, *args, **kw):
+    G = P.SpinSystem(*args, **kw)
+    if _PLAIN:
+        G.set_option(P.OPT_PLAIN_KERNELS, 1)
+    return G
+
+
 def _oracle_kind(oracle, coupling):
     return {"uniform": oracle.J_UNIFORM, "per_direction": oracle.J_PER_DIRECTION, "bond_pm1": oracle.J_BOND_PM1}[coupling]
 
 
 def _pair(P, oracle, dims, n=1, storage="int8", coupling="uniform", J=(1.0, 1.0, 1.0), replicas=1, replica_streams=0,
           seed=SEED, init=0):
-    G = P.SpinSystem(dims, n=n, storage=storage, coupling=coupling, J=J, replicas=replicas,
+    G = _system(P, dims, n=n, storage=storage, coupling=coupling, J=J, replicas=replicas,
                      replica_streams=replica_streams, seed=seed, init=init)
     O = oracle.System(dims, n=n, coupling_kind=_oracle_kind(oracle, coupling), J=J, n_replicas=replicas,
                       replica_streams=replica_streams, seed=seed, init=init)
@@ -105,6 +125,31 @@ def test_config1_L64_1000_sweeps_recorded(P, oracle, storage):
     assert G.sweep_counter == 1000
 
 
+@pytest.mark.parametrize("dims,storage,R,streams", [((64, 6, 1), "int8", 5, 1), ((64, 64, 1), "bitpack", 3, 1),
+                                                     ((64, 4, 4), "int8", 2, 1), ((128, 8, 2), "bitpack", 32, 1),
+                                                     ((256, 256, 1), "int8", 1, 0), ((256, 258, 1), "int8", 1, 0)])
+def test_recorded_sweeps_replicas_small_lattices(P, oracle, dims, storage, R, streams):
+    """spin_sweep_record on lattices around the limit of the shared-memory-resident kernel (1024 words per colour):
+    E, M of every replica after every sweep, then the spins, against the oracle; split calls continue the chain."""
+    import torch
+
+    beta = BETA_2D if dims[2] == 1 else BETA_3D
+    G, O = _pair(P, oracle, dims, storage=storage, replicas=R, replica_streams=streams)
+    n1, n2 = 7, 6
+    dE1, dM1 = G.sweep_record(beta, n1)
+    dE2, dM2 = G.sweep_record(beta, n2)
+    torch.cuda.synchronize()
+    Eg = np.concatenate([dE1.cpu().numpy(), dE2.cpu().numpy()])
+    Mg = np.concatenate([dM1.cpu().numpy(), dM2.cpu().numpy()])[:, :, 0]
+    for t in range(n1 + n2):
+        O.sweep(beta, 1)
+        e, m = O.measure()
+        assert np.array_equal(Eg[t], e), (t, Eg[t], e)
+        assert np.array_equal(Mg[t], m[:, 0]), (t, Mg[t], m[:, 0])
+    _assert_ising_equal(G, O, "after recorded sweeps %s" % (dims,))
+    assert G.sweep_counter == n1 + n2
+
+
 @pytest.mark.parametrize("dims,storage", [((64, 16, 1), "int8"), ((64, 16, 1), "bitpack"), ((64, 8, 4), "bitpack"),
                                           ((12, 8, 1), "int8")])
 def test_antiferromagnet(P, oracle, dims, storage):
@@ -160,7 +205,7 @@ def test_pm_j_user_bonds_and_replica_streams_uniform(P, oracle):
     N = dims[0] * dims[1] * dims[2]
     bonds = (1 - 2 * rng.integers(0, 2, size=(R, 3, N))).astype(np.int8)
     for storage in ("bitpack", "int8"):
-        G = P.SpinSystem(dims, storage=storage, coupling="bond_pm1", bonds=bonds, replicas=R, seed=3)
+        G = _system(P, dims, storage=storage, coupling="bond_pm1", bonds=bonds, replicas=R, seed=3)
         O = oracle.System(dims, coupling_kind=oracle.J_BOND_PM1, bonds=bonds, n_replicas=R, seed=3)
         assert np.array_equal(G.get_bonds(), bonds)
         for t in range(4):
@@ -179,8 +224,8 @@ def test_pm_j_user_bonds_and_replica_streams_uniform(P, oracle):
 @pytest.mark.parametrize("storage,dims", [("int8", (128, 10, 1)), ("bitpack", (128, 10, 6)), ("int8", (10, 6, 4))])
 def test_launch_shape_and_call_splitting_do_not_matter(P, oracle, storage, dims):
     beta = 0.3
-    A = P.SpinSystem(dims, storage=storage, seed=SEED)
-    B = P.SpinSystem(dims, storage=storage, seed=SEED)
+    A = _system(P, dims, storage=storage, seed=SEED)
+    B = _system(P, dims, storage=storage, seed=SEED)
     B.set_launch_shape(64, 1, 37)
     A.sweep(beta, 10)
     for _ in range(10):
@@ -190,7 +235,7 @@ def test_launch_shape_and_call_splitting_do_not_matter(P, oracle, storage, dims)
     O.sweep(beta, 10)
     assert np.array_equal(A.get_spins(), O.get_spins())
     # checkpoint / resume: state = spins + sweep counter
-    C2 = P.SpinSystem(dims, storage=storage, seed=SEED, init=P.INIT_COLD)
+    C2 = _system(P, dims, storage=storage, seed=SEED, init=P.INIT_COLD)
     C2.set_spins(A.get_spins())
     C2.sweep_counter = A.sweep_counter
     A.sweep(beta, 3)
@@ -209,7 +254,7 @@ def test_int8_strip_rows_do_not_matter(P, oracle, dims, J):
     Eo, Mo = O.measure()
     for rows in (1, 2, 4, 8, 16):
         for block in (64, 256):
-            G = P.SpinSystem(dims, storage="int8", J=(J, J, J), seed=SEED)
+            G = _system(P, dims, storage="int8", J=(J, J, J), seed=SEED)
             G.set_strip_rows(rows)
             G.set_launch_shape(block, 1, 1)
             G.sweep(beta, 3)
@@ -260,7 +305,7 @@ def test_measure_matches_oracle_on_identical_spins(P, oracle):
     for n, dims in [(3, (8, 6, 4)), (2, (12, 10, 1))]:
         O = oracle.System(dims, n=n, seed=7)
         O.sweep(0.6, 3)
-        G = P.SpinSystem(dims, n=n, storage="fp32", seed=1)
+        G = _system(P, dims, n=n, storage="fp32", seed=1)
         G.set_spins(O.get_spins())
         assert np.array_equal(G.get_spins(), O.get_spins())
         Eg, Mg = G.measure()
