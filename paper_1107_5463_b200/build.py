@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.path.join(HERE, "libspin.so")
+LIB = os.environ.get("LIBSPIN_PATH") or os.path.join(HERE, "libspin.so")  # override: a library built elsewhere
 SOURCES = [os.path.join(CSRC, "spin_api.cu")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -69,8 +69,36 @@ __device__ __forceinline__ uint32_t ising_flip_mask(const IsingArgs &a, uint32_t
     return ge3 | lt_mask_select<3>(a, t, colour, unit, rho, m);
 }
 
+// the 32 bytes of a unit as loaded, before packing (kept in flight while the previous row is being updated)
+struct Int8RawUnit {
+    uint4 lo, hi;
+};
+__device__ __forceinline__ Int8RawUnit int8_load_unit(const uint8_t *p) {
+    Int8RawUnit u;
+    u.lo = __ldg((const uint4 *)p);
+    u.hi = __ldg((const uint4 *)p + 1);
+    return u;
+}
+__device__ __forceinline__ uint32_t int8_pack_raw(const Int8RawUnit &u) {
+    uint32_t m = u.lo.x;
+    m = u.lo.y * 2u + m;
+    m = u.lo.z * 4u + m;
+    m = u.lo.w * 8u + m;
+    m = u.hi.x * 16u + m;
+    m = u.hi.y * 32u + m;
+    m = u.hi.z * 64u + m;
+    m = u.hi.w * 128u + m;
+    return m;
+}
+// the one byte of the x-neighbour outside the unit: p = 1 -> lane 0 of the next unit, p = 0 -> lane 31 of the previous
+__device__ __forceinline__ uint32_t int8_side_byte(const uint8_t *rowp, uint32_t p, uint32_t w, uint32_t WX) {
+    if (p) return __ldg(rowp + 32u * (w + 1u == WX ? 0u : w + 1u));
+    return __ldg(rowp + 32u * (w == 0u ? WX - 1u : w - 1u) + 31u);
+}
+
 // One thread per (replica, z, strip of K rows, unit column w); w is the fastest index, so a warp reads
-// 1 KB of consecutive bytes per row.
+// 1 KB of consecutive bytes per row.  Software-pipelined: the loads of row k + 1 are issued before the
+// update of row k is computed, so their latency hides behind the Philox / bit-slice work.
 template <int D, int K>
 __global__ void __launch_bounds__(256) ising_int8_halfsweep(const __grid_constant__ IsingArgs a) {
     const Geometry &g = a.g;
@@ -92,25 +120,43 @@ __global__ void __launch_bounds__(256) ising_int8_halfsweep(const __grid_constan
     const size_t zm_off = (D == 3) ? (size_t)(z == 0 ? Lz - 1 : z - 1) * plane : 0;
     const size_t zp_off = (D == 3) ? (size_t)(z == Lz - 1 ? 0 : z + 1) * plane : 0;
     const uint32_t ym0 = y0 == 0 ? Ly - 1 : y0 - 1;
-    uint32_t o_prev = int8_pack_unit(other + zoff + ym0 * rowbytes + 32u * w);
-    uint32_t o_cur = int8_pack_unit(other + zoff + y0 * rowbytes + 32u * w);
     uint32_t p = (y0 + z + a.colour) & 1u;
+    // prologue: rows y0 - 1 and y0 of the other colour, and everything row y0 needs
+    const Int8RawUnit r_prev = int8_load_unit(other + zoff + ym0 * rowbytes + 32u * w);
+    const Int8RawUnit r_cur = int8_load_unit(other + zoff + y0 * rowbytes + 32u * w);
+    Int8RawUnit pf_next, pf_mine, pf_zm, pf_zp;
+    uint32_t pf_side;
+    {
+        const uint32_t yp = y0 + 1 == Ly ? 0u : y0 + 1;
+        const size_t off = y0 * rowbytes + 32u * w;
+        pf_next = int8_load_unit(other + zoff + yp * rowbytes + 32u * w);
+        pf_mine = int8_load_unit(mine + zoff + off);
+        pf_side = int8_side_byte(other + zoff + y0 * rowbytes, p, w, WX);
+        if (D == 3) { pf_zm = int8_load_unit(other + zm_off + off); pf_zp = int8_load_unit(other + zp_off + off); }
+    }
+    uint32_t o_prev = int8_pack_raw(r_prev), o_cur = int8_pack_raw(r_cur);
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         if ((uint32_t)k < kend) {
             const uint32_t y = y0 + k;
-            const uint32_t yp = y + 1 == Ly ? 0u : y + 1;
             const size_t off = y * rowbytes + 32u * w;
-            const uint32_t o_next = int8_pack_unit(other + zoff + yp * rowbytes + 32u * w);
-            const uint32_t raw = int8_pack_unit(mine + zoff + off);
-            const uint32_t side = int8_side_mask(other + zoff + y * rowbytes, o_cur, p, w, WX);
+            const uint32_t o_next = int8_pack_raw(pf_next), raw = int8_pack_raw(pf_mine);
+            const uint32_t side = p ? ((o_cur >> 1) | (pf_side << 31)) : ((o_cur << 1) | pf_side);
+            uint32_t o_zm = 0u, o_zp = 0u;
+            if (D == 3) { o_zm = int8_pack_raw(pf_zm); o_zp = int8_pack_raw(pf_zp); }
+            if (k + 1 < K && (uint32_t)(k + 1) < kend) {
+                // row y + 1 <= Ly - 1 exists inside this strip: issue its loads now
+                const uint32_t y1 = y + 1, y2 = y1 + 1 == Ly ? 0u : y1 + 1;
+                const size_t off1 = y1 * rowbytes + 32u * w;
+                pf_next = int8_load_unit(other + zoff + y2 * rowbytes + 32u * w);
+                pf_mine = int8_load_unit(mine + zoff + off1);
+                pf_side = int8_side_byte(other + zoff + y1 * rowbytes, p ^ 1u, w, WX);
+                if (D == 3) { pf_zm = int8_load_unit(other + zm_off + off1); pf_zp = int8_load_unit(other + zp_off + off1); }
+            }
             const uint32_t s = raw ^ jflip;
             uint32_t av[6];
             av[0] = s ^ o_cur; av[1] = s ^ side; av[2] = s ^ o_prev; av[3] = s ^ o_next;
-            if (D == 3) {
-                av[4] = s ^ int8_pack_unit(other + zm_off + off);
-                av[5] = s ^ int8_pack_unit(other + zp_off + off);
-            }
+            if (D == 3) { av[4] = s ^ o_zm; av[5] = s ^ o_zp; }
             const uint32_t unit = (y + Ly * z) * WX + w;
             const uint32_t flip = ising_flip_mask<D>(a, a.t, a.colour, unit, rho, av);
             int8_store_unit(mine + zoff + off, raw ^ flip);

@@ -288,6 +288,26 @@ def test_vector_models_within_tolerance(P, oracle, n, dims, beta):
     assert np.max(np.abs(norm - 1.0)) < 4e-7
 
 
+@pytest.mark.parametrize("n,dims,J", [(3, (16, 6, 4), (1.0, 1.0, 1.0)), (2, (24, 10, 1), (1.0, 1.0, 1.0)),
+                                      (3, (8, 4, 2), (1.0, -1.0, 0.5)), (2, (8, 2, 6), (-1.0, -1.0, -1.0))])
+def test_vector_strip_rows_and_plain_kernel_agree_bitwise(P, n, dims, J):
+    """n >= 2: the strip kernel (quads of 4 sites, K = 1, 2, 4 rows per thread, several block sizes) and the plain
+    one-thread-per-site kernel perform the same fp32 operations in the same order: identical bits."""
+    beta = 0.7
+    coupling = "uniform" if J[0] == J[1] == J[2] else "per_direction"
+    ref = P.SpinSystem(dims, n=n, storage="fp32", coupling=coupling, J=J, seed=5)
+    ref.set_option(P.OPT_PLAIN_KERNELS, 1)
+    ref.sweep(beta, 4)
+    want = ref.get_spins()
+    for rows in (0, 1, 2, 4):
+        for block in (64, 128):
+            G = P.SpinSystem(dims, n=n, storage="fp32", coupling=coupling, J=J, seed=5)
+            G.set_strip_rows(rows)
+            G.set_launch_shape(block, 1, 1)
+            G.sweep(beta, 4)
+            assert np.array_equal(G.get_spins().view(np.uint32), want.view(np.uint32)), (rows, block)
+
+
 def test_vector_per_direction_and_replicas(P, oracle):
     G, O = _pair(P, oracle, (16, 8, 4), n=3, storage="fp32", coupling="per_direction", J=(1.0, 0.0, 0.5), replicas=3,
                  replica_streams=1)
