@@ -14,6 +14,7 @@ from . import build as _build
 
 J_UNIFORM, J_PER_DIRECTION, J_BOND_PM1 = 0, 1, 2
 INIT_HOT, INIT_COLD = 0, 1
+RULE_METROPOLIS, RULE_HEATBATH = 0, 1
 
 _lib = None
 
@@ -44,6 +45,12 @@ def lib():
         L.oracle_create.argtypes = [C.POINTER(C.c_int32), C.c_int32, C.c_int32, C.POINTER(C.c_double), C.c_void_p,
                                     C.c_int32, C.c_int32, C.c_int32, C.c_uint64]
         L.oracle_create.restype = C.c_void_p
+        L.oracle_set_update_rule.argtypes = [C.c_void_p, C.c_int32]
+        L.oracle_set_update_rule.restype = C.c_int
+        L.oracle_heatbath_threshold.argtypes = [C.c_double, C.c_int]
+        L.oracle_heatbath_threshold.restype = C.c_uint64
+        L.oracle_heatbath3.argtypes = [C.c_double, C.POINTER(C.c_float), C.c_uint32, C.c_uint32, C.POINTER(C.c_float)]
+        L.oracle_heatbath3.restype = None
         L.oracle_destroy.argtypes = [C.c_void_p]
         L.oracle_destroy.restype = None
         L.oracle_sweep.argtypes = [C.c_void_p, C.c_double, C.c_int64]
@@ -112,11 +119,22 @@ def vector_accept(beta, dE, w):
     return int(lib().oracle_vector_accept(float(beta), float(np.float32(dE)), int(w)))
 
 
+def heatbath_threshold(beta, h):
+    return int(lib().oracle_heatbath_threshold(float(beta), int(h)))
+
+
+def heatbath3(beta, h, w0, w1):
+    hv = (C.c_float * 3)(*[float(np.float32(v)) for v in h])
+    o = (C.c_float * 3)()
+    lib().oracle_heatbath3(float(beta), hv, int(w0), int(w1), o)
+    return np.array(list(o), dtype=np.float32)
+
+
 class System:
     """One oracle lattice system (R replicas).  Mirrors the product's handle, separately implemented."""
 
     def __init__(self, dims, n=1, coupling_kind=J_UNIFORM, J=(1.0, 1.0, 1.0), bonds=None, n_replicas=1,
-                 replica_streams=0, init=INIT_HOT, seed=0):
+                 replica_streams=0, init=INIT_HOT, seed=0, rule=RULE_METROPOLIS):
         dims = [int(v) for v in dims]
         if len(dims) == 2:
             dims = dims + [1]
@@ -140,6 +158,8 @@ class System:
                                       int(seed))
         if not self._h:
             raise ValueError("oracle_create: invalid arguments")
+        if rule != RULE_METROPOLIS and lib().oracle_set_update_rule(self._h, int(rule)):
+            raise ValueError("oracle_set_update_rule: rule not offered for this model")
 
     def close(self):
         if getattr(self, "_h", None):

@@ -139,6 +139,61 @@ int vector_accept(float beta_f, float dE, uint32_t w) {
     return u24(w) < p ? 1 : 0;
 }
 
+/* ------------------------------------------------------------ heat bath -- */
+/* PAPER.md:40 "updates according to the heat-bath prescription": the new value of
+ * the spin is drawn from its conditional Boltzmann distribution in the local field
+ * h = sum_j J_ij s_j, whatever the old value was.
+ *   n = 1: P(s = +1) = e^{beta h} / (e^{beta h} + e^{-beta h}) = 1 / (1 + e^{-2 beta h});
+ *          tabulated like the Metropolis factors: T_hb(h) = floor(P 2^32), s = +1 iff U < T_hb(h). */
+uint64_t heatbath_threshold(double beta, int h) {
+    const double p = 1.0 / (1.0 + std::exp(-2.0 * beta * (double)h));
+    const double scaled = std::ldexp(p, 32);
+    if (!(scaled < 4294967296.0)) return 4294967296ull;
+    if (!(scaled > 0.0)) return 0ull;
+    return (uint64_t)std::floor(scaled);
+}
+
+/*   n = 3: with H = beta |h| the cosine c of the angle between the new spin and h has density
+ *          proportional to e^{H c} on [-1, 1]; inverting its distribution function with a uniform u:
+ *          c = 1 + ln(1 - u (1 - e^{-2H})) / H.  The azimuth about h is uniform.  H = 0: uniform direction.
+ *   Frame: hhat = h / |h| and the branch-free orthonormal basis (e1, e2) of Duff et al. (JCGT 2017):
+ *          sg = copysign(1, hz), a = -1 / (sg + hz), b = hx hy a,
+ *          e1 = (1 + sg hx hx a, sg b, -sg hx), e2 = (b, sg + hy hy a, -hy).
+ *   s' = st (cp e1 + sp e2) + c hhat, st = sqrt(max(0, 1 - c c)), (sp, cp) = sincospi(2 u24(w1)).
+ *   fp32 throughout, every operation rounded separately in the order written; exp, log and sincospi are
+ *   evaluated in double and rounded once (as for the Metropolis proposal). */
+void heatbath3(float beta_f, const float h[3], uint32_t w0, uint32_t w1, float out[3]) {
+    const float hh = (h[0] * h[0] + h[1] * h[1]) + h[2] * h[2];
+    const float hn = std::sqrt(hh);
+    const float H = beta_f * hn;
+    if (!(H > 0.0f)) { direction3(w0, w1, out); return; }
+    const float u = u24(w0);
+    const float e2H = (float)std::exp((double)(-2.0f * H));
+    const float arg = 1.0f - u * (1.0f - e2H);          /* in (e^{-2H}, 1] */
+    const float lg = (float)std::log((double)arg);
+    float c = 1.0f + lg / H;
+    if (c < -1.0f) c = -1.0f;
+    if (c > 1.0f) c = 1.0f;
+    float omc = 1.0f - c * c;
+    if (omc < 0.0f) omc = 0.0f;
+    const float st = std::sqrt(omc);
+    double sd, cd;
+    sincospi_double((double)(2.0f * u24(w1)), &sd, &cd);
+    const float sp = (float)sd, cp = (float)cd;
+    const float inv = 1.0f / hn;
+    const float x = h[0] * inv, y = h[1] * inv, z = h[2] * inv;
+    const float sg = std::signbit(z) ? -1.0f : 1.0f;
+    const float a = -1.0f / (sg + z);
+    const float b = (x * y) * a;
+    const float e1[3] = {1.0f + (sg * (x * x)) * a, sg * b, (-sg) * x};
+    const float e2[3] = {b, sg + (y * y) * a, -y};
+    const float fa = st * cp, fb = st * sp;
+    for (int k = 0; k < 3; ++k) {
+        const float hk = (k == 0) ? x : (k == 1 ? y : z);
+        out[k] = (fa * e1[k] + fb * e2[k]) + c * hk;
+    }
+}
+
 }  // namespace
 
 /* ---------------------------------------------------------------- system -- */
@@ -147,6 +202,7 @@ struct oracle_system {
     int coupling_kind;
     double J[3];
     int R, replica_streams;
+    int rule; /* ORACLE_RULE_METROPOLIS (Eq. (2)) or ORACLE_RULE_HEATBATH */
     uint64_t seed;
     uint64_t t; /* sweeps done so far = Philox sweep counter */
     int64_t N;
@@ -194,8 +250,9 @@ int neighbours(const oracle_system &S, int r, int x, int y, int z, Neighbour nb[
 int64_t sweep_ising(oracle_system &S, double beta) {
     int64_t accepted = 0;
     /* table of the Boltzmann factors that can occur: dE = 2 s h, |h| <= 2d */
-    uint64_t T[13];
+    uint64_t T[13], Thb[13];
     for (int dE = 0; dE <= 12; ++dE) T[dE] = threshold(beta, dE);
+    for (int h = -6; h <= 6; ++h) Thb[h + 6] = heatbath_threshold(beta, h);
     const uint32_t t32 = (uint32_t)S.t;
     for (int colour = 0; colour < 2; ++colour) {
         for (int r = 0; r < S.R; ++r) {
@@ -219,6 +276,12 @@ int64_t sweep_ising(oracle_system &S, double beta) {
                         const int q = neighbours(S, r, x, y, z, nb);
                         int h = 0;
                         for (int k = 0; k < q; ++k) h += (int)nb[k].J * (int)s[nb[k].i];
+                        if (S.rule == ORACLE_RULE_HEATBATH) {
+                            const int8_t snew = ((uint64_t)U < Thb[h + 6]) ? (int8_t)1 : (int8_t)-1;
+                            if (snew != s[i]) ++accepted;
+                            s[i] = snew;
+                            continue;
+                        }
                         const int dE = 2 * (int)s[i] * h;
                         if (dE <= 0 || (uint64_t)U < T[dE]) {
                             s[i] = (int8_t)(-s[i]);
@@ -261,6 +324,13 @@ int64_t sweep_vector(oracle_system &S, double beta) {
                                 const float term = Jf * s[(size_t)nb[k].i * n + a];
                                 h[a] = h[a] + term;
                             }
+                        }
+                        if (S.rule == ORACLE_RULE_HEATBATH) {
+                            /* n = 3 only (oracle_set_update_rule refuses n = 2) */
+                            heatbath3(beta_f, h, w[0], w[1], snew);
+                            for (int a = 0; a < n; ++a) s[(size_t)i * n + a] = snew[a];
+                            ++accepted;
+                            continue;
                         }
                         float acc = 0.0f;
                         for (int a = 0; a < n; ++a) {
@@ -333,6 +403,7 @@ oracle_system *oracle_create(const int32_t dims[3], int32_t n, int32_t coupling_
     }
     S->R = n_replicas;
     S->replica_streams = replica_streams ? 1 : 0;
+    S->rule = ORACLE_RULE_METROPOLIS;
     S->seed = seed;
     S->t = 0;
     S->N = (int64_t)dims[0] * dims[1] * dims[2];
@@ -386,6 +457,18 @@ oracle_system *oracle_create(const int32_t dims[3], int32_t n, int32_t coupling_
 }
 
 void oracle_destroy(oracle_system *S) { delete S; }
+
+int oracle_set_update_rule(oracle_system *S, int32_t rule) {
+    if (!S || (rule != ORACLE_RULE_METROPOLIS && rule != ORACLE_RULE_HEATBATH)) return 1;
+    if (rule == ORACLE_RULE_HEATBATH && S->n == 2) return 1; /* no closed-form inverse for the von Mises law */
+    S->rule = rule;
+    return 0;
+}
+
+uint64_t oracle_heatbath_threshold(double beta, int h) { return heatbath_threshold(beta, h); }
+void oracle_heatbath3(double beta, const float h[3], uint32_t w0, uint32_t w1, float out[3]) {
+    heatbath3((float)beta, h, w0, w1, out);
+}
 
 int oracle_sweep_count(oracle_system *S, double beta, int64_t n_sweeps, int64_t *accepted) {
     if (!S || n_sweeps < 0 || !(beta >= 0.0)) return 1;

@@ -40,6 +40,8 @@ extern "C" {
 #define ORACLE_J_UNIFORM 0       /* J[0] on every bond                             */
 #define ORACLE_J_PER_DIRECTION 1 /* J[mu] on bonds in direction mu = x, y, z       */
 #define ORACLE_J_BOND_PM1 2      /* one +-1 per bond and replica                    */
+#define ORACLE_RULE_METROPOLIS 0  /* PAPER.md:37-38 Eq. (2)                            */
+#define ORACLE_RULE_HEATBATH 1    /* PAPER.md:40; n = 1 and n = 3                      */
 #define ORACLE_INIT_HOT 0
 #define ORACLE_INIT_COLD 1
 
@@ -76,6 +78,14 @@ oracle_system *oracle_create(const int32_t dims[3], int32_t n, int32_t coupling_
                              const int8_t *bonds, int32_t n_replicas, int32_t replica_streams, int32_t init,
                              uint64_t seed);
 void oracle_destroy(oracle_system *);
+
+/* Local update rule used by oracle_sweep: Metropolis (default) or heat bath.
+ * Heat bath: n = 1: s = +1 iff U < T_hb(h), T_hb(h) = floor(2^32 / (1 + exp(-2 beta h))), h = sum_j J s_j;
+ * n = 3: cosine about h by inversion, c = 1 + ln(1 - u (1 - e^{-2H})) / H, H = beta |h|, uniform azimuth
+ * (details in spin_oracle.cpp).  Returns nonzero for n = 2 (not offered) or a bad rule. */
+int oracle_set_update_rule(oracle_system *, int32_t rule);
+uint64_t oracle_heatbath_threshold(double beta, int h);
+void oracle_heatbath3(double beta, const float h[3], uint32_t w0, uint32_t w1, float out[3]);
 
 /* n_sweeps full sweeps (colour 0 then colour 1) at inverse temperature beta. */
 int oracle_sweep(oracle_system *, double beta, int64_t n_sweeps);

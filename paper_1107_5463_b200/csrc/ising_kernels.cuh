@@ -176,7 +176,7 @@ __device__ __forceinline__ uint32_t unsatisfied_bonds(const IsingArgs &a, uint32
                                                       const WordNbrs &n, uint32_t av[6]) {
     const uint32_t NW = a.g.NW;
     const uint32_t *__restrict__ other = (const uint32_t *)a.s[1 - colour] + (size_t)r * NW;
-    const uint32_t raw = ((const uint32_t *)a.s[colour])[(size_t)r * NW + gi];
+    const uint32_t raw = __ldg((const uint32_t *)a.s[colour] + (size_t)r * NW + gi);  // read only by its owner, before its write
     const uint32_t s = a.jneg ? ~raw : raw;
     const uint32_t o = other[gi], os = other[n.g_side];
     const uint32_t side = n.p ? ((o >> 1) | (os << 31)) : ((o << 1) | (os >> 31));
@@ -197,10 +197,41 @@ __device__ __forceinline__ uint32_t unsatisfied_bonds(const IsingArgs &a, uint32
     return raw;
 }
 
+// new value of word gi of replica r (see ising_bitpack_halfsweep)
+template <int D, bool BONDS, bool SHARED>
+__device__ __forceinline__ uint32_t bitpack_update_word(const IsingArgs &a, uint32_t r, uint32_t gi, const WordNbrs &n,
+                                                        const uint32_t ltf[D]) {
+    uint32_t av[6];
+    const uint32_t raw = unsatisfied_bonds<D, BONDS>(a, a.colour, r, gi, n, av);
+    uint32_t flip;
+    if (D == 2) {
+        const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
+        const uint32_t ge2 = c1 | (s1 & av[3]), ge1 = av[0] | av[1] | av[2] | av[3];
+        if (SHARED) flip = ge2 | (ge1 & ltf[0]) | ltf[1];
+        else {
+            const uint32_t m[2] = {ge1 & ~ge2, ~ge1};
+            flip = ge2 | lt_mask_select<2>(a, a.t, a.colour, gi, a.replica_streams ? r : 0u, m);
+        }
+    } else {
+        const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
+        const uint32_t s2 = av[3] ^ av[4] ^ av[5], c2 = maj3(av[3], av[4], av[5]);
+        const uint32_t b0 = s1 ^ s2, c3 = s1 & s2;
+        const uint32_t b1 = c1 ^ c2 ^ c3, b2 = maj3(c1, c2, c3);
+        const uint32_t ge3 = b2 | (b1 & b0);
+        if (SHARED) flip = ge3 | ((b1 | b2) & ltf[0]) | ((b0 | b1 | b2) & ltf[1]) | ltf[2];
+        else {
+            const uint32_t m[3] = {b1 & ~b0 & ~b2, b0 & ~b1 & ~b2, ~(b0 | b1 | b2)};
+            flip = ge3 | lt_mask_select<3>(a, a.t, a.colour, gi, a.replica_streams ? r : 0u, m);
+        }
+    }
+    return raw ^ flip;
+}
+
 // One thread per 32-site word of the active colour; loops over the replicas.  dE = 2q - 4 n_u with n_u
 // the number of unsatisfied bonds, counted bit-sliced with full adders.  SHARED: all replicas see
 // the same random numbers (R > 1, replica_streams = 0), so the masks are built once per word and
-// reused R times; otherwise each lane is compared against the one threshold it needs.
+// reused R times (batching four replicas' loads per thread was measured slower: 58 vs 40 us); otherwise each lane is compared against the one
+// threshold it needs.
 template <int D, bool BONDS, bool SHARED>
 __global__ void __launch_bounds__(256) ising_bitpack_halfsweep(const __grid_constant__ IsingArgs a) {
     constexpr int NT = D;  // thresholds: dE = 4, 8 (2D) and 12 (3D)
@@ -209,32 +240,13 @@ __global__ void __launch_bounds__(256) ising_bitpack_halfsweep(const __grid_cons
     for (uint32_t gi = blockIdx.x * blockDim.x + threadIdx.x; gi < NW; gi += gridDim.x * blockDim.x) {
         const WordNbrs n = word_neighbours<D>(a.g, a.colour, gi);
         uint32_t ltf[NT];
-        if (SHARED) lt_masks_full<NT>(a, a.t, a.colour, gi, 0u, ltf);
-        for (uint32_t r = 0; r < a.R; ++r) {
-            uint32_t av[6];
-            const uint32_t raw = unsatisfied_bonds<D, BONDS>(a, a.colour, r, gi, n, av);
-            uint32_t flip;
-            if (D == 2) {
-                const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
-                const uint32_t ge2 = c1 | (s1 & av[3]), ge1 = av[0] | av[1] | av[2] | av[3];
-                if (SHARED) flip = ge2 | (ge1 & ltf[0]) | ltf[1];
-                else {
-                    const uint32_t m[2] = {ge1 & ~ge2, ~ge1};
-                    flip = ge2 | lt_mask_select<2>(a, a.t, a.colour, gi, a.replica_streams ? r : 0u, m);
-                }
-            } else {
-                const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
-                const uint32_t s2 = av[3] ^ av[4] ^ av[5], c2 = maj3(av[3], av[4], av[5]);
-                const uint32_t b0 = s1 ^ s2, c3 = s1 & s2;
-                const uint32_t b1 = c1 ^ c2 ^ c3, b2 = maj3(c1, c2, c3);
-                const uint32_t ge3 = b2 | (b1 & b0);
-                if (SHARED) flip = ge3 | ((b1 | b2) & ltf[0]) | ((b0 | b1 | b2) & ltf[1]) | ltf[2];
-                else {
-                    const uint32_t m[3] = {b1 & ~b0 & ~b2, b0 & ~b1 & ~b2, ~(b0 | b1 | b2)};
-                    flip = ge3 | lt_mask_select<3>(a, a.t, a.colour, gi, a.replica_streams ? r : 0u, m);
-                }
-            }
-            mine_base[(size_t)r * NW + gi] = raw ^ flip;
+        if (SHARED) {
+            lt_masks_full<NT>(a, a.t, a.colour, gi, 0u, ltf);
+            for (uint32_t r = 0; r < a.R; ++r)
+                mine_base[(size_t)r * NW + gi] = bitpack_update_word<D, BONDS, true>(a, r, gi, n, ltf);
+        } else {
+            for (uint32_t r = 0; r < a.R; ++r)
+                mine_base[(size_t)r * NW + gi] = bitpack_update_word<D, BONDS, false>(a, r, gi, n, ltf);
         }
     }
 }
