@@ -131,14 +131,23 @@ def run_per_model(P, peak):
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1)
             out[name] = {"flips_per_ns": S.N * S.R * sweeps / (ms * 1e6), "us_per_sweep_recorded": 1e3 * ms / sweeps,
-                         "note": "launch-bound; E and M recorded every sweep"}
+                         "note": "one launch of the shared-memory-resident kernel for all sweeps; E and M recorded "
+                                 "every sweep; latency-bound (64 words per colour)"}
         else:
             ms_launch, fpn = time_sweeps(S, w["beta"], sweeps)
             bpu = P.workloads.BYTES_PER_UPDATE[name]
             out[name] = {"flips_per_ns": fpn, "ms_per_halfsweep": ms_launch, "algorithmic_GBps": fpn * bpu,
                          "hbm_frac": fpn * bpu / peak, "bytes_per_update": bpu}
-            if w["storage"] == "bitpack":
+            if w["storage"] == "bitpack" and name in WARP_INSTR:
+                gwips = WARP_INSTR[name] / (ms_launch * 1e6)
+                out[name]["roofline"] = {"bound": "alu", "achieved": gwips, "peak": ISSUE_PEAK_GWIPS,
+                                         "unit": "Gwarp-instr/s", "frac": gwips / ISSUE_PEAK_GWIPS,
+                                         "traffic": TRAFFIC.get(name),
+                                         "note": "instructions per launch from the committed ncu capture; peak = issue rate"}
                 out[name]["note"] = "state is L2-resident or nearly so; bound by integer issue, not HBM"
+            else:
+                out[name]["roofline"] = {"bound": "hbm", "achieved": fpn * bpu, "peak": peak, "unit": "GB/s",
+                                         "frac": fpn * bpu / peak, "traffic": TRAFFIC.get(name)}
         S.close()
         del S
         torch.cuda.empty_cache()
@@ -341,7 +350,19 @@ def run_graft(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
-TRAFFIC = {"ising2d_L16384_int8": 364969472}  # 268.50 MB read + 96.47 MB written, profiles/r01_int8_strip.md
+TRAFFIC = {  # profiles/r01c_all_kernels.md
+    "ising2d_L16384_int8": 362233344,      # 268.50 MB read + 93.74 MB written
+    "ising2d_L16384_bitpack": 33575680,    # state L2-resident: one read pass, no write-back inside the launch
+    "ising3d_L512_bitpack": 16801536,
+    "ea3d_L256_R16_bitpack": 144219648,
+    "heisenberg3d_L256_fp32": 265815808,
+    "xy3d_L256_fp32": 166819584,
+}
+# Executed warp-instructions per half-sweep launch (smsp__inst_executed.sum of the same captures), for the kernels whose
+# bound is integer arithmetic rather than HBM; the peak they are set against is the issue rate
+# 148 SMs x 4 sub-cores x 1 warp-instruction per clock x 1.965 GHz.
+WARP_INSTR = {"ising2d_L16384_bitpack": 41481418, "ising3d_L512_bitpack": 23959467, "ea3d_L256_R16_bitpack": 16541476}
+ISSUE_PEAK_GWIPS = 148 * 4 * 1.965
 
 
 def main():
