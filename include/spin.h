@@ -54,6 +54,12 @@ enum { SPIN_STORE_INT8 = 0,   /* n = 1: one byte per spin                       
 enum { SPIN_J_UNIFORM = 0,        /* J[0] on every bond                                               */
        SPIN_J_PER_DIRECTION = 1,  /* J[mu] on bonds in direction mu = x, y, z                         */
        SPIN_J_BOND_PM1 = 2 };     /* one +-1 per bond and replica (Edwards-Anderson); n = 1 */
+enum { SPIN_UPDATE_METROPOLIS = 0, /* Eq. (2): accept with min[1, exp(-beta dE)]          */
+       SPIN_UPDATE_HEATBATH = 1 }; /* the new spin is drawn from its conditional Boltzmann law in
+                                      the local field h = sum_j J_ij s_j, whatever the old value.  n = 1:
+                                      s = +1 iff U < floor(2^32 / (1 + exp(-2 beta h))); n = 3: cosine about h by
+                                      inversion, c = 1 + ln(1 - u (1 - e^{-2H})) / H, H = beta |h|, uniform azimuth
+                                      (DESIGN.md section 2).  n = 2 -> SPIN_ERR_UNSUPPORTED                   */
 enum { SPIN_INIT_HOT = 0,         /* iid uniform spins drawn from the seed                            */
        SPIN_INIT_COLD = 1 };      /* all +1 (n = 1), (1, 0) (n = 2), (0, 0, 1) (n = 3)                */
 
@@ -71,6 +77,7 @@ typedef struct {
                                 starts to be useful); 1: the replica index enters the Philox counter    */
     int32_t init;            /* SPIN_INIT_*                                                             */
     uint64_t seed;           /* Philox key                                                              */
+    int32_t update_rule;     /* SPIN_UPDATE_*                                                           */
 } spin_config;
 
 /* Bytes of device workspace spin_create() needs for this configuration. */

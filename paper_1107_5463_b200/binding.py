@@ -15,6 +15,8 @@ STORE_INT8, STORE_BITPACK, STORE_FP32 = 0, 1, 2
 J_UNIFORM, J_PER_DIRECTION, J_BOND_PM1 = 0, 1, 2
 INIT_HOT, INIT_COLD = 0, 1
 OPT_PLAIN_KERNELS = 0
+UPDATE_METROPOLIS, UPDATE_HEATBATH = 0, 1
+_RULE = {"metropolis": UPDATE_METROPOLIS, "heatbath": UPDATE_HEATBATH}
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE_TOO_SMALL, ERR_CUDA, ERR_STATE = range(6)
 
 _STORAGE = {"int8": STORE_INT8, "bitpack": STORE_BITPACK, "fp32": STORE_FP32}
@@ -32,7 +34,7 @@ class SpinConfig(C.Structure):
     _fields_ = [
         ("dims", C.c_int32 * 3), ("n", C.c_int32), ("storage", C.c_int32), ("coupling_kind", C.c_int32),
         ("J", C.c_double * 3), ("bonds", C.c_void_p), ("n_replicas", C.c_int32), ("replica_streams", C.c_int32),
-        ("init", C.c_int32), ("seed", C.c_uint64),
+        ("init", C.c_int32), ("seed", C.c_uint64), ("update_rule", C.c_int32),
     ]
 
 
@@ -93,7 +95,7 @@ def _check(status):
 
 
 def make_config(dims, n=1, storage="int8", coupling="uniform", J=(1.0, 1.0, 1.0), bonds=None, replicas=1,
-                replica_streams=0, init=INIT_HOT, seed=0):
+                replica_streams=0, init=INIT_HOT, seed=0, rule="metropolis"):
     dims = [int(v) for v in dims]
     if len(dims) == 2:
         dims.append(1)
@@ -116,6 +118,7 @@ def make_config(dims, n=1, storage="int8", coupling="uniform", J=(1.0, 1.0, 1.0)
     cfg.replica_streams = int(replica_streams)
     cfg.init = int(init)
     cfg.seed = int(seed)
+    cfg.update_rule = _RULE[rule] if isinstance(rule, str) else int(rule)
     return cfg, keep
 
 
@@ -130,14 +133,14 @@ class SpinSystem:
     sweep_record, get_spins, set_spins, get_bonds."""
 
     def __init__(self, dims, n=1, storage="int8", coupling="uniform", J=(1.0, 1.0, 1.0), bonds=None, replicas=1,
-                 replica_streams=0, init=INIT_HOT, seed=0, device="cuda:0"):
+                 replica_streams=0, init=INIT_HOT, seed=0, device="cuda:0", rule="metropolis"):
         import torch
 
         if not torch.cuda.is_available():
             raise RuntimeError("libspin needs a CUDA device (there is no CPU fallback)")
         self._torch = torch
         self.device = torch.device(device)
-        cfg, keep = make_config(dims, n, storage, coupling, J, bonds, replicas, replica_streams, init, seed)
+        cfg, keep = make_config(dims, n, storage, coupling, J, bonds, replicas, replica_streams, init, seed, rule)
         self.cfg = cfg
         self.dims = tuple(cfg.dims)
         self.n = int(cfg.n)

@@ -62,6 +62,16 @@ struct IsingTable {
     uint32_t Talways;     // bit dE set iff T(dE) = 2^32
 };
 
+// Heat-bath rule for n = 1: P(s = +1 | h) = 1 / (1 + exp(-2 beta h)), h = sum_j J s_j in {-q .. q},
+// tabulated as T_hb = floor(P 2^32).  The bit-sliced kernels index by the number k of neighbour terms J s_j that
+// equal -1 (h = q - 2 k, q = 2 d): digit[k][dg], always[k] as in IsingTable; T / Talways are indexed by h + 6.
+struct HeatBathTable {
+    uint32_t digit[7][32];
+    uint32_t always[7];
+    uint32_t T[13];
+    uint32_t Talways;
+};
+
 // Lattice geometry in the colour-compressed layout.  A colour-c site (x, y, z) has compressed
 // index j = (x >> 1) + RL (y + Ly z), RL = Lx / 2; all its neighbours are in the other colour's array:
 // same row at x >> 1 and at (x >> 1) -+ 1 (minus if x is even), rows y -+ 1 and planes z -+ 1 at x >> 1.

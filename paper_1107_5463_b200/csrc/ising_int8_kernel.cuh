@@ -69,6 +69,24 @@ __device__ __forceinline__ uint32_t ising_flip_mask(const IsingArgs &a, uint32_t
     return ge3 | lt_mask_select<3>(a, t, colour, unit, rho, m);
 }
 
+// New value of a unit's word (bit = 1: spin -1) from its own word `raw` and its unsatisfied-bond masks av[].
+//   HB = false (Metropolis, Eq. (2)): raw ^ flip mask.
+//   HB = true  (heat bath): av[k] ^ raw = lanes whose neighbour term J s_j is -1; with k of them the
+//   local field is h = 2 D - 2 k and the new spin is +1 iff U < T_hb(h).
+template <int D, bool HB>
+__device__ __forceinline__ uint32_t ising_new_word(const IsingArgs &a, uint32_t t, uint32_t colour, uint32_t unit, uint32_t rho,
+                                                   uint32_t raw, const uint32_t av[6]) {
+    if constexpr (!HB) {
+        return raw ^ ising_flip_mask<D>(a, t, colour, unit, rho, av);
+    } else {
+        uint32_t b[6], m[2 * D + 1];
+#pragma unroll
+        for (int k = 0; k < 6; ++k) b[k] = k < 2 * D ? av[k] ^ raw : 0u;
+        count_masks<D>(b, m);
+        return ~lt_mask_select<2 * D + 1, true>(a, t, colour, unit, rho, m);
+    }
+}
+
 // the 32 bytes of a unit as loaded, before packing (kept in flight while the previous row is being updated)
 struct Int8RawUnit {
     uint4 lo, hi;
@@ -99,7 +117,7 @@ __device__ __forceinline__ uint32_t int8_side_byte(const uint8_t *rowp, uint32_t
 // One thread per (replica, z, strip of K rows, unit column w); w is the fastest index, so a warp reads
 // 1 KB of consecutive bytes per row.  Software-pipelined: the loads of row k + 1 are issued before the
 // update of row k is computed, so their latency hides behind the Philox / bit-slice work.
-template <int D, int K>
+template <int D, int K, bool HB = false>
 __global__ void __launch_bounds__(256) ising_int8_halfsweep(const __grid_constant__ IsingArgs a) {
     const Geometry &g = a.g;
     const uint32_t WX = g.WX, Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz;
@@ -158,8 +176,8 @@ __global__ void __launch_bounds__(256) ising_int8_halfsweep(const __grid_constan
             av[0] = s ^ o_cur; av[1] = s ^ side; av[2] = s ^ o_prev; av[3] = s ^ o_next;
             if (D == 3) { av[4] = s ^ o_zm; av[5] = s ^ o_zp; }
             const uint32_t unit = (y + Ly * z) * WX + w;
-            const uint32_t flip = ising_flip_mask<D>(a, a.t, a.colour, unit, rho, av);
-            int8_store_unit(mine + zoff + off, raw ^ flip);
+            if (D == 2) { av[4] = 0u; av[5] = 0u; }
+            int8_store_unit(mine + zoff + off, ising_new_word<D, HB>(a, a.t, a.colour, unit, rho, raw, av));
             o_prev = o_cur;
             o_cur = o_next;
             p ^= 1u;

@@ -19,18 +19,31 @@ struct IsingArgs {
     int32_t coupling_kind;  // 0 uniform, 1 per direction, 2 per bond
     int32_t Jdir[3];        // generic kernel: coupling per direction in {-1, 0, +1}
     uint32_t jneg;          // fast kernels: 1 iff the uniform coupling is -1
+    uint32_t rule;          // 0 Metropolis (Eq. (2)), 1 heat bath
+    HeatBathTable hb;       // filled when rule = 1
 };
+
+// digit dg / "always" mask of threshold th of the table in use: HB = false -> Metropolis factors T(4 (th + 1)),
+// HB = true -> heat-bath probabilities of k = th neighbour terms equal to -1
+template <bool HB>
+__device__ __forceinline__ uint32_t tab_digit(const IsingArgs &a, int th, int dg) {
+    if constexpr (HB) return a.hb.digit[th][dg]; else return a.tab.digit[th < 3 ? th : 0][dg];
+}
+template <bool HB>
+__device__ __forceinline__ uint32_t tab_always(const IsingArgs &a, int th) {
+    if constexpr (HB) return a.hb.always[th]; else return a.tab.always[th < 3 ? th : 0];
+}
 
 // ------------------------------------------------------------------ bit-serial U < T ---------
 // Lane masks of U < T(4 (th + 1)) for th < NT, for all 32 lanes of `unit`.  Digits are consumed most
 // significant first, four per Philox call, until every lane is decided for every threshold
 // (about log2(32) + 1.3 digits on average; a warp runs until its slowest thread is done).
-template <int NT>
+template <int NT, bool HB = false>
 __device__ __forceinline__ void lt_masks_full(const IsingArgs &a, uint32_t t, uint32_t colour, uint32_t unit, uint32_t rho,
                                               uint32_t lt[NT]) {
     uint32_t eq[NT];
 #pragma unroll
-    for (int th = 0; th < NT; ++th) { lt[th] = a.tab.always[th]; eq[th] = ~a.tab.always[th]; }
+    for (int th = 0; th < NT; ++th) { lt[th] = tab_always<HB>(a, th); eq[th] = ~tab_always<HB>(a, th); }
 #pragma unroll
     for (int call = 0; call < 8; ++call) {
         uint32_t any = eq[0];
@@ -43,7 +56,7 @@ __device__ __forceinline__ void lt_masks_full(const IsingArgs &a, uint32_t t, ui
         for (int k = 0; k < 4; ++k) {
 #pragma unroll
             for (int th = 0; th < NT; ++th) {
-                const uint32_t tb = a.tab.digit[th][4 * call + k];
+                const uint32_t tb = tab_digit<HB>(a, th, 4 * call + k);
                 lt[th] |= eq[th] & ~w[k] & tb;
                 eq[th] &= ~(w[k] ^ tb);
             }
@@ -54,12 +67,12 @@ __device__ __forceinline__ void lt_masks_full(const IsingArgs &a, uint32_t t, ui
 // The same comparison when every lane needs only ONE threshold: m[th] are disjoint lane masks
 // (lane in m[th] compares against T(4 (th + 1)); lanes in none are not compared).  Returns the
 // mask of lanes with U < their threshold.
-template <int NT>
+template <int NT, bool HB = false>
 __device__ __forceinline__ uint32_t lt_mask_select(const IsingArgs &a, uint32_t t, uint32_t colour, uint32_t unit, uint32_t rho,
                                                    const uint32_t m[NT]) {
     uint32_t lt = 0u, eq = 0u;
 #pragma unroll
-    for (int th = 0; th < NT; ++th) { lt |= m[th] & a.tab.always[th]; eq |= m[th] & ~a.tab.always[th]; }
+    for (int th = 0; th < NT; ++th) { lt |= m[th] & tab_always<HB>(a, th); eq |= m[th] & ~tab_always<HB>(a, th); }
 #pragma unroll
     for (int call = 0; call < 8; ++call) {
         if (eq == 0u) break;
@@ -68,9 +81,9 @@ __device__ __forceinline__ uint32_t lt_mask_select(const IsingArgs &a, uint32_t 
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             const int dg = 4 * call + k;
-            uint32_t tk = a.tab.digit[NT - 1][dg];
+            uint32_t tk = tab_digit<HB>(a, NT - 1, dg);
 #pragma unroll
-            for (int th = NT - 2; th >= 0; --th) tk = (m[th] & a.tab.digit[th][dg]) | (~m[th] & tk);
+            for (int th = NT - 2; th >= 0; --th) tk = (m[th] & tab_digit<HB>(a, th, dg)) | (~m[th] & tk);
             lt |= eq & ~w[k] & tk;
             eq &= ~(w[k] ^ tk);
         }
@@ -79,6 +92,24 @@ __device__ __forceinline__ uint32_t lt_mask_select(const IsingArgs &a, uint32_t 
 }
 
 __device__ __forceinline__ uint32_t maj3(uint32_t x, uint32_t y, uint32_t z) { return (x & y) | (z & (x | y)); }
+
+// m[k] = lanes in which exactly k of the 2 D masks b[] are set (k = 0 .. 2 D), bit-sliced with full adders
+template <int D>
+__device__ __forceinline__ void count_masks(const uint32_t b[6], uint32_t m[2 * D + 1]) {
+    if (D == 2) {
+        const uint32_t s1 = b[0] ^ b[1] ^ b[2], c1 = maj3(b[0], b[1], b[2]);
+        const uint32_t b0 = s1 ^ b[3], c2 = s1 & b[3];
+        const uint32_t b1 = c1 ^ c2, b2 = c1 & c2;
+        m[0] = ~(b0 | b1 | b2); m[1] = b0 & ~b1; m[2] = b1 & ~b0; m[3] = b0 & b1; m[4] = b2;
+    } else {
+        const uint32_t s1 = b[0] ^ b[1] ^ b[2], c1 = maj3(b[0], b[1], b[2]);
+        const uint32_t s2 = b[3] ^ b[4] ^ b[5], c2 = maj3(b[3], b[4], b[5]);
+        const uint32_t b0 = s1 ^ s2, c3 = s1 & s2;
+        const uint32_t b1 = c1 ^ c2 ^ c3, b2 = maj3(c1, c2, c3);
+        m[0] = ~(b0 | b1 | b2); m[1] = b0 & ~b1 & ~b2; m[2] = b1 & ~b0 & ~b2; m[3] = b0 & b1;
+        m[4] = b2 & ~b0 & ~b1; m[5] = b2 & b0; m[6] = b2 & b1;
+    }
+}
 
 // ------------------------------------------------------------------ generic kernel -----------
 // One thread per (replica, site of the active colour).  Handles size-2 dimensions (the -mu and +mu
@@ -122,9 +153,11 @@ __global__ void __launch_bounds__(256) ising_generic_halfsweep(const __grid_cons
             h += J * (1 - 2 * nb[k]);
         }
         const int dE = 2 * s * h;
-        bool flip = dE <= 0 || ((a.tab.Talways >> dE) & 1u);
+        // Metropolis: flip iff dE <= 0 or U < T(dE).  Heat bath: s' = +1 iff U < T_hb(h); `flip` then means "U < T_hb"
+        const bool hb = a.rule != 0u;
+        bool flip = hb ? ((a.hb.Talways >> (h + 6)) & 1u) != 0u : (dE <= 0 || ((a.tab.Talways >> dE) & 1u));
         if (!flip) {
-            const uint32_t T = a.tab.T[dE];
+            const uint32_t T = hb ? a.hb.T[h + 6] : a.tab.T[dE];
             const uint32_t unit = j >> 5, lane = j & 31u;
             const uint32_t rho = a.replica_streams ? r : 0u;
             bool decided = false;
@@ -139,7 +172,8 @@ __global__ void __launch_bounds__(256) ising_generic_halfsweep(const __grid_cons
                 }
             }
         }
-        if (flip) mine_base[(size_t)r * g.Nh + j] = (uint8_t)(s > 0 ? 1 : 0);
+        if (hb) mine_base[(size_t)r * g.Nh + j] = (uint8_t)(flip ? 0 : 1);
+        else if (flip) mine_base[(size_t)r * g.Nh + j] = (uint8_t)(s > 0 ? 1 : 0);
     }
 }
 
@@ -247,6 +281,37 @@ __global__ void __launch_bounds__(256) ising_bitpack_halfsweep(const __grid_cons
         } else {
             for (uint32_t r = 0; r < a.R; ++r)
                 mine_base[(size_t)r * NW + gi] = bitpack_update_word<D, BONDS, false>(a, r, gi, n, ltf);
+        }
+    }
+}
+
+// Heat-bath version of ising_bitpack_halfsweep: av[k] ^ raw = lanes whose neighbour term J s_j is -1;
+// with k of them the local field is h = 2 D - 2 k and the new spin is +1 iff U < T_hb(h) (HeatBathTable).
+// SHARED: the 2 D + 1 masks U < T_hb are built once per word and reused by every replica.
+template <int D, bool BONDS, bool SHARED>
+__global__ void __launch_bounds__(256) ising_bitpack_halfsweep_hb(const __grid_constant__ IsingArgs a) {
+    constexpr int NT = 2 * D + 1;
+    const uint32_t NW = a.g.NW;
+    uint32_t *mine_base = (uint32_t *)a.s[a.colour];
+    for (uint32_t gi = blockIdx.x * blockDim.x + threadIdx.x; gi < NW; gi += gridDim.x * blockDim.x) {
+        const WordNbrs n = word_neighbours<D>(a.g, a.colour, gi);
+        uint32_t ltf[NT];
+        if (SHARED) lt_masks_full<NT, true>(a, a.t, a.colour, gi, 0u, ltf);
+        for (uint32_t r = 0; r < a.R; ++r) {
+            uint32_t av[6], b[6], m[NT];
+            const uint32_t raw = unsatisfied_bonds<D, BONDS>(a, a.colour, r, gi, n, av);
+#pragma unroll
+            for (int k = 0; k < 6; ++k) b[k] = k < 2 * D ? av[k] ^ raw : 0u;
+            count_masks<D>(b, m);
+            uint32_t up;   // lanes whose new spin is +1
+            if (SHARED) {
+                up = 0u;
+#pragma unroll
+                for (int k = 0; k < NT; ++k) up |= m[k] & ltf[k];
+            } else {
+                up = lt_mask_select<NT, true>(a, a.t, a.colour, gi, a.replica_streams ? r : 0u, m);
+            }
+            mine_base[(size_t)r * NW + gi] = ~up;
         }
     }
 }

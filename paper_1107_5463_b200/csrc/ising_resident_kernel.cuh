@@ -30,7 +30,7 @@ __device__ __forceinline__ void resident_bonds(const uint32_t *oth, uint32_t rb,
 
 // INT8: the global arrays are the int8 fast layout (ising_int8_kernel.cuh), else bit-packed words.
 // d_E / d_M: NULL, or device arrays [n_sweeps][R] that receive E and M after every sweep.
-template <int D, bool INT8>
+template <int D, bool INT8, bool HB = false>
 __global__ void __launch_bounds__(RESIDENT_MAX_WORDS) ising_resident_sweeps(const __grid_constant__ IsingArgs a, uint32_t n_sweeps,
                                                                              double *d_E, double *d_M) {
     __shared__ uint32_t sp[2][RESIDENT_MAX_WORDS];
@@ -65,8 +65,9 @@ __global__ void __launch_bounds__(RESIDENT_MAX_WORDS) ising_resident_sweeps(cons
             if (live) {
                 uint32_t av[6];
                 resident_bonds<D>(sp[1 - c], rb, gi, nb[c], w[c] ^ jflip, av);
-                const uint32_t flip = ising_flip_mask<D>(a, t, (uint32_t)c, gi, rho, av);
-                w[c] ^= flip;
+                const uint32_t fresh = ising_new_word<D, HB>(a, t, (uint32_t)c, gi, rho, w[c], av);
+                const uint32_t flip = fresh ^ w[c];
+                w[c] = fresh;
                 sp[c][i] = w[c];
                 if (c == 1 && record) {
                     // after the flip the bond masks of the flipped lanes are inverted

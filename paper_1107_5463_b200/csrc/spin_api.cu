@@ -67,6 +67,7 @@ struct spin_system {
     uint32_t mblocks;    // CTAs (per replica) of the measurement kernels
     double table_beta;   // beta the cached table was built for (NaN = none)
     IsingTable tab;
+    HeatBathTable hb;    // n = 1 heat bath: built with the table above
 };
 
 static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
@@ -102,6 +103,10 @@ static spin_status derive(const spin_config *c, Derived *out) {
     if (c->coupling_kind < SPIN_J_UNIFORM || c->coupling_kind > SPIN_J_BOND_PM1)
         return fail(SPIN_ERR_INVALID_ARG, "bad coupling_kind");
     if (c->init != SPIN_INIT_HOT && c->init != SPIN_INIT_COLD) return fail(SPIN_ERR_INVALID_ARG, "bad init");
+    if (c->update_rule != SPIN_UPDATE_METROPOLIS && c->update_rule != SPIN_UPDATE_HEATBATH)
+        return fail(SPIN_ERR_INVALID_ARG, "bad update_rule");
+    if (c->update_rule == SPIN_UPDATE_HEATBATH && c->n == 2)
+        return fail(SPIN_ERR_UNSUPPORTED, "heat bath is offered for n = 1 and n = 3 (no closed-form inverse for n = 2)");
     if (c->storage < SPIN_STORE_INT8 || c->storage > SPIN_STORE_FP32) return fail(SPIN_ERR_INVALID_ARG, "bad storage");
     if (c->n == 1 && c->storage == SPIN_STORE_FP32) return fail(SPIN_ERR_INVALID_ARG, "n = 1 needs INT8 or BITPACK storage");
     if (c->n > 1 && c->storage != SPIN_STORE_FP32) return fail(SPIN_ERR_INVALID_ARG, "n >= 2 needs FP32 storage");
@@ -196,6 +201,29 @@ static void build_table(double beta, IsingTable *tab) {
     }
 }
 
+// Heat-bath probabilities: T_hb(h) = floor(2^32 / (1 + exp(-2 beta h))), h = -6 .. 6, in double.
+// digit[k] / always[k] serve the bit-sliced kernels, indexed by the number k of neighbour terms equal to -1
+// (h = q - 2 k, q = 2 d neighbours).
+static void build_hb_table(double beta, int q, HeatBathTable *hb) {
+    std::memset(hb, 0, sizeof *hb);
+    uint64_t T[13];
+    for (int h = -6; h <= 6; ++h) {
+        const double scaled = std::ldexp(1.0 / (1.0 + std::exp(-2.0 * beta * (double)h)), 32);
+        uint64_t v;
+        if (!(scaled < 4294967296.0)) v = 4294967296ull;
+        else if (!(scaled > 0.0)) v = 0ull;
+        else v = (uint64_t)std::floor(scaled);
+        T[h + 6] = v;
+        if (v >= 4294967296ull) { hb->Talways |= 1u << (h + 6); hb->T[h + 6] = 0xFFFFFFFFu; }
+        else hb->T[h + 6] = (uint32_t)v;
+    }
+    for (int k = 0; k <= q && k < 7; ++k) {
+        const int h = q - 2 * k;
+        hb->always[k] = T[h + 6] >= 4294967296ull ? 0xFFFFFFFFu : 0u;
+        for (int dg = 0; dg < 32; ++dg) hb->digit[k][dg] = ((hb->T[h + 6] >> (31 - dg)) & 1u) ? 0xFFFFFFFFu : 0u;
+    }
+}
+
 static IsingArgs ising_args(const spin_system *s) {
     IsingArgs a;
     a.g = s->g; a.keys = s->keys; a.tab = s->tab;
@@ -209,6 +237,8 @@ static IsingArgs ising_args(const spin_system *s) {
         a.Jdir[mu] = s->cfg.coupling_kind == SPIN_J_UNIFORM ? (int)s->cfg.J[0]
                    : (s->cfg.coupling_kind == SPIN_J_PER_DIRECTION ? (mu < s->d ? (int)s->cfg.J[mu] : 0) : 0);
     a.jneg = (s->cfg.coupling_kind == SPIN_J_UNIFORM && s->cfg.J[0] < 0.0) ? 1u : 0u;
+    a.rule = s->cfg.update_rule == SPIN_UPDATE_HEATBATH ? 1u : 0u;
+    a.hb = s->hb;
     return a;
 }
 
@@ -222,6 +252,7 @@ static VectorArgs vector_args(const spin_system *s, double beta) {
     for (int mu = 0; mu < 3; ++mu)
         a.Jdir[mu] = s->cfg.coupling_kind == SPIN_J_UNIFORM ? (float)s->cfg.J[0] : (mu < s->d ? (float)s->cfg.J[mu] : 0.0f);
     a.beta = (float)beta;
+    a.rule = s->cfg.update_rule == SPIN_UPDATE_HEATBATH ? 1u : 0u;
     return a;
 }
 
@@ -234,16 +265,22 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
         ising_generic_halfsweep<<<grid_for(s, (uint64_t)s->g.Nh * s->R), B, 0, st>>>(a);
     } else if (s->path == PATH_ISING_INT8) {
         // one thread per (replica, z, strip of K rows, unit column)
-        const int K = s->strip_rows;
+        const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
+        const int K = hb ? 4 : s->strip_rows;   // the heat-bath kernel is instantiated for K = 4 only
         const uint64_t items = (uint64_t)s->g.WX * ((s->g.Ly + K - 1) / K) * s->g.Lz * s->R;
         const int G = (int)((items + B - 1) / B);
 #define I8(D_, K_) ising_int8_halfsweep<D_, K_><<<G, B, 0, st>>>(a)
-        if (s->d == 2) { if (K == 1) I8(2, 1); else if (K == 2) I8(2, 2); else if (K == 4) I8(2, 4); else if (K == 8) I8(2, 8); else I8(2, 16); }
+        if (hb) { if (s->d == 2) ising_int8_halfsweep<2, 4, true><<<G, B, 0, st>>>(a); else ising_int8_halfsweep<3, 4, true><<<G, B, 0, st>>>(a); }
+        else if (s->d == 2) { if (K == 1) I8(2, 1); else if (K == 2) I8(2, 2); else if (K == 4) I8(2, 4); else if (K == 8) I8(2, 8); else I8(2, 16); }
         else { if (K == 1) I8(3, 1); else if (K == 2) I8(3, 2); else if (K == 4) I8(3, 4); else if (K == 8) I8(3, 8); else I8(3, 16); }
 #undef I8
     } else {
         const int G = grid_for(s, s->g.NW);
-#define BP(D_, BONDS_, SH_) ising_bitpack_halfsweep<D_, BONDS_, SH_><<<G, B, 0, st>>>(a)
+#define BP(D_, BONDS_, SH_)                                                                      \
+    do {                                                                                         \
+        if (s->cfg.update_rule == SPIN_UPDATE_HEATBATH) ising_bitpack_halfsweep_hb<D_, BONDS_, SH_><<<G, B, 0, st>>>(a); \
+        else ising_bitpack_halfsweep<D_, BONDS_, SH_><<<G, B, 0, st>>>(a);                     \
+    } while (0)
         if (s->d == 2) {
             if (bonds) { if (shared) BP(2, true, true); else BP(2, true, false); }
             else { if (shared) BP(2, false, true); else BP(2, false, false); }
@@ -262,7 +299,17 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
 // the one-thread-per-site kernel otherwise.
 static spin_status launch_halfsweep_vector(spin_system *s, const VectorArgs &a, cudaStream_t st) {
     const Geometry &g = s->g;
-    if (g.RL % 4 == 0 && !s->vector_generic) {
+    const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
+    if (g.RL % 4 == 0 && !s->vector_generic && hb) {
+        // heat bath (n = 3): the strip kernel with one row per thread
+        bool unitj = true;
+        for (int mu = 0; mu < s->d; ++mu) unitj = unitj && a.Jdir[mu] == 1.0f;
+        const int B = s->block > 128 ? 128 : s->block;
+        const uint64_t items = (uint64_t)(g.RL / 4) * g.Ly * g.Lz * s->R;
+        const int G = (int)((items + B - 1) / B);
+        if (s->d == 2) { if (unitj) vector_strip_halfsweep<3, 2, true, 1, true><<<G, B, 0, st>>>(a); else vector_strip_halfsweep<3, 2, false, 1, true><<<G, B, 0, st>>>(a); }
+        else { if (unitj) vector_strip_halfsweep<3, 3, true, 1, true><<<G, B, 0, st>>>(a); else vector_strip_halfsweep<3, 3, false, 1, true><<<G, B, 0, st>>>(a); }
+    } else if (g.RL % 4 == 0 && !s->vector_generic) {
         bool unitj = true;
         for (int mu = 0; mu < s->d; ++mu) unitj = unitj && a.Jdir[mu] == 1.0f;
         const int K = s->strip_rows_set ? (s->strip_rows >= 4 ? 4 : s->strip_rows) : 1;  // default 1 (measured fastest)
@@ -354,8 +401,13 @@ static spin_status enqueue_resident(spin_system *s, int64_t n_sweeps, double *d_
         const uint32_t chunk = (uint32_t)(n_sweeps > (1 << 20) ? (1 << 20) : n_sweeps);
         const IsingArgs a = ising_args(s);
         const bool i8 = s->path == PATH_ISING_INT8;
-        if (s->d == 2) { if (i8) ising_resident_sweeps<2, true><<<1, B, 0, st>>>(a, chunk, d_E, d_M); else ising_resident_sweeps<2, false><<<1, B, 0, st>>>(a, chunk, d_E, d_M); }
-        else { if (i8) ising_resident_sweeps<3, true><<<1, B, 0, st>>>(a, chunk, d_E, d_M); else ising_resident_sweeps<3, false><<<1, B, 0, st>>>(a, chunk, d_E, d_M); }
+        const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
+#define RS(D_, I8_, HB_) ising_resident_sweeps<D_, I8_, HB_><<<1, B, 0, st>>>(a, chunk, d_E, d_M)
+#define RS2(D_, I8_) do { if (hb) RS(D_, I8_, true); else RS(D_, I8_, false); } while (0)
+        if (s->d == 2) { if (i8) RS2(2, true); else RS2(2, false); }
+        else { if (i8) RS2(3, true); else RS2(3, false); }
+#undef RS2
+#undef RS
         CUDA_TRY(cudaGetLastError());
         s->launches += 1;
         s->t += chunk;
@@ -370,7 +422,11 @@ static spin_status check_sweep_args(spin_system *s, double beta, int64_t n_sweep
     if (!(beta >= 0.0) || !std::isfinite(beta)) return fail(SPIN_ERR_INVALID_ARG, "beta must be finite and >= 0");
     if (n_sweeps < 0) return fail(SPIN_ERR_INVALID_ARG, "n_sweeps must be >= 0");
     if (s->t + (uint64_t)n_sweeps > 0x100000000ull) return fail(SPIN_ERR_STATE, "sweep counter would pass 2^32");
-    if (s->n == 1 && !(beta == s->table_beta)) { build_table(beta, &s->tab); s->table_beta = beta; }
+    if (s->n == 1 && !(beta == s->table_beta)) {
+        build_table(beta, &s->tab);
+        if (s->cfg.update_rule == SPIN_UPDATE_HEATBATH) build_hb_table(beta, 2 * s->d, &s->hb);
+        s->table_beta = beta;
+    }
     return SPIN_OK;
 }
 

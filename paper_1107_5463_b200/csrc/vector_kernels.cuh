@@ -18,6 +18,7 @@ struct VectorArgs {
     uint32_t R, replica_streams, t, colour;
     float Jdir[3];
     float beta;
+    uint32_t rule;        // 0 Metropolis (Eq. (2)), 1 heat bath (n = 3 only)
 };
 
 __device__ __forceinline__ float u24(uint32_t w) { return (float)(w >> 8) * 5.9604644775390625e-08f; }
@@ -40,6 +41,38 @@ __device__ __forceinline__ void direction2(uint32_t w0, float out[2]) {
     sincospif(two_u24(w0), &sn, &cs);
     out[0] = cs;
     out[1] = sn;
+}
+
+// Heat bath for n = 3: the new spin is drawn from exp(beta s.h) on the sphere.
+// With H = beta |h| the cosine about h is c = 1 + ln(1 - u (1 - e^{-2H})) / H (inversion of its distribution
+// function), the azimuth is uniform, and the frame is hhat plus the branch-free orthonormal pair of Duff et al.
+// Every fp32 operation is rounded separately, in the order the oracle states them; only expf, logf and sincospif
+// can differ from its double-evaluated, once-rounded values.
+__device__ __forceinline__ void heatbath3(float beta, const float h[3], uint32_t w0, uint32_t w1, float out[3]) {
+    const float hh = __fadd_rn(__fadd_rn(__fmul_rn(h[0], h[0]), __fmul_rn(h[1], h[1])), __fmul_rn(h[2], h[2]));
+    const float hn = __fsqrt_rn(hh);
+    const float H = __fmul_rn(beta, hn);
+    if (!(H > 0.0f)) { direction3(w0, w1, out); return; }
+    const float u = u24(w0);
+    const float e2H = expf(__fmul_rn(-2.0f, H));
+    const float arg = __fsub_rn(1.0f, __fmul_rn(u, __fsub_rn(1.0f, e2H)));
+    float c = __fadd_rn(1.0f, __fdiv_rn(logf(arg), H));
+    c = fminf(fmaxf(c, -1.0f), 1.0f);
+    const float st = __fsqrt_rn(fmaxf(__fsub_rn(1.0f, __fmul_rn(c, c)), 0.0f));
+    float sp, cp;
+    sincospif(two_u24(w1), &sp, &cp);
+    const float inv = __fdiv_rn(1.0f, hn);
+    const float x = __fmul_rn(h[0], inv), y = __fmul_rn(h[1], inv), z = __fmul_rn(h[2], inv);
+    const float sg = signbit(z) ? -1.0f : 1.0f;
+    const float a = __fdiv_rn(-1.0f, __fadd_rn(sg, z));
+    const float b = __fmul_rn(__fmul_rn(x, y), a);
+    const float e1[3] = {__fadd_rn(1.0f, __fmul_rn(__fmul_rn(sg, __fmul_rn(x, x)), a)), __fmul_rn(sg, b), __fmul_rn(-sg, x)};
+    const float e2[3] = {b, __fadd_rn(sg, __fmul_rn(__fmul_rn(y, y), a)), -y};
+    const float fa = __fmul_rn(st, cp), fb = __fmul_rn(st, sp);
+    const float hk[3] = {x, y, z};
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+        out[k] = __fadd_rn(__fadd_rn(__fmul_rn(fa, e1[k]), __fmul_rn(fb, e2[k])), __fmul_rn(c, hk[k]));
 }
 
 // neighbour indices (compressed, other colour) of site j of colour `colour`, order -x,+x,-y,+y,-z,+z
@@ -84,6 +117,13 @@ __global__ void __launch_bounds__(256) vector_halfsweep(const __grid_constant__ 
         philox4x32_10(j, a.replica_streams ? r : 0u, a.t, make_tag(a.colour, DOM_VECTOR_UPDATE, 0), a.keys, w);
         float sn[NC];
         uint32_t wacc;
+        if (NC == 3 && a.rule != 0u) {
+            float h3[3] = {h[0], h[1], h[NC - 1]}, s3[3];
+            heatbath3(a.beta, h3, w[0], w[1], s3);
+#pragma unroll
+            for (int c = 0; c < NC; ++c) mine[(size_t)c * g.Nh + j] = s3[c];
+            continue;
+        }
         if (NC == 3) { direction3(w[0], w[1], sn); wacc = w[2]; }
         else { direction2(w[0], sn); wacc = w[1]; }
         float so[NC];
@@ -129,7 +169,7 @@ __device__ __forceinline__ float add_nb(float h, float J, float s) {
     return UNITJ ? __fadd_rn(h, s) : __fadd_rn(h, __fmul_rn(J, s));
 }
 
-template <int NC, int D, bool UNITJ, int K>
+template <int NC, int D, bool UNITJ, int K, bool HB = false>
 __global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_constant__ VectorArgs a) {
     const Geometry &g = a.g;
     const uint32_t RL = g.RL, QX = RL >> 2, Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz, Nh = g.Nh;
@@ -203,6 +243,13 @@ __global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_const
                 philox4x32_10(off + i, rho, a.t, tag, a.keys, w);
                 float sn[NC], so[NC];
                 uint32_t wacc;
+                if (HB && NC == 3) {
+                    float h3[3] = {h[i][0], h[i][1], h[i][NC - 1]}, s3[3];
+                    heatbath3(a.beta, h3, w[0], w[1], s3);
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) res[c][i] = s3[c];
+                    continue;
+                }
                 if (NC == 3) { direction3(w[0], w[1], sn); wacc = w[2]; }
                 else { direction2(w[0], sn); wacc = w[1]; }
 #pragma unroll

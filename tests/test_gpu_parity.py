@@ -51,11 +51,12 @@ def _oracle_kind(oracle, coupling):
 
 
 def _pair(P, oracle, dims, n=1, storage="int8", coupling="uniform", J=(1.0, 1.0, 1.0), replicas=1, replica_streams=0,
-          seed=SEED, init=0):
+          seed=SEED, init=0, rule="metropolis"):
     G = _system(P, dims, n=n, storage=storage, coupling=coupling, J=J, replicas=replicas,
-                     replica_streams=replica_streams, seed=seed, init=init)
+                     replica_streams=replica_streams, seed=seed, init=init, rule=rule)
     O = oracle.System(dims, n=n, coupling_kind=_oracle_kind(oracle, coupling), J=J, n_replicas=replicas,
-                      replica_streams=replica_streams, seed=seed, init=init)
+                      replica_streams=replica_streams, seed=seed, init=init,
+                      rule=oracle.RULE_HEATBATH if rule == "heatbath" else oracle.RULE_METROPOLIS)
     return G, O
 
 
@@ -352,3 +353,80 @@ def test_error_paths(P):
     with pytest.raises(P.SpinError) as e:
         S.sweep(0.4, 1)
     assert e.value.status == 5
+
+
+# --------------------------------------------------------------------------- heat bath
+HEATBATH_CASES = [
+    # dims, storage, coupling, J, R, streams, beta
+    ((8, 6, 1), "int8", "uniform", 1.0, 1, 0, BETA_2D),            # generic kernel
+    ((6, 4, 8), "int8", "uniform", 1.0, 2, 1, BETA_3D),
+    ((4, 2, 2), "int8", "bond_pm1", 1.0, 3, 1, 0.6),               # size-2 dimensions, per-bond couplings
+    ((66, 4, 1), "int8", "per_direction", 1.0, 1, 0, 0.7),         # zero coupling in z / odd local fields
+    ((128, 10, 1), "int8", "uniform", 1.0, 1, 0, BETA_2D),         # int8 fast kernel, ragged strips
+    ((192, 6, 4), "int8", "uniform", -1.0, 1, 0, BETA_3D),         # antiferromagnet
+    ((2048, 34, 1), "int8", "uniform", 1.0, 1, 0, BETA_2D),        # beyond the resident kernel's limit
+    ((128, 6, 1), "bitpack", "uniform", 1.0, 1, 0, BETA_2D),
+    ((192, 10, 6), "bitpack", "uniform", 1.0, 1, 0, BETA_3D),
+    ((64, 130, 4), "bitpack", "uniform", 1.0, 2, 1, BETA_3D),      # one-launch-per-half-sweep bit-packed kernel
+    ((64, 6, 4), "bitpack", "bond_pm1", 1.0, 4, 0, 1.0 / 1.1),     # +-J, shared update stream (config 4 shape)
+    ((64, 6, 4), "bitpack", "bond_pm1", 1.0, 3, 1, 1.0 / 1.1),
+    ((64, 12, 1), "bitpack", "bond_pm1", 1.0, 5, 0, 0.8),
+]
+
+
+@pytest.mark.parametrize("dims,storage,coupling,J,R,streams,beta", HEATBATH_CASES)
+def test_ising_heatbath_bit_exact_every_sweep(P, oracle, dims, storage, coupling, J, R, streams, beta):
+    Jv = (J, J, 0.0) if coupling == "per_direction" else (J, J, J)
+    G, O = _pair(P, oracle, dims, storage=storage, coupling=coupling, J=Jv, replicas=R, replica_streams=streams,
+                 rule="heatbath")
+    for t in range(5):
+        G.sweep(beta, 1)
+        O.sweep(beta, 1)
+        _assert_ising_equal(G, O, "heat bath %s %s sweep %d" % (dims, storage, t))
+    # limits: beta = 0 is a fair coin per site (still bit-exact); beta = 50 aligns every spin with its field
+    for b in (0.0, 50.0):
+        G.sweep(b, 2)
+        O.sweep(b, 2)
+        _assert_ising_equal(G, O, "heat bath %s beta %g" % (dims, b))
+
+
+def test_heatbath_recorded_sweeps(P, oracle):
+    import torch
+
+    G, O = _pair(P, oracle, (64, 64, 1), storage="int8", replicas=2, replica_streams=1, rule="heatbath")
+    dE, dM = G.sweep_record(BETA_2D, 40)
+    torch.cuda.synchronize()
+    Eg, Mg = dE.cpu().numpy(), dM.cpu().numpy()[:, :, 0]
+    for t in range(40):
+        O.sweep(BETA_2D, 1)
+        e, m = O.measure()
+        assert np.array_equal(Eg[t], e) and np.array_equal(Mg[t], m[:, 0]), t
+    _assert_ising_equal(G, O, "heat bath recorded")
+
+
+@pytest.mark.parametrize("dims,J", [((16, 16, 16), (1.0, 1.0, 1.0)), ((32, 32, 1), (1.0, 1.0, 1.0)),
+                                    ((8, 6, 4), (1.0, -1.0, 0.5)), ((6, 4, 4), (1.0, 1.0, 1.0))])
+def test_heisenberg_heatbath_within_tolerance(P, oracle, dims, J):
+    """n = 3 heat bath: per-sweep energy within 1e-5 relative over the first 10 sweeps, spins within 1e-4
+    (both sides fp32 in the same order; only expf / logf / sincospif differ from the oracle's once-rounded values)."""
+    coupling = "uniform" if J[0] == J[1] == J[2] else "per_direction"
+    G, O = _pair(P, oracle, dims, n=3, storage="fp32", coupling=coupling, J=J, rule="heatbath")
+    N = dims[0] * dims[1] * dims[2]
+    bad = 0
+    for t in range(10):
+        G.sweep(0.693, 1)
+        O.sweep(0.693, 1)
+        Eg, Mg = G.measure()
+        Eo, Mo = O.measure()
+        assert abs(Eg[0] - Eo[0]) <= 1e-5 * abs(Eo[0]), (t, Eg, Eo)
+        assert np.max(np.abs(Mg - Mo)) <= 1e-5 * N
+        diff = np.max(np.abs(G.get_spins() - O.get_spins()), axis=2)
+        bad += int(np.count_nonzero(diff > 1e-4))
+        assert np.max(np.abs(np.linalg.norm(G.get_spins()[0].astype(np.float64), axis=1) - 1.0)) < 1e-5
+    assert bad <= max(0, int(1e-6 * 10 * N)), bad
+
+
+def test_heatbath_is_unsupported_for_xy(P):
+    with pytest.raises(P.SpinError) as e:
+        P.SpinSystem((8, 8, 1), n=2, storage="fp32", rule="heatbath")
+    assert e.value.status == 2
