@@ -230,9 +230,9 @@ def run_graft(args):
     import numpy as np
     import torch
 
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+    from paper_1107_5463_b200 import ranks
+
+    rank, local_rank, world = ranks.env_rank()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     torch.cuda.set_device(local_rank)
@@ -247,7 +247,7 @@ def run_graft(args):
     P.lib()
     peak, peak_src = measured_peaks()
     w = P.workloads.WORKLOADS[args.workload]
-    S = P.from_workload(w, P.workloads.SEED + rank, device=dev)  # every rank: its own independent lattice
+    S = P.from_workload(w, ranks.rank_seed(P.workloads.SEED, rank), device=dev)  # every rank: its own independent lattice
     beta, SPS = w["beta"], args.sweeps_per_step
     updates_per_step = S.N * S.R * SPS
 
@@ -257,11 +257,7 @@ def run_graft(args):
         torch.cuda.synchronize()
 
     def max_over_ranks(x):
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return ranks.max_over_ranks(x, dist, dev)
 
     # ---- device-resident arm -------------------------------------------------------------------
     for _ in range(args.warmup):

@@ -1,0 +1,73 @@
+"""The N > 1 host logic of bench.py (paper_1107_5463_b200/ranks.py) under a real world_size-2 process group on CPU
+(gloo): per-rank seeds give independent lattices, the timed region is the slowest rank's, the metric sums the updates
+of all ranks.  There is no data-path collective to test: the path shards by independent lattices.
+The lattices themselves are driven here by the oracle, standing in for the GPU handle (no GPU in this test)."""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, out):
+    sys.path.insert(0, ROOT)
+    import torch.distributed as dist
+
+    import oracle
+    from paper_1107_5463_b200 import ranks, workloads
+
+    dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%d" % port, rank=rank, world_size=world)
+    try:
+        seed = ranks.rank_seed(workloads.SEED, rank)
+        S = oracle.System((16, 16, 1), seed=seed)
+        S.sweep(0.4406868, 3)
+        E, M = S.measure()
+        spins = S.get_spins()
+        # pretend rank r needed (10 + 5 r) ms for 1e6 updates
+        value, ms = ranks.whole_job_flips_per_ns(1e6, 10.0 + 5.0 * rank, dist)
+        mx = ranks.max_over_ranks(float(rank), dist)
+        out.put((rank, seed, float(E[0]), spins.tobytes(), value, ms, mx))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_world_size_two_gloo():
+    import torch.multiprocessing as mp
+
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    (r0, s0, e0, sp0, v0, ms0, mx0), (r1, s1, e1, sp1, v1, ms1, mx1) = res
+    assert (r0, r1) == (0, 1) and s1 == s0 + 1
+    assert sp0 != sp1, "ranks must simulate different lattices"
+    # slowest rank defines the time; both ranks' updates count
+    assert ms0 == ms1 == 15.0 and mx0 == mx1 == 1.0
+    assert v0 == v1 == pytest.approx(2e6 / (15.0 * 1e6))
+
+
+def test_single_process_defaults():
+    sys.path.insert(0, ROOT)
+    from paper_1107_5463_b200 import ranks
+
+    assert ranks.max_over_ranks(3.5) == 3.5
+    v, ms = ranks.whole_job_flips_per_ns(4e6, 2.0)
+    assert ms == 2.0 and v == pytest.approx(2.0)
+    assert ranks.rank_seed(7, 3) == 10
