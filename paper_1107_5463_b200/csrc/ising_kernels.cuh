@@ -275,8 +275,11 @@ __global__ void __launch_bounds__(256) ising_bitpack_halfsweep(const __grid_cons
         const WordNbrs n = word_neighbours<D>(a.g, a.colour, gi);
         uint32_t ltf[NT];
         if (SHARED) {
+            // gridDim.y > 1: the replicas are split into gridDim.y chunks (many realisations of a small lattice)
+            const uint32_t chunk = (a.R + gridDim.y - 1) / gridDim.y;
+            const uint32_t r0 = blockIdx.y * chunk, r1 = min(a.R, r0 + chunk);
             lt_masks_full<NT>(a, a.t, a.colour, gi, 0u, ltf);
-            for (uint32_t r = 0; r < a.R; ++r)
+            for (uint32_t r = r0; r < r1; ++r)
                 mine_base[(size_t)r * NW + gi] = bitpack_update_word<D, BONDS, true>(a, r, gi, n, ltf);
         } else {
             for (uint32_t r = 0; r < a.R; ++r)
@@ -297,7 +300,9 @@ __global__ void __launch_bounds__(256) ising_bitpack_halfsweep_hb(const __grid_c
         const WordNbrs n = word_neighbours<D>(a.g, a.colour, gi);
         uint32_t ltf[NT];
         if (SHARED) lt_masks_full<NT, true>(a, a.t, a.colour, gi, 0u, ltf);
-        for (uint32_t r = 0; r < a.R; ++r) {
+        const uint32_t chunk = SHARED ? (a.R + gridDim.y - 1) / gridDim.y : a.R;
+        const uint32_t r0 = SHARED ? blockIdx.y * chunk : 0u, r1 = min(a.R, r0 + chunk);
+        for (uint32_t r = r0; r < r1; ++r) {
             uint32_t av[6], b[6], m[NT];
             const uint32_t raw = unsatisfied_bonds<D, BONDS>(a, a.colour, r, gi, n, av);
 #pragma unroll

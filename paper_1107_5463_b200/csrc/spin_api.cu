@@ -275,11 +275,25 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
         else { if (K == 1) I8(3, 1); else if (K == 2) I8(3, 2); else if (K == 4) I8(3, 4); else if (K == 8) I8(3, 8); else I8(3, 16); }
 #undef I8
     } else {
-        const int G = grid_for(s, s->g.NW);
+        // shared update stream: chunks of >= 16 replicas per thread (the masks of a word are built once per chunk);
+        // more chunks only when the lattice alone cannot fill the GPU (many realisations of a small lattice)
+        int Bq = B;
+        while (Bq > 32 && (uint32_t)(Bq / 2) >= s->g.NW) Bq /= 2;   // small lattices: no dead threads
+        const int Gx = (int)((s->g.NW + Bq - 1) / Bq) < grid_for(s, s->g.NW) ? (int)((s->g.NW + Bq - 1) / Bq) : grid_for(s, s->g.NW);
+        int Gy = 1;
+        if (shared && s->R > 16) {
+            // replicas per thread: 16 when the lattice fills the GPU, down to 4 when it is the replicas that must
+            uint64_t per = (uint64_t)s->g.NW * s->R / ((uint64_t)s->sm_count * 1024);
+            if (per > 16) per = 16;
+            if (per < 4) per = 4;
+            Gy = (int)((s->R + per - 1) / per);
+            if (Gy > 65535) Gy = 65535;
+        }
+        const dim3 G(Gx, Gy);
 #define BP(D_, BONDS_, SH_)                                                                      \
     do {                                                                                         \
-        if (s->cfg.update_rule == SPIN_UPDATE_HEATBATH) ising_bitpack_halfsweep_hb<D_, BONDS_, SH_><<<G, B, 0, st>>>(a); \
-        else ising_bitpack_halfsweep<D_, BONDS_, SH_><<<G, B, 0, st>>>(a);                     \
+        if (s->cfg.update_rule == SPIN_UPDATE_HEATBATH) ising_bitpack_halfsweep_hb<D_, BONDS_, SH_><<<G, Bq, 0, st>>>(a); \
+        else ising_bitpack_halfsweep<D_, BONDS_, SH_><<<G, Bq, 0, st>>>(a);                     \
     } while (0)
         if (s->d == 2) {
             if (bonds) { if (shared) BP(2, true, true); else BP(2, true, false); }

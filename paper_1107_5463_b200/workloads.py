@@ -30,6 +30,11 @@ WORKLOADS = {
     # extra: 3D XY (named by north_star, absent from the configs)
     "xy3d_L256_fp32": dict(dims=(256, 256, 256), n=2, storage="fp32", coupling="uniform", J=(1.0, 1.0, 1.0),
                            beta=0.4542, sweeps=500, replicas=1, replica_streams=0, record=False),
+    # extra: the shape of the paper's fastest Metropolis row (Table 1: 2D +-J, many
+    # realisations, multi-spin coded, one random number per site for all realisations); L = 64 is the smallest
+    # lattice the bit-packed layout takes (the paper used L = 32)
+    "ea2d_L64_R4096_bitpack": dict(dims=(64, 64, 1), n=1, storage="bitpack", coupling="bond_pm1", J=(1.0, 1.0, 1.0),
+                                   beta=1.0, sweeps=1000, replicas=4096, replica_streams=0, record=False),
 }
 
 # Algorithmic bytes moved per attempted update: read the target colour, read the
@@ -40,6 +45,7 @@ BYTES_PER_UPDATE = {
     "ising2d_L16384_bitpack": 0.375,
     "ising3d_L512_bitpack": 0.375,
     "ea3d_L256_R16_bitpack": 1.125,
+    "ea2d_L64_R4096_bitpack": 0.875,   # 3 spin bits + 2 forward bonds from each end = 7 bits
     "heisenberg3d_L256_fp32": 36.0,
     "xy3d_L256_fp32": 24.0,
 }

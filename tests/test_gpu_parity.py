@@ -200,6 +200,18 @@ def test_pm_j_spin_glass_bit_exact(P, oracle, dims, storage, R, streams):
         _assert_ising_equal(G, O, "+-J %s %s R=%d sweep %d" % (dims, storage, R, t))
 
 
+@pytest.mark.parametrize("dims,R,rule", [((64, 8, 1), 80, "metropolis"), ((64, 4, 2), 40, "metropolis"),
+                                         ((64, 8, 1), 80, "heatbath"), ((64, 4, 2), 33, "heatbath")])
+def test_many_realisations_shared_stream(P, oracle, dims, R, rule):
+    """many +-J realisations of a small lattice, one random number per site for all of them
+    (PAPER.md:52); the replica axis is then split over gridDim.y chunks."""
+    G, O = _pair(P, oracle, dims, storage="bitpack", coupling="bond_pm1", replicas=R, replica_streams=0, rule=rule)
+    for t in range(4):
+        G.sweep(1.0, 1)
+        O.sweep(1.0, 1)
+        _assert_ising_equal(G, O, "many realisations %s R=%d sweep %d" % (dims, R, t))
+
+
 def test_pm_j_user_bonds_and_replica_streams_uniform(P, oracle):
     rng = np.random.default_rng(5)
     dims, R = (64, 4, 2), 4
