@@ -18,8 +18,9 @@
  *   - Every call returns a spin_status; nothing throws or aborts across the ABI; outputs are
  *     written only on SPIN_OK.  spin_last_error() gives a thread-local message.
  *   - The CALLER owns device memory: spin_create() carves everything it needs out of the
- *     device workspace passed in (size from spin_workspace_bytes()); the library allocates
- *     device memory only transiently inside the get/set calls (staging of canonical arrays).
+ *     device workspace passed in (size from spin_workspace_bytes()).  The only device memory the
+ *     library allocates itself is one staging buffer for canonical arrays, created by the first
+ *     get/set call, reused by later ones and freed by spin_destroy().
  *   - "stream" arguments are cudaStream_t passed as void* (NULL = the legacy default stream).
  *   - spin_sweep / spin_sweep_record only enqueue work; spin_measure and the get/set calls block.
  *   - A handle is not thread-safe; different handles are independent.

@@ -68,6 +68,8 @@ struct spin_system {
     double table_beta;   // beta the cached table was built for (NaN = none)
     IsingTable tab;
     HeatBathTable hb;    // n = 1 heat bath: built with the table above
+    void *staging;       // device buffer for canonical arrays (get / set calls), kept until spin_destroy
+    size_t staging_bytes;
 };
 
 static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
@@ -314,22 +316,23 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
 static spin_status launch_halfsweep_vector(spin_system *s, const VectorArgs &a, cudaStream_t st) {
     const Geometry &g = s->g;
     const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
-    if (g.RL % 4 == 0 && !s->vector_generic && hb) {
+    const bool strip_ok = g.RL % 4 == 0 && !s->vector_generic && s->R <= 65535;
+    if (strip_ok && hb) {
         // heat bath (n = 3): the strip kernel with one row per thread
         bool unitj = true;
         for (int mu = 0; mu < s->d; ++mu) unitj = unitj && a.Jdir[mu] == 1.0f;
         const int B = s->block > 128 ? 128 : s->block;
-        const uint64_t items = (uint64_t)(g.RL / 4) * g.Ly * g.Lz * s->R;
-        const int G = (int)((items + B - 1) / B);
+        const uint64_t items = (uint64_t)(g.RL / 4) * g.Ly * g.Lz;
+        const dim3 G((unsigned)((items + B - 1) / B), s->R);
         if (s->d == 2) { if (unitj) vector_strip_halfsweep<3, 2, true, 1, true><<<G, B, 0, st>>>(a); else vector_strip_halfsweep<3, 2, false, 1, true><<<G, B, 0, st>>>(a); }
         else { if (unitj) vector_strip_halfsweep<3, 3, true, 1, true><<<G, B, 0, st>>>(a); else vector_strip_halfsweep<3, 3, false, 1, true><<<G, B, 0, st>>>(a); }
-    } else if (g.RL % 4 == 0 && !s->vector_generic) {
+    } else if (strip_ok) {
         bool unitj = true;
         for (int mu = 0; mu < s->d; ++mu) unitj = unitj && a.Jdir[mu] == 1.0f;
         const int K = s->strip_rows_set ? (s->strip_rows >= 4 ? 4 : s->strip_rows) : 1;  // default 1 (measured fastest)
         const int B = s->block > 128 ? 128 : s->block;
-        const uint64_t items = (uint64_t)(g.RL / 4) * ((g.Ly + K - 1) / K) * g.Lz * s->R;
-        const int G = (int)((items + B - 1) / B);
+        const uint64_t items = (uint64_t)(g.RL / 4) * ((g.Ly + K - 1) / K) * g.Lz;
+        const dim3 G((unsigned)((items + B - 1) / B), s->R);
 #define VS4(NC_, D_, U_, K_) vector_strip_halfsweep<NC_, D_, U_, K_><<<G, B, 0, st>>>(a)
 #define VS3(NC_, D_, U_) do { if (K == 1) VS4(NC_, D_, U_, 1); else if (K == 2) VS4(NC_, D_, U_, 2); else VS4(NC_, D_, U_, 4); } while (0)
 #define VS2(NC_, D_) do { if (unitj) VS3(NC_, D_, true); else VS3(NC_, D_, false); } while (0)
@@ -486,7 +489,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
         return fail(SPIN_ERR_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, %zu needed", bytes, need);
     }
     s->ws = (char *)d_workspace;
-    s->t = 0; s->launches = 0;
+    s->t = 0; s->launches = 0; s->staging = nullptr; s->staging_bytes = 0;
     s->block = dv.path == PATH_ISING_INT8 ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0;
     s->table_beta = std::nan("");
     Geometry &g = s->g;
@@ -549,6 +552,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
 }
 
 spin_status spin_destroy(spin_system *s) {
+    if (s && s->staging) cudaFree(s->staging);
     delete s;
     return SPIN_OK;
 }
@@ -597,6 +601,15 @@ spin_status spin_measure(spin_system *s, double *E, double *M, void *stream) {
     return SPIN_OK;
 }
 
+// the handle's staging buffer, grown on demand (cudaMalloc / cudaFree cost milliseconds at these sizes)
+static cudaError_t ensure_staging(spin_system *s, size_t bytes) {
+    if (s->staging && s->staging_bytes >= bytes) return cudaSuccess;
+    if (s->staging) { cudaFree(s->staging); s->staging = nullptr; s->staging_bytes = 0; }
+    cudaError_t e = cudaMalloc(&s->staging, bytes);
+    if (e == cudaSuccess) s->staging_bytes = bytes;
+    return e;
+}
+
 static size_t canonical_spin_bytes(const spin_system *s) {
     return s->n == 1 ? (size_t)s->R * s->N : (size_t)s->R * s->N * s->n * sizeof(float);
 }
@@ -605,9 +618,9 @@ spin_status spin_get_spins(spin_system *s, void *host, size_t bytes) {
     if (!s || !host) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
     const size_t need = canonical_spin_bytes(s);
     if (bytes != need) return fail(SPIN_ERR_INVALID_ARG, "spins need exactly %zu bytes, got %zu", need, bytes);
-    void *staging = nullptr;
     CUDA_TRY(cudaDeviceSynchronize());
-    CUDA_TRY(cudaMalloc(&staging, need));
+    CUDA_TRY(ensure_staging(s, need));
+    void *staging = s->staging;
     const SetupArgs sa = setup_args(s);
     const int G = grid_for(s, 2ull * s->R * s->g.Nh);
     void *s0 = s->ws + s->lay.off_s[0], *s1 = s->ws + s->lay.off_s[1];
@@ -616,7 +629,6 @@ spin_status spin_get_spins(spin_system *s, void *host, size_t bytes) {
     else vector_to_canonical<3><<<G, 256>>>(sa, (const float *)s0, (const float *)s1, (float *)staging);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpy(host, staging, need, cudaMemcpyDeviceToHost);
-    cudaFree(staging);
     if (e != cudaSuccess) return fail(SPIN_ERR_CUDA, "get_spins: %s", cudaGetErrorString(e));
     return SPIN_OK;
 }
@@ -625,9 +637,9 @@ spin_status spin_set_spins(spin_system *s, const void *host, size_t bytes) {
     if (!s || !host) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
     const size_t need = canonical_spin_bytes(s);
     if (bytes != need) return fail(SPIN_ERR_INVALID_ARG, "spins need exactly %zu bytes, got %zu", need, bytes);
-    char *staging = nullptr;
     CUDA_TRY(cudaDeviceSynchronize());
-    CUDA_TRY(cudaMalloc((void **)&staging, need + 256));
+    CUDA_TRY(ensure_staging(s, need + 512));
+    char *staging = (char *)s->staging;
     int *d_bad = (int *)(staging + need + (256 - need % 256) % 256);  // 4 aligned bytes after the spins
     int bad = 0;
     cudaError_t e = cudaMemcpy(staging, host, need, cudaMemcpyHostToDevice);
@@ -640,10 +652,7 @@ spin_status spin_set_spins(spin_system *s, const void *host, size_t bytes) {
         }
         if (e == cudaSuccess) e = cudaMemcpy(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost);
     }
-    if (e == cudaSuccess && bad) {
-        cudaFree(staging);
-        return fail(SPIN_ERR_INVALID_ARG, "Ising spins must be +-1");
-    }
+    if (e == cudaSuccess && bad) return fail(SPIN_ERR_INVALID_ARG, "Ising spins must be +-1");
     if (e == cudaSuccess) {
         const SetupArgs sa = setup_args(s);
         const int G = grid_for(s, 2ull * s->R * s->g.Nh);
@@ -654,7 +663,6 @@ spin_status spin_set_spins(spin_system *s, const void *host, size_t bytes) {
         e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaDeviceSynchronize();
     }
-    cudaFree(staging);
     if (e != cudaSuccess) return fail(SPIN_ERR_CUDA, "set_spins: %s", cudaGetErrorString(e));
     return SPIN_OK;
 }
@@ -669,12 +677,11 @@ spin_status spin_get_bonds(spin_system *s, int8_t *host, size_t bytes) {
         CUDA_TRY(cudaMemcpy(host, s->ws + s->lay.off_bonds, need, cudaMemcpyDeviceToHost));
         return SPIN_OK;
     }
-    void *staging = nullptr;
-    CUDA_TRY(cudaMalloc(&staging, need));
+    CUDA_TRY(ensure_staging(s, need));
+    void *staging = s->staging;
     bonds_unpack<<<grid_for(s, 2ull * s->R * s->g.Nh), 256>>>(setup_args(s), (const uint32_t *)(s->ws + s->lay.off_bonds), (int8_t *)staging);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpy(host, staging, need, cudaMemcpyDeviceToHost);
-    cudaFree(staging);
     if (e != cudaSuccess) return fail(SPIN_ERR_CUDA, "get_bonds: %s", cudaGetErrorString(e));
     return SPIN_OK;
 }

@@ -175,9 +175,11 @@ __global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_const
     const uint32_t RL = g.RL, QX = RL >> 2, Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz, Nh = g.Nh;
     const uint32_t nstrip = (Ly + K - 1) / K;
     const uint32_t per_replica = QX * nstrip * Lz;
-    const uint32_t item = blockIdx.x * blockDim.x + threadIdx.x;
-    if (item >= per_replica * a.R) return;
-    const uint32_t r = item / per_replica, it = item - r * per_replica;
+    // the replica is blockIdx.y (host: gridDim.y = R), so the plane base pointers are warp-uniform and every access is
+    // "uniform 64-bit base + 32-bit offset" (no per-thread 64-bit address arithmetic)
+    const uint32_t it = blockIdx.x * blockDim.x + threadIdx.x;
+    if (it >= per_replica) return;
+    const uint32_t r = blockIdx.y;
     const uint32_t sz = fdiv(it, g.divQX), q = it - sz * QX;       // sz = strip + nstrip * z
     const uint32_t z = sz / nstrip, y0 = (sz - z * nstrip) * K;
     const uint32_t kend = min((uint32_t)K, Ly - y0);
