@@ -79,6 +79,13 @@ typedef struct {
     int32_t init;            /* SPIN_INIT_*                                                             */
     uint64_t seed;           /* Philox key                                                              */
     int32_t update_rule;     /* SPIN_UPDATE_*                                                           */
+    /* Slab decomposition over several handles / GPUs; both 0 = the handle holds the whole lattice.
+     * dims[] are then the LOCAL extents: the handle owns planes [slab_offset, slab_offset + dims[axis]) of a lattice
+     * whose extent along the slowest axis (z for d = 3, y for d = 2) is slab_global.  Both even.  Random numbers are
+     * keyed by GLOBAL site indices, so the slabs together reproduce the unsharded lattice bit for bit.  Uniform or
+     * per-direction couplings only.  Drive with spin_halfsweep + spin_halo_get / spin_halo_put. */
+    int32_t slab_global;
+    int32_t slab_offset;
 } spin_config;
 
 /* Bytes of device workspace spin_create() needs for this configuration. */
@@ -98,6 +105,18 @@ spin_status spin_sweep(spin_system *s, double beta, int64_t n_sweeps, void *stre
  * aggregates).  E, M are HOST pointers to R and R*n doubles.  n = 1: both are exact integers.
  * Runs on `stream` and blocks until the result is on the host. */
 spin_status spin_measure(spin_system *s, double *E, double *M, void *stream);
+
+/* One half-sweep (colour 0, then colour 1, alternating; the sweep counter advances after colour 1), enqueued on
+ * `stream`.  For slab handles the caller exchanges halos in between: before the half-sweep of colour c every handle
+ * needs its neighbours' boundary planes of colour 1 - c (spin_halo_get on the owner, spin_halo_put here). */
+spin_status spin_halfsweep(spin_system *s, double beta, int32_t colour, void *stream);
+
+/* Slab handles: bytes of one face (one boundary plane of one colour, all replicas / components). */
+spin_status spin_halo_bytes(const spin_system *s, size_t *bytes);
+/* Copy the OWNED boundary plane of colour `colour` on side 0 (lowest owned plane) or 1 (highest) into the contiguous
+ * DEVICE buffer d_buf / copy d_buf into the GHOST plane below (side 0) or above (side 1) the owned planes.  Async. */
+spin_status spin_halo_get(spin_system *s, int32_t colour, int32_t side, void *d_buf, void *stream);
+spin_status spin_halo_put(spin_system *s, int32_t colour, int32_t side, const void *d_buf, void *stream);
 
 /* As spin_sweep, recording E and M after every sweep into DEVICE arrays d_E[n_sweeps][R] and
  * d_M[n_sweeps][R][n] (doubles).  Enqueues only. */

@@ -26,7 +26,8 @@ _COUPLING = {"uniform": J_UNIFORM, "per_direction": J_PER_DIRECTION, "bond_pm1":
 SYMBOLS = [
     "spin_workspace_bytes", "spin_create", "spin_sweep", "spin_measure", "spin_sweep_record", "spin_get_spins",
     "spin_set_spins", "spin_get_bonds", "spin_get_sweep_count", "spin_set_sweep_count", "spin_get_launch_count",
-    "spin_set_launch_shape", "spin_set_strip_rows", "spin_set_option", "spin_destroy", "spin_last_error", "spin_version",
+    "spin_set_launch_shape", "spin_set_strip_rows", "spin_set_option", "spin_halfsweep", "spin_halo_bytes",
+    "spin_halo_get", "spin_halo_put", "spin_destroy", "spin_last_error", "spin_version",
 ]
 
 
@@ -35,6 +36,7 @@ class SpinConfig(C.Structure):
         ("dims", C.c_int32 * 3), ("n", C.c_int32), ("storage", C.c_int32), ("coupling_kind", C.c_int32),
         ("J", C.c_double * 3), ("bonds", C.c_void_p), ("n_replicas", C.c_int32), ("replica_streams", C.c_int32),
         ("init", C.c_int32), ("seed", C.c_uint64), ("update_rule", C.c_int32),
+        ("slab_global", C.c_int32), ("slab_offset", C.c_int32),
     ]
 
 
@@ -78,6 +80,10 @@ def lib():
         L.spin_set_launch_shape.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32]
         L.spin_set_strip_rows.argtypes = [vp, C.c_int32]
         L.spin_set_option.argtypes = [vp, C.c_int32, C.c_int64]
+        L.spin_halfsweep.argtypes = [vp, C.c_double, C.c_int32, vp]
+        L.spin_halo_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
+        L.spin_halo_get.argtypes = [vp, C.c_int32, C.c_int32, vp, vp]
+        L.spin_halo_put.argtypes = [vp, C.c_int32, C.c_int32, vp, vp]
         L.spin_destroy.argtypes = [vp]
         for name in SYMBOLS:
             getattr(L, name).restype = C.c_int
@@ -95,7 +101,7 @@ def _check(status):
 
 
 def make_config(dims, n=1, storage="int8", coupling="uniform", J=(1.0, 1.0, 1.0), bonds=None, replicas=1,
-                replica_streams=0, init=INIT_HOT, seed=0, rule="metropolis"):
+                replica_streams=0, init=INIT_HOT, seed=0, rule="metropolis", slab_global=0, slab_offset=0):
     dims = [int(v) for v in dims]
     if len(dims) == 2:
         dims.append(1)
@@ -119,6 +125,8 @@ def make_config(dims, n=1, storage="int8", coupling="uniform", J=(1.0, 1.0, 1.0)
     cfg.init = int(init)
     cfg.seed = int(seed)
     cfg.update_rule = _RULE[rule] if isinstance(rule, str) else int(rule)
+    cfg.slab_global = int(slab_global)
+    cfg.slab_offset = int(slab_offset)
     return cfg, keep
 
 
@@ -133,14 +141,16 @@ class SpinSystem:
     sweep_record, get_spins, set_spins, get_bonds."""
 
     def __init__(self, dims, n=1, storage="int8", coupling="uniform", J=(1.0, 1.0, 1.0), bonds=None, replicas=1,
-                 replica_streams=0, init=INIT_HOT, seed=0, device="cuda:0", rule="metropolis"):
+                 replica_streams=0, init=INIT_HOT, seed=0, device="cuda:0", rule="metropolis", slab_global=0,
+                 slab_offset=0):
         import torch
 
         if not torch.cuda.is_available():
             raise RuntimeError("libspin needs a CUDA device (there is no CPU fallback)")
         self._torch = torch
         self.device = torch.device(device)
-        cfg, keep = make_config(dims, n, storage, coupling, J, bonds, replicas, replica_streams, init, seed, rule)
+        cfg, keep = make_config(dims, n, storage, coupling, J, bonds, replicas, replica_streams, init, seed, rule,
+                                slab_global, slab_offset)
         self.cfg = cfg
         self.dims = tuple(cfg.dims)
         self.n = int(cfg.n)
@@ -171,6 +181,25 @@ class SpinSystem:
     def sweep(self, beta, n_sweeps=1):
         with self._torch.cuda.device(self.device):
             _check(lib().spin_sweep(self._h, float(beta), int(n_sweeps), self._stream()))
+
+    def halfsweep(self, beta, colour):
+        with self._torch.cuda.device(self.device):
+            _check(lib().spin_halfsweep(self._h, float(beta), int(colour), self._stream()))
+
+    def halo_bytes(self):
+        out = C.c_size_t(0)
+        _check(lib().spin_halo_bytes(self._h, C.byref(out)))
+        return int(out.value)
+
+    def halo_get(self, colour, side, buf):
+        """owned boundary plane (side 0: lowest, 1: highest) of colour `colour` -> contiguous CUDA uint8 tensor buf"""
+        with self._torch.cuda.device(self.device):
+            _check(lib().spin_halo_get(self._h, int(colour), int(side), C.c_void_p(buf.data_ptr()), self._stream()))
+
+    def halo_put(self, colour, side, buf):
+        """contiguous CUDA uint8 tensor buf -> ghost plane below (side 0) / above (side 1) the owned planes"""
+        with self._torch.cuda.device(self.device):
+            _check(lib().spin_halo_put(self._h, int(colour), int(side), C.c_void_p(buf.data_ptr()), self._stream()))
 
     def measure(self):
         E = np.zeros(self.R, dtype=np.float64)

@@ -84,6 +84,17 @@ struct Geometry {
     uint32_t NW;      // words per colour = Nh / 32 (fast kernels only)
     FastDiv divRL, divWX, divLy;
     FastDiv divQX;    // by RL / 4 (quads of 4 sites per row and colour; strip kernel of the n >= 2 models)
+    // Slab decomposition: this handle holds planes [slab_offset, slab_offset + L_own) of a larger
+    // lattice along its slowest axis (z for d = 3, y for d = 2), stored with two ghost planes on either side, so the
+    // local arrays look like a periodic lattice of L_own + 4 planes.  The kernels sweep all of it (the ghost planes are
+    // overwritten by the halo exchange before they are read) and only need the offsets that turn a local index into
+    // the global one that feeds Philox, and the owned range for the measurements and the canonical get / set.
+    // Not sharded: offsets 0, owned range = everything.
+    uint32_t j_off;     // + local compressed index  -> global compressed index (mod 2^32)
+    uint32_t unit_off;  // + local 32-site unit      -> global unit             (mod 2^32; fast layouts)
+    uint32_t i_off;     // + local lexicographic idx -> global lexicographic index (mod 2^32)
+    uint32_t own_j0, own_j1;   // owned compressed indices [own_j0, own_j1) of either colour
+    uint32_t own_i0, own_in;   // owned lexicographic indices [own_i0, own_i0 + own_in)
 };
 
 }  // namespace spin

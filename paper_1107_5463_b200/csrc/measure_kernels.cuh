@@ -38,7 +38,7 @@ __global__ void __launch_bounds__(256) ising_generic_measure(const __grid_consta
     const int8_t *__restrict__ bonds = (const int8_t *)a.bonds;
     const uint32_t N = 2u * g.Nh;
     long long e = 0, m = 0;
-    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < g.Nh; j += gridDim.x * blockDim.x) {
+    for (uint32_t j = g.own_j0 + blockIdx.x * blockDim.x + threadIdx.x; j < g.own_j1; j += gridDim.x * blockDim.x) {
         const uint32_t row = fdiv(j, g.divRL), xh = j - row * g.RL;
         const uint32_t z = fdiv(row, g.divLy), y = row - z * (uint32_t)g.Ly;
         const uint32_t p = (y + z + 1u) & 1u;  // colour-1 site
@@ -81,7 +81,7 @@ __global__ void __launch_bounds__(256) ising_bitpack_measure(const __grid_consta
     const uint32_t r = blockIdx.y, NW = a.g.NW;
     const uint32_t *__restrict__ s0 = (const uint32_t *)a.s[0] + (size_t)r * NW;
     long long e = 0, m = 0;
-    for (uint32_t gi = blockIdx.x * blockDim.x + threadIdx.x; gi < NW; gi += gridDim.x * blockDim.x) {
+    for (uint32_t gi = (a.g.own_j0 >> 5) + blockIdx.x * blockDim.x + threadIdx.x; gi < (a.g.own_j1 >> 5); gi += gridDim.x * blockDim.x) {
         const WordNbrs n = word_neighbours<D>(a.g, 1u, gi);
         uint32_t av[6];
         const uint32_t raw = unsatisfied_bonds<D, BONDS>(a, 1u, r, gi, n, av);
@@ -103,12 +103,12 @@ template <int D>
 __global__ void __launch_bounds__(256) ising_int8_measure(const __grid_constant__ IsingArgs a, long long *acc) {
     __shared__ long long sm[32];
     const Geometry &g = a.g;
-    const uint32_t r = blockIdx.y, NW = g.NW;
+    const uint32_t r = blockIdx.y;
     const uint8_t *__restrict__ s0 = (const uint8_t *)a.s[0] + (size_t)r * g.Nh;
     const uint8_t *__restrict__ s1 = (const uint8_t *)a.s[1] + (size_t)r * g.Nh;
     const uint32_t jflip = a.jneg ? 0xFFFFFFFFu : 0u;
     long long e = 0, m = 0;
-    for (uint32_t gi = blockIdx.x * blockDim.x + threadIdx.x; gi < NW; gi += gridDim.x * blockDim.x) {
+    for (uint32_t gi = (g.own_j0 >> 5) + blockIdx.x * blockDim.x + threadIdx.x; gi < (g.own_j1 >> 5); gi += gridDim.x * blockDim.x) {
         const WordNbrs n = word_neighbours<D>(g, 1u, gi);
         const uint32_t row = fdiv(gi, g.divWX), w = gi - row * g.WX;
         const uint32_t raw = int8_pack_unit(s1 + 32u * (size_t)gi);
@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(256) vector_measure(const __grid_constant__ Ve
 #pragma unroll
     for (int c = 0; c < NC; ++c) m[c] = 0.0;
     const int q = 2 * g.d;
-    for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < g.Nh; j += gridDim.x * blockDim.x) {
+    for (uint32_t j = g.own_j0 + blockIdx.x * blockDim.x + threadIdx.x; j < g.own_j1; j += gridDim.x * blockDim.x) {
         uint32_t nb[6];
         neighbour_indices(g, 1u, j, nb);
         float si[NC];

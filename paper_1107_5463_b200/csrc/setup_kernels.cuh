@@ -37,7 +37,7 @@ __device__ __forceinline__ uint32_t lex_index(const Geometry &g, uint32_t c, uin
 __global__ void __launch_bounds__(256) ising_fill(const __grid_constant__ SetupArgs a, int mode, const int8_t *canon,
                                                   void *s0, void *s1) {
     const Geometry &g = a.g;
-    const uint32_t per_colour = a.R * g.Nh, total = 2u * per_colour, N = 2u * g.Nh;
+    const uint32_t per_colour = a.R * g.Nh, total = 2u * per_colour;
     for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
         const uint32_t c = idx / per_colour, rem = idx - c * per_colour;
         const uint32_t r = rem / g.Nh, j = rem - r * g.Nh;
@@ -45,10 +45,15 @@ __global__ void __launch_bounds__(256) ising_fill(const __grid_constant__ SetupA
         uint32_t bit = 0u;
         if (mode == 1) {
             uint32_t w[4];
-            philox4x32_10(i >> 7, r, 0u, make_tag(0u, DOM_INIT, 0u), a.keys, w);
-            bit = (w[(i >> 5) & 3u] >> (i & 31u)) & 1u;
+            const uint32_t ig = i + g.i_off;   // global site index (slab decomposition)
+            philox4x32_10(ig >> 7, r, 0u, make_tag(0u, DOM_INIT, 0u), a.keys, w);
+            bit = (w[(ig >> 5) & 3u] >> (ig & 31u)) & 1u;
         } else if (mode == 2) {
-            bit = canon[(size_t)r * N + i] < 0 ? 1u : 0u;
+            // canonical arrays hold the owned sites only (ghost planes of a slab keep what the halo exchange wrote)
+            const uint32_t io = i - g.own_i0;
+            if (io < g.own_in) bit = canon[(size_t)r * g.own_in + io] < 0 ? 1u : 0u;
+            else if (a.bitpack) bit = (((const uint32_t *)(c ? s1 : s0))[(size_t)r * g.NW + (j >> 5)] >> (j & 31u)) & 1u;
+            else bit = ((const uint8_t *)(c ? s1 : s0))[(size_t)r * g.Nh + int8_byte_index(a, j)];
         }
         void *dst = c ? s1 : s0;
         if (a.bitpack) {
@@ -73,7 +78,7 @@ __global__ void __launch_bounds__(256) ising_validate_canonical(const int8_t *ca
 __global__ void __launch_bounds__(256) ising_to_canonical(const __grid_constant__ SetupArgs a, const void *s0, const void *s1,
                                                           int8_t *canon) {
     const Geometry &g = a.g;
-    const uint32_t per_colour = a.R * g.Nh, total = 2u * per_colour, N = 2u * g.Nh;
+    const uint32_t per_colour = a.R * g.Nh, total = 2u * per_colour;
     for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
         const uint32_t c = idx / per_colour, rem = idx - c * per_colour;
         const uint32_t r = rem / g.Nh, j = rem - r * g.Nh;
@@ -82,7 +87,8 @@ __global__ void __launch_bounds__(256) ising_to_canonical(const __grid_constant_
         uint32_t bit;
         if (a.bitpack) bit = (((const uint32_t *)src)[(size_t)r * g.NW + (j >> 5)] >> (j & 31u)) & 1u;
         else bit = ((const uint8_t *)src)[(size_t)r * g.Nh + int8_byte_index(a, j)];
-        canon[(size_t)r * N + i] = bit ? (int8_t)-1 : (int8_t)1;
+        const uint32_t io = i - g.own_i0;
+        if (io < g.own_in) canon[(size_t)r * g.own_in + io] = bit ? (int8_t)-1 : (int8_t)1;
     }
 }
 
@@ -91,7 +97,7 @@ template <int NC>
 __global__ void __launch_bounds__(256) vector_fill(const __grid_constant__ SetupArgs a, int mode, const float *canon,
                                                    float *s0, float *s1) {
     const Geometry &g = a.g;
-    const uint32_t per_colour = a.R * g.Nh, total = 2u * per_colour, N = 2u * g.Nh;
+    const uint32_t per_colour = a.R * g.Nh, total = 2u * per_colour;
     for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
         const uint32_t c = idx / per_colour, rem = idx - c * per_colour;
         const uint32_t r = rem / g.Nh, j = rem - r * g.Nh;
@@ -101,11 +107,13 @@ __global__ void __launch_bounds__(256) vector_fill(const __grid_constant__ Setup
             if (NC == 3) v[2] = 1.0f; else v[0] = 1.0f;
         } else if (mode == 1) {
             uint32_t w[4];
-            philox4x32_10(i, r, 0u, make_tag(0u, DOM_INIT, 0u), a.keys, w);
+            philox4x32_10(i + g.i_off, r, 0u, make_tag(0u, DOM_INIT, 0u), a.keys, w);
             if (NC == 3) direction3(w[0], w[1], v); else direction2(w[0], v);
         } else {
+            const uint32_t io = i - g.own_i0;
+            if (io >= g.own_in) continue;   // ghost planes keep what the halo exchange wrote
 #pragma unroll
-            for (int k = 0; k < NC; ++k) v[k] = canon[((size_t)r * N + i) * NC + k];
+            for (int k = 0; k < NC; ++k) v[k] = canon[((size_t)r * g.own_in + io) * NC + k];
         }
         float *dst = (c ? s1 : s0) + (size_t)r * NC * g.Nh;
 #pragma unroll
@@ -117,14 +125,16 @@ template <int NC>
 __global__ void __launch_bounds__(256) vector_to_canonical(const __grid_constant__ SetupArgs a, const float *s0, const float *s1,
                                                            float *canon) {
     const Geometry &g = a.g;
-    const uint32_t per_colour = a.R * g.Nh, total = 2u * per_colour, N = 2u * g.Nh;
+    const uint32_t per_colour = a.R * g.Nh, total = 2u * per_colour;
     for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
         const uint32_t c = idx / per_colour, rem = idx - c * per_colour;
         const uint32_t r = rem / g.Nh, j = rem - r * g.Nh;
         const uint32_t i = lex_index(g, c, j);
         const float *src = (c ? s1 : s0) + (size_t)r * NC * g.Nh;
+        const uint32_t io = i - g.own_i0;
+        if (io >= g.own_in) continue;
 #pragma unroll
-        for (int k = 0; k < NC; ++k) canon[((size_t)r * N + i) * NC + k] = src[(size_t)k * g.Nh + j];
+        for (int k = 0; k < NC; ++k) canon[((size_t)r * g.own_in + io) * NC + k] = src[(size_t)k * g.Nh + j];
     }
 }
 

@@ -62,6 +62,8 @@ struct spin_system {
     int block;           // threads per CTA
     int strip_rows;      // strip kernels: rows per thread (1, 2, 4, 8, 16)
     int strip_rows_set;  // the caller chose strip_rows (otherwise each kernel family uses its own default)
+    int axis, own_planes; // slab decomposition: axis (2 z, 1 y, -1 none) and owned planes along it
+    uint32_t next_colour; // spin_halfsweep: colour expected next
     int vector_generic;  // n >= 2: force the one-thread-per-site kernel (test knob)
     int grid_num, grid_den;
     uint32_t mblocks;    // CTAs (per replica) of the measurement kernels
@@ -90,7 +92,10 @@ static FastDiv make_fastdiv(uint32_t d) {
 
 struct Derived {
     int d;
-    uint64_t N;
+    uint64_t N;        // sites of the local arrays (with the ghost planes of a slab)
+    uint64_t Nown;     // owned sites (= N when the handle holds the whole lattice)
+    int32_t pad[3];    // dims of the local arrays
+    int axis;          // slab axis (2: z, 1: y) or -1
     Path path;
 };
 
@@ -113,7 +118,24 @@ static spin_status derive(const spin_config *c, Derived *out) {
     if (c->n == 1 && c->storage == SPIN_STORE_FP32) return fail(SPIN_ERR_INVALID_ARG, "n = 1 needs INT8 or BITPACK storage");
     if (c->n > 1 && c->storage != SPIN_STORE_FP32) return fail(SPIN_ERR_INVALID_ARG, "n >= 2 needs FP32 storage");
     out->d = L[2] == 1 ? 2 : 3;
-    out->N = (uint64_t)L[0] * (uint64_t)L[1] * (uint64_t)L[2];
+    out->Nown = (uint64_t)L[0] * (uint64_t)L[1] * (uint64_t)L[2];
+    out->pad[0] = L[0]; out->pad[1] = L[1]; out->pad[2] = L[2];
+    out->axis = -1;
+    if (c->slab_global != 0) {
+        // slab of a larger lattice along the slowest axis: two ghost planes on either side (even, so colours keep
+        // their parity); the update sequence is that of the global lattice (global indices feed Philox)
+        const int ax = out->d == 3 ? 2 : 1;
+        if (c->slab_global < L[ax] || (c->slab_global & 1) || c->slab_offset < 0 || (c->slab_offset & 1) ||
+            c->slab_offset + L[ax] > c->slab_global)
+            return fail(SPIN_ERR_INVALID_ARG, "slab: need even global extent >= local, even offset, offset + local <= global");
+        if (c->coupling_kind == SPIN_J_BOND_PM1) return fail(SPIN_ERR_UNSUPPORTED, "slab decomposition with per-bond couplings");
+        if ((uint64_t)L[0] * L[1] * (out->d == 3 ? (uint64_t)c->slab_global : 1ull) >= (1ull << 32) ||
+            (out->d == 2 && (uint64_t)L[0] * c->slab_global >= (1ull << 32)))
+            return fail(SPIN_ERR_UNSUPPORTED, "slab: the global lattice must have fewer than 2^32 sites");
+        out->axis = ax;
+        out->pad[ax] = L[ax] + 4;
+    }
+    out->N = (uint64_t)out->pad[0] * (uint64_t)out->pad[1] * (uint64_t)out->pad[2];
     if (out->N * (uint64_t)c->n_replicas >= (1ull << 31))
         return fail(SPIN_ERR_UNSUPPORTED, "N * n_replicas must stay below 2^31");
     const int used = c->coupling_kind == SPIN_J_UNIFORM ? 1 : (c->coupling_kind == SPIN_J_PER_DIRECTION ? out->d : 0);
@@ -405,7 +427,7 @@ static spin_status enqueue_measure(spin_system *s, double *dE, double *dM, cudaS
 // Small uniform-coupling Ising systems (at most RESIDENT_MAX_WORDS 32-site words per colour over all replicas):
 // all n_sweeps sweeps, and the per-sweep E and M if asked for, in ONE launch of the shared-memory-resident kernel.
 static bool resident_ok(const spin_system *s, bool record) {
-    if (s->vector_generic || s->n != 1) return false;
+    if (s->vector_generic || s->n != 1 || s->axis >= 0) return false;
     if (!(s->path == PATH_ISING_INT8 || s->path == PATH_ISING_BITPACK)) return false;
     if (s->cfg.coupling_kind != SPIN_J_UNIFORM) return false;
     if ((uint64_t)s->g.NW * s->R > (uint64_t)RESIDENT_MAX_WORDS) return false;
@@ -481,7 +503,8 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
     if (!s) return fail(SPIN_ERR_INVALID_ARG, "out of host memory");
     s->cfg = *cfg;
     s->cfg.bonds = nullptr;  // host array is read here only
-    s->d = dv.d; s->n = cfg->n; s->R = (uint32_t)cfg->n_replicas; s->N = dv.N; s->path = dv.path;
+    s->d = dv.d; s->n = cfg->n; s->R = (uint32_t)cfg->n_replicas; s->N = dv.Nown; s->path = dv.path;
+    s->axis = dv.axis; s->own_planes = dv.axis >= 0 ? cfg->dims[dv.axis] : 0; s->next_colour = 0;
     make_layout(cfg, dv, &s->lay, &s->mblocks);
     if (bytes < s->lay.total) {
         const size_t need = s->lay.total;
@@ -493,11 +516,21 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
     s->block = dv.path == PATH_ISING_INT8 ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0;
     s->table_beta = std::nan("");
     Geometry &g = s->g;
-    g.Lx = cfg->dims[0]; g.Ly = cfg->dims[1]; g.Lz = cfg->dims[2]; g.d = dv.d;
+    g.Lx = dv.pad[0]; g.Ly = dv.pad[1]; g.Lz = dv.pad[2]; g.d = dv.d;
     g.RL = (uint32_t)(g.Lx / 2); g.rows = (uint32_t)(g.Ly * g.Lz); g.Nh = (uint32_t)(dv.N / 2);
     g.WX = g.RL / 32; g.NW = g.Nh / 32;
     g.divRL = make_fastdiv(g.RL); g.divWX = make_fastdiv(g.WX ? g.WX : 1); g.divLy = make_fastdiv((uint32_t)g.Ly);
     g.divQX = make_fastdiv(g.RL / 4 ? g.RL / 4 : 1);
+    g.j_off = 0; g.unit_off = 0; g.i_off = 0; g.own_j0 = 0; g.own_j1 = g.Nh; g.own_i0 = 0; g.own_in = (uint32_t)dv.N;
+    if (dv.axis >= 0) {
+        const int64_t plane_sites = dv.axis == 2 ? (int64_t)g.Lx * g.Ly : (int64_t)g.Lx, plane_h = plane_sites / 2;
+        const int64_t shift = (int64_t)cfg->slab_offset - 2;   // local plane p is global plane p + shift
+        g.j_off = (uint32_t)(shift * plane_h);
+        g.unit_off = (uint32_t)(shift * plane_h / 32);        // exact for the fast layouts (plane_h % 32 == 0)
+        g.i_off = (uint32_t)(shift * plane_sites);
+        g.own_j0 = (uint32_t)(2 * plane_h); g.own_j1 = (uint32_t)((2 + cfg->dims[dv.axis]) * plane_h);
+        g.own_i0 = (uint32_t)(2 * plane_sites); g.own_in = (uint32_t)dv.Nown;
+    }
     for (int r = 0; r < 10; ++r) {
         s->keys.k0[r] = (uint32_t)(cfg->seed & 0xFFFFFFFFull) + (uint32_t)r * 0x9E3779B9u;
         s->keys.k1[r] = (uint32_t)(cfg->seed >> 32) + (uint32_t)r * 0xBB67AE85u;
@@ -560,6 +593,8 @@ spin_status spin_destroy(spin_system *s) {
 spin_status spin_sweep(spin_system *s, double beta, int64_t n_sweeps, void *stream) {
     spin_status rc = check_sweep_args(s, beta, n_sweeps);
     if (rc != SPIN_OK) return rc;
+    if (s->axis >= 0) return fail(SPIN_ERR_STATE, "slab handle: drive it with spin_halfsweep and the halo calls");
+    if (s->next_colour != 0) return fail(SPIN_ERR_STATE, "a spin_halfsweep of colour 1 is pending");
     if (resident_ok(s, false)) return enqueue_resident(s, n_sweeps, nullptr, nullptr, (cudaStream_t)stream);
     for (int64_t k = 0; k < n_sweeps; ++k) {
         rc = enqueue_sweep(s, beta, (cudaStream_t)stream);
@@ -572,6 +607,8 @@ spin_status spin_sweep_record(spin_system *s, double beta, int64_t n_sweeps, dou
     spin_status rc = check_sweep_args(s, beta, n_sweeps);
     if (rc != SPIN_OK) return rc;
     if (!d_E || !d_M) return fail(SPIN_ERR_INVALID_ARG, "d_E / d_M is NULL");
+    if (s->axis >= 0) return fail(SPIN_ERR_STATE, "slab handle: drive it with spin_halfsweep and the halo calls");
+    if (s->next_colour != 0) return fail(SPIN_ERR_STATE, "a spin_halfsweep of colour 1 is pending");
     if (resident_ok(s, true)) return enqueue_resident(s, n_sweeps, d_E, d_M, (cudaStream_t)stream);
     for (int64_t k = 0; k < n_sweeps; ++k) {
         rc = enqueue_sweep(s, beta, (cudaStream_t)stream);
@@ -580,6 +617,70 @@ spin_status spin_sweep_record(spin_system *s, double beta, int64_t n_sweeps, dou
         if (rc != SPIN_OK) return rc;
     }
     return SPIN_OK;
+}
+
+spin_status spin_halfsweep(spin_system *s, double beta, int32_t colour, void *stream) {
+    spin_status rc = check_sweep_args(s, beta, colour == 1 ? 1 : 0);
+    if (rc != SPIN_OK) return rc;
+    if (colour != 0 && colour != 1) return fail(SPIN_ERR_INVALID_ARG, "colour must be 0 or 1");
+    if ((uint32_t)colour != s->next_colour) return fail(SPIN_ERR_STATE, "half-sweeps alternate: colour %u is next", s->next_colour);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (s->n == 1) {
+        IsingArgs a = ising_args(s);
+        a.colour = (uint32_t)colour;
+        rc = launch_halfsweep_ising(s, a, st);
+    } else {
+        VectorArgs a = vector_args(s, beta);
+        a.colour = (uint32_t)colour;
+        rc = launch_halfsweep_vector(s, a, st);
+    }
+    if (rc != SPIN_OK) return rc;
+    s->next_colour = 1u - (uint32_t)colour;
+    if (colour == 1) s->t += 1;
+    return SPIN_OK;
+}
+
+// one face of one colour: per (replica, component) one contiguous plane of the colour array
+struct Face {
+    size_t plane_bytes, stride_bytes, rows;
+};
+static Face face_of(const spin_system *s) {
+    const Geometry &g = s->g;
+    const size_t plane_h = s->axis == 2 ? (size_t)g.RL * g.Ly : (size_t)g.RL;
+    Face f;
+    if (s->path == PATH_ISING_BITPACK) { f.plane_bytes = plane_h / 8; f.stride_bytes = (size_t)g.NW * 4; f.rows = s->R; }
+    else if (s->path == PATH_VECTOR) { f.plane_bytes = plane_h * 4; f.stride_bytes = (size_t)g.Nh * 4; f.rows = (size_t)s->R * s->n; }
+    else { f.plane_bytes = plane_h; f.stride_bytes = g.Nh; f.rows = s->R; }
+    return f;
+}
+
+spin_status spin_halo_bytes(const spin_system *s, size_t *bytes) {
+    if (!s || !bytes) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    if (s->axis < 0) return fail(SPIN_ERR_STATE, "not a slab handle");
+    const Face f = face_of(s);
+    *bytes = f.plane_bytes * f.rows;
+    return SPIN_OK;
+}
+
+static spin_status halo_copy(spin_system *s, int32_t colour, int32_t side, void *d_buf, bool get, cudaStream_t st) {
+    if (!s || !d_buf) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    if (s->axis < 0) return fail(SPIN_ERR_STATE, "not a slab handle");
+    if ((colour != 0 && colour != 1) || (side != 0 && side != 1)) return fail(SPIN_ERR_INVALID_ARG, "colour and side must be 0 or 1");
+    const Face f = face_of(s);
+    // local planes: 0, 1 low ghosts (1 is read), 2 .. own + 1 owned, own + 2, own + 3 high ghosts (own + 2 is read)
+    const size_t plane = get ? (side == 0 ? 2 : (size_t)s->own_planes + 1) : (side == 0 ? 1 : (size_t)s->own_planes + 2);
+    char *arr = s->ws + s->lay.off_s[colour] + plane * f.plane_bytes;
+    if (get) CUDA_TRY(cudaMemcpy2DAsync(d_buf, f.plane_bytes, arr, f.stride_bytes, f.plane_bytes, f.rows, cudaMemcpyDeviceToDevice, st));
+    else CUDA_TRY(cudaMemcpy2DAsync(arr, f.stride_bytes, d_buf, f.plane_bytes, f.plane_bytes, f.rows, cudaMemcpyDeviceToDevice, st));
+    return SPIN_OK;
+}
+
+spin_status spin_halo_get(spin_system *s, int32_t colour, int32_t side, void *d_buf, void *stream) {
+    return halo_copy(s, colour, side, d_buf, true, (cudaStream_t)stream);
+}
+
+spin_status spin_halo_put(spin_system *s, int32_t colour, int32_t side, const void *d_buf, void *stream) {
+    return halo_copy(s, colour, side, const_cast<void *>(d_buf), false, (cudaStream_t)stream);
 }
 
 spin_status spin_measure(spin_system *s, double *E, double *M, void *stream) {

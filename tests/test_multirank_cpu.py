@@ -71,3 +71,69 @@ def test_single_process_defaults():
     v, ms = ranks.whole_job_flips_per_ns(4e6, 2.0)
     assert ms == 2.0 and v == pytest.approx(2.0)
     assert ranks.rank_seed(7, 3) == 10
+
+
+# --------------------------------------------------------------------------- slab decomposition: who sends what to whom
+def _slab_worker(rank, world, port, out):
+    sys.path.insert(0, ROOT)
+    import torch
+    import torch.distributed as dist
+
+    from paper_1107_5463_b200 import slab
+
+    dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%d" % port, rank=rank, world_size=world)
+    try:
+        # a fake slab: owned planes hold 10 * rank + plane index, ghosts start at -1
+        own = 4
+        planes = {c: torch.full((own + 4, 3), -1.0) for c in (0, 1)}
+        for c in (0, 1):
+            for p in range(own):
+                planes[c][2 + p] = 100.0 * c + 10.0 * rank + p
+
+        def get_face(colour, side):
+            return planes[colour][2 if side == 0 else own + 1].clone()
+
+        def put_face(colour, side, t):
+            planes[colour][1 if side == 0 else own + 2] = t
+
+        for c in (0, 1):
+            slab.exchange_faces(get_face, put_face, c, dist, rank, world)
+        out.put((rank, {c: (planes[c][1, 0].item(), planes[c][own + 2, 0].item()) for c in (0, 1)}))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_slab_halo_exchange_ring_gloo(world):
+    """exchange_faces over a real process group: my lower ghost = highest plane of the rank below, my upper ghost =
+    lowest plane of the rank above (periodic), for both colours; world 2 (both neighbours are the same rank) and 3."""
+    import torch.multiprocessing as mp
+
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_slab_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = dict(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    own = 4
+    for r in range(world):
+        below, above = (r - 1) % world, (r + 1) % world
+        for c in (0, 1):
+            low_ghost, high_ghost = res[r][c]
+            assert low_ghost == 100.0 * c + 10.0 * below + (own - 1)
+            assert high_ghost == 100.0 * c + 10.0 * above + 0
+
+
+def test_slab_plan():
+    sys.path.insert(0, ROOT)
+    from paper_1107_5463_b200 import slab
+
+    assert slab.plan((512, 512, 512), 8) == [((512, 512, 64), 64 * k) for k in range(8)]
+    assert slab.plan((16384, 16384), 4)[3] == ((16384, 4096, 1), 12288)
+    assert slab.ring_neighbours(0, 4) == (3, 1) and slab.ring_neighbours(3, 4) == (2, 0)
+    with pytest.raises(ValueError):
+        slab.plan((64, 64, 6), 2)
