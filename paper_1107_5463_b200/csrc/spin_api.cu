@@ -43,6 +43,7 @@ struct Layout {
     size_t off_bonds, bytes_bonds;
     size_t off_acc, bytes_acc;  // n = 1: int64 [R][2]; n >= 2: double [R][mblocks][1 + n]
     size_t off_res, bytes_res;  // double [R] E then [R][n] M
+    size_t off_t;               // uint32: sweep counter read by graph-replayed launches
     size_t total;
 };
 
@@ -70,6 +71,10 @@ struct spin_system {
     double table_beta;   // beta the cached table was built for (NaN = none)
     IsingTable tab;
     HeatBathTable hb;    // n = 1 heat bath: built with the table above
+    cudaGraphExec_t gexec;      // GRAPH_SWEEPS sweeps for (g_beta, launch shape); NULL until first used
+    cudaStream_t cap_stream;    // capture-only stream (nothing ever runs on it)
+    double g_beta;
+    int g_block, g_rows, g_rows_set, g_num, g_den;
     void *staging;       // device buffer for canonical arrays (get / set calls), kept until spin_destroy
     size_t staging_bytes;
 };
@@ -184,6 +189,7 @@ static void make_layout(const spin_config *c, const Derived &dv, Layout *l, uint
     l->off_acc = off; off += align_up(l->bytes_acc);
     l->bytes_res = (size_t)(R * (1 + c->n) * sizeof(double));
     l->off_res = off; off += align_up(l->bytes_res);
+    l->off_t = off; off += 256;
     l->total = off;
 }
 
@@ -255,7 +261,7 @@ static IsingArgs ising_args(const spin_system *s) {
     a.s[1] = s->ws + s->lay.off_s[1];
     a.bonds = s->lay.bytes_bonds ? s->ws + s->lay.off_bonds : nullptr;
     a.R = s->R; a.replica_streams = s->cfg.replica_streams ? 1u : 0u;
-    a.t = (uint32_t)s->t; a.colour = 0;
+    a.t = (uint32_t)s->t; a.colour = 0; a.t_base = nullptr;
     a.coupling_kind = s->cfg.coupling_kind;
     for (int mu = 0; mu < 3; ++mu)
         a.Jdir[mu] = s->cfg.coupling_kind == SPIN_J_UNIFORM ? (int)s->cfg.J[0]
@@ -272,7 +278,7 @@ static VectorArgs vector_args(const spin_system *s, double beta) {
     a.s[0] = (float *)(s->ws + s->lay.off_s[0]);
     a.s[1] = (float *)(s->ws + s->lay.off_s[1]);
     a.R = s->R; a.replica_streams = s->cfg.replica_streams ? 1u : 0u;
-    a.t = (uint32_t)s->t; a.colour = 0;
+    a.t = (uint32_t)s->t; a.colour = 0; a.t_base = nullptr;
     for (int mu = 0; mu < 3; ++mu)
         a.Jdir[mu] = s->cfg.coupling_kind == SPIN_J_UNIFORM ? (float)s->cfg.J[0] : (mu < s->d ? (float)s->cfg.J[mu] : 0.0f);
     a.beta = (float)beta;
@@ -290,7 +296,15 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
     } else if (s->path == PATH_ISING_INT8) {
         // one thread per (replica, z, strip of K rows, unit column)
         const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
-        const int K = hb ? 4 : s->strip_rows;   // the heat-bath kernel is instantiated for K = 4 only
+        // rows per thread: the caller's choice, else 4 when that still leaves every SM several CTAs and 1 otherwise
+        // (a thread walks its rows one after the other: on small grids more threads beat fewer halo loads);
+        // the heat-bath kernel is instantiated for K = 4 only
+        int K = s->strip_rows;
+        if (!s->strip_rows_set) {
+            const uint64_t threads4 = (uint64_t)s->g.WX * ((s->g.Ly + 3) / 4) * s->g.Lz * s->R;
+            K = threads4 >= (uint64_t)s->sm_count * 2048 ? 4 : 1;
+        }
+        if (hb) K = 4;
         const uint64_t items = (uint64_t)s->g.WX * ((s->g.Ly + K - 1) / K) * s->g.Lz * s->R;
         const int G = (int)((items + B - 1) / B);
 #define I8(D_, K_) ising_int8_halfsweep<D_, K_><<<G, B, 0, st>>>(a)
@@ -373,9 +387,13 @@ static spin_status launch_halfsweep_vector(spin_system *s, const VectorArgs &a, 
     return SPIN_OK;
 }
 
-static spin_status enqueue_sweep(spin_system *s, double beta, cudaStream_t st) {
+// One sweep.  t_base == NULL: an ordinary sweep at the handle's counter, which then advances.  Otherwise (graph
+// capture) the launches carry the offset t_rel and read the counter from device memory; the handle is not advanced.
+static spin_status enqueue_sweep(spin_system *s, double beta, cudaStream_t st, const uint32_t *t_base = nullptr,
+                                 uint32_t t_rel = 0) {
     if (s->n == 1) {
         IsingArgs a = ising_args(s);
+        if (t_base) { a.t = t_rel; a.t_base = t_base; }
         for (uint32_t colour = 0; colour < 2; ++colour) {
             a.colour = colour;
             spin_status rc = launch_halfsweep_ising(s, a, st);
@@ -383,13 +401,73 @@ static spin_status enqueue_sweep(spin_system *s, double beta, cudaStream_t st) {
         }
     } else {
         VectorArgs a = vector_args(s, beta);
+        if (t_base) { a.t = t_rel; a.t_base = t_base; }
         for (uint32_t colour = 0; colour < 2; ++colour) {
             a.colour = colour;
             spin_status rc = launch_halfsweep_vector(s, a, st);
             if (rc != SPIN_OK) return rc;
         }
     }
-    s->t += 1;
+    if (!t_base) s->t += 1;
+    return SPIN_OK;
+}
+
+// ------------------------------------------------------------------------- CUDA graphs -------
+// Lattices between the resident kernel's limit and a few million sites are launch-bound: a half-sweep takes less
+// time than its launch (the argument block with the tables is ~3 KB).  spin_sweep then replays a graph of
+// GRAPH_SWEEPS sweeps whose nodes read the sweep counter from device memory; its last node advances the counter.
+constexpr int GRAPH_SWEEPS = 16;
+
+__global__ void counter_set(uint32_t *t, uint32_t v) { *t = v; }
+__global__ void counter_add(uint32_t *t, uint32_t v) { *t += v; }
+
+static bool graph_ok(const spin_system *s, int64_t n_sweeps) {
+    if (s->vector_generic || s->axis >= 0 || n_sweeps < 2 * GRAPH_SWEEPS) return false;
+    // threads of a half-sweep launch; beyond a few full waves the kernel outlasts its launch
+    const uint64_t per_thread = s->n == 1 ? 32 : 4;
+    return s->N * s->R / 2 / per_thread <= (uint64_t)s->sm_count * 2048 * 2;
+}
+
+static spin_status graph_prepare(spin_system *s, double beta) {
+    const bool same = s->gexec && s->g_beta == beta && s->g_block == s->block && s->g_rows == s->strip_rows &&
+                      s->g_rows_set == s->strip_rows_set && s->g_num == s->grid_num && s->g_den == s->grid_den;
+    if (same) return SPIN_OK;
+    if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
+    if (!s->cap_stream) CUDA_TRY(cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
+    uint32_t *d_t = (uint32_t *)(s->ws + s->lay.off_t);
+    const uint64_t launches0 = s->launches;
+    CUDA_TRY(cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
+    spin_status rc = SPIN_OK;
+    for (int k = 0; k < GRAPH_SWEEPS && rc == SPIN_OK; ++k) rc = enqueue_sweep(s, beta, s->cap_stream, d_t, (uint32_t)k);
+    counter_add<<<1, 1, 0, s->cap_stream>>>(d_t, (uint32_t)GRAPH_SWEEPS);
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamEndCapture(s->cap_stream, &graph);
+    s->launches = launches0;   // capturing launched nothing
+    if (rc != SPIN_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) return fail(SPIN_ERR_CUDA, "graph capture: %s", cudaGetErrorString(e));
+    e = cudaGraphInstantiate(&s->gexec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) { s->gexec = nullptr; return fail(SPIN_ERR_CUDA, "graph instantiate: %s", cudaGetErrorString(e)); }
+    s->g_beta = beta; s->g_block = s->block; s->g_rows = s->strip_rows; s->g_rows_set = s->strip_rows_set;
+    s->g_num = s->grid_num; s->g_den = s->grid_den;
+    return SPIN_OK;
+}
+
+// as many whole graphs as fit into n_sweeps; returns the sweeps done
+static spin_status graph_sweeps(spin_system *s, double beta, int64_t n_sweeps, cudaStream_t st, int64_t *done) {
+    *done = 0;
+    spin_status rc = graph_prepare(s, beta);
+    if (rc != SPIN_OK) return rc;
+    uint32_t *d_t = (uint32_t *)(s->ws + s->lay.off_t);
+    counter_set<<<1, 1, 0, st>>>(d_t, (uint32_t)s->t);
+    CUDA_TRY(cudaGetLastError());
+    s->launches += 1;
+    while (n_sweeps - *done >= GRAPH_SWEEPS) {
+        CUDA_TRY(cudaGraphLaunch(s->gexec, st));
+        s->t += GRAPH_SWEEPS;
+        s->launches += 2 * GRAPH_SWEEPS + 1;
+        *done += GRAPH_SWEEPS;
+    }
     return SPIN_OK;
 }
 
@@ -512,7 +590,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
         return fail(SPIN_ERR_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, %zu needed", bytes, need);
     }
     s->ws = (char *)d_workspace;
-    s->t = 0; s->launches = 0; s->staging = nullptr; s->staging_bytes = 0;
+    s->t = 0; s->launches = 0; s->staging = nullptr; s->staging_bytes = 0; s->gexec = nullptr; s->cap_stream = nullptr;
     s->block = dv.path == PATH_ISING_INT8 ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0;
     s->table_beta = std::nan("");
     Geometry &g = s->g;
@@ -586,6 +664,8 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
 
 spin_status spin_destroy(spin_system *s) {
     if (s && s->staging) cudaFree(s->staging);
+    if (s && s->gexec) cudaGraphExecDestroy(s->gexec);
+    if (s && s->cap_stream) cudaStreamDestroy(s->cap_stream);
     delete s;
     return SPIN_OK;
 }
@@ -596,6 +676,12 @@ spin_status spin_sweep(spin_system *s, double beta, int64_t n_sweeps, void *stre
     if (s->axis >= 0) return fail(SPIN_ERR_STATE, "slab handle: drive it with spin_halfsweep and the halo calls");
     if (s->next_colour != 0) return fail(SPIN_ERR_STATE, "a spin_halfsweep of colour 1 is pending");
     if (resident_ok(s, false)) return enqueue_resident(s, n_sweeps, nullptr, nullptr, (cudaStream_t)stream);
+    if (graph_ok(s, n_sweeps)) {
+        int64_t done = 0;
+        rc = graph_sweeps(s, beta, n_sweeps, (cudaStream_t)stream, &done);
+        if (rc != SPIN_OK) return rc;
+        n_sweeps -= done;
+    }
     for (int64_t k = 0; k < n_sweeps; ++k) {
         rc = enqueue_sweep(s, beta, (cudaStream_t)stream);
         if (rc != SPIN_OK) return rc;

@@ -442,3 +442,36 @@ def test_heatbath_is_unsupported_for_xy(P):
     with pytest.raises(P.SpinError) as e:
         P.SpinSystem((8, 8, 1), n=2, storage="fp32", rule="heatbath")
     assert e.value.status == 2
+
+
+# --------------------------------------------------------------------------- CUDA-graph replay (launch-bound sizes)
+@pytest.mark.parametrize("dims,storage,rule", [((128, 600, 1), "int8", "metropolis"), ((64, 70, 20), "bitpack", "metropolis"),
+                                               ((128, 520, 1), "bitpack", "heatbath")])
+def test_graph_replayed_sweeps_ising(P, oracle, dims, storage, rule):
+    """spin_sweep with many sweeps on a lattice beyond the resident kernel's limit replays a CUDA graph of 16 sweeps
+    whose launches read the sweep counter from device memory: 40 sweeps = 2 graphs + 8 plain sweeps, then another beta
+    (graph rebuilt), a changed launch shape, and a counter set by hand -- bit-exact against the oracle throughout."""
+    G, O = _pair(P, oracle, dims, storage=storage, rule=rule)
+    for beta, n in ((0.4406868, 40), (0.3, 33)):
+        G.sweep(beta, n)
+        O.sweep(beta, n)
+        _assert_ising_equal(G, O, "graph %s beta %g" % (dims, beta))
+    G.set_launch_shape(64, 1, 1)
+    G.sweep_counter = 1000
+    O.sweep_counter = 1000
+    G.sweep(0.3, 32)
+    O.sweep(0.3, 32)
+    _assert_ising_equal(G, O, "graph after counter change")
+    assert G.sweep_counter == 1032
+
+
+@pytest.mark.parametrize("n", [2, 3])
+def test_graph_replayed_sweeps_vector(P, n):
+    dims = (32, 32, 16)
+    A = P.SpinSystem(dims, n=n, storage="fp32", seed=9)
+    B = P.SpinSystem(dims, n=n, storage="fp32", seed=9)
+    A.sweep(0.6, 37)                 # 2 graphs + 5 plain sweeps
+    for _ in range(37):
+        B.sweep(0.6, 1)              # never reaches the graph threshold
+    assert np.array_equal(A.get_spins().view(np.uint32), B.get_spins().view(np.uint32))
+    assert A.sweep_counter == B.sweep_counter == 37
