@@ -152,6 +152,17 @@ def run_per_model(P, peak):
         S.close()
         del S
         torch.cuda.empty_cache()
+    # heat-bath rule ("very similar speed-ups"): the same lattices, update_rule = heat bath
+    for name, sweeps in (("ising2d_L16384_int8", 20), ("ising3d_L512_bitpack", 20), ("heisenberg3d_L256_fp32", 10)):
+        w = P.workloads.WORKLOADS[name]
+        S = P.from_workload(w, P.workloads.SEED, rule="heatbath")
+        ms_launch, fpn = time_sweeps(S, w["beta"], sweeps)
+        bpu = P.workloads.BYTES_PER_UPDATE[name]
+        out[name + "_heatbath"] = {"flips_per_ns": fpn, "ms_per_halfsweep": ms_launch, "algorithmic_GBps": fpn * bpu,
+                                   "hbm_frac": fpn * bpu / peak, "bytes_per_update": bpu, "update_rule": "heat bath"}
+        S.close()
+        del S
+        torch.cuda.empty_cache()
     return out
 
 

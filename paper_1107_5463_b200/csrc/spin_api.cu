@@ -290,7 +290,7 @@ static VectorArgs vector_args(const spin_system *s, double beta) {
 static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cudaStream_t st) {
     const bool bonds = s->cfg.coupling_kind == SPIN_J_BOND_PM1;
     const bool shared = s->R > 1 && !s->cfg.replica_streams;
-    const int B = s->block;
+    const int B = s->path == PATH_ISING_INT8 && s->block > 128 ? 128 : s->block;   // the int8 kernel is built for <= 128 threads
     if (s->path == PATH_ISING_GENERIC) {
         ising_generic_halfsweep<<<grid_for(s, (uint64_t)s->g.Nh * s->R), B, 0, st>>>(a);
     } else if (s->path == PATH_ISING_INT8) {
