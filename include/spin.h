@@ -73,7 +73,7 @@ typedef struct {
     const int8_t *bonds;     /* BOND_PM1: HOST array [replica][mu][i] (mu < d) of +-1, the coupling of
                                 the bond leaving site i in direction +mu; NULL -> drawn iid +-1, p = 1/2,
                                 from the seed.  Read during spin_create only.                          */
-    int32_t n_replicas;      /* R >= 1 independent systems stored side by side            */
+    int32_t n_replicas;      /* 1 <= R <= 65535 independent systems stored side by side   */
     int32_t replica_streams; /* 0: all replicas see the same random numbers (needs distinct bonds or
                                 starts to be useful); 1: the replica index enters the Philox counter    */
     int32_t init;            /* SPIN_INIT_*                                                             */

@@ -112,6 +112,7 @@ static spin_status derive(const spin_config *c, Derived *out) {
         return fail(SPIN_ERR_INVALID_ARG, "every lattice dimension must be even (checkerboard + periodic)");
     if (c->n < 1 || c->n > 3) return fail(SPIN_ERR_INVALID_ARG, "n must be 1, 2 or 3");
     if (c->n_replicas < 1) return fail(SPIN_ERR_INVALID_ARG, "n_replicas must be >= 1");
+    if (c->n_replicas > 65535) return fail(SPIN_ERR_UNSUPPORTED, "at most 65535 replicas per handle (replicas map to a grid dimension)");
     if (c->coupling_kind < SPIN_J_UNIFORM || c->coupling_kind > SPIN_J_BOND_PM1)
         return fail(SPIN_ERR_INVALID_ARG, "bad coupling_kind");
     if (c->init != SPIN_INIT_HOT && c->init != SPIN_INIT_COLD) return fail(SPIN_ERR_INVALID_ARG, "bad init");

@@ -1,0 +1,138 @@
+"""The physics pins of the oracle, applied to the GPU path ITSELF with the statistics
+a B200 affords in seconds, and north_star's long-run clause for the continuous models: <E> and <|m|> of the library and
+of the oracle agree within 3 standard errors (same seeds and independent seeds).
+
+Exact references: Kaufman's finite-lattice energy (-sqrt(2) is its L -> infinity limit), Onsager / Yang, exact
+enumeration of the 4 x 4 lattice, the 1D-chain closed forms, the simple-cubic high-temperature series.
+Seeds are fixed, so every 3-sigma statement is decided once."""
+import numpy as np
+import pytest
+
+import exact_results as X
+from test_oracle_physics import check_histogram
+
+pytestmark = pytest.mark.gpu
+
+BETA_C2 = 0.4406868
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1107_5463_b200 as pkg
+
+    pkg.lib()
+    return pkg
+
+
+def _recorded_means(S, beta, therm, sweeps, chunk=2000):
+    """per-replica time averages of e and |m| from spin_sweep_record (device arrays, one copy per chunk)"""
+    import torch
+
+    S.sweep(beta, therm)
+    e_acc = np.zeros(S.R)
+    m_acc = np.zeros(S.R)
+    done = 0
+    while done < sweeps:
+        k = min(chunk, sweeps - done)
+        dE, dM = S.sweep_record(beta, k)
+        torch.cuda.synchronize()
+        e_acc += dE.sum(dim=0).cpu().numpy()
+        m_acc += torch.sqrt((dM ** 2).sum(dim=2)).sum(dim=0).cpu().numpy()
+        done += k
+    return e_acc / sweeps / S.N, m_acc / sweeps / S.N
+
+
+def _mean_err(x):
+    return float(x.mean()), float(x.std(ddof=1) / np.sqrt(x.size))
+
+
+@pytest.mark.parametrize("rule", ["metropolis", "heatbath"])
+@pytest.mark.parametrize("storage", ["int8", "bitpack"])
+def test_2d_ising_critical_energy_L64_is_kaufmans_value(P, storage, rule):
+    """BASELINE config 1's lattice (64 x 64 at beta = 0.4406868) run long enough to test it: 16 independent replicas x
+    60 000 recorded sweeps through the shared-memory-resident kernel.  e_64 = -1.4239384631, not -sqrt(2)."""
+    exact = X.kaufman_energy_per_spin(64, BETA_C2)
+    assert exact == pytest.approx(-1.4239384631, abs=2e-9)
+    S = P.SpinSystem((64, 64, 1), storage=storage, replicas=16, replica_streams=1, seed=2024, rule=rule)
+    e, _ = _recorded_means(S, BETA_C2, 2000, 60000)
+    mean, err = _mean_err(e)
+    assert err < 1.5e-3
+    assert abs(mean - exact) < 3 * err, (mean, err, exact)
+    assert abs(mean + np.sqrt(2.0)) > 4 * err          # the infinite-lattice value is resolvably different
+    assert abs(X.kaufman_energy_per_spin(64, 1.01 * BETA_C2) - exact) > 5 * err   # resolving power: 1 % in beta
+
+
+def test_2d_ising_ordered_phase_onsager_yang_L128(P):
+    """beta = 0.5, cold start, 128 x 128 (not resident: one launch per half-sweep, CUDA-graph replayed)."""
+    S = P.SpinSystem((128, 128, 1), storage="int8", replicas=8, replica_streams=1, seed=7, init=P.INIT_COLD)
+    e, m = _recorded_means(S, 0.5, 500, 6000, chunk=1000)
+    em, ee = _mean_err(e)
+    mm, me = _mean_err(m)
+    assert ee < 5e-4 and me < 5e-4
+    assert abs(em - X.onsager_energy_per_spin(0.5)) < 3 * ee + 2e-5, (em, ee)
+    assert abs(mm - X.yang_magnetisation(0.5)) < 3 * me + 1e-4, (mm, me)
+
+
+@pytest.mark.parametrize("rule", ["metropolis", "heatbath"])
+def test_4x4_energy_histogram_matches_exact_enumeration(P, rule):
+    """60 000 independent 4 x 4 lattices (generic kernel), one sample each after 80 sweeps: multinomial test of the
+    energy histogram against the brute-force Boltzmann weights; 2 % off in beta must fail."""
+    dims = (4, 4, 1)
+    PE = X.boltzmann_moments(dims, BETA_C2)[3]
+    for beta, must_pass in ((BETA_C2, True), (1.02 * BETA_C2, False)):
+        S = P.SpinSystem(dims, storage="int8", replicas=60000, replica_streams=1, seed=99, rule=rule)
+        S.sweep(beta, 80)
+        E, _ = S.measure()
+        worst, chi2 = check_histogram(E, PE)
+        if must_pass:
+            assert worst < 3.5 and chi2 < 2.5, (worst, chi2)
+        else:
+            assert worst > 8.0
+
+
+def test_3d_ising_high_temperature_series(P):
+    val, nxt = X.sc_ising_series_minus_e(0.1)
+    S = P.SpinSystem((64, 16, 16), storage="bitpack", replicas=8, replica_streams=1, seed=3)
+    e, _ = _recorded_means(S, 0.1, 200, 4000, chunk=1000)
+    mean, err = _mean_err(-e)
+    assert err < 2e-4
+    assert abs(mean - val) < 3 * err + nxt, (mean, err, val, nxt)
+
+
+@pytest.mark.parametrize("n,K,rule", [(2, 1.0, "metropolis"), (3, 1.0, "metropolis"), (3, 2.0, "heatbath")])
+def test_vector_chains_closed_form(P, n, K, rule):
+    """couplings (1, 0, 0): independent periodic chains of length 64: I_1/I_0 (n = 2), coth K - 1/K (n = 3)."""
+    S = P.SpinSystem((64, 64, 1), n=n, storage="fp32", coupling="per_direction", J=(1.0, 0.0, 0.0), replicas=8,
+                     replica_streams=1, seed=10 + n, rule=rule)
+    e, _ = _recorded_means(S, K, 500, 4000, chunk=1000)
+    mean, err = _mean_err(-e)
+    exact = X.chain_bond_average(n, K, 64)
+    assert err < 1.5e-3
+    assert abs(mean - exact) < 3 * err, (n, K, mean, err, exact)
+
+
+@pytest.mark.parametrize("n,beta", [(3, 0.693), (2, 0.4542)])
+def test_long_run_averages_agree_with_the_oracle(P, oracle, n, beta):
+    """north_star: long-run <E> and <|m|> of the library and of the oracle within 3 standard errors, 8^3 lattice,
+    once with the same seed (the two chains then differ only through rare rounding-level decisions) and once with
+    independent seeds."""
+    dims, R, therm, sweeps = (8, 8, 8), 8, 300, 1500
+    O = oracle.System(dims, n=n, n_replicas=R, replica_streams=1, seed=41)
+    O.sweep(beta, therm)
+    eo, mo = np.zeros(R), np.zeros(R)
+    for _ in range(sweeps):
+        O.sweep(beta, 1)
+        E, M = O.measure()
+        eo += E
+        mo += np.sqrt((M ** 2).sum(axis=1))
+    eo, mo = eo / sweeps / 512, mo / sweeps / 512
+    for seed in (41, 4242):
+        S = P.SpinSystem(dims, n=n, storage="fp32", replicas=R, replica_streams=1, seed=seed)
+        eg, mg = _recorded_means(S, beta, therm, sweeps, chunk=500)
+        for a, b, what in ((eg, eo, "e"), (mg, mo, "|m|")):
+            (ma, ea), (mb, eb) = _mean_err(a), _mean_err(b)
+            assert abs(ma - mb) < 3 * np.hypot(ea, eb) + 1e-6, (n, seed, what, ma, ea, mb, eb)
