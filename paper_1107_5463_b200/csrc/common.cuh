@@ -37,14 +37,6 @@ __host__ __device__ __forceinline__ uint32_t make_tag(uint32_t colour, uint32_t 
     return colour + 16u * domain + 256u * call;
 }
 
-// Sweep index (the Philox counter word t) of a launch.  Plain launches carry it in the argument block; launches
-// replayed from a CUDA graph carry only their offset inside the graph and add the handle's counter, which lives in
-// device memory and is advanced by the last node of the graph.
-template <class Args>
-__device__ __forceinline__ uint32_t sweep_index(const Args &a) {
-    return a.t_base ? a.t + __ldg(a.t_base) : a.t;
-}
-
 // ---------------------------------------------------------------------------------------------
 // Division by a run-time constant fixed at handle creation: q = (n * mul) >> (32 + shift) for
 // n < 2^31 (round-up method).  Two instructions instead of ~20.

@@ -180,7 +180,7 @@ __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(cons
             if (D == 3) { av[4] = s ^ o_zm; av[5] = s ^ o_zp; }
             const uint32_t unit = unit0 + (uint32_t)k * WX;
             if (D == 2) { av[4] = 0u; av[5] = 0u; }
-            int8_store_unit(mine + zoff + off, ising_new_word<D, HB>(a, sweep_index(a), a.colour, unit, rho, raw, av));
+            int8_store_unit(mine + zoff + off, ising_new_word<D, HB>(a, a.t, a.colour, unit, rho, raw, av));
             o_prev = o_cur;
             o_cur = o_next;
             p ^= 1u;

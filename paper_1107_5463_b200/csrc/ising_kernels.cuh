@@ -16,7 +16,6 @@ struct IsingArgs {
     void *s[2];          // per colour: int8 -> uint8_t [R][Nh] (0 = +1, 1 = -1); bitpack -> uint32_t [R][NW]
     const void *bonds;   // bitpack: uint32_t [2][R][3][NW] (bit = 1: J = -1); generic: int8 [R][d][N] of +-1
     uint32_t R, replica_streams, t, colour;
-    const uint32_t *t_base;  // NULL, or device counter added to t (CUDA-graph replays; common.cuh sweep_index)
     int32_t coupling_kind;  // 0 uniform, 1 per direction, 2 per bond
     int32_t Jdir[3];        // generic kernel: coupling per direction in {-1, 0, +1}
     uint32_t jneg;          // fast kernels: 1 iff the uniform coupling is -1
@@ -165,7 +164,7 @@ __global__ void __launch_bounds__(256) ising_generic_halfsweep(const __grid_cons
             bool decided = false;
             for (int call = 0; call < 8 && !decided; ++call) {
                 uint32_t w[4];
-                philox4x32_10(unit, rho, sweep_index(a), make_tag(a.colour, DOM_ISING_UPDATE, call), a.keys, w);
+                philox4x32_10(unit, rho, a.t, make_tag(a.colour, DOM_ISING_UPDATE, call), a.keys, w);
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                     if (decided) continue;
@@ -246,7 +245,7 @@ __device__ __forceinline__ uint32_t bitpack_update_word(const IsingArgs &a, uint
         if (SHARED) flip = ge2 | (ge1 & ltf[0]) | ltf[1];
         else {
             const uint32_t m[2] = {ge1 & ~ge2, ~ge1};
-            flip = ge2 | lt_mask_select<2>(a, sweep_index(a), a.colour, gi + a.g.unit_off, a.replica_streams ? r : 0u, m);
+            flip = ge2 | lt_mask_select<2>(a, a.t, a.colour, gi + a.g.unit_off, a.replica_streams ? r : 0u, m);
         }
     } else {
         const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
@@ -257,7 +256,7 @@ __device__ __forceinline__ uint32_t bitpack_update_word(const IsingArgs &a, uint
         if (SHARED) flip = ge3 | ((b1 | b2) & ltf[0]) | ((b0 | b1 | b2) & ltf[1]) | ltf[2];
         else {
             const uint32_t m[3] = {b1 & ~b0 & ~b2, b0 & ~b1 & ~b2, ~(b0 | b1 | b2)};
-            flip = ge3 | lt_mask_select<3>(a, sweep_index(a), a.colour, gi + a.g.unit_off, a.replica_streams ? r : 0u, m);
+            flip = ge3 | lt_mask_select<3>(a, a.t, a.colour, gi + a.g.unit_off, a.replica_streams ? r : 0u, m);
         }
     }
     return raw ^ flip;
@@ -280,7 +279,7 @@ __global__ void __launch_bounds__(256) ising_bitpack_halfsweep(const __grid_cons
             // gridDim.y > 1: the replicas are split into gridDim.y chunks (many realisations of a small lattice)
             const uint32_t chunk = (a.R + gridDim.y - 1) / gridDim.y;
             const uint32_t r0 = blockIdx.y * chunk, r1 = min(a.R, r0 + chunk);
-            lt_masks_full<NT>(a, sweep_index(a), a.colour, gi + a.g.unit_off, 0u, ltf);
+            lt_masks_full<NT>(a, a.t, a.colour, gi + a.g.unit_off, 0u, ltf);
             for (uint32_t r = r0; r < r1; ++r)
                 mine_base[(size_t)r * NW + gi] = bitpack_update_word<D, BONDS, true>(a, r, gi, n, ltf);
         } else {
@@ -301,7 +300,7 @@ __global__ void __launch_bounds__(256) ising_bitpack_halfsweep_hb(const __grid_c
     for (uint32_t gi = blockIdx.x * blockDim.x + threadIdx.x; gi < NW; gi += gridDim.x * blockDim.x) {
         const WordNbrs n = word_neighbours<D>(a.g, a.colour, gi);
         uint32_t ltf[NT];
-        if (SHARED) lt_masks_full<NT, true>(a, sweep_index(a), a.colour, gi + a.g.unit_off, 0u, ltf);
+        if (SHARED) lt_masks_full<NT, true>(a, a.t, a.colour, gi + a.g.unit_off, 0u, ltf);
         const uint32_t chunk = SHARED ? (a.R + gridDim.y - 1) / gridDim.y : a.R;
         const uint32_t r0 = SHARED ? blockIdx.y * chunk : 0u, r1 = min(a.R, r0 + chunk);
         for (uint32_t r = r0; r < r1; ++r) {
@@ -316,7 +315,7 @@ __global__ void __launch_bounds__(256) ising_bitpack_halfsweep_hb(const __grid_c
 #pragma unroll
                 for (int k = 0; k < NT; ++k) up |= m[k] & ltf[k];
             } else {
-                up = lt_mask_select<NT, true>(a, sweep_index(a), a.colour, gi + a.g.unit_off, a.replica_streams ? r : 0u, m);
+                up = lt_mask_select<NT, true>(a, a.t, a.colour, gi + a.g.unit_off, a.replica_streams ? r : 0u, m);
             }
             mine_base[(size_t)r * NW + gi] = ~up;
         }

@@ -43,7 +43,6 @@ struct Layout {
     size_t off_bonds, bytes_bonds;
     size_t off_acc, bytes_acc;  // n = 1: int64 [R][2]; n >= 2: double [R][mblocks][1 + n]
     size_t off_res, bytes_res;  // double [R] E then [R][n] M
-    size_t off_t;               // uint32: sweep counter read by graph-replayed launches
     size_t total;
 };
 
@@ -72,6 +71,9 @@ struct spin_system {
     IsingTable tab;
     HeatBathTable hb;    // n = 1 heat bath: built with the table above
     cudaGraphExec_t gexec;      // GRAPH_SWEEPS sweeps for (g_beta, launch shape); NULL until first used
+    cudaGraph_t graph;          // the captured graph (its node handles address the kernel nodes of gexec)
+    struct GraphNode *gnodes;   // its kernel nodes with host copies of their argument blocks
+    size_t n_gnodes;
     cudaStream_t cap_stream;    // capture-only stream (nothing ever runs on it)
     double g_beta;
     int g_block, g_rows, g_rows_set, g_num, g_den;
@@ -190,7 +192,6 @@ static void make_layout(const spin_config *c, const Derived &dv, Layout *l, uint
     l->off_acc = off; off += align_up(l->bytes_acc);
     l->bytes_res = (size_t)(R * (1 + c->n) * sizeof(double));
     l->off_res = off; off += align_up(l->bytes_res);
-    l->off_t = off; off += 256;
     l->total = off;
 }
 
@@ -262,7 +263,7 @@ static IsingArgs ising_args(const spin_system *s) {
     a.s[1] = s->ws + s->lay.off_s[1];
     a.bonds = s->lay.bytes_bonds ? s->ws + s->lay.off_bonds : nullptr;
     a.R = s->R; a.replica_streams = s->cfg.replica_streams ? 1u : 0u;
-    a.t = (uint32_t)s->t; a.colour = 0; a.t_base = nullptr;
+    a.t = (uint32_t)s->t; a.colour = 0;
     a.coupling_kind = s->cfg.coupling_kind;
     for (int mu = 0; mu < 3; ++mu)
         a.Jdir[mu] = s->cfg.coupling_kind == SPIN_J_UNIFORM ? (int)s->cfg.J[0]
@@ -279,7 +280,7 @@ static VectorArgs vector_args(const spin_system *s, double beta) {
     a.s[0] = (float *)(s->ws + s->lay.off_s[0]);
     a.s[1] = (float *)(s->ws + s->lay.off_s[1]);
     a.R = s->R; a.replica_streams = s->cfg.replica_streams ? 1u : 0u;
-    a.t = (uint32_t)s->t; a.colour = 0; a.t_base = nullptr;
+    a.t = (uint32_t)s->t; a.colour = 0;
     for (int mu = 0; mu < 3; ++mu)
         a.Jdir[mu] = s->cfg.coupling_kind == SPIN_J_UNIFORM ? (float)s->cfg.J[0] : (mu < s->d ? (float)s->cfg.J[mu] : 0.0f);
     a.beta = (float)beta;
@@ -388,13 +389,11 @@ static spin_status launch_halfsweep_vector(spin_system *s, const VectorArgs &a, 
     return SPIN_OK;
 }
 
-// One sweep.  t_base == NULL: an ordinary sweep at the handle's counter, which then advances.  Otherwise (graph
-// capture) the launches carry the offset t_rel and read the counter from device memory; the handle is not advanced.
-static spin_status enqueue_sweep(spin_system *s, double beta, cudaStream_t st, const uint32_t *t_base = nullptr,
-                                 uint32_t t_rel = 0) {
+// One sweep at sweep index t_override (graph capture: the handle is not advanced) or at the handle's counter.
+static spin_status enqueue_sweep(spin_system *s, double beta, cudaStream_t st, bool capture = false, uint32_t t_override = 0) {
     if (s->n == 1) {
         IsingArgs a = ising_args(s);
-        if (t_base) { a.t = t_rel; a.t_base = t_base; }
+        if (capture) a.t = t_override;
         for (uint32_t colour = 0; colour < 2; ++colour) {
             a.colour = colour;
             spin_status rc = launch_halfsweep_ising(s, a, st);
@@ -402,25 +401,32 @@ static spin_status enqueue_sweep(spin_system *s, double beta, cudaStream_t st, c
         }
     } else {
         VectorArgs a = vector_args(s, beta);
-        if (t_base) { a.t = t_rel; a.t_base = t_base; }
+        if (capture) a.t = t_override;
         for (uint32_t colour = 0; colour < 2; ++colour) {
             a.colour = colour;
             spin_status rc = launch_halfsweep_vector(s, a, st);
             if (rc != SPIN_OK) return rc;
         }
     }
-    if (!t_base) s->t += 1;
+    if (!capture) s->t += 1;
     return SPIN_OK;
 }
 
 // ------------------------------------------------------------------------- CUDA graphs -------
 // Lattices between the resident kernel's limit and a few million sites are launch-bound: a half-sweep takes less
 // time than its launch (the argument block with the tables is ~3 KB).  spin_sweep then replays a graph of
-// GRAPH_SWEEPS sweeps whose nodes read the sweep counter from device memory; its last node advances the counter.
+// GRAPH_SWEEPS sweeps.  The kernels are the ordinary ones (the sweep index is an ordinary kernel argument, so the large
+// lattices pay nothing for this): before each replay the host rewrites that one argument of every kernel node
+// (cudaGraphExecKernelNodeSetParams), which costs about a microsecond per node and runs ahead of the GPU.
 constexpr int GRAPH_SWEEPS = 16;
 
-__global__ void counter_set(uint32_t *t, uint32_t v) { *t = v; }
-__global__ void counter_add(uint32_t *t, uint32_t v) { *t += v; }
+struct GraphNode {
+    cudaGraphNode_t node;
+    cudaKernelNodeParams params;   // kernelParams is re-pointed at `args` before every update
+    uint32_t k;                    // sweep offset of this launch inside the graph
+    union { IsingArgs ising; VectorArgs vec; } args;
+    GraphNode() {}
+};
 
 static bool graph_ok(const spin_system *s, int64_t n_sweeps) {
     if (s->vector_generic || s->axis >= 0 || n_sweeps < 2 * GRAPH_SWEEPS) return false;
@@ -429,26 +435,51 @@ static bool graph_ok(const spin_system *s, int64_t n_sweeps) {
     return s->N * s->R / 2 / per_thread <= (uint64_t)s->sm_count * 2048 * 2;
 }
 
+static void graph_drop(spin_system *s) {
+    if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
+    if (s->graph) { cudaGraphDestroy(s->graph); s->graph = nullptr; }
+    delete[] s->gnodes; s->gnodes = nullptr; s->n_gnodes = 0; s->graph = nullptr;
+}
+
 static spin_status graph_prepare(spin_system *s, double beta) {
     const bool same = s->gexec && s->g_beta == beta && s->g_block == s->block && s->g_rows == s->strip_rows &&
                       s->g_rows_set == s->strip_rows_set && s->g_num == s->grid_num && s->g_den == s->grid_den;
     if (same) return SPIN_OK;
-    if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
+    graph_drop(s);
     if (!s->cap_stream) CUDA_TRY(cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
-    uint32_t *d_t = (uint32_t *)(s->ws + s->lay.off_t);
     const uint64_t launches0 = s->launches;
     CUDA_TRY(cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
     spin_status rc = SPIN_OK;
-    for (int k = 0; k < GRAPH_SWEEPS && rc == SPIN_OK; ++k) rc = enqueue_sweep(s, beta, s->cap_stream, d_t, (uint32_t)k);
-    counter_add<<<1, 1, 0, s->cap_stream>>>(d_t, (uint32_t)GRAPH_SWEEPS);
+    for (int k = 0; k < GRAPH_SWEEPS && rc == SPIN_OK; ++k) rc = enqueue_sweep(s, beta, s->cap_stream, true, (uint32_t)k);
     cudaGraph_t graph = nullptr;
     cudaError_t e = cudaStreamEndCapture(s->cap_stream, &graph);
     s->launches = launches0;   // capturing launched nothing
     if (rc != SPIN_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
     if (e != cudaSuccess) return fail(SPIN_ERR_CUDA, "graph capture: %s", cudaGetErrorString(e));
-    e = cudaGraphInstantiate(&s->gexec, graph, 0);
-    cudaGraphDestroy(graph);
-    if (e != cudaSuccess) { s->gexec = nullptr; return fail(SPIN_ERR_CUDA, "graph instantiate: %s", cudaGetErrorString(e)); }
+    // every kernel node with a copy of its argument block; the captured sweep offset is read back from that block
+    size_t n_nodes = 0;
+    e = cudaGraphGetNodes(graph, nullptr, &n_nodes);
+    cudaGraphNode_t *nodes = (e == cudaSuccess && n_nodes) ? new (std::nothrow) cudaGraphNode_t[n_nodes] : nullptr;
+    s->gnodes = nodes ? new (std::nothrow) GraphNode[n_nodes] : nullptr;
+    if (e == cudaSuccess && (!nodes || !s->gnodes)) e = cudaErrorMemoryAllocation;
+    if (e == cudaSuccess) e = cudaGraphGetNodes(graph, nodes, &n_nodes);
+    for (size_t i = 0; e == cudaSuccess && i < n_nodes; ++i) {
+        cudaGraphNodeType type;
+        e = cudaGraphNodeGetType(nodes[i], &type);
+        if (e != cudaSuccess || type != cudaGraphNodeTypeKernel) continue;
+        GraphNode &gn = s->gnodes[s->n_gnodes];
+        gn.node = nodes[i];
+        e = cudaGraphKernelNodeGetParams(nodes[i], &gn.params);
+        if (e != cudaSuccess) break;
+        if (s->n == 1) { std::memcpy(&gn.args.ising, gn.params.kernelParams[0], sizeof(IsingArgs)); gn.k = gn.args.ising.t; }
+        else { std::memcpy(&gn.args.vec, gn.params.kernelParams[0], sizeof(VectorArgs)); gn.k = gn.args.vec.t; }
+        s->n_gnodes += 1;
+    }
+    delete[] nodes;
+    if (e == cudaSuccess && s->n_gnodes != 2 * GRAPH_SWEEPS) e = cudaErrorUnknown;
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&s->gexec, graph, 0);
+    s->graph = graph;   // kept: node handles stay valid as long as it lives
+    if (e != cudaSuccess) { s->gexec = nullptr; graph_drop(s); return fail(SPIN_ERR_CUDA, "graph build: %s", cudaGetErrorString(e)); }
     s->g_beta = beta; s->g_block = s->block; s->g_rows = s->strip_rows; s->g_rows_set = s->strip_rows_set;
     s->g_num = s->grid_num; s->g_den = s->grid_den;
     return SPIN_OK;
@@ -459,14 +490,19 @@ static spin_status graph_sweeps(spin_system *s, double beta, int64_t n_sweeps, c
     *done = 0;
     spin_status rc = graph_prepare(s, beta);
     if (rc != SPIN_OK) return rc;
-    uint32_t *d_t = (uint32_t *)(s->ws + s->lay.off_t);
-    counter_set<<<1, 1, 0, st>>>(d_t, (uint32_t)s->t);
-    CUDA_TRY(cudaGetLastError());
-    s->launches += 1;
     while (n_sweeps - *done >= GRAPH_SWEEPS) {
+        for (size_t i = 0; i < s->n_gnodes; ++i) {
+            GraphNode &gn = s->gnodes[i];
+            void *argp[1];
+            if (s->n == 1) { gn.args.ising.t = (uint32_t)s->t + gn.k; argp[0] = &gn.args.ising; }
+            else { gn.args.vec.t = (uint32_t)s->t + gn.k; argp[0] = &gn.args.vec; }
+            gn.params.kernelParams = argp;
+            gn.params.extra = nullptr;
+            CUDA_TRY(cudaGraphExecKernelNodeSetParams(s->gexec, gn.node, &gn.params));
+        }
         CUDA_TRY(cudaGraphLaunch(s->gexec, st));
         s->t += GRAPH_SWEEPS;
-        s->launches += 2 * GRAPH_SWEEPS + 1;
+        s->launches += 2 * GRAPH_SWEEPS;
         *done += GRAPH_SWEEPS;
     }
     return SPIN_OK;
@@ -591,7 +627,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
         return fail(SPIN_ERR_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, %zu needed", bytes, need);
     }
     s->ws = (char *)d_workspace;
-    s->t = 0; s->launches = 0; s->staging = nullptr; s->staging_bytes = 0; s->gexec = nullptr; s->cap_stream = nullptr;
+    s->t = 0; s->launches = 0; s->staging = nullptr; s->staging_bytes = 0; s->gexec = nullptr; s->cap_stream = nullptr; s->gnodes = nullptr; s->n_gnodes = 0;
     s->block = dv.path == PATH_ISING_INT8 ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0;
     s->table_beta = std::nan("");
     Geometry &g = s->g;
@@ -665,7 +701,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
 
 spin_status spin_destroy(spin_system *s) {
     if (s && s->staging) cudaFree(s->staging);
-    if (s && s->gexec) cudaGraphExecDestroy(s->gexec);
+    if (s) graph_drop(s);
     if (s && s->cap_stream) cudaStreamDestroy(s->cap_stream);
     delete s;
     return SPIN_OK;

@@ -16,7 +16,6 @@ struct VectorArgs {
     PhiloxKeys keys;
     float *s[2];          // per colour: float [R][NC][Nh]
     uint32_t R, replica_streams, t, colour;
-    const uint32_t *t_base;  // NULL, or device counter added to t (CUDA-graph replays)
     float Jdir[3];
     float beta;
     uint32_t rule;        // 0 Metropolis (Eq. (2)), 1 heat bath (n = 3 only)
@@ -115,7 +114,7 @@ __global__ void __launch_bounds__(256) vector_halfsweep(const __grid_constant__ 
             }
         }
         uint32_t w[4];
-        philox4x32_10(j + g.j_off, a.replica_streams ? r : 0u, sweep_index(a), make_tag(a.colour, DOM_VECTOR_UPDATE, 0), a.keys, w);
+        philox4x32_10(j + g.j_off, a.replica_streams ? r : 0u, a.t, make_tag(a.colour, DOM_VECTOR_UPDATE, 0), a.keys, w);
         float sn[NC];
         uint32_t wacc;
         if (NC == 3 && a.rule != 0u) {
@@ -243,7 +242,7 @@ __global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_const
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 uint32_t w[4];
-                philox4x32_10(off + i + g.j_off, rho, sweep_index(a), tag, a.keys, w);
+                philox4x32_10(off + i + g.j_off, rho, a.t, tag, a.keys, w);
                 float sn[NC], so[NC];
                 uint32_t wacc;
                 if (HB && NC == 3) {
