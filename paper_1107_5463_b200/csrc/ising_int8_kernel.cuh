@@ -188,4 +188,65 @@ __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(cons
     }
 }
 
+// The same strip walk for BIT-PACKED storage with uniform couplings (own random stream per replica or one replica):
+// one thread per (replica, z, strip of K rows, word column w); words of the other colour are rolled through
+// registers over the rows, the loads of row k + 1 are issued before row k is computed, and the index arithmetic is
+// paid once per strip instead of once per word.  Results are bit-identical to ising_bitpack_halfsweep.
+template <int D, int K, bool HB = false>
+__global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __grid_constant__ IsingArgs a) {
+    const Geometry &g = a.g;
+    const uint32_t WX = g.WX, Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz;
+    const uint32_t nstrip = (Ly + K - 1) / K;
+    const uint32_t per_replica = WX * nstrip * Lz;
+    const uint32_t item = blockIdx.x * blockDim.x + threadIdx.x;
+    if (item >= per_replica * a.R) return;
+    const uint32_t r = item / per_replica, it = item - r * per_replica;
+    const uint32_t sz = fdiv(it, g.divWX), w = it - sz * WX;      // sz = strip + nstrip * z
+    const uint32_t z = sz / nstrip, y0 = (sz - z * nstrip) * K;
+    const uint32_t kend = min((uint32_t)K, Ly - y0);
+    const uint32_t *__restrict__ other = (const uint32_t *)a.s[1 - a.colour] + (size_t)r * g.NW;
+    uint32_t *mine = (uint32_t *)a.s[a.colour] + (size_t)r * g.NW;
+    const uint32_t rho = a.replica_streams ? r : 0u;
+    const uint32_t jflip = a.jneg ? 0xFFFFFFFFu : 0u;
+    const uint32_t plane = WX * Ly, zoff = z * plane;
+    const uint32_t zm_off = (D == 3) ? (z == 0 ? Lz - 1 : z - 1) * plane : 0u;
+    const uint32_t zp_off = (D == 3) ? (z == Lz - 1 ? 0u : z + 1) * plane : 0u;
+    const uint32_t w_next = w + 1u == WX ? 0u : w + 1u, w_prev = w == 0u ? WX - 1u : w - 1u;
+    const uint32_t ym0 = y0 == 0 ? Ly - 1 : y0 - 1;
+    uint32_t p = (y0 + z + a.colour) & 1u;
+    uint32_t o_prev = __ldg(other + zoff + ym0 * WX + w), o_cur = __ldg(other + zoff + y0 * WX + w);
+    uint32_t pf_next, pf_mine, pf_side, pf_zm = 0u, pf_zp = 0u;
+    {
+        const uint32_t yp = y0 + 1 == Ly ? 0u : y0 + 1, off = y0 * WX + w;
+        pf_next = __ldg(other + zoff + yp * WX + w);
+        pf_mine = __ldg(mine + zoff + off);
+        pf_side = __ldg(other + zoff + y0 * WX + (p ? w_next : w_prev));
+        if (D == 3) { pf_zm = __ldg(other + zm_off + off); pf_zp = __ldg(other + zp_off + off); }
+    }
+    const uint32_t unit0 = (y0 + Ly * z) * WX + w + g.unit_off;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        if ((uint32_t)k < kend) {
+            const uint32_t y = y0 + k, off = y * WX + w;
+            const uint32_t o_next = pf_next, raw = pf_mine, o_zm = pf_zm, o_zp = pf_zp;
+            const uint32_t side = p ? ((o_cur >> 1) | (pf_side << 31)) : ((o_cur << 1) | (pf_side >> 31));
+            if (k + 1 < K && (uint32_t)(k + 1) < kend) {
+                const uint32_t y1 = y + 1, y2 = y1 + 1 == Ly ? 0u : y1 + 1, off1 = y1 * WX + w;
+                pf_next = __ldg(other + zoff + y2 * WX + w);
+                pf_mine = __ldg(mine + zoff + off1);
+                pf_side = __ldg(other + zoff + y1 * WX + (p ? w_prev : w_next));   // row y + 1 has the other parity
+                if (D == 3) { pf_zm = __ldg(other + zm_off + off1); pf_zp = __ldg(other + zp_off + off1); }
+            }
+            const uint32_t s = raw ^ jflip;
+            uint32_t av[6];
+            av[0] = s ^ o_cur; av[1] = s ^ side; av[2] = s ^ o_prev; av[3] = s ^ o_next;
+            av[4] = D == 3 ? s ^ o_zm : 0u; av[5] = D == 3 ? s ^ o_zp : 0u;
+            mine[zoff + off] = ising_new_word<D, HB>(a, a.t, a.colour, unit0 + (uint32_t)k * WX, rho, raw, av);
+            o_prev = o_cur;
+            o_cur = o_next;
+            p ^= 1u;
+        }
+    }
+}
+
 }  // namespace spin

@@ -314,6 +314,23 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
         else if (s->d == 2) { if (K == 1) I8(2, 1); else if (K == 2) I8(2, 2); else if (K == 4) I8(2, 4); else if (K == 8) I8(2, 8); else I8(2, 16); }
         else { if (K == 1) I8(3, 1); else if (K == 2) I8(3, 2); else if (K == 4) I8(3, 4); else if (K == 8) I8(3, 8); else I8(3, 16); }
 #undef I8
+    } else if (!bonds && !shared && !s->vector_generic) {
+        // uniform couplings, own random numbers per word: the strip kernel (K rows per thread, as for int8)
+        int K = s->strip_rows_set ? s->strip_rows : 0;
+        if (!K) {
+            const uint64_t threads4 = (uint64_t)s->g.WX * ((s->g.Ly + 3) / 4) * s->g.Lz * s->R;
+            K = threads4 >= (uint64_t)s->sm_count * 2048 ? 4 : 1;
+        }
+        if (K > 4) K = 4;
+        const int Bs = B > 128 ? 128 : B;
+        const uint64_t items = (uint64_t)s->g.WX * ((s->g.Ly + K - 1) / K) * s->g.Lz * s->R;
+        const int G = (int)((items + Bs - 1) / Bs);
+        const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
+#define BS3(D_, K_) do { if (hb) ising_bitpack_strip_halfsweep<D_, K_, true><<<G, Bs, 0, st>>>(a); else ising_bitpack_strip_halfsweep<D_, K_, false><<<G, Bs, 0, st>>>(a); } while (0)
+#define BS2(D_) do { if (K == 1) BS3(D_, 1); else if (K == 2) BS3(D_, 2); else BS3(D_, 4); } while (0)
+        if (s->d == 2) BS2(2); else BS2(3);
+#undef BS2
+#undef BS3
     } else {
         // shared update stream: chunks of >= 16 replicas per thread (the masks of a word are built once per chunk);
         // more chunks only when the lattice alone cannot fill the GPU (many realisations of a small lattice)
