@@ -315,7 +315,8 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
         else { if (K == 1) I8(3, 1); else if (K == 2) I8(3, 2); else if (K == 4) I8(3, 4); else if (K == 8) I8(3, 8); else I8(3, 16); }
 #undef I8
     } else if (!bonds && !shared && !s->vector_generic) {
-        // uniform couplings, own random numbers per word: the strip kernel (K rows per thread, as for int8)
+        // uniform couplings, own random numbers per word: the strip kernel (K rows per thread, as for int8;
+        // measured at L = 16384: 65.7 / 61.6 / 58.4 / 65.8 / 71.9 us for K = 1 / 2 / 4 / 8 / 16)
         int K = s->strip_rows_set ? s->strip_rows : 0;
         if (!K) {
             const uint64_t threads4 = (uint64_t)s->g.WX * ((s->g.Ly + 3) / 4) * s->g.Lz * s->R;
