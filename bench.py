@@ -358,18 +358,19 @@ def run_graft(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
-TRAFFIC = {  # profiles/r01c_all_kernels.md
-    "ising2d_L16384_int8": 362233344,      # 268.50 MB read + 93.74 MB written
-    "ising2d_L16384_bitpack": 33575680,    # state L2-resident: one read pass, no write-back inside the launch
-    "ising3d_L512_bitpack": 16801536,
-    "ea3d_L256_R16_bitpack": 144219648,
-    "heisenberg3d_L256_fp32": 265815808,
-    "xy3d_L256_fp32": 166819584,
+TRAFFIC = {  # profiles/r01d_all_kernels.md
+    "ising2d_L16384_int8": 362360064,      # 268.50 MB read + 93.86 MB written
+    "ising2d_L16384_bitpack": 33593088,    # state L2-resident: one read pass, no write-back inside the launch
+    "ising3d_L512_bitpack": 16820224,
+    "ea3d_L256_R16_bitpack": 144403456,
+    "ea2d_L64_R4096_bitpack": 6305280,
+    "heisenberg3d_L256_fp32": 266009856,
+    "xy3d_L256_fp32": 166662144,
 }
 # Executed warp-instructions per half-sweep launch (smsp__inst_executed.sum of the same captures), for the kernels whose
 # bound is integer arithmetic rather than HBM; the peak they are set against is the issue rate
 # 148 SMs x 4 sub-cores x 1 warp-instruction per clock x 1.965 GHz.
-WARP_INSTR = {"ising2d_L16384_bitpack": 40863300, "ising3d_L512_bitpack": 23410766}   # profiles/r01d_all_kernels.md
+WARP_INSTR = {"ising2d_L16384_bitpack": 38098807, "ising3d_L512_bitpack": 21948915}
 ISSUE_PEAK_GWIPS = 148 * 4 * 1.965
 
 
