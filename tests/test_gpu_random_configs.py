@@ -26,7 +26,7 @@ def _draw(rng):
     Ly = 2 * int(rng.integers(1, 12))
     Lz = 2 * int(rng.integers(1, 6)) if d3 else 1
     n = int(rng.choice([1, 1, 1, 2, 3]))
-    cfg = dict(dims=(Lx, Ly, Lz), n=n, seed=int(rng.integers(0, 2 ** 62)), R=int(rng.choice([1, 1, 2, 3, 5])),
+    cfg = dict(dims=(Lx, Ly, Lz), n=n, seed=int(rng.integers(0, 2 ** 62)), R=int(rng.choice([1, 1, 2, 3, 4, 5, 8])),
                streams=int(rng.integers(0, 2)), beta=float(rng.choice([0.0, 0.1, 0.2216546, 0.4406868, 0.7, 1.3, 5.0])),
                init=int(rng.integers(0, 2)))
     if n == 1:
