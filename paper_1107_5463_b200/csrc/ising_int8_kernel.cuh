@@ -87,6 +87,28 @@ __device__ __forceinline__ uint32_t ising_new_word(const IsingArgs &a, uint32_t 
     }
 }
 
+// Fused measurement: every bond joins the two colours, so the colour-1 half-sweep
+// has, in the masks it formed anyway, everything E and M need.  Per 32-site word of colour 1 after its update:
+// E += 2 (#unsatisfied bonds) - (#bonds), M += 64 - 2 (minus spins of this word and of the colour-0 word at the same
+// index).  Lanes of a warp that serve the same replica are summed with one warp reduction, then one atomic each.
+template <int D>
+__device__ __forceinline__ void fused_word_sums(const uint32_t av[6], uint32_t raw, uint32_t fresh, uint32_t o_same, int &e, int &m) {
+    const uint32_t flip = raw ^ fresh;   // a flipped lane inverts all its bond masks
+    int unsat = __popc(av[0] ^ flip) + __popc(av[1] ^ flip) + __popc(av[2] ^ flip) + __popc(av[3] ^ flip);
+    if (D == 3) unsat += __popc(av[4] ^ flip) + __popc(av[5] ^ flip);
+    e += 2 * unsat - 2 * D * 32;
+    m += 64 - 2 * (__popc(fresh) + __popc(o_same));
+}
+__device__ __forceinline__ void fused_commit(long long *acc, uint32_t r, int e, int m) {
+    const unsigned active = __activemask();
+    const unsigned peers = __match_any_sync(active, r);
+    const int es = __reduce_add_sync(peers, e), ms = __reduce_add_sync(peers, m);
+    if ((threadIdx.x & 31u) == (uint32_t)(__ffs(peers) - 1)) {
+        atomicAdd((unsigned long long *)&acc[2 * r], (unsigned long long)(long long)es);
+        atomicAdd((unsigned long long *)&acc[2 * r + 1], (unsigned long long)(long long)ms);
+    }
+}
+
 // the 32 bytes of a unit as loaded, before packing (kept in flight while the previous row is being updated)
 struct Int8RawUnit {
     uint4 lo, hi;
@@ -119,7 +141,7 @@ __device__ __forceinline__ uint32_t int8_side_byte(const uint8_t *rowp, uint32_t
 // update of row k is computed, so their latency hides behind the Philox / bit-slice work.
 // At most 128 threads per CTA; d = 2: 7 CTAs per SM, i.e. at most 72 registers (one more costs a whole CTA of occupancy:
 // measured 72.6 vs 75.0 us at L = 16384).
-template <int D, int K, bool HB = false>
+template <int D, int K, bool HB = false, bool MEAS = false>
 __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(const __grid_constant__ IsingArgs a) {
     const Geometry &g = a.g;
     const uint32_t WX = g.WX, Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz;
@@ -156,6 +178,7 @@ __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(cons
     }
     uint32_t o_prev = int8_pack_raw(r_prev), o_cur = int8_pack_raw(r_cur);
     const uint32_t unit0 = (y0 + Ly * z) * WX + w + g.unit_off;   // global Philox unit of row y0 (slab offset included)
+    int e_sum = 0, m_sum = 0;
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         if ((uint32_t)k < kend) {
@@ -180,19 +203,22 @@ __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(cons
             if (D == 3) { av[4] = s ^ o_zm; av[5] = s ^ o_zp; }
             const uint32_t unit = unit0 + (uint32_t)k * WX;
             if (D == 2) { av[4] = 0u; av[5] = 0u; }
-            int8_store_unit(mine + zoff + off, ising_new_word<D, HB>(a, a.t, a.colour, unit, rho, raw, av));
+            const uint32_t fresh = ising_new_word<D, HB>(a, a.t, a.colour, unit, rho, raw, av);
+            int8_store_unit(mine + zoff + off, fresh);
+            if (MEAS) fused_word_sums<D>(av, raw, fresh, o_cur, e_sum, m_sum);
             o_prev = o_cur;
             o_cur = o_next;
             p ^= 1u;
         }
     }
+    if (MEAS) fused_commit(a.acc, r, e_sum, m_sum);
 }
 
 // The same strip walk for BIT-PACKED storage with uniform couplings (own random stream per replica or one replica):
 // one thread per (replica, z, strip of K rows, word column w); words of the other colour are rolled through
 // registers over the rows, the loads of row k + 1 are issued before row k is computed, and the index arithmetic is
 // paid once per strip instead of once per word.  Results are bit-identical to ising_bitpack_halfsweep.
-template <int D, int K, bool HB = false>
+template <int D, int K, bool HB = false, bool MEAS = false>
 __global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __grid_constant__ IsingArgs a) {
     const Geometry &g = a.g;
     const uint32_t WX = g.WX, Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz;
@@ -224,6 +250,7 @@ __global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __gri
         if (D == 3) { pf_zm = __ldg(other + zm_off + off); pf_zp = __ldg(other + zp_off + off); }
     }
     const uint32_t unit0 = (y0 + Ly * z) * WX + w + g.unit_off;
+    int e_sum = 0, m_sum = 0;
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         if ((uint32_t)k < kend) {
@@ -241,12 +268,15 @@ __global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __gri
             uint32_t av[6];
             av[0] = s ^ o_cur; av[1] = s ^ side; av[2] = s ^ o_prev; av[3] = s ^ o_next;
             av[4] = D == 3 ? s ^ o_zm : 0u; av[5] = D == 3 ? s ^ o_zp : 0u;
-            mine[zoff + off] = ising_new_word<D, HB>(a, a.t, a.colour, unit0 + (uint32_t)k * WX, rho, raw, av);
+            const uint32_t fresh = ising_new_word<D, HB>(a, a.t, a.colour, unit0 + (uint32_t)k * WX, rho, raw, av);
+            mine[zoff + off] = fresh;
+            if (MEAS) fused_word_sums<D>(av, raw, fresh, o_cur, e_sum, m_sum);
             o_prev = o_cur;
             o_cur = o_next;
             p ^= 1u;
         }
     }
+    if (MEAS) fused_commit(a.acc, r, e_sum, m_sum);
 }
 
 }  // namespace spin

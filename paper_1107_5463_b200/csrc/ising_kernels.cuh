@@ -20,6 +20,7 @@ struct IsingArgs {
     int32_t Jdir[3];        // generic kernel: coupling per direction in {-1, 0, +1}
     uint32_t jneg;          // fast kernels: 1 iff the uniform coupling is -1
     uint32_t rule;          // 0 Metropolis (Eq. (2)), 1 heat bath
+    long long *acc;         // [R][2] energy / magnetisation accumulators (fused measurement of the strip kernels)
     HeatBathTable hb;       // filled when rule = 1
 };
 

@@ -271,6 +271,7 @@ static IsingArgs ising_args(const spin_system *s) {
     a.jneg = (s->cfg.coupling_kind == SPIN_J_UNIFORM && s->cfg.J[0] < 0.0) ? 1u : 0u;
     a.rule = s->cfg.update_rule == SPIN_UPDATE_HEATBATH ? 1u : 0u;
     a.hb = s->hb;
+    a.acc = (long long *)(s->ws + s->lay.off_acc);
     return a;
 }
 
@@ -289,10 +290,13 @@ static VectorArgs vector_args(const spin_system *s, double beta) {
 }
 
 // ----------------------------------------------------------------------------- launches ------
-static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cudaStream_t st) {
+// fused: NULL, or (colour 1 only) ask for E / M to be accumulated into a.acc by the half-sweep itself;
+// *fused tells whether the kernel that ran could do it (the strip kernels with 1 or 4 rows per thread).
+static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cudaStream_t st, bool *fused = nullptr) {
     const bool bonds = s->cfg.coupling_kind == SPIN_J_BOND_PM1;
     const bool shared = s->R > 1 && !s->cfg.replica_streams;
     const int B = s->path == PATH_ISING_INT8 && s->block > 128 ? 128 : s->block;   // the int8 kernel is built for <= 128 threads
+    if (fused) *fused = false;
     if (s->path == PATH_ISING_GENERIC) {
         ising_generic_halfsweep<<<grid_for(s, (uint64_t)s->g.Nh * s->R), B, 0, st>>>(a);
     } else if (s->path == PATH_ISING_INT8) {
@@ -309,6 +313,14 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
         if (hb) K = 4;
         const uint64_t items = (uint64_t)s->g.WX * ((s->g.Ly + K - 1) / K) * s->g.Lz * s->R;
         const int G = (int)((items + B - 1) / B);
+        if (fused && (K == 1 || K == 4) && a.colour == 1u) {
+            *fused = true;
+#define I8M(D_, K_, HB_) ising_int8_halfsweep<D_, K_, HB_, true><<<G, B, 0, st>>>(a)
+            if (hb) { if (s->d == 2) I8M(2, 4, true); else I8M(3, 4, true); }
+            else if (s->d == 2) { if (K == 1) I8M(2, 1, false); else I8M(2, 4, false); }
+            else { if (K == 1) I8M(3, 1, false); else I8M(3, 4, false); }
+#undef I8M
+        } else
 #define I8(D_, K_) ising_int8_halfsweep<D_, K_><<<G, B, 0, st>>>(a)
         if (hb) { if (s->d == 2) ising_int8_halfsweep<2, 4, true><<<G, B, 0, st>>>(a); else ising_int8_halfsweep<3, 4, true><<<G, B, 0, st>>>(a); }
         else if (s->d == 2) { if (K == 1) I8(2, 1); else if (K == 2) I8(2, 2); else if (K == 4) I8(2, 4); else if (K == 8) I8(2, 8); else I8(2, 16); }
@@ -329,7 +341,13 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
         const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
 #define BS3(D_, K_) do { if (hb) ising_bitpack_strip_halfsweep<D_, K_, true><<<G, Bs, 0, st>>>(a); else ising_bitpack_strip_halfsweep<D_, K_, false><<<G, Bs, 0, st>>>(a); } while (0)
 #define BS2(D_) do { if (K == 1) BS3(D_, 1); else if (K == 2) BS3(D_, 2); else BS3(D_, 4); } while (0)
+#define BM3(D_, K_) do { if (hb) ising_bitpack_strip_halfsweep<D_, K_, true, true><<<G, Bs, 0, st>>>(a); else ising_bitpack_strip_halfsweep<D_, K_, false, true><<<G, Bs, 0, st>>>(a); } while (0)
+        if (fused && (K == 1 || K == 4) && a.colour == 1u) {
+            *fused = true;
+            if (s->d == 2) { if (K == 1) BM3(2, 1); else BM3(2, 4); } else { if (K == 1) BM3(3, 1); else BM3(3, 4); }
+        } else
         if (s->d == 2) BS2(2); else BS2(3);
+#undef BM3
 #undef BS2
 #undef BS3
     } else {
@@ -752,10 +770,31 @@ spin_status spin_sweep_record(spin_system *s, double beta, int64_t n_sweeps, dou
     if (s->axis >= 0) return fail(SPIN_ERR_STATE, "slab handle: drive it with spin_halfsweep and the halo calls");
     if (s->next_colour != 0) return fail(SPIN_ERR_STATE, "a spin_halfsweep of colour 1 is pending");
     if (resident_ok(s, true)) return enqueue_resident(s, n_sweeps, d_E, d_M, (cudaStream_t)stream);
+    cudaStream_t st = (cudaStream_t)stream;
     for (int64_t k = 0; k < n_sweeps; ++k) {
-        rc = enqueue_sweep(s, beta, (cudaStream_t)stream);
-        if (rc != SPIN_OK) return rc;
-        rc = enqueue_measure(s, d_E + (size_t)k * s->R, d_M + (size_t)k * s->R * s->n, (cudaStream_t)stream);
+        double *oE = d_E + (size_t)k * s->R, *oM = d_M + (size_t)k * s->R * s->n;
+        if (s->n == 1 && !s->vector_generic) {
+            // E and M for free inside the colour-1 half-sweep where the kernel can (strip kernels), else a measurement pass
+            IsingArgs a = ising_args(s);
+            bool fused = false;
+            a.colour = 0;
+            rc = launch_halfsweep_ising(s, a, st);
+            if (rc != SPIN_OK) return rc;
+            a.colour = 1;
+            rc = launch_halfsweep_ising(s, a, st, &fused);
+            if (rc != SPIN_OK) return rc;
+            s->t += 1;
+            if (fused) {
+                ising_measure_finalize<<<(s->R + 63) / 64, 64, 0, st>>>(a.acc, s->R, oE, oM);
+                s->launches += 1;
+                CUDA_TRY(cudaGetLastError());
+                continue;
+            }
+        } else {
+            rc = enqueue_sweep(s, beta, st);
+            if (rc != SPIN_OK) return rc;
+        }
+        rc = enqueue_measure(s, oE, oM, st);
         if (rc != SPIN_OK) return rc;
     }
     return SPIN_OK;

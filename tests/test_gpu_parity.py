@@ -475,3 +475,24 @@ def test_graph_replayed_sweeps_vector(P, n):
         B.sweep(0.6, 1)              # never reaches the graph threshold
     assert np.array_equal(A.get_spins().view(np.uint32), B.get_spins().view(np.uint32))
     assert A.sweep_counter == B.sweep_counter == 37
+
+
+@pytest.mark.parametrize("dims,storage,J,R,rule", [((128, 600, 1), "int8", 1.0, 1, "metropolis"), ((128, 520, 1), "bitpack", -1.0, 2, "metropolis"),
+                                                   ((64, 70, 20), "bitpack", 1.0, 1, "heatbath"), ((64, 34, 22), "int8", 1.0, 3, "heatbath"),
+                                                   ((192, 300, 1), "int8", -1.0, 1, "metropolis")])
+def test_fused_measurement_in_recorded_sweeps(P, oracle, dims, storage, J, R, rule):
+    """spin_sweep_record beyond the resident kernel's limit: E and M are accumulated by the colour-1 half-sweep itself
+    (every bond joins the two colours) and must equal the oracle's sums after every sweep; warps that
+    straddle two replicas, ragged strips, antiferromagnet, both rules."""
+    import torch
+
+    beta = BETA_2D if dims[2] == 1 else BETA_3D
+    G, O = _pair(P, oracle, dims, storage=storage, J=(J, J, J), replicas=R, replica_streams=1, rule=rule)
+    dE, dM = G.sweep_record(beta, 6)
+    torch.cuda.synchronize()
+    Eg, Mg = dE.cpu().numpy(), dM.cpu().numpy()[:, :, 0]
+    for t in range(6):
+        O.sweep(beta, 1)
+        e, m = O.measure()
+        assert np.array_equal(Eg[t], e) and np.array_equal(Mg[t], m[:, 0]), (t, Eg[t], e, Mg[t], m[:, 0])
+    _assert_ising_equal(G, O, "after fused recorded sweeps")     # spin_measure (separate pass) agrees as well
