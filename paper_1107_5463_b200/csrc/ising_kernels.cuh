@@ -323,4 +323,69 @@ __global__ void __launch_bounds__(256) ising_bitpack_halfsweep_hb(const __grid_c
     }
 }
 
+// ------------------------------------------------------------------ +-J, shared stream, one thread per row of 4 words ----
+// Lx = 256 (BASELINE config 4): a row of one colour is exactly four 32-site words = one 128-bit access, and the
+// periodic x-neighbour of every word lies in the same four words.  One thread updates a whole row for all replicas
+// of its chunk: twelve 128-bit loads and one 128-bit store per replica, no scalar loads at all.
+__device__ __forceinline__ uint32_t u4c(const uint4 &v, int i) { return i == 0 ? v.x : (i == 1 ? v.y : (i == 2 ? v.z : v.w)); }
+
+template <bool HB>
+__global__ void __launch_bounds__(128) ising_pmj_row4_halfsweep(const __grid_constant__ IsingArgs a) {
+    constexpr int D = 3, NT = HB ? 2 * D + 1 : D;
+    const Geometry &g = a.g;
+    const uint32_t Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz, rows = Ly * Lz, NW = g.NW;
+    const uint32_t row = blockIdx.x * blockDim.x + threadIdx.x;
+    if (row >= rows) return;
+    const uint32_t z = fdiv(row, g.divLy), y = row - z * Ly;
+    const uint32_t p = (y + z + a.colour) & 1u;
+    const uint32_t r_ym = y == 0 ? row + (Ly - 1) : row - 1, r_yp = y == Ly - 1 ? row - (Ly - 1) : row + 1;
+    const uint32_t r_zm = z == 0 ? row + Ly * (Lz - 1) : row - Ly, r_zp = z == Lz - 1 ? row - Ly * (Lz - 1) : row + Ly;
+    uint32_t ltf[4][NT];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) lt_masks_full<NT, HB>(a, a.t, a.colour, 4u * row + (uint32_t)i + g.unit_off, 0u, ltf[i]);
+    const uint32_t chunk = (a.R + gridDim.y - 1) / gridDim.y;
+    const uint32_t r0 = blockIdx.y * chunk, r1 = min(a.R, r0 + chunk);
+    const uint32_t oc = 1u - a.colour;
+    const uint32_t NW4 = NW >> 2;   // uint4 per (replica, plane)
+    for (uint32_t r = r0; r < r1; ++r) {
+        const uint4 *__restrict__ So = (const uint4 *)a.s[oc] + (size_t)r * NW4;
+        uint4 *Sc = (uint4 *)a.s[a.colour] + (size_t)r * NW4;
+        const uint4 *__restrict__ Bo = (const uint4 *)a.bonds + ((size_t)(a.colour * a.R + r) * 3) * NW4;   // own forward bonds
+        const uint4 *__restrict__ Bt = (const uint4 *)a.bonds + ((size_t)(oc * a.R + r) * 3) * NW4;         // other colour's
+        const uint4 raw = __ldg((const uint4 *)Sc + row);
+        const uint4 o = __ldg(So + row), ym = __ldg(So + r_ym), yp = __ldg(So + r_yp), zm = __ldg(So + r_zm), zp = __ldg(So + r_zp);
+        const uint4 bx_own = __ldg(Bo + row), bx_oth = __ldg(Bt + row);
+        const uint4 by_m = __ldg(Bt + NW4 + r_ym), by_own = __ldg(Bo + NW4 + row);
+        const uint4 bz_m = __ldg(Bt + 2 * (size_t)NW4 + r_zm), bz_own = __ldg(Bo + 2 * (size_t)NW4 + row);
+        uint32_t out[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const uint32_t rw = u4c(raw, i), s = a.jneg ? ~rw : rw, oi = u4c(o, i);
+            const int in = (i + 1) & 3, ip = (i + 3) & 3;   // periodic inside the row
+            uint32_t av[6];
+            if (p) { av[0] = s ^ oi ^ u4c(bx_oth, i); av[1] = s ^ ((oi >> 1) | (u4c(o, in) << 31)) ^ u4c(bx_own, i); }
+            else { av[0] = s ^ oi ^ u4c(bx_own, i); av[1] = s ^ ((oi << 1) | (u4c(o, ip) >> 31)) ^ ((u4c(bx_oth, i) << 1) | (u4c(bx_oth, ip) >> 31)); }
+            av[2] = s ^ u4c(ym, i) ^ u4c(by_m, i); av[3] = s ^ u4c(yp, i) ^ u4c(by_own, i);
+            av[4] = s ^ u4c(zm, i) ^ u4c(bz_m, i); av[5] = s ^ u4c(zp, i) ^ u4c(bz_own, i);
+            if constexpr (HB) {
+                uint32_t b[6], m[NT];
+#pragma unroll
+                for (int k = 0; k < 6; ++k) b[k] = av[k] ^ rw;
+                count_masks<D>(b, m);
+                uint32_t up = 0u;
+#pragma unroll
+                for (int k = 0; k < NT; ++k) up |= m[k] & ltf[i][k];
+                out[i] = ~up;
+            } else {
+                const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
+                const uint32_t s2 = av[3] ^ av[4] ^ av[5], c2 = maj3(av[3], av[4], av[5]);
+                const uint32_t b0 = s1 ^ s2, c3 = s1 & s2;
+                const uint32_t b1 = c1 ^ c2 ^ c3, b2 = maj3(c1, c2, c3);
+                out[i] = rw ^ ((b2 | (b1 & b0)) | ((b1 | b2) & ltf[i][0]) | ((b0 | b1 | b2) & ltf[i][1]) | ltf[i][2]);
+            }
+        }
+        Sc[row] = make_uint4(out[0], out[1], out[2], out[3]);
+    }
+}
+
 }  // namespace spin

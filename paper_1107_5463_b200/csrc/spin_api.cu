@@ -350,6 +350,22 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
 #undef BM3
 #undef BS2
 #undef BS3
+    } else if (bonds && shared && s->d == 3 && s->g.WX == 4 && !s->vector_generic) {
+        // Lx = 256: a row of one colour is one 128-bit word group; one thread per row (ising_pmj_row4_halfsweep).
+        // All replicas in one thread when the rows alone give every SM >= 256 threads (measured at 256^3, R = 16:
+        // 35.2 / 37.1 / 35.2 / 47.4 / 78.1 us for 1 / 2 / 4 / 8 / 16 replica chunks), else chunks of >= 4 replicas
+        const int Bq = 128;
+        const uint32_t rows = (uint32_t)(s->g.Ly * s->g.Lz);
+        unsigned Gy = 1;
+        if ((uint64_t)rows < (uint64_t)s->sm_count * 256) {
+            uint64_t want = ((uint64_t)s->sm_count * 256 + rows - 1) / rows;   // chunks that would fill the GPU
+            const uint64_t most = (s->R + 3) / 4;
+            if (want > most) want = most;
+            Gy = (unsigned)(want < 1 ? 1 : want);
+        }
+        const dim3 G((rows + Bq - 1) / Bq, Gy);
+        if (s->cfg.update_rule == SPIN_UPDATE_HEATBATH) ising_pmj_row4_halfsweep<true><<<G, Bq, 0, st>>>(a);
+        else ising_pmj_row4_halfsweep<false><<<G, Bq, 0, st>>>(a);
     } else {
         // shared update stream: chunks of >= 16 replicas per thread (the masks of a word are built once per chunk);
         // more chunks only when the lattice alone cannot fill the GPU (many realisations of a small lattice)

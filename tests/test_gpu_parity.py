@@ -183,6 +183,8 @@ def test_per_direction_couplings_generic(P, oracle):
 
 @pytest.mark.parametrize("dims,storage,R,streams", [
     ((64, 6, 4), "bitpack", 16, 0),   # config 4 shape: 16 realisations, shared update stream
+    ((256, 6, 4), "bitpack", 5, 0),   # Lx = 256: one thread per row of four words (config 4's own kernel)
+    ((256, 2, 2), "bitpack", 18, 0),  # the same with size-2 dimensions and replica chunks
     ((128, 4, 6), "bitpack", 3, 1),
     ((64, 8, 1), "bitpack", 5, 0),
     ((64, 8, 1), "bitpack", 2, 1),
@@ -383,6 +385,7 @@ HEATBATH_CASES = [
     ((64, 6, 4), "bitpack", "bond_pm1", 1.0, 4, 0, 1.0 / 1.1),     # +-J, shared update stream (config 4 shape)
     ((64, 6, 4), "bitpack", "bond_pm1", 1.0, 3, 1, 1.0 / 1.1),
     ((64, 12, 1), "bitpack", "bond_pm1", 1.0, 5, 0, 0.8),
+    ((256, 4, 6), "bitpack", "bond_pm1", 1.0, 6, 0, 1.0 / 1.1),    # Lx = 256: the row kernel
 ]
 
 
