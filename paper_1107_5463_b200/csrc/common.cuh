@@ -83,6 +83,7 @@ struct Geometry {
     uint32_t WX;      // 32-site words per row and colour = RL / 32 (fast kernels only)
     uint32_t NW;      // words per colour = Nh / 32 (fast kernels only)
     FastDiv divRL, divWX, divLy;
+    FastDiv divQW;    // by WX / 4 (quads of four words per row and colour; +-J quad kernel)
     FastDiv divQX;    // by RL / 4 (quads of 4 sites per row and colour; strip kernel of the n >= 2 models)
     // Slab decomposition: this handle holds planes [slab_offset, slab_offset + L_own) of a larger
     // lattice along its slowest axis (z for d = 3, y for d = 2), stored with two ghost planes on either side, so the

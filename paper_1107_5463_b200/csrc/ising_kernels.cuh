@@ -323,68 +323,93 @@ __global__ void __launch_bounds__(256) ising_bitpack_halfsweep_hb(const __grid_c
     }
 }
 
-// ------------------------------------------------------------------ +-J, shared stream, one thread per row of 4 words ----
-// Lx = 256 (BASELINE config 4): a row of one colour is exactly four 32-site words = one 128-bit access, and the
-// periodic x-neighbour of every word lies in the same four words.  One thread updates a whole row for all replicas
-// of its chunk: twelve 128-bit loads and one 128-bit store per replica, no scalar loads at all.
+// ------------------------------------------------------------------ +-J, shared stream, one thread per quad of words ----
+// Lx % 256 == 0: a row of one colour is a whole number of quads of four 32-site words, and a quad is one aligned 128-bit
+// access in the spin arrays and in every coupling plane.  One thread updates a quad for all replicas of its chunk:
+// 8 (d = 2) or 12 (d = 3) 128-bit loads and one 128-bit store per replica, plus, when the row is longer than one quad,
+// two scalar loads for the x-neighbour word (and its coupling word) in the adjacent quad.  At Lx = 256 (BASELINE
+// config 4) the row is the quad and the periodic x-neighbour of every word is inside it: no scalar loads at all.
 __device__ __forceinline__ uint32_t u4c(const uint4 &v, int i) { return i == 0 ? v.x : (i == 1 ? v.y : (i == 2 ? v.z : v.w)); }
 
-template <bool HB>
-__global__ void __launch_bounds__(128) ising_pmj_row4_halfsweep(const __grid_constant__ IsingArgs a) {
-    constexpr int D = 3, NT = HB ? 2 * D + 1 : D;
+template <int D, bool HB>
+__global__ void __launch_bounds__(128) ising_pmj_quad_halfsweep(const __grid_constant__ IsingArgs a) {
+    constexpr int NT = HB ? 2 * D + 1 : D;
     const Geometry &g = a.g;
-    const uint32_t Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz, rows = Ly * Lz, NW = g.NW;
-    const uint32_t row = blockIdx.x * blockDim.x + threadIdx.x;
-    if (row >= rows) return;
+    const uint32_t Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz, NW = g.NW, QX = g.WX >> 2, rows = Ly * Lz;
+    const uint32_t item = blockIdx.x * blockDim.x + threadIdx.x;
+    if (item >= rows * QX) return;
+    const uint32_t row = QX == 1u ? item : fdiv(item, g.divQW), q = item - row * QX;
     const uint32_t z = fdiv(row, g.divLy), y = row - z * Ly;
     const uint32_t p = (y + z + a.colour) & 1u;
-    const uint32_t r_ym = y == 0 ? row + (Ly - 1) : row - 1, r_yp = y == Ly - 1 ? row - (Ly - 1) : row + 1;
-    const uint32_t r_zm = z == 0 ? row + Ly * (Lz - 1) : row - Ly, r_zp = z == Lz - 1 ? row - Ly * (Lz - 1) : row + Ly;
+    // uint4 indices (inside one replica's array) of this quad and of the quads at y -+ 1, z -+ 1
+    const uint32_t me = item;
+    const uint32_t q_ym = y == 0 ? me + QX * (Ly - 1) : me - QX, q_yp = y == Ly - 1 ? me - QX * (Ly - 1) : me + QX;
+    const uint32_t q_zm = D == 3 ? (z == 0 ? me + QX * Ly * (Lz - 1) : me - QX * Ly) : me;
+    const uint32_t q_zp = D == 3 ? (z == Lz - 1 ? me - QX * Ly * (Lz - 1) : me + QX * Ly) : me;
+    // word index of the x-neighbour outside the quad: p = 1 -> first word of the next quad, p = 0 -> last of the previous
+    const uint32_t w_edge = row * (4u * QX) + (p ? (q + 1u == QX ? 0u : 4u * q + 4u) : (q == 0u ? 4u * QX - 1u : 4u * q - 1u));
     uint32_t ltf[4][NT];
 #pragma unroll
-    for (int i = 0; i < 4; ++i) lt_masks_full<NT, HB>(a, a.t, a.colour, 4u * row + (uint32_t)i + g.unit_off, 0u, ltf[i]);
+    for (int i = 0; i < 4; ++i) lt_masks_full<NT, HB>(a, a.t, a.colour, 4u * me + (uint32_t)i + g.unit_off, 0u, ltf[i]);
     const uint32_t chunk = (a.R + gridDim.y - 1) / gridDim.y;
     const uint32_t r0 = blockIdx.y * chunk, r1 = min(a.R, r0 + chunk);
     const uint32_t oc = 1u - a.colour;
     const uint32_t NW4 = NW >> 2;   // uint4 per (replica, plane)
+    const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
     for (uint32_t r = r0; r < r1; ++r) {
         const uint4 *__restrict__ So = (const uint4 *)a.s[oc] + (size_t)r * NW4;
         uint4 *Sc = (uint4 *)a.s[a.colour] + (size_t)r * NW4;
         const uint4 *__restrict__ Bo = (const uint4 *)a.bonds + ((size_t)(a.colour * a.R + r) * 3) * NW4;   // own forward bonds
         const uint4 *__restrict__ Bt = (const uint4 *)a.bonds + ((size_t)(oc * a.R + r) * 3) * NW4;         // other colour's
-        const uint4 raw = __ldg((const uint4 *)Sc + row);
-        const uint4 o = __ldg(So + row), ym = __ldg(So + r_ym), yp = __ldg(So + r_yp), zm = __ldg(So + r_zm), zp = __ldg(So + r_zp);
-        const uint4 bx_own = __ldg(Bo + row), bx_oth = __ldg(Bt + row);
-        const uint4 by_m = __ldg(Bt + NW4 + r_ym), by_own = __ldg(Bo + NW4 + row);
-        const uint4 bz_m = __ldg(Bt + 2 * (size_t)NW4 + r_zm), bz_own = __ldg(Bo + 2 * (size_t)NW4 + row);
+        const uint4 raw = __ldg((const uint4 *)Sc + me);
+        const uint4 o = __ldg(So + me), ym = __ldg(So + q_ym), yp = __ldg(So + q_yp);
+        const uint4 zm = D == 3 ? __ldg(So + q_zm) : zero, zp = D == 3 ? __ldg(So + q_zp) : zero;
+        const uint4 bx_own = __ldg(Bo + me), bx_oth = __ldg(Bt + me);
+        const uint4 by_m = __ldg(Bt + NW4 + q_ym), by_own = __ldg(Bo + NW4 + me);
+        const uint4 bz_m = D == 3 ? __ldg(Bt + 2 * (size_t)NW4 + q_zm) : zero, bz_own = D == 3 ? __ldg(Bo + 2 * (size_t)NW4 + me) : zero;
+        // the neighbour word outside the quad and (p = 0 only) its forward x coupling; inside the quad when QX == 1
+        uint32_t o_edge, b_edge = 0u;
+        if (QX == 1u) { o_edge = p ? o.x : o.w; b_edge = bx_oth.w; }
+        else {
+            o_edge = __ldg((const uint32_t *)So + w_edge);
+            if (!p) b_edge = __ldg((const uint32_t *)Bt + w_edge);
+        }
         uint32_t out[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const uint32_t rw = u4c(raw, i), s = a.jneg ? ~rw : rw, oi = u4c(o, i);
-            const int in = (i + 1) & 3, ip = (i + 3) & 3;   // periodic inside the row
             uint32_t av[6];
-            if (p) { av[0] = s ^ oi ^ u4c(bx_oth, i); av[1] = s ^ ((oi >> 1) | (u4c(o, in) << 31)) ^ u4c(bx_own, i); }
-            else { av[0] = s ^ oi ^ u4c(bx_own, i); av[1] = s ^ ((oi << 1) | (u4c(o, ip) >> 31)) ^ ((u4c(bx_oth, i) << 1) | (u4c(bx_oth, ip) >> 31)); }
+            if (p) {
+                const uint32_t nx = i == 3 ? o_edge : u4c(o, (i + 1) & 3);
+                av[0] = s ^ oi ^ u4c(bx_oth, i); av[1] = s ^ ((oi >> 1) | (nx << 31)) ^ u4c(bx_own, i);
+            } else {
+                const uint32_t pv = i == 0 ? o_edge : u4c(o, (i + 3) & 3), bp = i == 0 ? b_edge : u4c(bx_oth, (i + 3) & 3);
+                av[0] = s ^ oi ^ u4c(bx_own, i); av[1] = s ^ ((oi << 1) | (pv >> 31)) ^ ((u4c(bx_oth, i) << 1) | (bp >> 31));
+            }
             av[2] = s ^ u4c(ym, i) ^ u4c(by_m, i); av[3] = s ^ u4c(yp, i) ^ u4c(by_own, i);
-            av[4] = s ^ u4c(zm, i) ^ u4c(bz_m, i); av[5] = s ^ u4c(zp, i) ^ u4c(bz_own, i);
+            av[4] = D == 3 ? s ^ u4c(zm, i) ^ u4c(bz_m, i) : 0u; av[5] = D == 3 ? s ^ u4c(zp, i) ^ u4c(bz_own, i) : 0u;
             if constexpr (HB) {
                 uint32_t b[6], m[NT];
 #pragma unroll
-                for (int k = 0; k < 6; ++k) b[k] = av[k] ^ rw;
+                for (int k = 0; k < 6; ++k) b[k] = k < 2 * D ? av[k] ^ rw : 0u;
                 count_masks<D>(b, m);
                 uint32_t up = 0u;
 #pragma unroll
                 for (int k = 0; k < NT; ++k) up |= m[k] & ltf[i][k];
                 out[i] = ~up;
+            } else if (D == 2) {
+                const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
+                const uint32_t ge2 = c1 | (s1 & av[3]), ge1 = av[0] | av[1] | av[2] | av[3];
+                out[i] = rw ^ (ge2 | (ge1 & ltf[i][0]) | ltf[i][1]);
             } else {
                 const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
                 const uint32_t s2 = av[3] ^ av[4] ^ av[5], c2 = maj3(av[3], av[4], av[5]);
                 const uint32_t b0 = s1 ^ s2, c3 = s1 & s2;
                 const uint32_t b1 = c1 ^ c2 ^ c3, b2 = maj3(c1, c2, c3);
-                out[i] = rw ^ ((b2 | (b1 & b0)) | ((b1 | b2) & ltf[i][0]) | ((b0 | b1 | b2) & ltf[i][1]) | ltf[i][2]);
+                out[i] = rw ^ ((b2 | (b1 & b0)) | ((b1 | b2) & ltf[i][0]) | ((b0 | b1 | b2) & ltf[i][1]) | ltf[i][D - 1]);
             }
         }
-        Sc[row] = make_uint4(out[0], out[1], out[2], out[3]);
+        Sc[me] = make_uint4(out[0], out[1], out[2], out[3]);
     }
 }
 

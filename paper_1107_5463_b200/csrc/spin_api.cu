@@ -350,22 +350,23 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
 #undef BM3
 #undef BS2
 #undef BS3
-    } else if (bonds && shared && s->d == 3 && s->g.WX == 4 && !s->vector_generic) {
-        // Lx = 256: a row of one colour is one 128-bit word group; one thread per row (ising_pmj_row4_halfsweep).
-        // All replicas in one thread when the rows alone give every SM >= 256 threads (measured at 256^3, R = 16:
+    } else if (bonds && shared && s->g.WX % 4 == 0 && !s->vector_generic) {
+        // Lx % 256 == 0: one thread per quad of four words, 128-bit accesses (ising_pmj_quad_halfsweep).
+        // All replicas in one thread when the quads alone give every SM >= 256 threads (measured at 256^3, R = 16:
         // 35.2 / 37.1 / 35.2 / 47.4 / 78.1 us for 1 / 2 / 4 / 8 / 16 replica chunks), else chunks of >= 4 replicas
         const int Bq = 128;
-        const uint32_t rows = (uint32_t)(s->g.Ly * s->g.Lz);
+        const uint64_t quads = (uint64_t)s->g.NW / 4;
         unsigned Gy = 1;
-        if ((uint64_t)rows < (uint64_t)s->sm_count * 256) {
-            uint64_t want = ((uint64_t)s->sm_count * 256 + rows - 1) / rows;   // chunks that would fill the GPU
+        if (quads < (uint64_t)s->sm_count * 256) {
+            uint64_t want = ((uint64_t)s->sm_count * 256 + quads - 1) / quads;   // chunks that would fill the GPU
             const uint64_t most = (s->R + 3) / 4;
             if (want > most) want = most;
             Gy = (unsigned)(want < 1 ? 1 : want);
         }
-        const dim3 G((rows + Bq - 1) / Bq, Gy);
-        if (s->cfg.update_rule == SPIN_UPDATE_HEATBATH) ising_pmj_row4_halfsweep<true><<<G, Bq, 0, st>>>(a);
-        else ising_pmj_row4_halfsweep<false><<<G, Bq, 0, st>>>(a);
+        const dim3 G((unsigned)((quads + Bq - 1) / Bq), Gy);
+        const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
+        if (s->d == 2) { if (hb) ising_pmj_quad_halfsweep<2, true><<<G, Bq, 0, st>>>(a); else ising_pmj_quad_halfsweep<2, false><<<G, Bq, 0, st>>>(a); }
+        else { if (hb) ising_pmj_quad_halfsweep<3, true><<<G, Bq, 0, st>>>(a); else ising_pmj_quad_halfsweep<3, false><<<G, Bq, 0, st>>>(a); }
     } else {
         // shared update stream: chunks of >= 16 replicas per thread (the masks of a word are built once per chunk);
         // more chunks only when the lattice alone cannot fill the GPU (many realisations of a small lattice)
@@ -689,6 +690,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
     g.WX = g.RL / 32; g.NW = g.Nh / 32;
     g.divRL = make_fastdiv(g.RL); g.divWX = make_fastdiv(g.WX ? g.WX : 1); g.divLy = make_fastdiv((uint32_t)g.Ly);
     g.divQX = make_fastdiv(g.RL / 4 ? g.RL / 4 : 1);
+    g.divQW = make_fastdiv(g.WX / 4 ? g.WX / 4 : 1);
     g.j_off = 0; g.unit_off = 0; g.i_off = 0; g.own_j0 = 0; g.own_j1 = g.Nh; g.own_i0 = 0; g.own_in = (uint32_t)dv.N;
     if (dv.axis >= 0) {
         const int64_t plane_sites = dv.axis == 2 ? (int64_t)g.Lx * g.Ly : (int64_t)g.Lx, plane_h = plane_sites / 2;

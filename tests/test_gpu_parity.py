@@ -185,6 +185,9 @@ def test_per_direction_couplings_generic(P, oracle):
     ((64, 6, 4), "bitpack", 16, 0),   # config 4 shape: 16 realisations, shared update stream
     ((256, 6, 4), "bitpack", 5, 0),   # Lx = 256: one thread per row of four words (config 4's own kernel)
     ((256, 2, 2), "bitpack", 18, 0),  # the same with size-2 dimensions and replica chunks
+    ((512, 4, 4), "bitpack", 3, 0),   # two quads per row: the x-neighbour word comes from the adjacent quad
+    ((768, 6, 1), "bitpack", 4, 0),   # d = 2, three quads per row
+    ((256, 8, 1), "bitpack", 7, 0),   # d = 2, the row is the quad
     ((128, 4, 6), "bitpack", 3, 1),
     ((64, 8, 1), "bitpack", 5, 0),
     ((64, 8, 1), "bitpack", 2, 1),
@@ -385,7 +388,8 @@ HEATBATH_CASES = [
     ((64, 6, 4), "bitpack", "bond_pm1", 1.0, 4, 0, 1.0 / 1.1),     # +-J, shared update stream (config 4 shape)
     ((64, 6, 4), "bitpack", "bond_pm1", 1.0, 3, 1, 1.0 / 1.1),
     ((64, 12, 1), "bitpack", "bond_pm1", 1.0, 5, 0, 0.8),
-    ((256, 4, 6), "bitpack", "bond_pm1", 1.0, 6, 0, 1.0 / 1.1),    # Lx = 256: the row kernel
+    ((256, 4, 6), "bitpack", "bond_pm1", 1.0, 6, 0, 1.0 / 1.1),    # Lx = 256: the quad kernel, row = quad
+    ((512, 6, 1), "bitpack", "bond_pm1", 1.0, 5, 0, 0.8),          # d = 2, two quads per row
 ]
 
 
