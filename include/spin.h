@@ -144,7 +144,13 @@ spin_status spin_set_strip_rows(spin_system *s, int32_t rows);
 
 /* Test knob: value 1 selects the plain kernels (one launch per half-sweep, one thread per site for n >= 2,
  * no resident small-lattice kernel), 0 (default) the tuned ones.  Results never depend on it bit for bit. */
-enum { SPIN_OPT_PLAIN_KERNELS = 0 };
+enum { SPIN_OPT_PLAIN_KERNELS = 0,
+       /* The TMA-staged kernel of the n >= 2 models (d = 3, Lx <= 512: tiles and halos staged in shared memory by
+        * cp.async.bulk.tensor, PAPER.md:42 tile + boundary layer): 1 = every half-sweep, 0 = never (strip kernel),
+        * -1 (default) = only for the colour-1 half-sweep of spin_sweep_record, where its fused E / M saves the
+        * measurement pass; elsewhere the strip kernel is the faster one on B200 (profiles/).  Spins are bit-identical
+        * whichever kernel runs. */
+       SPIN_OPT_TMA_KERNELS = 1 };
 spin_status spin_set_option(spin_system *s, int32_t option, int64_t value);
 
 /* Frees the handle only; never the workspace. */

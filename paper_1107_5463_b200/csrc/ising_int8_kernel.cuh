@@ -119,6 +119,14 @@ __device__ __forceinline__ Int8RawUnit int8_load_unit(const uint8_t *p) {
     u.hi = __ldg((const uint4 *)p + 1);
     return u;
 }
+// the same for the array being updated: plain (coherent) loads -- the non-coherent path is for data that stays
+// read-only for the whole kernel
+__device__ __forceinline__ Int8RawUnit int8_load_unit_rw(const uint8_t *p) {
+    Int8RawUnit u;
+    u.lo = *((const uint4 *)p);
+    u.hi = *((const uint4 *)p + 1);
+    return u;
+}
 __device__ __forceinline__ uint32_t int8_pack_raw(const Int8RawUnit &u) {
     uint32_t m = u.lo.x;
     m = u.lo.y * 2u + m;
@@ -172,7 +180,7 @@ __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(cons
         const uint32_t yp = y0 + 1 == Ly ? 0u : y0 + 1;
         const size_t off = y0 * rowbytes + 32u * w;
         pf_next = int8_load_unit(other + zoff + yp * rowbytes + 32u * w);
-        pf_mine = int8_load_unit(mine + zoff + off);
+        pf_mine = int8_load_unit_rw(mine + zoff + off);
         pf_side = int8_side_byte(other + zoff + y0 * rowbytes, p, w, WX);
         if (D == 3) { pf_zm = int8_load_unit(other + zm_off + off); pf_zp = int8_load_unit(other + zp_off + off); }
     }
@@ -193,7 +201,7 @@ __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(cons
                 const uint32_t y1 = y + 1, y2 = y1 + 1 == Ly ? 0u : y1 + 1;
                 const size_t off1 = y1 * rowbytes + 32u * w;
                 pf_next = int8_load_unit(other + zoff + y2 * rowbytes + 32u * w);
-                pf_mine = int8_load_unit(mine + zoff + off1);
+                pf_mine = int8_load_unit_rw(mine + zoff + off1);
                 pf_side = int8_side_byte(other + zoff + y1 * rowbytes, p ^ 1u, w, WX);
                 if (D == 3) { pf_zm = int8_load_unit(other + zm_off + off1); pf_zp = int8_load_unit(other + zp_off + off1); }
             }
@@ -245,7 +253,7 @@ __global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __gri
     {
         const uint32_t yp = y0 + 1 == Ly ? 0u : y0 + 1, off = y0 * WX + w;
         pf_next = __ldg(other + zoff + yp * WX + w);
-        pf_mine = __ldg(mine + zoff + off);
+        pf_mine = mine[zoff + off];
         pf_side = __ldg(other + zoff + y0 * WX + (p ? w_next : w_prev));
         if (D == 3) { pf_zm = __ldg(other + zm_off + off); pf_zp = __ldg(other + zp_off + off); }
     }
@@ -260,7 +268,7 @@ __global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __gri
             if (k + 1 < K && (uint32_t)(k + 1) < kend) {
                 const uint32_t y1 = y + 1, y2 = y1 + 1 == Ly ? 0u : y1 + 1, off1 = y1 * WX + w;
                 pf_next = __ldg(other + zoff + y2 * WX + w);
-                pf_mine = __ldg(mine + zoff + off1);
+                pf_mine = mine[zoff + off1];
                 pf_side = __ldg(other + zoff + y1 * WX + (p ? w_prev : w_next));   // row y + 1 has the other parity
                 if (D == 3) { pf_zm = __ldg(other + zm_off + off1); pf_zp = __ldg(other + zp_off + off1); }
             }

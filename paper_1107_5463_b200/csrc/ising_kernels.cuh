@@ -212,7 +212,7 @@ __device__ __forceinline__ uint32_t unsatisfied_bonds(const IsingArgs &a, uint32
                                                       const WordNbrs &n, uint32_t av[6]) {
     const uint32_t NW = a.g.NW;
     const uint32_t *__restrict__ other = (const uint32_t *)a.s[1 - colour] + (size_t)r * NW;
-    const uint32_t raw = __ldg((const uint32_t *)a.s[colour] + (size_t)r * NW + gi);  // read only by its owner, before its write
+    const uint32_t raw = ((const uint32_t *)a.s[colour])[(size_t)r * NW + gi];  // plain load: this array is written by the kernel
     const uint32_t s = a.jneg ? ~raw : raw;
     const uint32_t o = other[gi], os = other[n.g_side];
     const uint32_t side = n.p ? ((o >> 1) | (os << 31)) : ((o << 1) | (os >> 31));
@@ -361,7 +361,7 @@ __global__ void __launch_bounds__(128) ising_pmj_quad_halfsweep(const __grid_con
         uint4 *Sc = (uint4 *)a.s[a.colour] + (size_t)r * NW4;
         const uint4 *__restrict__ Bo = (const uint4 *)a.bonds + ((size_t)(a.colour * a.R + r) * 3) * NW4;   // own forward bonds
         const uint4 *__restrict__ Bt = (const uint4 *)a.bonds + ((size_t)(oc * a.R + r) * 3) * NW4;         // other colour's
-        const uint4 raw = __ldg((const uint4 *)Sc + me);
+        const uint4 raw = Sc[me];   // plain load: this array is written by the kernel
         const uint4 o = __ldg(So + me), ym = __ldg(So + q_ym), yp = __ldg(So + q_yp);
         const uint4 zm = D == 3 ? __ldg(So + q_zm) : zero, zp = D == 3 ? __ldg(So + q_zp) : zero;
         const uint4 bx_own = __ldg(Bo + me), bx_oth = __ldg(Bt + me);

@@ -15,6 +15,7 @@
 #include "measure_kernels.cuh"
 #include "setup_kernels.cuh"
 #include "vector_kernels.cuh"
+#include "vector_tma_kernel.cuh"
 
 using namespace spin;
 
@@ -79,6 +80,11 @@ struct spin_system {
     int g_block, g_rows, g_rows_set, g_num, g_den;
     void *staging;       // device buffer for canonical arrays (get / set calls), kept until spin_destroy
     size_t staging_bytes;
+    // n >= 2, d = 3: TMA-staged kernel (vector_tma_kernel.cuh)
+    int tma_ok;          // tensor maps encoded (rows of <= 256 sites per colour, driver entry point found)
+    int use_tma;         // SPIN_OPT_TMA_KERNELS: 1 every half-sweep, 0 never, -1 (default) only where its fused E / M pays
+    uint32_t tma_ty;     // rows per tile
+    CUtensorMap tma_main[2], tma_row[2];
 };
 
 static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
@@ -176,6 +182,16 @@ static uint32_t measure_blocks(uint64_t work_items) {
     return (uint32_t)b;
 }
 
+// TMA-staged kernel of the n >= 2 models: rows per tile, and CTAs per replica for S steps, R replicas and room for `cap` CTAs
+static uint32_t tma_tile_rows(uint32_t RL) { return RL <= 128 ? 8u : 4u; }
+static uint32_t tma_grid_x(uint64_t S, uint64_t R, uint64_t cap) {
+    uint64_t gx = cap / R;
+    if (gx < 1) gx = 1;
+    if (gx > S) gx = S;
+    return (uint32_t)gx;
+}
+constexpr uint64_t TMA_MAX_CTAS = 512;
+
 static void make_layout(const spin_config *c, const Derived &dv, Layout *l, uint32_t *mblocks) {
     const uint64_t Nh = dv.N / 2, R = (uint64_t)c->n_replicas;
     size_t off = 0;
@@ -188,7 +204,14 @@ static void make_layout(const spin_config *c, const Derived &dv, Layout *l, uint
         l->bytes_bonds = dv.path == PATH_ISING_BITPACK ? (size_t)(2 * R * 3 * (Nh / 32) * 4) : (size_t)(R * dv.d * dv.N);
     l->off_bonds = off; off += align_up(l->bytes_bonds);
     *mblocks = measure_blocks(dv.path == PATH_ISING_BITPACK || dv.path == PATH_ISING_INT8 ? Nh / 32 : Nh);
-    l->bytes_acc = c->n == 1 ? (size_t)(R * 2 * sizeof(long long)) : (size_t)(R * *mblocks * (1 + c->n) * sizeof(double));
+    uint64_t pblocks = *mblocks;   // n >= 2: per-CTA partials of the measurement pass or of the fused TMA half-sweep
+    if (c->n > 1 && dv.d == 3) {
+        const uint32_t ty = tma_tile_rows((uint32_t)dv.pad[0] / 2);
+        const uint64_t S = (uint64_t)((dv.pad[1] + ty - 1) / ty) * dv.pad[2];
+        const uint64_t gx = tma_grid_x(S, R, TMA_MAX_CTAS);
+        if (gx > pblocks) pblocks = gx;
+    }
+    l->bytes_acc = c->n == 1 ? (size_t)(R * 2 * sizeof(long long)) : (size_t)(R * pblocks * (1 + c->n) * sizeof(double));
     l->off_acc = off; off += align_up(l->bytes_acc);
     l->bytes_res = (size_t)(R * (1 + c->n) * sizeof(double));
     l->off_res = off; off += align_up(l->bytes_res);
@@ -402,12 +425,109 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
     return SPIN_OK;
 }
 
-// n >= 2: the strip kernel (128-bit accesses, K rows per thread) when a row holds whole quads of 4 sites,
-// the one-thread-per-site kernel otherwise.
-static spin_status launch_halfsweep_vector(spin_system *s, const VectorArgs &a, cudaStream_t st) {
+// cuTensorMapEncodeTiled through the runtime (no link against libcuda); NULL if the driver does not offer it
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+// Tensor maps of the two colour arrays float [R][NC][Lz][Ly][RL] for the TMA-staged kernel: a box of TY rows and a
+// box of one row, each over all NC components.  Leaves tma_ok = 0 (strip kernel) when the shape does not qualify.
+static void tma_prepare(spin_system *s) {
+    s->tma_ok = 0;
+    const Geometry &g = s->g;
+    if (s->path != PATH_VECTOR || s->d != 3 || g.RL % 4 != 0 || g.RL > 256 || s->R > 65535) return;
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return;
+    s->tma_ty = tma_tile_rows(g.RL);
+    const cuuint64_t dims[5] = {g.RL, (cuuint64_t)g.Ly, (cuuint64_t)g.Lz, (cuuint64_t)s->n, s->R};
+    const cuuint64_t strides[4] = {(cuuint64_t)g.RL * 4, (cuuint64_t)g.RL * g.Ly * 4, (cuuint64_t)g.Nh * 4, (cuuint64_t)g.Nh * 4 * s->n};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    for (int c = 0; c < 2; ++c) {
+        void *base = s->ws + s->lay.off_s[c];
+        const cuuint32_t box_main[5] = {g.RL, s->tma_ty, 1, (cuuint32_t)s->n, 1};
+        const cuuint32_t box_row[5] = {g.RL, 1, 1, (cuuint32_t)s->n, 1};
+        if (enc(&s->tma_main[c], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, base, dims, strides, box_main, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return;
+        if (enc(&s->tma_row[c], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, base, dims, strides, box_row, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return;
+    }
+    s->tma_ok = 1;
+}
+
+template <int NC, bool UNITJ, bool HB, bool MEAS>
+static cudaError_t launch_tma(const VectorTmaArgs &ta, dim3 G, size_t smem, cudaStream_t st) {
+    static size_t configured = 0;   // dynamic shared memory this instantiation has been allowed so far
+    if (configured < smem) {
+        cudaError_t e = cudaFuncSetAttribute(vector_tma_halfsweep<NC, UNITJ, HB, MEAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = smem;
+    }
+    vector_tma_halfsweep<NC, UNITJ, HB, MEAS><<<G, TMA_THREADS, smem, st>>>(ta);
+    return cudaGetLastError();
+}
+
+// CTAs per replica of the TMA-staged kernel on this device
+static uint32_t tma_ctas(const spin_system *s, bool hb, bool meas) {
+    const uint64_t S = (uint64_t)((s->g.Ly + s->tma_ty - 1) / s->tma_ty) * s->g.Lz;
+    uint64_t cap = (uint64_t)s->sm_count * tma_ctas_per_sm(hb, meas) * (uint64_t)s->grid_num / (uint64_t)s->grid_den;
+    if (cap > TMA_MAX_CTAS) cap = TMA_MAX_CTAS;
+    if (cap < 1) cap = 1;
+    return tma_grid_x(S, s->R, cap);
+}
+
+// n >= 2.  d = 3 with rows of at most 256 sites per colour: the TMA-staged kernel (tiles + halo in shared memory, ring over
+// z); otherwise the strip kernel (128-bit accesses, K rows per thread) when a row holds whole quads of 4 sites, else the
+// one-thread-per-site kernel.  fused: NULL, or (colour 1) ask for E / M partials from the half-sweep itself (row a7);
+// *fused = number of per-replica partials written (0: this kernel cannot, run the measurement pass).
+static spin_status launch_halfsweep_vector(spin_system *s, const VectorArgs &a, cudaStream_t st, bool allow_tma = true,
+                                           uint32_t *fused = nullptr) {
     const Geometry &g = s->g;
     const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
     const bool strip_ok = g.RL % 4 == 0 && !s->vector_generic && s->R <= 65535;
+    if (fused) *fused = 0;
+    // the staged kernel serves (a) every half-sweep when SPIN_OPT_TMA_KERNELS is on, (b) by default only the colour-1 half-sweep
+    // of a recorded sweep, whose fused E / M saves the measurement pass (the strip kernel is faster otherwise: profiles/)
+    const bool want_fused = fused && a.colour == 1u;
+    if (allow_tma && s->tma_ok && (s->use_tma == 1 || (s->use_tma < 0 && want_fused)) && !s->vector_generic) {
+        bool unitj = true;
+        for (int mu = 0; mu < s->d; ++mu) unitj = unitj && a.Jdir[mu] == 1.0f;
+        VectorTmaArgs ta;
+        ta.v = a;
+        for (int c = 0; c < 2; ++c) { ta.main_map[c] = s->tma_main[c]; ta.row_map[c] = s->tma_row[c]; }
+        ta.TY = s->tma_ty;
+        ta.nyb = ((uint32_t)g.Ly + s->tma_ty - 1) / s->tma_ty;
+        ta.part = (double *)(s->ws + s->lay.off_acc);
+        const bool meas = fused && a.colour == 1u;
+        const dim3 G(tma_ctas(s, hb, meas), s->R);
+        const size_t smem = tma_smem_bytes(s->n, (int)s->tma_ty, g.RL);
+        cudaError_t e;
+#define TM4(NC_, U_, HB_, M_) e = launch_tma<NC_, U_, HB_, M_>(ta, G, smem, st)
+#define TM3(NC_, U_, HB_) do { if (meas) TM4(NC_, U_, HB_, true); else TM4(NC_, U_, HB_, false); } while (0)
+#define TM2(NC_, HB_) do { if (unitj) TM3(NC_, true, HB_); else TM3(NC_, false, HB_); } while (0)
+        if (s->n == 2) TM2(2, false);
+        else if (hb) TM2(3, true);
+        else TM2(3, false);
+#undef TM2
+#undef TM3
+#undef TM4
+        if (e != cudaSuccess) return fail(SPIN_ERR_CUDA, "TMA half-sweep launch: %s", cudaGetErrorString(e));
+        if (meas) *fused = G.x;
+        s->launches += 1;
+        return SPIN_OK;
+    }
     if (strip_ok && hb) {
         // heat bath (n = 3): the strip kernel with one row per thread
         bool unitj = true;
@@ -457,7 +577,8 @@ static spin_status enqueue_sweep(spin_system *s, double beta, cudaStream_t st, b
         if (capture) a.t = t_override;
         for (uint32_t colour = 0; colour < 2; ++colour) {
             a.colour = colour;
-            spin_status rc = launch_halfsweep_vector(s, a, st);
+            // graph replay patches the sweep index into VectorArgs-sized argument blocks: strip kernel only
+            spin_status rc = launch_halfsweep_vector(s, a, st, !capture);
             if (rc != SPIN_OK) return rc;
         }
     }
@@ -680,6 +801,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
         return fail(SPIN_ERR_WORKSPACE_TOO_SMALL, "workspace has %zu bytes, %zu needed", bytes, need);
     }
     s->ws = (char *)d_workspace;
+    s->tma_ok = 0; s->use_tma = -1; s->tma_ty = 0;
     s->t = 0; s->launches = 0; s->staging = nullptr; s->staging_bytes = 0; s->gexec = nullptr; s->cap_stream = nullptr; s->gnodes = nullptr; s->n_gnodes = 0;
     // 128 threads per CTA for the Ising fast paths (measured: +-J R = 16 39.1 vs 40.4 us with 256)
     s->block = (dv.path == PATH_ISING_INT8 || dv.path == PATH_ISING_BITPACK) ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0;
@@ -713,6 +835,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
         delete s;
         return fail(SPIN_ERR_CUDA, "no usable CUDA device: %s", cudaGetErrorString(e));
     }
+    tma_prepare(s);
 #define CREATE_TRY(expr)                                                                              \
     do {                                                                                              \
         cudaError_t e2_ = (expr);                                                                     \
@@ -808,6 +931,23 @@ spin_status spin_sweep_record(spin_system *s, double beta, int64_t n_sweeps, dou
                 CUDA_TRY(cudaGetLastError());
                 continue;
             }
+        } else if (s->n > 1) {
+            // n >= 2: the TMA-staged colour-1 half-sweep leaves per-CTA partial sums of E and M (row a7)
+            VectorArgs a = vector_args(s, beta);
+            uint32_t parts = 0;
+            a.colour = 0;
+            rc = launch_halfsweep_vector(s, a, st);
+            if (rc != SPIN_OK) return rc;
+            a.colour = 1;
+            rc = launch_halfsweep_vector(s, a, st, true, &parts);
+            if (rc != SPIN_OK) return rc;
+            s->t += 1;
+            if (parts) {
+                vector_measure_finalize<<<s->R, 256, 0, st>>>((const double *)(s->ws + s->lay.off_acc), parts, s->n, oE, oM);
+                s->launches += 1;
+                CUDA_TRY(cudaGetLastError());
+                continue;
+            }
         } else {
             rc = enqueue_sweep(s, beta, st);
             if (rc != SPIN_OK) return rc;
@@ -819,7 +959,8 @@ spin_status spin_sweep_record(spin_system *s, double beta, int64_t n_sweeps, dou
 }
 
 spin_status spin_halfsweep(spin_system *s, double beta, int32_t colour, void *stream) {
-    spin_status rc = check_sweep_args(s, beta, colour == 1 ? 1 : 0);
+    // either colour needs a sweep index below 2^32 (colour 0 at t = 2^32 would silently reuse the numbers of sweep 0)
+    spin_status rc = check_sweep_args(s, beta, 1);
     if (rc != SPIN_OK) return rc;
     if (colour != 0 && colour != 1) return fail(SPIN_ERR_INVALID_ARG, "colour must be 0 or 1");
     if ((uint32_t)colour != s->next_colour) return fail(SPIN_ERR_STATE, "half-sweeps alternate: colour %u is next", s->next_colour);
@@ -1030,6 +1171,11 @@ spin_status spin_set_option(spin_system *s, int32_t option, int64_t value) {
     if (option == SPIN_OPT_PLAIN_KERNELS) {
         if (value != 0 && value != 1) return fail(SPIN_ERR_INVALID_ARG, "SPIN_OPT_PLAIN_KERNELS takes 0 or 1");
         s->vector_generic = (int)value;
+        return SPIN_OK;
+    }
+    if (option == SPIN_OPT_TMA_KERNELS) {
+        if (value != 0 && value != 1 && value != -1) return fail(SPIN_ERR_INVALID_ARG, "SPIN_OPT_TMA_KERNELS takes 0, 1 or -1");
+        s->use_tma = (int)value;
         return SPIN_OK;
     }
     return fail(SPIN_ERR_INVALID_ARG, "unknown option %d", (int)option);

@@ -193,6 +193,148 @@ __device__ __forceinline__ float add_nb(float h, float J, float s) {
     return UNITJ ? __fadd_rn(h, s) : __fadd_rn(h, __fmul_rn(J, s));
 }
 
+// ---------------------------------------------------------------------------------------------
+// Packed fp32 arithmetic (sm_100: add / mul / fma.rn.f32x2 -> FADD2 / FMUL2 / FFMA2, two IEEE operations per issued
+// instruction).  Each half of a packed operation is the correctly rounded scalar operation, so a pair of sites computed
+// this way carries exactly the bits the one-thread-per-site kernel produces with __fadd_rn / __fmul_rn / fmaf; what is
+// saved is issue slots, which is what bounds these kernels (profiles/).
+__device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
+__device__ __forceinline__ float2 f2s(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
+
+// sincospi_u24 for two sites at once: integer range reduction per site, the two polynomials packed
+__device__ __forceinline__ void sincospi_u24_x2(uint32_t wa, uint32_t wb, float2 *sn, float2 *cs) {
+    const uint32_t ka = wa >> 8, kb = wb >> 8;
+    const uint32_t qa = (ka + (1u << 21)) >> 22, qb = (kb + (1u << 21)) >> 22;
+    const float2 r = __fmul2_rn(f2((float)(int)(ka - (qa << 22)), (float)(int)(kb - (qb << 22))), f2s(1.1920928955078125e-07f));
+    const float2 u = __fmul2_rn(r, r);
+    float2 ps = __ffma2_rn(f2s(-0.589078654592815f), u, f2s(2.5497672980581947f));
+    ps = __ffma2_rn(ps, u, f2s(-5.167707829131533f));
+    ps = __ffma2_rn(ps, u, f2s(3.1415926439336053f));
+    const float2 sr = __fmul2_rn(ps, r);
+    float2 cr = __ffma2_rn(f2s(0.2313297165900991f), u, f2s(-1.3350445644556512f));
+    cr = __ffma2_rn(cr, u, f2s(4.058707263029904f));
+    cr = __ffma2_rn(cr, u, f2s(-4.934802162589503f));
+    cr = __ffma2_rn(cr, u, f2s(1.0f));
+    const float aa = (qa & 1u) ? cr.x : sr.x, ba = (qa & 1u) ? sr.x : cr.x;
+    const float ab = (qb & 1u) ? cr.y : sr.y, bb = (qb & 1u) ? sr.y : cr.y;
+    sn->x = __uint_as_float(__float_as_uint(aa) ^ ((qa & 2u) << 30));
+    cs->x = __uint_as_float(__float_as_uint(ba) ^ (((qa + 1u) & 2u) << 30));
+    sn->y = __uint_as_float(__float_as_uint(ab) ^ ((qb & 2u) << 30));
+    cs->y = __uint_as_float(__float_as_uint(bb) ^ (((qb + 1u) & 2u) << 30));
+}
+
+// direction3 / direction2 for two sites (site a in .x, site b in .y); out[c] = component c of both
+__device__ __forceinline__ void direction3_x2(uint32_t w0a, uint32_t w1a, uint32_t w0b, uint32_t w1b, float2 out[3]) {
+    // z = 2 u24(w) - 1 = k 2^-23 - 1 with k < 2^24: product and difference are exact, so one fma gives the same float
+    const float2 z = __ffma2_rn(f2((float)(w0a >> 8), (float)(w0b >> 8)), f2s(1.1920928955078125e-07f), f2s(-1.0f));
+    const float2 om = __fadd2_rn(f2s(1.0f), neg2(__fmul2_rn(z, z)));
+    const float2 rho = f2(__fsqrt_rn(fmaxf(om.x, 0.0f)), __fsqrt_rn(fmaxf(om.y, 0.0f)));
+    float2 sn, cs;
+    sincospi_u24_x2(w1a, w1b, &sn, &cs);
+    out[0] = __fmul2_rn(rho, cs);
+    out[1] = __fmul2_rn(rho, sn);
+    out[2] = z;
+}
+__device__ __forceinline__ void direction2_x2(uint32_t w0a, uint32_t w0b, float2 out[2]) {
+    float2 sn, cs;
+    sincospi_u24_x2(w0a, w0b, &sn, &cs);
+    out[0] = cs;
+    out[1] = sn;
+}
+
+template <bool UNITJ>
+__device__ __forceinline__ float2 add_nb2(float2 h, float J, float sa, float sb) {
+    return UNITJ ? __fadd2_rn(h, f2(sa, sb)) : __fadd2_rn(h, __fmul2_rn(f2s(J), f2(sa, sb)));
+}
+
+// The update of one quad of 4 consecutive same-colour sites of a row, shared by the strip kernel and the TMA-staged
+// kernel (vector_tma_kernel.cuh) so that both perform the same fp32 operations in the same order as the one-thread-per-
+// site kernel (bit-identical results); the sites are handled as two pairs with packed arithmetic.  o_cur = other colour
+// at the same compressed indices, side[c] = the one x-neighbour outside the quad (p = 1: first site of the next quad,
+// p = 0: last site of the previous one), o_prev / o_next = rows y -+ 1, o_zm / o_zp = planes z -+ 1 (D = 3), own = the
+// quad's spins, ctr0 = GLOBAL compressed index of the quad's first site (Philox counter word 0 of site i is ctr0 + i).
+// phase 1: the local fields of the four sites, hp[pr][c] = component c of sites 2 pr and 2 pr + 1
+template <int NC, int D, bool UNITJ>
+__device__ __forceinline__ void vector_quad_field(float Jx, float Jy, float Jz, uint32_t p, const Quad<NC> &o_cur,
+                                                  const float side[NC], const Quad<NC> &o_prev, const Quad<NC> &o_next,
+                                                  const Quad<NC> &o_zm, const Quad<NC> &o_zp, float2 hp[2][NC]) {
+    // order -x, +x, -y, +y, -z, +z, every product and sum rounded separately
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+        // the two x-neighbours are o (same compressed index) and sh (index + 1 if p, index - 1 if not); the
+        // first sum J x(-x) + J x(+x) is commutative, so which of the two is "-x" does not matter
+        const float4 o = o_cur.c[c];
+        const float4 sh = p ? make_float4(o.y, o.z, o.w, side[c]) : make_float4(side[c], o.x, o.y, o.z);
+        float2 v01 = UNITJ ? __fadd2_rn(f2(o.x, o.y), f2(sh.x, sh.y))
+                           : __fadd2_rn(__fmul2_rn(f2s(Jx), f2(o.x, o.y)), __fmul2_rn(f2s(Jx), f2(sh.x, sh.y)));
+        float2 v23 = UNITJ ? __fadd2_rn(f2(o.z, o.w), f2(sh.z, sh.w))
+                           : __fadd2_rn(__fmul2_rn(f2s(Jx), f2(o.z, o.w)), __fmul2_rn(f2s(Jx), f2(sh.z, sh.w)));
+        v01 = add_nb2<UNITJ>(v01, Jy, o_prev.c[c].x, o_prev.c[c].y);
+        v23 = add_nb2<UNITJ>(v23, Jy, o_prev.c[c].z, o_prev.c[c].w);
+        v01 = add_nb2<UNITJ>(v01, Jy, o_next.c[c].x, o_next.c[c].y);
+        v23 = add_nb2<UNITJ>(v23, Jy, o_next.c[c].z, o_next.c[c].w);
+        if (D == 3) {
+            v01 = add_nb2<UNITJ>(v01, Jz, o_zm.c[c].x, o_zm.c[c].y);
+            v23 = add_nb2<UNITJ>(v23, Jz, o_zm.c[c].z, o_zm.c[c].w);
+            v01 = add_nb2<UNITJ>(v01, Jz, o_zp.c[c].x, o_zp.c[c].y);
+            v23 = add_nb2<UNITJ>(v23, Jz, o_zp.c[c].z, o_zp.c[c].w);
+        }
+        hp[0][c] = v01;
+        hp[1][c] = v23;
+    }
+}
+
+// phase 2: proposals, acceptance and the new spins res[c][i] of the four sites from their fields and old spins
+template <int NC, bool HB>
+__device__ __forceinline__ void vector_quad_accept(const VectorArgs &a, const float2 hp[2][NC], const Quad<NC> &own,
+                                                   uint32_t ctr0, uint32_t rho, uint32_t tag, float res[NC][4]) {
+#pragma unroll
+    for (int pr = 0; pr < 2; ++pr) {
+        uint32_t wa[4], wb[4];
+        philox4x32_10(ctr0 + 2 * pr, rho, a.t, tag, a.keys, wa);
+        philox4x32_10(ctr0 + 2 * pr + 1, rho, a.t, tag, a.keys, wb);
+        if (HB && NC == 3) {
+            float ha[3] = {hp[pr][0].x, hp[pr][1].x, hp[pr][NC - 1].x}, hb[3] = {hp[pr][0].y, hp[pr][1].y, hp[pr][NC - 1].y};
+            float sa[3], sb[3];
+            heatbath3(a.beta, ha, wa[0], wa[1], sa);
+            heatbath3(a.beta, hb, wb[0], wb[1], sb);
+#pragma unroll
+            for (int c = 0; c < NC; ++c) { res[c][2 * pr] = sa[c]; res[c][2 * pr + 1] = sb[c]; }
+            continue;
+        }
+        float2 sn[NC], so[NC];
+        uint32_t wacc_a, wacc_b;
+        if (NC == 3) { direction3_x2(wa[0], wa[1], wb[0], wb[1], sn); wacc_a = wa[2]; wacc_b = wb[2]; }
+        else { direction2_x2(wa[0], wb[0], sn); wacc_a = wa[1]; wacc_b = wb[1]; }
+#pragma unroll
+        for (int c = 0; c < NC; ++c) so[c] = pr == 0 ? f2(own.c[c].x, own.c[c].y) : f2(own.c[c].z, own.c[c].w);
+        // acc = (s' - s) . h = -dE; accept iff dE <= 0 (acc >= 0) or u < exp(-beta dE) = exp(beta acc)
+        float2 acc = __fmul2_rn(__fadd2_rn(sn[0], neg2(so[0])), hp[pr][0]);
+#pragma unroll
+        for (int c = 1; c < NC; ++c) acc = __fadd2_rn(acc, __fmul2_rn(__fadd2_rn(sn[c], neg2(so[c])), hp[pr][c]));
+        const float2 arg = __fmul2_rn(f2s(a.beta), acc);
+        const bool acc_a = acc.x >= 0.0f || u24(wacc_a) < expf(arg.x);
+        const bool acc_b = acc.y >= 0.0f || u24(wacc_b) < expf(arg.y);
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            res[c][2 * pr] = acc_a ? sn[c].x : so[c].x;
+            res[c][2 * pr + 1] = acc_b ? sn[c].y : so[c].y;
+        }
+    }
+}
+
+template <int NC, int D, bool UNITJ, bool HB>
+__device__ __forceinline__ void vector_quad_update(const VectorArgs &a, float Jx, float Jy, float Jz, uint32_t p,
+                                                   const Quad<NC> &o_cur, const float side[NC], const Quad<NC> &o_prev,
+                                                   const Quad<NC> &o_next, const Quad<NC> &o_zm, const Quad<NC> &o_zp,
+                                                   const Quad<NC> &own, uint32_t ctr0, uint32_t rho, uint32_t tag,
+                                                   float res[NC][4]) {
+    float2 hp[2][NC];
+    vector_quad_field<NC, D, UNITJ>(Jx, Jy, Jz, p, o_cur, side, o_prev, o_next, o_zm, o_zp, hp);
+    vector_quad_accept<NC, HB>(a, hp, own, ctr0, rho, tag, res);
+}
+
 template <int NC, int D, bool UNITJ, int K, bool HB = false>
 __global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_constant__ VectorArgs a) {
     const Geometry &g = a.g;
@@ -241,53 +383,9 @@ __global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_const
             float side[NC];
 #pragma unroll
             for (int c = 0; c < NC; ++c) side[c] = __ldg(other + (size_t)c * Nh + row + (p ? side_p1 : side_p0));
-            // local field, order -x, +x, -y, +y, -z, +z, every product and sum rounded separately
-            float h[4][NC];
-#pragma unroll
-            for (int c = 0; c < NC; ++c) {
-                // the two x-neighbours are o (same compressed index) and sh (index + 1 if p, index - 1 if not); the
-                // first sum J x(-x) + J x(+x) is commutative, so which of the two is "-x" does not matter
-                const float4 o = o_cur.c[c];
-                const float4 sh = p ? make_float4(o.y, o.z, o.w, side[c]) : make_float4(side[c], o.x, o.y, o.z);
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    float v = UNITJ ? __fadd_rn(lane_of(o, i), lane_of(sh, i))
-                                    : __fadd_rn(__fmul_rn(Jx, lane_of(o, i)), __fmul_rn(Jx, lane_of(sh, i)));
-                    v = add_nb<UNITJ>(v, Jy, lane_of(o_prev.c[c], i));
-                    v = add_nb<UNITJ>(v, Jy, lane_of(o_next.c[c], i));
-                    if (D == 3) {
-                        v = add_nb<UNITJ>(v, Jz, lane_of(o_zm.c[c], i));
-                        v = add_nb<UNITJ>(v, Jz, lane_of(o_zp.c[c], i));
-                    }
-                    h[i][c] = v;
-                }
-            }
             float res[NC][4];
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                uint32_t w[4];
-                philox4x32_10(off + i + g.j_off, rho, a.t, tag, a.keys, w);
-                float sn[NC], so[NC];
-                uint32_t wacc;
-                if (HB && NC == 3) {
-                    float h3[3] = {h[i][0], h[i][1], h[i][NC - 1]}, s3[3];
-                    heatbath3(a.beta, h3, w[0], w[1], s3);
-#pragma unroll
-                    for (int c = 0; c < NC; ++c) res[c][i] = s3[c];
-                    continue;
-                }
-                if (NC == 3) { direction3(w[0], w[1], sn); wacc = w[2]; }
-                else { direction2(w[0], sn); wacc = w[1]; }
-#pragma unroll
-                for (int c = 0; c < NC; ++c) so[c] = lane_of(own.c[c], i);
-                float acc = __fmul_rn(__fsub_rn(sn[0], so[0]), h[i][0]);
-#pragma unroll
-                for (int c = 1; c < NC; ++c) acc = __fadd_rn(acc, __fmul_rn(__fsub_rn(sn[c], so[c]), h[i][c]));
-                const float dE = -acc;
-                const bool accept = dE <= 0.0f || u24(wacc) < expf(__fmul_rn(-a.beta, dE));
-#pragma unroll
-                for (int c = 0; c < NC; ++c) res[c][i] = accept ? sn[c] : so[c];
-            }
+            vector_quad_update<NC, D, UNITJ, HB>(a, Jx, Jy, Jz, p, o_cur, side, o_prev, o_next, o_zm, o_zp, own,
+                                                 off + g.j_off, rho, tag, res);
 #pragma unroll
             for (int c = 0; c < NC; ++c)
                 *(float4 *)(mine + (size_t)c * Nh + off) = make_float4(res[c][0], res[c][1], res[c][2], res[c][3]);

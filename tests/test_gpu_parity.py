@@ -320,6 +320,7 @@ def test_vector_strip_rows_and_plain_kernel_agree_bitwise(P, n, dims, J):
     for rows in (0, 1, 2, 4):
         for block in (64, 128):
             G = P.SpinSystem(dims, n=n, storage="fp32", coupling=coupling, J=J, seed=5)
+            G.set_option(P.OPT_TMA_KERNELS, 0)   # the strip kernel itself (d = 3 would take the TMA-staged one: test_gpu_tma.py)
             G.set_strip_rows(rows)
             G.set_launch_shape(block, 1, 1)
             G.sweep(beta, 4)
