@@ -87,6 +87,59 @@ __device__ __forceinline__ uint32_t ising_new_word(const IsingArgs &a, uint32_t 
     }
 }
 
+// Metropolis word with the comparison cut after DEFER_CALLS calls: returns raw ^ (flip mask so far); eq = lanes still
+// undecided (their final flip bits are lt_mask_select_tail of the same unit and masks m[], XORed into the word)
+template <int D>
+__device__ __forceinline__ uint32_t ising_new_word_head(const IsingArgs &a, uint32_t t, uint32_t colour, uint32_t unit, uint32_t rho,
+                                                        uint32_t raw, const uint32_t av[6], uint32_t &eq, uint32_t m[D]) {
+    if (D == 2) {
+        const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
+        const uint32_t ge2 = c1 | (s1 & av[3]), ge1 = av[0] | av[1] | av[2] | av[3];
+        m[0] = ge1 & ~ge2; m[1] = ~ge1;
+        return raw ^ (ge2 | lt_mask_select_head<D>(a, t, colour, unit, rho, m, eq));
+    }
+    const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
+    const uint32_t s2 = av[3] ^ av[4] ^ av[5], c2 = maj3(av[3], av[4], av[5]);
+    const uint32_t b0 = s1 ^ s2, c3 = s1 & s2;
+    const uint32_t b1 = c1 ^ c2 ^ c3, b2 = maj3(c1, c2, c3);
+    const uint32_t ge3 = b2 | (b1 & b0);
+    m[0] = b1 & ~b0 & ~b2; m[1] = b0 & ~b1 & ~b2; m[D - 1] = ~(b0 | b1 | b2);
+    return raw ^ (ge3 | lt_mask_select_head<D>(a, t, colour, unit, rho, m, eq));
+}
+
+// Owner side of the deferred tail: the word is complete (returns true: store it) or it went into the warp's queue
+// (returns false: the drain stores it); a full queue makes the owner finish the unit itself.
+template <int D>
+__device__ __forceinline__ bool defer_or_finish(const IsingArgs &a, DeferQueue &q, uint32_t warp, uint32_t unit, uint32_t rho,
+                                                uint32_t eq, const uint32_t m[D], uint32_t &word, uint32_t index) {
+    if (eq == 0u) return true;
+    const uint32_t pos = atomicAdd(&q.n[warp], 1u);
+    if (pos >= (uint32_t)DEFER_CAP) {
+        word ^= lt_mask_select_tail<D>(a, a.t, a.colour, unit, rho, m, eq);
+        return true;
+    }
+    q.f[warp][0][pos] = unit; q.f[warp][1][pos] = rho; q.f[warp][2][pos] = eq;
+    q.f[warp][3][pos] = m[0]; q.f[warp][4][pos] = D == 3 ? m[1] : 0u;
+    q.f[warp][5][pos] = word; q.f[warp][6][pos] = index;
+    return false;
+}
+
+// Drain: lane l finishes pending unit l (l + 32, ... never: the queue holds at most DEFER_CAP = 32 entries).
+// store(index, word) writes the finished word.  Call with the whole warp converged.
+template <int D, typename Store>
+__device__ __forceinline__ void defer_drain(const IsingArgs &a, DeferQueue &q, uint32_t warp, uint32_t lane, Store store) {
+    __syncwarp();
+    const uint32_t n = min(q.n[warp], (uint32_t)DEFER_CAP);
+    if (lane < n) {
+        uint32_t m[D];
+        m[0] = q.f[warp][3][lane];
+        if (D == 3) m[1] = q.f[warp][4][lane];
+        m[D - 1] = 0u;   // the last mask never enters select_digit (its lanes take the default digit)
+        const uint32_t lt = lt_mask_select_tail<D>(a, a.t, a.colour, q.f[warp][0][lane], q.f[warp][1][lane], m, q.f[warp][2][lane]);
+        store(q.f[warp][6][lane], q.f[warp][5][lane] ^ lt);
+    }
+}
+
 // Fused measurement: every bond joins the two colours, so the colour-1 half-sweep
 // has, in the masks it formed anyway, everything E and M need.  Per 32-site word of colour 1 after its update:
 // E += 2 (#unsatisfied bonds) - (#bonds), M += 64 - 2 (minus spins of this word and of the colour-0 word at the same
@@ -156,7 +209,13 @@ __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(cons
     const uint32_t nstrip = (Ly + K - 1) / K;
     const uint32_t per_replica = WX * nstrip * Lz;
     const uint32_t item = blockIdx.x * blockDim.x + threadIdx.x;
-    if (item >= per_replica * a.R) return;
+    // The deferred tail of the digit comparison (ising_bitpack_strip_halfsweep) is compiled out here: measured on B200 the
+    // queue's live state pushes the d = 2 instance past its 72 registers (7 CTAs per SM): 87.7 us against 72.8 us without
+    constexpr bool DEFER = false;
+    __shared__ DeferQueue dq;
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
+    if (DEFER) { if (lane == 0u) dq.n[warp] = 0u; __syncwarp(); }
+    if (item < per_replica * a.R) {
     const uint32_t r = item / per_replica, it = item - r * per_replica;
     const uint32_t sz = fdiv(it, g.divWX), w = it - sz * WX;      // sz = strip + nstrip * z
     const uint32_t z = sz / nstrip, y0 = (sz - z * nstrip) * K;
@@ -211,15 +270,28 @@ __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(cons
             if (D == 3) { av[4] = s ^ o_zm; av[5] = s ^ o_zp; }
             const uint32_t unit = unit0 + (uint32_t)k * WX;
             if (D == 2) { av[4] = 0u; av[5] = 0u; }
-            const uint32_t fresh = ising_new_word<D, HB>(a, a.t, a.colour, unit, rho, raw, av);
-            int8_store_unit(mine + zoff + off, fresh);
-            if (MEAS) fused_word_sums<D>(av, raw, fresh, o_cur, e_sum, m_sum);
+            if constexpr (DEFER) {
+                uint32_t eq, mm[D];
+                uint32_t fresh = ising_new_word_head<D>(a, a.t, a.colour, unit, rho, raw, av, eq, mm);
+                // index of the unit in the whole colour array (32-byte units)
+                const uint32_t uidx = (uint32_t)(((size_t)r * g.Nh + zoff + off) >> 5);
+                if (defer_or_finish<D>(a, dq, warp, unit, rho, eq, mm, fresh, uidx)) int8_store_unit(mine + zoff + off, fresh);
+            } else {
+                const uint32_t fresh = ising_new_word<D, HB>(a, a.t, a.colour, unit, rho, raw, av);
+                int8_store_unit(mine + zoff + off, fresh);
+                if (MEAS) fused_word_sums<D>(av, raw, fresh, o_cur, e_sum, m_sum);
+            }
             o_prev = o_cur;
             o_cur = o_next;
             p ^= 1u;
         }
     }
     if (MEAS) fused_commit(a.acc, r, e_sum, m_sum);
+    }
+    if constexpr (DEFER) {
+        uint8_t *base = (uint8_t *)a.s[a.colour];
+        defer_drain<D>(a, dq, warp, lane, [&](uint32_t uidx, uint32_t word) { int8_store_unit(base + 32u * (size_t)uidx, word); });
+    }
 }
 
 // The same strip walk for BIT-PACKED storage with uniform couplings (own random stream per replica or one replica):
@@ -233,7 +305,11 @@ __global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __gri
     const uint32_t nstrip = (Ly + K - 1) / K;
     const uint32_t per_replica = WX * nstrip * Lz;
     const uint32_t item = blockIdx.x * blockDim.x + threadIdx.x;
-    if (item >= per_replica * a.R) return;
+    constexpr bool DEFER = !HB && !MEAS;   // deferred tail of the digit comparison, as in ising_int8_halfsweep
+    __shared__ DeferQueue dq;
+    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
+    if (DEFER) { if (lane == 0u) dq.n[warp] = 0u; __syncwarp(); }
+    if (item < per_replica * a.R) {
     const uint32_t r = item / per_replica, it = item - r * per_replica;
     const uint32_t sz = fdiv(it, g.divWX), w = it - sz * WX;      // sz = strip + nstrip * z
     const uint32_t z = sz / nstrip, y0 = (sz - z * nstrip) * K;
@@ -276,15 +352,27 @@ __global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __gri
             uint32_t av[6];
             av[0] = s ^ o_cur; av[1] = s ^ side; av[2] = s ^ o_prev; av[3] = s ^ o_next;
             av[4] = D == 3 ? s ^ o_zm : 0u; av[5] = D == 3 ? s ^ o_zp : 0u;
-            const uint32_t fresh = ising_new_word<D, HB>(a, a.t, a.colour, unit0 + (uint32_t)k * WX, rho, raw, av);
-            mine[zoff + off] = fresh;
-            if (MEAS) fused_word_sums<D>(av, raw, fresh, o_cur, e_sum, m_sum);
+            if constexpr (DEFER) {
+                uint32_t eq, mm[D];
+                const uint32_t unit = unit0 + (uint32_t)k * WX;
+                uint32_t fresh = ising_new_word_head<D>(a, a.t, a.colour, unit, rho, raw, av, eq, mm);
+                if (defer_or_finish<D>(a, dq, warp, unit, rho, eq, mm, fresh, r * g.NW + zoff + off)) mine[zoff + off] = fresh;
+            } else {
+                const uint32_t fresh = ising_new_word<D, HB>(a, a.t, a.colour, unit0 + (uint32_t)k * WX, rho, raw, av);
+                mine[zoff + off] = fresh;
+                if (MEAS) fused_word_sums<D>(av, raw, fresh, o_cur, e_sum, m_sum);
+            }
             o_prev = o_cur;
             o_cur = o_next;
             p ^= 1u;
         }
     }
     if (MEAS) fused_commit(a.acc, r, e_sum, m_sum);
+    }
+    if constexpr (DEFER) {
+        uint32_t *base = (uint32_t *)a.s[a.colour];
+        defer_drain<D>(a, dq, warp, lane, [&](uint32_t widx, uint32_t word) { base[widx] = word; });
+    }
 }
 
 }  // namespace spin

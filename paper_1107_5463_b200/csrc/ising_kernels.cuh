@@ -92,6 +92,71 @@ __device__ __forceinline__ uint32_t lt_mask_select(const IsingArgs &a, uint32_t 
     return lt;
 }
 
+// ------------------------------------------------------------------ deferred tail of U < T ----
+// A warp that runs the lazy digit loop above pays for its slowest thread: 3.45 Philox calls per warp against 2.25 per
+// thread (profiles/r01d).  The strip kernels therefore split the comparison: DEFER_CALLS calls are made unconditionally
+// by every thread (no divergence, the calls interleave), and a unit that still has undecided lanes afterwards (about one
+// in ten) is pushed into a per-warp shared-memory queue; after its strip the warp drains the queue with one pending unit
+// per lane, so the tail calls run with all lanes busy.  The contract (R-16) is unchanged: every lane's
+// decision is still "U < T" on the same digits.
+constexpr int DEFER_CALLS = 2;
+constexpr int DEFER_CAP = 32;          // queue entries per warp; a thread that finds it full finishes its unit itself
+constexpr int DEFER_FIELDS = 6;        // unit, rho, eq, m[0], m[1], provisional word; + the word's index in its array
+struct DeferQueue {
+    uint32_t n[4];
+    uint32_t f[4][DEFER_FIELDS + 1][DEFER_CAP];
+};
+
+// digit k of the threshold each lane compares against: lanes of m[th] use T(4 (th + 1)), the rest the last one
+template <int NT>
+__device__ __forceinline__ uint32_t select_digit(const IsingArgs &a, const uint32_t m[NT], int dg) {
+    uint32_t tk = tab_digit<false>(a, NT - 1, dg);
+#pragma unroll
+    for (int th = NT - 2; th >= 0; --th) tk = (m[th] & tab_digit<false>(a, th, dg)) | (~m[th] & tk);
+    return tk;
+}
+
+// calls [0, DEFER_CALLS) of the comparison, unconditionally; returns lt, leaves the undecided lanes in eq
+template <int NT>
+__device__ __forceinline__ uint32_t lt_mask_select_head(const IsingArgs &a, uint32_t t, uint32_t colour, uint32_t unit, uint32_t rho,
+                                                        const uint32_t m[NT], uint32_t &eq_out) {
+    uint32_t lt = 0u, eq = 0u;
+#pragma unroll
+    for (int th = 0; th < NT; ++th) { lt |= m[th] & tab_always<false>(a, th); eq |= m[th] & ~tab_always<false>(a, th); }
+#pragma unroll
+    for (int call = 0; call < DEFER_CALLS; ++call) {
+        uint32_t w[4];
+        philox4x32_10(unit, rho, t, make_tag(colour, DOM_ISING_UPDATE, call), a.keys, w);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const uint32_t tk = select_digit<NT>(a, m, 4 * call + k);
+            lt |= eq & ~w[k] & tk;
+            eq &= ~(w[k] ^ tk);
+        }
+    }
+    eq_out = eq;
+    return lt;
+}
+
+// calls [DEFER_CALLS, 8) for the lanes still in eq, lazily; returns the lanes that turn out to have U < T
+template <int NT>
+__device__ __forceinline__ uint32_t lt_mask_select_tail(const IsingArgs &a, uint32_t t, uint32_t colour, uint32_t unit, uint32_t rho,
+                                                        const uint32_t m[NT], uint32_t eq) {
+    uint32_t lt = 0u;
+    for (int call = DEFER_CALLS; call < 8; ++call) {
+        if (eq == 0u) break;
+        uint32_t w[4];
+        philox4x32_10(unit, rho, t, make_tag(colour, DOM_ISING_UPDATE, call), a.keys, w);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const uint32_t tk = select_digit<NT>(a, m, 4 * call + k);
+            lt |= eq & ~w[k] & tk;
+            eq &= ~(w[k] ^ tk);
+        }
+    }
+    return lt;
+}
+
 __device__ __forceinline__ uint32_t maj3(uint32_t x, uint32_t y, uint32_t z) { return (x & y) | (z & (x | y)); }
 
 // m[k] = lanes in which exactly k of the 2 D masks b[] are set (k = 0 .. 2 D), bit-sliced with full adders
