@@ -57,6 +57,8 @@ def lib():
         L.oracle_sweep.restype = C.c_int
         L.oracle_sweep_count.argtypes = [C.c_void_p, C.c_double, C.c_int64, C.POINTER(C.c_int64)]
         L.oracle_sweep_count.restype = C.c_int
+        L.oracle_last_sweep_dE.argtypes = [C.c_void_p]
+        L.oracle_last_sweep_dE.restype = C.c_double
         L.oracle_measure.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.oracle_measure.restype = C.c_int
         L.oracle_get_spins.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64]
@@ -179,6 +181,10 @@ class System:
         if rc:
             raise RuntimeError("oracle_sweep_count failed (%d)" % rc)
         return acc
+
+    def last_sweep_dE(self):
+        """Sum of the dE of every move accepted in the last Metropolis sweep (bookkeeping)."""
+        return float(lib().oracle_last_sweep_dE(self._h))
 
     def measure(self):
         E = np.zeros(self.R, dtype=np.float64)

@@ -209,6 +209,9 @@ struct oracle_system {
     std::vector<int8_t> s1;    /* n = 1 : [r][i]          */
     std::vector<float> sv;     /* n >= 2: [r][i][n]       */
     std::vector<int8_t> bonds; /* BOND_PM1: [r][mu][i]    */
+    /* bookkeeping only (the accepted move changes H by dE): sum over the last sweep, all replicas, of
+     * the dE of every accepted Metropolis move, as the sweep itself computed it; never read by the update */
+    double dE_accepted = 0.0;
 
     int64_t site(int x, int y, int z) const { return (int64_t)x + (int64_t)Lx * ((int64_t)y + (int64_t)Ly * (int64_t)z); }
     int64_t compressed(int x, int y, int z) const { return (int64_t)(x >> 1) + (int64_t)(Lx / 2) * ((int64_t)y + (int64_t)Ly * (int64_t)z); }
@@ -249,6 +252,7 @@ int neighbours(const oracle_system &S, int r, int x, int y, int z, Neighbour nb[
 
 int64_t sweep_ising(oracle_system &S, double beta) {
     int64_t accepted = 0;
+    S.dE_accepted = 0.0;
     /* table of the Boltzmann factors that can occur: dE = 2 s h, |h| <= 2d */
     uint64_t T[13], Thb[13];
     for (int dE = 0; dE <= 12; ++dE) T[dE] = threshold(beta, dE);
@@ -286,6 +290,7 @@ int64_t sweep_ising(oracle_system &S, double beta) {
                         if (dE <= 0 || (uint64_t)U < T[dE]) {
                             s[i] = (int8_t)(-s[i]);
                             ++accepted;
+                            S.dE_accepted += (double)dE;
                         }
                     }
         }
@@ -296,6 +301,7 @@ int64_t sweep_ising(oracle_system &S, double beta) {
 
 int64_t sweep_vector(oracle_system &S, double beta) {
     int64_t accepted = 0;
+    S.dE_accepted = 0.0;
     const float beta_f = (float)beta;
     const uint32_t t32 = (uint32_t)S.t;
     const int n = S.n;
@@ -342,6 +348,7 @@ int64_t sweep_vector(oracle_system &S, double beta) {
                         if (vector_accept(beta_f, dE, w_accept)) {
                             for (int a = 0; a < n; ++a) s[(size_t)i * n + a] = snew[a];
                             ++accepted;
+                            S.dE_accepted += (double)dE;
                         }
                     }
         }
@@ -479,6 +486,8 @@ int oracle_sweep_count(oracle_system *S, double beta, int64_t n_sweeps, int64_t 
     }
     return 0;
 }
+
+double oracle_last_sweep_dE(const oracle_system *S) { return S ? S->dE_accepted : 0.0; }
 
 int oracle_sweep(oracle_system *S, double beta, int64_t n_sweeps) { return oracle_sweep_count(S, beta, n_sweeps, nullptr); }
 

@@ -91,6 +91,9 @@ void oracle_heatbath3(double beta, const float h[3], uint32_t w0, uint32_t w1, f
 int oracle_sweep(oracle_system *, double beta, int64_t n_sweeps);
 /* Same, but also returns, per sweep, how many proposals were accepted. */
 int oracle_sweep_count(oracle_system *, double beta, int64_t n_sweeps, int64_t *accepted);
+/* Bookkeeping: the sum, over the LAST Metropolis sweep and all replicas, of the energy change dE of
+ * every accepted move, as the sweep computed it from its local field.  The update never reads it. */
+double oracle_last_sweep_dE(const oracle_system *);
 
 /* E[r] = -sum_bonds J s.s ; M[r*n + a] = sum_i s_i^a. */
 int oracle_measure(const oracle_system *, double *E, double *M);

@@ -166,3 +166,30 @@ def sc_ising_series_minus_e(K):
     dv = 1 - v * v
     val = 3 * v + (12 * v ** 3 + 132 * v ** 5 + 1500 * v ** 7) * dv
     return float(val), float(1980 * 10 * v ** 9)  # crude bound on the first omitted term
+
+
+# ----------------------------------------------------------------- 3D high-T series, O(n)
+def on_bond_function(n, K):
+    """t(K) = <s.s'> of two O(n) unit spins joined by one bond: tanh K, I_1/I_0, coth K - 1/K (n = 1, 2, 3)."""
+    mp.mp.dps = 40
+    K = mp.mpf(K)
+    if n == 1:
+        return mp.tanh(K)
+    if n == 2:
+        return mp.besseli(1, K) / mp.besseli(0, K)
+    if n == 3:
+        return mp.coth(K) - 1 / K
+    raise ValueError(n)
+
+
+def sc_on_series_minus_e(n, K):
+    """-e of the simple-cubic O(n) model to the first lattice term of the high-temperature expansion, derived from the
+    definition (Eq. (1)): integrating out bond by bond, ln Z / N = const + 3 ln lambda_0(K) + 3 n t^4 + O(t^6)
+    -- 3 bonds per site, 3 elementary plaquettes per site, a closed loop of four bonds weighs n t^4 (the trace over the n
+    components; n = 1 gives the Ising series' 3 v^4) -- and -e = d(ln Z / N)/dK with (ln lambda_0)' = t:
+        -e = 3 t + 12 n t^3 t'(K).
+    Returns (value, scale of the first omitted term ~ 22 n 6 t^5 t')."""
+    t = on_bond_function(n, K)
+    dt = 1 - t * t - (n - 1) * t / mp.mpf(K)   # t' of the three bond functions above (Bessel-ratio identity)
+    val = 3 * t + 12 * n * t ** 3 * dt
+    return float(val), float(132 * n * t ** 5 * dt)

@@ -77,3 +77,19 @@ def test_chain_values():
 
 def test_series():
     assert X.sc_ising_series_minus_e(0.1)[0] == pytest.approx(G["series3d_K0.1"], abs=1e-7)
+
+
+def test_on_series_reduces_to_the_ising_series_and_to_its_leading_term():
+    """sc_on_series_minus_e: n = 1 must reproduce the first two terms of the Ising series 3 v + 12 v^3 (1 - v^2), and
+    for every n the leading behaviour is 3 K / n."""
+    import numpy as np
+    K = 0.05
+    v = np.tanh(K)
+    val, omitted = X.sc_on_series_minus_e(1, K)
+    assert abs(val - (3 * v + 12 * v ** 3 * (1 - v * v))) < 1e-12
+    full, _ = X.sc_ising_series_minus_e(K)
+    assert abs(val - full) < 2 * omitted
+    for n in (2, 3):
+        val, omitted = X.sc_on_series_minus_e(n, K)
+        assert abs(val - 3 * K / n) < 3 * K / n * 4 * K * K
+        assert omitted < 3e-6

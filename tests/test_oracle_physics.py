@@ -176,6 +176,18 @@ def test_2d_ising_critical_energy_is_kaufmans_finite_lattice_value(oracle):
     assert abs(X.kaufman_energy_per_spin(L, 1.02 * BETA_C2) - exact) > 10 * err
 
 
+def test_2d_ising_critical_energy_kaufman_L32(oracle):
+    """SURVEY.md P7 asks for L = 16 and 32: the same pin on the 32 x 32 torus (16 chains x 30 000 sweeps)."""
+    L = 32
+    exact = X.kaufman_energy_per_spin(L, BETA_C2)
+    e, _ = _replica_means(oracle, (L, L, 1), BETA_C2, R=16, therm=1500, sweeps=30000, seed=1107)
+    mean, err = _mean_and_error(e)
+    assert err < 3.5e-3
+    assert abs(mean - exact) < 3 * err, (mean, err, exact)
+    assert abs(mean + np.sqrt(2.0)) > 4 * err
+    assert abs(exact - X.kaufman_energy_per_spin(16, BETA_C2)) > 4 * err   # L = 32 is told apart from L = 16
+
+
 def test_2d_ising_ordered_phase_matches_onsager_yang(oracle):
     """P8: beta = 0.5, cold start, L = 32: <|m|> = (1 - sinh^-4 2beta)^(1/8), <e> = Onsager."""
     L = 32
@@ -241,6 +253,20 @@ def test_3d_ising_high_temperature_series(oracle):
     mean, err = _mean_and_error(-e)
     assert err < 6e-4
     assert abs(mean - minus_e) < 3 * err + 2 * omitted, (mean, err, minus_e)
+
+
+@pytest.mark.parametrize("n", [2, 3])
+def test_3d_vector_models_high_temperature_series(oracle, n):
+    """The genuinely three-dimensional n >= 2 path (all six neighbour terms of sweep_vector): 8^3 at
+    K = 0.05 against -e = 3 t + 12 n t^3 t' (exact_results.sc_on_series_minus_e, derived from the definition).  A dropped
+    or doubled y / z term in the local field moves -e by a third of its value, a missing lattice term by 0.25 %."""
+    K = 0.05
+    minus_e, omitted = X.sc_on_series_minus_e(n, K)
+    e, _ = _replica_means(oracle, (8, 8, 8), K, R=16, therm=50, sweeps=1500, seed=40 + n, n=n)
+    mean, err = _mean_and_error(-e)
+    assert err < 6e-4
+    assert abs(mean - minus_e) < 3 * err + 2 * omitted, (n, mean, err, minus_e)
+    assert abs(2.0 / 3.0 * minus_e - mean) > 10 * err     # resolving power: one missing direction is a many-sigma effect
 
 
 # --------------------------------------------------------------------------- P14: continuous spins

@@ -183,19 +183,40 @@ def test_sweep_counter_composition_and_resume(oracle):
 
 
 def test_energy_change_equals_sum_of_accepted_dE_vector_models(oracle):
-    """P14 (bookkeeping part): unit norm is preserved and measure() is consistent with the local field."""
+    """P14 (bookkeeping part): over one sweep the energy of Eq. (1), re-measured from the spins, changes
+    by exactly the sum of the dE of the accepted moves as the sweep computed them from its local field (fp32 there, so
+    equal up to rounding).  A wrong neighbour, sign or coupling in any of the six field terms breaks the balance."""
     for n in (2, 3):
         S = oracle.System((8, 6, 4), n=n, seed=12)
         s = S.get_spins()[0].astype(np.float64)
         assert np.allclose((s ** 2).sum(axis=1), 1.0, atol=4e-7)
-        S.sweep(0.7, 3)
+        for beta in (0.7, 0.7, 2.5, 0.0):
+            E0, _ = S.measure()
+            acc = S.sweep_count(beta, 1)
+            E1, M = S.measure()
+            assert 0 < acc[0] <= S.N
+            dE = S.last_sweep_dE()
+            assert abs((E1[0] - E0[0]) - dE) <= 1e-6 * S.N, (n, beta, E1[0] - E0[0], dE)
+            assert abs(E1[0] - E0[0]) > 1e-3        # the balance is not 0 = 0
         s = S.get_spins()[0].astype(np.float64)
         assert np.allclose((s ** 2).sum(axis=1), 1.0, atol=4e-7)
-        E, M = S.measure()
         g = s.reshape(4, 6, 8, n)
         e = -sum((g * np.roll(g, -1, axis=2 - mu)).sum() for mu in range(3))
-        assert E[0] == pytest.approx(e, rel=1e-12)
+        assert E1[0] == pytest.approx(e, rel=1e-12)
         assert np.allclose(M[0], s.sum(axis=0), rtol=1e-12)
+
+
+def test_energy_change_equals_sum_of_accepted_dE_ising(oracle):
+    """The same balance for n = 1, exact in integers: uniform, per-direction and +-J couplings, 2D and 3D."""
+    cases = [dict(dims=(8, 6, 4)), dict(dims=(8, 6, 1)), dict(dims=(6, 4, 2), coupling_kind=oracle.J_PER_DIRECTION, J=(1.0, -1.0, 0.0)),
+             dict(dims=(8, 6, 4), coupling_kind=oracle.J_BOND_PM1, n_replicas=2)]
+    for kw in cases:
+        S = oracle.System(kw.pop("dims"), n=1, seed=5, **kw)
+        for beta in (0.3, 0.3, 1.0, 0.0):
+            E0, _ = S.measure()
+            S.sweep(beta, 1)
+            E1, _ = S.measure()
+            assert (E1 - E0).sum() == S.last_sweep_dE()
 
 
 def test_invalid_arguments_are_rejected(oracle):
