@@ -150,7 +150,15 @@ enum { SPIN_OPT_PLAIN_KERNELS = 0,
         * -1 (default) = only for the colour-1 half-sweep of spin_sweep_record, where its fused E / M saves the
         * measurement pass; elsewhere the strip kernel is the faster one on B200 (profiles/).  Spins are bit-identical
         * whichever kernel runs. */
-       SPIN_OPT_TMA_KERNELS = 1 };
+       SPIN_OPT_TMA_KERNELS = 1,
+       /* Bulk L2 prefetch (cp.async.bulk.prefetch.L2) issued by the +-J quad kernel (value = replicas ahead) and the
+        * n >= 2 strip kernel (value = CTAs ahead): -1 (default) = each kernel's own distance, 0 = off.  A pure
+        * performance hint: results never depend on it. */
+       SPIN_OPT_L2_PREFETCH = 2,
+       /* A/B knob: 0 (default) = the tuned kernel of each family; 1 = the alternative kept beside it
+        * (+-J shared stream: the cooperative kernel, one CTA of replica-chunk warps per 32 quads, instead of one thread per quad and all replicas).  Results never
+        * depend on it. */
+       SPIN_OPT_KERNEL_VARIANT = 3 };
 spin_status spin_set_option(spin_system *s, int32_t option, int64_t value);
 
 /* Frees the handle only; never the workspace. */

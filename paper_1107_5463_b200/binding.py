@@ -16,6 +16,8 @@ J_UNIFORM, J_PER_DIRECTION, J_BOND_PM1 = 0, 1, 2
 INIT_HOT, INIT_COLD = 0, 1
 OPT_PLAIN_KERNELS = 0
 OPT_TMA_KERNELS = 1
+OPT_L2_PREFETCH = 2
+OPT_KERNEL_VARIANT = 3
 UPDATE_METROPOLIS, UPDATE_HEATBATH = 0, 1
 _RULE = {"metropolis": UPDATE_METROPOLIS, "heatbath": UPDATE_HEATBATH}
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE_TOO_SMALL, ERR_CUDA, ERR_STATE = range(6)

@@ -38,6 +38,14 @@ __host__ __device__ __forceinline__ uint32_t make_tag(uint32_t colour, uint32_t 
 }
 
 // ---------------------------------------------------------------------------------------------
+// Bulk L2 prefetch (sm_90+: cp.async.bulk.prefetch.L2): one thread asks the memory system to bring `bytes` contiguous
+// bytes (a multiple of 16, 16-byte aligned) from HBM into L2.  No register or shared-memory cost; the half-sweep kernels
+// use it to turn the DRAM latency of data that a later CTA / the next replica iteration will load into an L2 hit.
+__device__ __forceinline__ void l2_prefetch_bulk(const void *p, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------
 // Division by a run-time constant fixed at handle creation: q = (n * mul) >> (32 + shift) for
 // n < 2^31 (round-up method).  Two instructions instead of ~20.
 struct FastDiv {

@@ -140,28 +140,6 @@ __device__ __forceinline__ void defer_drain(const IsingArgs &a, DeferQueue &q, u
     }
 }
 
-// Fused measurement: every bond joins the two colours, so the colour-1 half-sweep
-// has, in the masks it formed anyway, everything E and M need.  Per 32-site word of colour 1 after its update:
-// E += 2 (#unsatisfied bonds) - (#bonds), M += 64 - 2 (minus spins of this word and of the colour-0 word at the same
-// index).  Lanes of a warp that serve the same replica are summed with one warp reduction, then one atomic each.
-template <int D>
-__device__ __forceinline__ void fused_word_sums(const uint32_t av[6], uint32_t raw, uint32_t fresh, uint32_t o_same, int &e, int &m) {
-    const uint32_t flip = raw ^ fresh;   // a flipped lane inverts all its bond masks
-    int unsat = __popc(av[0] ^ flip) + __popc(av[1] ^ flip) + __popc(av[2] ^ flip) + __popc(av[3] ^ flip);
-    if (D == 3) unsat += __popc(av[4] ^ flip) + __popc(av[5] ^ flip);
-    e += 2 * unsat - 2 * D * 32;
-    m += 64 - 2 * (__popc(fresh) + __popc(o_same));
-}
-__device__ __forceinline__ void fused_commit(long long *acc, uint32_t r, int e, int m) {
-    const unsigned active = __activemask();
-    const unsigned peers = __match_any_sync(active, r);
-    const int es = __reduce_add_sync(peers, e), ms = __reduce_add_sync(peers, m);
-    if ((threadIdx.x & 31u) == (uint32_t)(__ffs(peers) - 1)) {
-        atomicAdd((unsigned long long *)&acc[2 * r], (unsigned long long)(long long)es);
-        atomicAdd((unsigned long long *)&acc[2 * r + 1], (unsigned long long)(long long)ms);
-    }
-}
-
 // the 32 bytes of a unit as loaded, before packing (kept in flight while the previous row is being updated)
 struct Int8RawUnit {
     uint4 lo, hi;
@@ -286,7 +264,7 @@ __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(cons
             p ^= 1u;
         }
     }
-    if (MEAS) fused_commit(a.acc, r, e_sum, m_sum);
+    if (MEAS) fused_commit(a, r, e_sum, m_sum);
     }
     if constexpr (DEFER) {
         uint8_t *base = (uint8_t *)a.s[a.colour];
@@ -367,7 +345,7 @@ __global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __gri
             p ^= 1u;
         }
     }
-    if (MEAS) fused_commit(a.acc, r, e_sum, m_sum);
+    if (MEAS) fused_commit(a, r, e_sum, m_sum);
     }
     if constexpr (DEFER) {
         uint32_t *base = (uint32_t *)a.s[a.colour];

@@ -20,8 +20,11 @@ struct IsingArgs {
     int32_t Jdir[3];        // generic kernel: coupling per direction in {-1, 0, +1}
     uint32_t jneg;          // fast kernels: 1 iff the uniform coupling is -1
     uint32_t rule;          // 0 Metropolis (Eq. (2)), 1 heat bath
-    long long *acc;         // [R][2] energy / magnetisation accumulators (fused measurement of the strip kernels)
+    long long *acc;         // [acc_slots][R][2] energy / magnetisation accumulators (measurement kernels and fused measurement)
+    uint32_t acc_slots;     // power of two: a CTA adds into slot blockIdx.x & (acc_slots - 1), so that atomics on one address
+                            // do not serialise (65 536 of them per launch on two addresses cost 18 us); the finalize sums the slots
     HeatBathTable hb;       // filled when rule = 1
+    uint32_t prefetch;      // L2 prefetch distance (0 = off): replicas ahead (+-J quad kernel) / CTAs ahead (strip kernels)
 };
 
 // digit dg / "always" mask of threshold th of the table in use: HB = false -> Metropolis factors T(4 (th + 1)),
@@ -158,6 +161,34 @@ __device__ __forceinline__ uint32_t lt_mask_select_tail(const IsingArgs &a, uint
 }
 
 __device__ __forceinline__ uint32_t maj3(uint32_t x, uint32_t y, uint32_t z) { return (x & y) | (z & (x | y)); }
+
+// Fused measurement: every bond joins the two colours, so the colour-1 half-sweep
+// has, in the masks it formed anyway, everything E and M need.  Per 32-site word of colour 1 after its update:
+// E += 2 (#unsatisfied bonds) - (#bonds), M += 64 - 2 (minus spins of this word and of the colour-0 word at the same
+// index).  Lanes of a warp that serve the same replica are summed with one warp reduction, then one atomic each.
+template <int D>
+__device__ __forceinline__ void fused_word_sums(const uint32_t av[6], uint32_t raw, uint32_t fresh, uint32_t o_same, int &e, int &m) {
+    const uint32_t flip = raw ^ fresh;   // a flipped lane inverts all its bond masks
+    int unsat = __popc(av[0] ^ flip) + __popc(av[1] ^ flip) + __popc(av[2] ^ flip) + __popc(av[3] ^ flip);
+    if (D == 3) unsat += __popc(av[4] ^ flip) + __popc(av[5] ^ flip);
+    e += 2 * unsat - 2 * D * 32;
+    m += 64 - 2 * (__popc(fresh) + __popc(o_same));
+}
+// the accumulator pair of replica r this CTA adds into
+__device__ __forceinline__ unsigned long long *acc_slot(const IsingArgs &a, uint32_t r) {
+    return (unsigned long long *)a.acc + 2 * ((size_t)(blockIdx.x & (a.acc_slots - 1u)) * a.R + r);
+}
+__device__ __forceinline__ void acc_add(const IsingArgs &a, uint32_t r, long long e, long long m) {
+    unsigned long long *p = acc_slot(a, r);
+    atomicAdd(p, (unsigned long long)e);
+    atomicAdd(p + 1, (unsigned long long)m);
+}
+__device__ __forceinline__ void fused_commit(const IsingArgs &a, uint32_t r, int e, int m) {
+    const unsigned active = __activemask();
+    const unsigned peers = __match_any_sync(active, r);
+    const int es = __reduce_add_sync(peers, e), ms = __reduce_add_sync(peers, m);
+    if ((threadIdx.x & 31u) == (uint32_t)(__ffs(peers) - 1)) acc_add(a, r, es, ms);
+}
 
 // m[k] = lanes in which exactly k of the 2 D masks b[] are set (k = 0 .. 2 D), bit-sliced with full adders
 template <int D>
@@ -299,11 +330,15 @@ __device__ __forceinline__ uint32_t unsatisfied_bonds(const IsingArgs &a, uint32
 }
 
 // new value of word gi of replica r (see ising_bitpack_halfsweep)
-template <int D, bool BONDS, bool SHARED>
+template <int D, bool BONDS, bool SHARED, bool MEAS = false>
 __device__ __forceinline__ uint32_t bitpack_update_word(const IsingArgs &a, uint32_t r, uint32_t gi, const WordNbrs &n,
-                                                        const uint32_t ltf[D]) {
+                                                        const uint32_t ltf[D], int *e_sum = nullptr, int *m_sum = nullptr) {
     uint32_t av[6];
     const uint32_t raw = unsatisfied_bonds<D, BONDS>(a, a.colour, r, gi, n, av);
+    [[maybe_unused]] const auto finish = [&](uint32_t flip) {
+        if (MEAS) fused_word_sums<D>(av, raw, raw ^ flip, ((const uint32_t *)a.s[1 - a.colour])[(size_t)r * a.g.NW + gi], *e_sum, *m_sum);
+        return raw ^ flip;
+    };
     uint32_t flip;
     if (D == 2) {
         const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
@@ -325,7 +360,7 @@ __device__ __forceinline__ uint32_t bitpack_update_word(const IsingArgs &a, uint
             flip = ge3 | lt_mask_select<3>(a, a.t, a.colour, gi + a.g.unit_off, a.replica_streams ? r : 0u, m);
         }
     }
-    return raw ^ flip;
+    return finish(flip);
 }
 
 // One thread per 32-site word of the active colour; loops over the replicas.  dE = 2q - 4 n_u with n_u
@@ -333,24 +368,32 @@ __device__ __forceinline__ uint32_t bitpack_update_word(const IsingArgs &a, uint
 // the same random numbers (R > 1, replica_streams = 0), so the masks are built once per word and
 // reused R times (batching four replicas' loads per thread was measured slower: 58 vs 40 us); otherwise each lane is compared against the one
 // threshold it needs.
-template <int D, bool BONDS, bool SHARED>
+// MEAS: the colour-1 half-sweep of a recorded sweep also accumulates E and M into a.acc (fused_word_sums).
+template <int D, bool BONDS, bool SHARED, bool MEAS = false>
 __global__ void __launch_bounds__(256) ising_bitpack_halfsweep(const __grid_constant__ IsingArgs a) {
     constexpr int NT = D;  // thresholds: dE = 4, 8 (2D) and 12 (3D)
     const uint32_t NW = a.g.NW;
     uint32_t *mine_base = (uint32_t *)a.s[a.colour];
     for (uint32_t gi = blockIdx.x * blockDim.x + threadIdx.x; gi < NW; gi += gridDim.x * blockDim.x) {
         const WordNbrs n = word_neighbours<D>(a.g, a.colour, gi);
+        const bool owned = gi >= (a.g.own_j0 >> 5) && gi < (a.g.own_j1 >> 5);
         uint32_t ltf[NT];
+        uint32_t r0 = 0u, r1 = a.R;
         if (SHARED) {
             // gridDim.y > 1: the replicas are split into gridDim.y chunks (many realisations of a small lattice)
             const uint32_t chunk = (a.R + gridDim.y - 1) / gridDim.y;
-            const uint32_t r0 = blockIdx.y * chunk, r1 = min(a.R, r0 + chunk);
+            r0 = blockIdx.y * chunk; r1 = min(a.R, r0 + chunk);
             lt_masks_full<NT>(a, a.t, a.colour, gi + a.g.unit_off, 0u, ltf);
-            for (uint32_t r = r0; r < r1; ++r)
-                mine_base[(size_t)r * NW + gi] = bitpack_update_word<D, BONDS, true>(a, r, gi, n, ltf);
-        } else {
-            for (uint32_t r = 0; r < a.R; ++r)
-                mine_base[(size_t)r * NW + gi] = bitpack_update_word<D, BONDS, false>(a, r, gi, n, ltf);
+        }
+        for (uint32_t r = r0; r < r1; ++r) {
+            int e = 0, m = 0;
+            mine_base[(size_t)r * NW + gi] = bitpack_update_word<D, BONDS, SHARED, MEAS>(a, r, gi, n, ltf, &e, &m);
+            if (MEAS && owned) {
+                // every lane of the warp that is in this loop serves replica r: one reduction, one atomic pair
+                const unsigned act = __activemask();
+                const int es = __reduce_add_sync(act, e), ms = __reduce_add_sync(act, m);
+                if ((threadIdx.x & 31u) == (uint32_t)(__ffs(act) - 1)) acc_add(a, r, es, ms);
+            }
         }
     }
 }
@@ -396,85 +439,181 @@ __global__ void __launch_bounds__(256) ising_bitpack_halfsweep_hb(const __grid_c
 // config 4) the row is the quad and the periodic x-neighbour of every word is inside it: no scalar loads at all.
 __device__ __forceinline__ uint32_t u4c(const uint4 &v, int i) { return i == 0 ? v.x : (i == 1 ? v.y : (i == 2 ? v.z : v.w)); }
 
-template <int D, bool HB>
+// geometry of one quad (uint4 index `me` inside one replica's array) of the active colour
+struct QuadGeom {
+    uint32_t me, p, q_ym, q_yp, q_zm, q_zp, w_edge, QX, NW4;
+};
+template <int D>
+__device__ __forceinline__ QuadGeom quad_geometry(const IsingArgs &a, uint32_t item) {
+    const Geometry &g = a.g;
+    const uint32_t Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz, QX = g.WX >> 2;
+    QuadGeom k;
+    const uint32_t row = QX == 1u ? item : fdiv(item, g.divQW), q = item - row * QX;
+    const uint32_t z = fdiv(row, g.divLy), y = row - z * Ly;
+    k.p = (y + z + a.colour) & 1u;
+    k.me = item; k.QX = QX; k.NW4 = g.NW >> 2;   // uint4 per (replica, plane)
+    // uint4 indices of the quads at y -+ 1, z -+ 1
+    k.q_ym = y == 0 ? item + QX * (Ly - 1) : item - QX; k.q_yp = y == Ly - 1 ? item - QX * (Ly - 1) : item + QX;
+    k.q_zm = D == 3 ? (z == 0 ? item + QX * Ly * (Lz - 1) : item - QX * Ly) : item;
+    k.q_zp = D == 3 ? (z == Lz - 1 ? item - QX * Ly * (Lz - 1) : item + QX * Ly) : item;
+    // word index of the x-neighbour outside the quad: p = 1 -> first word of the next quad, p = 0 -> last of the previous
+    k.w_edge = row * (4u * QX) + (k.p ? (q + 1u == QX ? 0u : 4u * q + 4u) : (q == 0u ? 4u * QX - 1u : 4u * q - 1u));
+    return k;
+}
+
+// the update of quad k of replica r: ltf[i][th] = lanes of word i with U < threshold th (shared by all replicas)
+template <int D, bool HB, int NT, bool MEAS = false>
+__device__ __forceinline__ void pmj_quad_replica(const IsingArgs &a, const QuadGeom &k, uint32_t r, const uint32_t ltf[4][NT]) {
+    int e_sum = 0, m_sum = 0;
+    const uint32_t oc = 1u - a.colour, me = k.me, p = k.p, NW4 = k.NW4;
+    const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
+    const uint4 *__restrict__ So = (const uint4 *)a.s[oc] + (size_t)r * NW4;
+    uint4 *Sc = (uint4 *)a.s[a.colour] + (size_t)r * NW4;
+    const uint4 *__restrict__ Bo = (const uint4 *)a.bonds + ((size_t)(a.colour * a.R + r) * 3) * NW4;   // own forward bonds
+    const uint4 *__restrict__ Bt = (const uint4 *)a.bonds + ((size_t)(oc * a.R + r) * 3) * NW4;         // other colour's
+    const uint4 raw = Sc[me];   // plain load: this array is written by the kernel
+    const uint4 o = __ldg(So + me), ym = __ldg(So + k.q_ym), yp = __ldg(So + k.q_yp);
+    const uint4 zm = D == 3 ? __ldg(So + k.q_zm) : zero, zp = D == 3 ? __ldg(So + k.q_zp) : zero;
+    const uint4 bx_own = __ldg(Bo + me), bx_oth = __ldg(Bt + me);
+    const uint4 by_m = __ldg(Bt + NW4 + k.q_ym), by_own = __ldg(Bo + NW4 + me);
+    const uint4 bz_m = D == 3 ? __ldg(Bt + 2 * (size_t)NW4 + k.q_zm) : zero, bz_own = D == 3 ? __ldg(Bo + 2 * (size_t)NW4 + me) : zero;
+    // the neighbour word outside the quad and (p = 0 only) its forward x coupling; inside the quad when QX == 1
+    uint32_t o_edge, b_edge = 0u;
+    if (k.QX == 1u) { o_edge = p ? o.x : o.w; b_edge = bx_oth.w; }
+    else {
+        o_edge = __ldg((const uint32_t *)So + k.w_edge);
+        if (!p) b_edge = __ldg((const uint32_t *)Bt + k.w_edge);
+    }
+    uint32_t out[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const uint32_t rw = u4c(raw, i), s = a.jneg ? ~rw : rw, oi = u4c(o, i);
+        uint32_t av[6];
+        if (p) {
+            const uint32_t nx = i == 3 ? o_edge : u4c(o, (i + 1) & 3);
+            av[0] = s ^ oi ^ u4c(bx_oth, i); av[1] = s ^ ((oi >> 1) | (nx << 31)) ^ u4c(bx_own, i);
+        } else {
+            const uint32_t pv = i == 0 ? o_edge : u4c(o, (i + 3) & 3), bp = i == 0 ? b_edge : u4c(bx_oth, (i + 3) & 3);
+            av[0] = s ^ oi ^ u4c(bx_own, i); av[1] = s ^ ((oi << 1) | (pv >> 31)) ^ ((u4c(bx_oth, i) << 1) | (bp >> 31));
+        }
+        av[2] = s ^ u4c(ym, i) ^ u4c(by_m, i); av[3] = s ^ u4c(yp, i) ^ u4c(by_own, i);
+        av[4] = D == 3 ? s ^ u4c(zm, i) ^ u4c(bz_m, i) : 0u; av[5] = D == 3 ? s ^ u4c(zp, i) ^ u4c(bz_own, i) : 0u;
+        if constexpr (HB) {
+            uint32_t b[6], m[NT];
+#pragma unroll
+            for (int kk = 0; kk < 6; ++kk) b[kk] = kk < 2 * D ? av[kk] ^ rw : 0u;
+            count_masks<D>(b, m);
+            uint32_t up = 0u;
+#pragma unroll
+            for (int kk = 0; kk < NT; ++kk) up |= m[kk] & ltf[i][kk];
+            out[i] = ~up;
+        } else if (D == 2) {
+            const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
+            const uint32_t ge2 = c1 | (s1 & av[3]), ge1 = av[0] | av[1] | av[2] | av[3];
+            out[i] = rw ^ (ge2 | (ge1 & ltf[i][0]) | ltf[i][1]);
+        } else {
+            const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
+            const uint32_t s2 = av[3] ^ av[4] ^ av[5], c2 = maj3(av[3], av[4], av[5]);
+            const uint32_t b0 = s1 ^ s2, c3 = s1 & s2;
+            const uint32_t b1 = c1 ^ c2 ^ c3, b2 = maj3(c1, c2, c3);
+            out[i] = rw ^ ((b2 | (b1 & b0)) | ((b1 | b2) & ltf[i][0]) | ((b0 | b1 | b2) & ltf[i][1]) | ltf[i][D - 1]);
+        }
+        if (MEAS) fused_word_sums<D>(av, rw, out[i], oi, e_sum, m_sum);
+    }
+    Sc[me] = make_uint4(out[0], out[1], out[2], out[3]);
+    if (MEAS) {
+        // all live lanes of the warp are at replica r: one reduction, one atomic pair per warp
+        const unsigned act = __activemask();
+        const int es = __reduce_add_sync(act, e_sum), ms = __reduce_add_sync(act, m_sum);
+        if ((threadIdx.x & 31u) == (uint32_t)(__ffs(act) - 1)) acc_add(a, r, es, ms);
+    }
+}
+
+// L2 prefetch of replica rn's rows for the warp whose first quad is me0 (one lane calls this): eight bulk requests
+template <int D>
+__device__ __forceinline__ void pmj_quad_prefetch(const IsingArgs &a, uint32_t rn, uint32_t me0, uint32_t pf_bytes, uint32_t pf_ym,
+                                                  uint32_t pf_zm, uint32_t NW4) {
+    const uint32_t oc = 1u - a.colour;
+    const uint4 *Sn = (const uint4 *)a.s[oc] + (size_t)rn * NW4, *Cn = (const uint4 *)a.s[a.colour] + (size_t)rn * NW4;
+    const uint4 *Bon = (const uint4 *)a.bonds + ((size_t)(a.colour * a.R + rn) * 3) * NW4;
+    const uint4 *Btn = (const uint4 *)a.bonds + ((size_t)(oc * a.R + rn) * 3) * NW4;
+    l2_prefetch_bulk(Cn + me0, pf_bytes);
+    l2_prefetch_bulk(Sn + me0, pf_bytes);
+    l2_prefetch_bulk(Bon + me0, pf_bytes);
+    l2_prefetch_bulk(Btn + me0, pf_bytes);
+    l2_prefetch_bulk(Bon + NW4 + me0, pf_bytes);
+    l2_prefetch_bulk(Btn + NW4 + pf_ym, 512u);
+    if (D == 3) {
+        l2_prefetch_bulk(Bon + 2 * (size_t)NW4 + me0, pf_bytes);
+        l2_prefetch_bulk(Btn + 2 * (size_t)NW4 + pf_zm, 512u);
+    }
+}
+
+// One thread per quad; the thread builds the masks of its four words and loops over the replicas of its chunk
+// (blockIdx.y).  Kept for rows of fewer than 32 quads per CTA column and as the A/B partner of the cooperative kernel.
+template <int D, bool HB, bool MEAS = false>
 __global__ void __launch_bounds__(128) ising_pmj_quad_halfsweep(const __grid_constant__ IsingArgs a) {
     constexpr int NT = HB ? 2 * D + 1 : D;
     const Geometry &g = a.g;
-    const uint32_t Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz, NW = g.NW, QX = g.WX >> 2, rows = Ly * Lz;
+    const uint32_t items = (uint32_t)g.Ly * (uint32_t)g.Lz * (g.WX >> 2);
     const uint32_t item = blockIdx.x * blockDim.x + threadIdx.x;
-    if (item >= rows * QX) return;
-    const uint32_t row = QX == 1u ? item : fdiv(item, g.divQW), q = item - row * QX;
-    const uint32_t z = fdiv(row, g.divLy), y = row - z * Ly;
-    const uint32_t p = (y + z + a.colour) & 1u;
-    // uint4 indices (inside one replica's array) of this quad and of the quads at y -+ 1, z -+ 1
-    const uint32_t me = item;
-    const uint32_t q_ym = y == 0 ? me + QX * (Ly - 1) : me - QX, q_yp = y == Ly - 1 ? me - QX * (Ly - 1) : me + QX;
-    const uint32_t q_zm = D == 3 ? (z == 0 ? me + QX * Ly * (Lz - 1) : me - QX * Ly) : me;
-    const uint32_t q_zp = D == 3 ? (z == Lz - 1 ? me - QX * Ly * (Lz - 1) : me + QX * Ly) : me;
-    // word index of the x-neighbour outside the quad: p = 1 -> first word of the next quad, p = 0 -> last of the previous
-    const uint32_t w_edge = row * (4u * QX) + (p ? (q + 1u == QX ? 0u : 4u * q + 4u) : (q == 0u ? 4u * QX - 1u : 4u * q - 1u));
+    if (item >= items) return;
+    const QuadGeom k = quad_geometry<D>(a, item);
     uint32_t ltf[4][NT];
 #pragma unroll
-    for (int i = 0; i < 4; ++i) lt_masks_full<NT, HB>(a, a.t, a.colour, 4u * me + (uint32_t)i + g.unit_off, 0u, ltf[i]);
+    for (int i = 0; i < 4; ++i) lt_masks_full<NT, HB>(a, a.t, a.colour, 4u * item + (uint32_t)i + g.unit_off, 0u, ltf[i]);
     const uint32_t chunk = (a.R + gridDim.y - 1) / gridDim.y;
     const uint32_t r0 = blockIdx.y * chunk, r1 = min(a.R, r0 + chunk);
-    const uint32_t oc = 1u - a.colour;
-    const uint32_t NW4 = NW >> 2;   // uint4 per (replica, plane)
-    const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
+    // L2 prefetch of the next replica's rows (one lane per warp): the replica loop is a chain of dependent DRAM round
+    // trips otherwise (61 % of the stall samples were long-scoreboard waits, profiles/r02a)
+    const uint32_t lane = threadIdx.x & 31u, me0 = item - lane;
+    const uint32_t pf_bytes = 16u * min(32u, items - me0);
+    const uint32_t pf_ym = min(__shfl_sync(__activemask(), k.q_ym, 0), k.NW4 - 32u), pf_zm = min(__shfl_sync(__activemask(), k.q_zm, 0), k.NW4 - 32u);
     for (uint32_t r = r0; r < r1; ++r) {
-        const uint4 *__restrict__ So = (const uint4 *)a.s[oc] + (size_t)r * NW4;
-        uint4 *Sc = (uint4 *)a.s[a.colour] + (size_t)r * NW4;
-        const uint4 *__restrict__ Bo = (const uint4 *)a.bonds + ((size_t)(a.colour * a.R + r) * 3) * NW4;   // own forward bonds
-        const uint4 *__restrict__ Bt = (const uint4 *)a.bonds + ((size_t)(oc * a.R + r) * 3) * NW4;         // other colour's
-        const uint4 raw = Sc[me];   // plain load: this array is written by the kernel
-        const uint4 o = __ldg(So + me), ym = __ldg(So + q_ym), yp = __ldg(So + q_yp);
-        const uint4 zm = D == 3 ? __ldg(So + q_zm) : zero, zp = D == 3 ? __ldg(So + q_zp) : zero;
-        const uint4 bx_own = __ldg(Bo + me), bx_oth = __ldg(Bt + me);
-        const uint4 by_m = __ldg(Bt + NW4 + q_ym), by_own = __ldg(Bo + NW4 + me);
-        const uint4 bz_m = D == 3 ? __ldg(Bt + 2 * (size_t)NW4 + q_zm) : zero, bz_own = D == 3 ? __ldg(Bo + 2 * (size_t)NW4 + me) : zero;
-        // the neighbour word outside the quad and (p = 0 only) its forward x coupling; inside the quad when QX == 1
-        uint32_t o_edge, b_edge = 0u;
-        if (QX == 1u) { o_edge = p ? o.x : o.w; b_edge = bx_oth.w; }
-        else {
-            o_edge = __ldg((const uint32_t *)So + w_edge);
-            if (!p) b_edge = __ldg((const uint32_t *)Bt + w_edge);
+        if (a.prefetch && lane == 0u && r + a.prefetch < r1 && k.NW4 >= 32u) pmj_quad_prefetch<D>(a, r + a.prefetch, me0, pf_bytes, pf_ym, pf_zm, k.NW4);
+        pmj_quad_replica<D, HB, NT, MEAS>(a, k, r, ltf);
+    }
+}
+
+// Cooperative version: a CTA of CH warps serves 32 consecutive quads.  Phase 1: its threads build the masks of the 128
+// words of those quads, one word per thread (stride blockDim.x), into shared memory.  Phase 2: warp c updates the 32
+// quads (one per lane: coalesced 512-byte accesses) for the replicas of chunk c, reading the masks from shared memory.
+// Against the one-thread-per-quad kernel the Philox work per thread is 1 / 4 (the total is unchanged), the replica loop is
+// CH times shorter and CH times more warps keep loads in flight; CTAs in different phases overlap on an SM.
+template <int D, bool HB>
+__global__ void __launch_bounds__(256) ising_pmj_quad_coop_halfsweep(const __grid_constant__ IsingArgs a) {
+    constexpr int NT = HB ? 2 * D + 1 : D;
+    __shared__ __align__(16) uint32_t sm_lt[NT][128];   // [threshold][word of the CTA's 32 quads]
+    const Geometry &g = a.g;
+    const uint32_t items = (uint32_t)g.Ly * (uint32_t)g.Lz * (g.WX >> 2);
+    const uint32_t me0 = blockIdx.x * 32u, lane = threadIdx.x & 31u, warp = threadIdx.x >> 5, CH = blockDim.x >> 5;
+    for (uint32_t wi = threadIdx.x; wi < 128u; wi += blockDim.x) {
+        if (me0 + (wi >> 2) < items) {
+            uint32_t lt[NT];
+            lt_masks_full<NT, HB>(a, a.t, a.colour, 4u * me0 + wi + g.unit_off, 0u, lt);
+#pragma unroll
+            for (int th = 0; th < NT; ++th) sm_lt[th][wi] = lt[th];
         }
-        uint32_t out[4];
+    }
+    const uint32_t item = me0 + lane;
+    const uint32_t chunk = (a.R + CH - 1) / CH;
+    const uint32_t r0 = warp * chunk, r1 = min(a.R, r0 + chunk);
+    const bool live = item < items;
+    const QuadGeom k = quad_geometry<D>(a, live ? item : 0u);
+    const uint32_t pf_bytes = 16u * min(32u, items - me0);
+    const uint32_t pf_ym = min(__shfl_sync(0xFFFFFFFFu, k.q_ym, 0), k.NW4 - 32u), pf_zm = min(__shfl_sync(0xFFFFFFFFu, k.q_zm, 0), k.NW4 - 32u);
+    if (a.prefetch && lane == 0u && r0 < r1 && k.NW4 >= 32u) pmj_quad_prefetch<D>(a, r0, me0, pf_bytes, pf_ym, pf_zm, k.NW4);
+    __syncthreads();
+    if (!live) return;
+    uint32_t ltf[4][NT];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const uint32_t rw = u4c(raw, i), s = a.jneg ? ~rw : rw, oi = u4c(o, i);
-            uint32_t av[6];
-            if (p) {
-                const uint32_t nx = i == 3 ? o_edge : u4c(o, (i + 1) & 3);
-                av[0] = s ^ oi ^ u4c(bx_oth, i); av[1] = s ^ ((oi >> 1) | (nx << 31)) ^ u4c(bx_own, i);
-            } else {
-                const uint32_t pv = i == 0 ? o_edge : u4c(o, (i + 3) & 3), bp = i == 0 ? b_edge : u4c(bx_oth, (i + 3) & 3);
-                av[0] = s ^ oi ^ u4c(bx_own, i); av[1] = s ^ ((oi << 1) | (pv >> 31)) ^ ((u4c(bx_oth, i) << 1) | (bp >> 31));
-            }
-            av[2] = s ^ u4c(ym, i) ^ u4c(by_m, i); av[3] = s ^ u4c(yp, i) ^ u4c(by_own, i);
-            av[4] = D == 3 ? s ^ u4c(zm, i) ^ u4c(bz_m, i) : 0u; av[5] = D == 3 ? s ^ u4c(zp, i) ^ u4c(bz_own, i) : 0u;
-            if constexpr (HB) {
-                uint32_t b[6], m[NT];
-#pragma unroll
-                for (int k = 0; k < 6; ++k) b[k] = k < 2 * D ? av[k] ^ rw : 0u;
-                count_masks<D>(b, m);
-                uint32_t up = 0u;
-#pragma unroll
-                for (int k = 0; k < NT; ++k) up |= m[k] & ltf[i][k];
-                out[i] = ~up;
-            } else if (D == 2) {
-                const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
-                const uint32_t ge2 = c1 | (s1 & av[3]), ge1 = av[0] | av[1] | av[2] | av[3];
-                out[i] = rw ^ (ge2 | (ge1 & ltf[i][0]) | ltf[i][1]);
-            } else {
-                const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
-                const uint32_t s2 = av[3] ^ av[4] ^ av[5], c2 = maj3(av[3], av[4], av[5]);
-                const uint32_t b0 = s1 ^ s2, c3 = s1 & s2;
-                const uint32_t b1 = c1 ^ c2 ^ c3, b2 = maj3(c1, c2, c3);
-                out[i] = rw ^ ((b2 | (b1 & b0)) | ((b1 | b2) & ltf[i][0]) | ((b0 | b1 | b2) & ltf[i][1]) | ltf[i][D - 1]);
-            }
-        }
-        Sc[me] = make_uint4(out[0], out[1], out[2], out[3]);
+    for (int th = 0; th < NT; ++th) {
+        const uint4 v = *(const uint4 *)&sm_lt[th][4u * lane];
+        ltf[0][th] = v.x; ltf[1][th] = v.y; ltf[2][th] = v.z; ltf[3][th] = v.w;
+    }
+    for (uint32_t r = r0; r < r1; ++r) {
+        if (a.prefetch && lane == 0u && r + a.prefetch < r1 && k.NW4 >= 32u) pmj_quad_prefetch<D>(a, r + a.prefetch, me0, pf_bytes, pf_ym, pf_zm, k.NW4);
+        pmj_quad_replica<D, HB, NT>(a, k, r, ltf);
     }
 }
 

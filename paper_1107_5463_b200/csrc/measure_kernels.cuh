@@ -28,8 +28,8 @@ __device__ __forceinline__ T block_sum(T v, T *smem /* >= 32 */) {
     return v;  // valid in thread 0
 }
 
-// acc[r][0] += E, acc[r][1] += M for int8 storage (any dims / couplings).  grid = (blocks, R).
-__global__ void __launch_bounds__(256) ising_generic_measure(const __grid_constant__ IsingArgs a, long long *acc) {
+// a.acc[slot][r][0] += E, [1] += M for int8 storage (any dims / couplings).  grid = (blocks, R).
+__global__ void __launch_bounds__(256) ising_generic_measure(const __grid_constant__ IsingArgs a) {
     __shared__ long long sm[32];
     const Geometry &g = a.g;
     const uint32_t r = blockIdx.y;
@@ -68,15 +68,12 @@ __global__ void __launch_bounds__(256) ising_generic_measure(const __grid_consta
     }
     e = block_sum(e, sm);
     m = block_sum(m, sm);
-    if (threadIdx.x == 0) {
-        atomicAdd((unsigned long long *)&acc[2 * r], (unsigned long long)e);
-        atomicAdd((unsigned long long *)&acc[2 * r + 1], (unsigned long long)m);
-    }
+    if (threadIdx.x == 0) acc_add(a, r, e, m);
 }
 
 // Bit-packed storage: E = 2 n_unsatisfied - n_bonds, M = N - 2 popcount.  grid = (blocks, R).
 template <int D, bool BONDS>
-__global__ void __launch_bounds__(256) ising_bitpack_measure(const __grid_constant__ IsingArgs a, long long *acc) {
+__global__ void __launch_bounds__(256) ising_bitpack_measure(const __grid_constant__ IsingArgs a) {
     __shared__ long long sm[32];
     const uint32_t r = blockIdx.y, NW = a.g.NW;
     const uint32_t *__restrict__ s0 = (const uint32_t *)a.s[0] + (size_t)r * NW;
@@ -92,15 +89,12 @@ __global__ void __launch_bounds__(256) ising_bitpack_measure(const __grid_consta
     }
     e = block_sum(e, sm);
     m = block_sum(m, sm);
-    if (threadIdx.x == 0) {
-        atomicAdd((unsigned long long *)&acc[2 * r], (unsigned long long)e);
-        atomicAdd((unsigned long long *)&acc[2 * r + 1], (unsigned long long)m);
-    }
+    if (threadIdx.x == 0) acc_add(a, r, e, m);
 }
 
 // int8 fast layout (uniform J = +-1): units packed to lane masks, then as the bit-packed kernel.  grid = (blocks, R).
 template <int D>
-__global__ void __launch_bounds__(256) ising_int8_measure(const __grid_constant__ IsingArgs a, long long *acc) {
+__global__ void __launch_bounds__(256) ising_int8_measure(const __grid_constant__ IsingArgs a) {
     __shared__ long long sm[32];
     const Geometry &g = a.g;
     const uint32_t r = blockIdx.y;
@@ -124,21 +118,24 @@ __global__ void __launch_bounds__(256) ising_int8_measure(const __grid_constant_
     }
     e = block_sum(e, sm);
     m = block_sum(m, sm);
-    if (threadIdx.x == 0) {
-        atomicAdd((unsigned long long *)&acc[2 * r], (unsigned long long)e);
-        atomicAdd((unsigned long long *)&acc[2 * r + 1], (unsigned long long)m);
-    }
+    if (threadIdx.x == 0) acc_add(a, r, e, m);
 }
 
-// acc -> doubles at outE[r], outM[r]; clears acc for the next measurement.  One thread per replica.
-__global__ void ising_measure_finalize(long long *acc, uint32_t R, double *outE, double *outM) {
-    const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
-    if (r < R) {
-        outE[r] = (double)acc[2 * r];
-        outM[r] = (double)acc[2 * r + 1];
-        acc[2 * r] = 0;
-        acc[2 * r + 1] = 0;
+// sum of the slots of acc -> doubles at outE[r], outM[r]; clears acc for the next measurement.  One warp per replica,
+// lane k takes slots k, k + 32, ... (integer sums: exact in any order).  block = 128 threads = 4 replicas.
+__global__ void __launch_bounds__(128) ising_measure_finalize(long long *acc, uint32_t R, uint32_t slots, double *outE, double *outM) {
+    const uint32_t r = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31u;
+    if (r >= R) return;
+    long long e = 0, m = 0;
+    for (uint32_t k = lane; k < slots; k += 32u) {
+        longlong2 *p = (longlong2 *)(acc + 2 * ((size_t)k * R + r));
+        const longlong2 v = *p;
+        e += v.x; m += v.y;
+        *p = make_longlong2(0, 0);
     }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { e += __shfl_down_sync(0xFFFFFFFFu, e, o); m += __shfl_down_sync(0xFFFFFFFFu, m, o); }
+    if (lane == 0u) { outE[r] = (double)e; outM[r] = (double)m; }
 }
 
 // n >= 2: part[r][block][1 + NC].  grid = (blocks, R).
@@ -193,6 +190,41 @@ __global__ void __launch_bounds__(256) vector_measure_finalize(const double *par
             else outM[(size_t)r * nc + (k - 1)] = v;
         }
     }
+}
+
+// Two-level, single-launch version for many partials (the fused strip kernel leaves one per warp): grid = (F, R).
+// Block (f, r) sums its contiguous share of part[r][0 .. nparts) in a fixed order into mid[r][f]; the block that finishes
+// last for replica r (ticket from counter[r]) sums mid[r][0 .. F) in a fixed order.  Which block is last does not change
+// any order of summation, so the result is deterministic.
+__global__ void __launch_bounds__(256) vector_partials_finalize(const double *part, uint32_t nparts, int nc, double *mid,
+                                                                unsigned int *counter, double *outE, double *outM) {
+    __shared__ double sm[32];
+    __shared__ unsigned int ticket;
+    const uint32_t r = blockIdx.y, F = gridDim.x, f = blockIdx.x;
+    const uint32_t share = (nparts + F - 1) / F, b0 = f * share, b1 = min(nparts, b0 + share);
+    for (int k = 0; k < 1 + nc; ++k) {
+        double v = 0.0;
+        for (uint32_t b = b0 + threadIdx.x; b < b1; b += blockDim.x) v += part[((size_t)r * nparts + b) * (1 + nc) + k];
+        v = block_sum(v, sm);
+        if (threadIdx.x == 0) mid[((size_t)r * F + f) * (1 + nc) + k] = v;
+    }
+    if (threadIdx.x == 0) {
+        __threadfence();
+        ticket = atomicAdd(&counter[r], 1u);
+    }
+    __syncthreads();
+    if (ticket != F - 1) return;
+    __threadfence();
+    for (int k = 0; k < 1 + nc; ++k) {
+        double v = 0.0;
+        for (uint32_t b = threadIdx.x; b < F; b += blockDim.x) v += __ldcg(&mid[((size_t)r * F + b) * (1 + nc) + k]);
+        v = block_sum(v, sm);
+        if (threadIdx.x == 0) {
+            if (k == 0) outE[r] = v;
+            else outM[(size_t)r * nc + (k - 1)] = v;
+        }
+    }
+    if (threadIdx.x == 0) counter[r] = 0u;
 }
 
 }  // namespace spin

@@ -42,7 +42,8 @@ enum Path { PATH_ISING_GENERIC, PATH_ISING_INT8, PATH_ISING_BITPACK, PATH_VECTOR
 struct Layout {
     size_t off_s[2], bytes_s;   // one colour array
     size_t off_bonds, bytes_bonds;
-    size_t off_acc, bytes_acc;  // n = 1: int64 [R][2]; n >= 2: double [R][mblocks][1 + n]
+    size_t off_acc, bytes_acc;  // n = 1: int64 [R][2]; n >= 2: double [R][partials][1 + n], then the two below
+    size_t off_mid, off_cnt;    // n >= 2: double [R][FINALIZE_BLOCKS][1 + n] and unsigned [R] of vector_partials_finalize
     size_t off_res, bytes_res;  // double [R] E then [R][n] M
     size_t total;
 };
@@ -66,6 +67,8 @@ struct spin_system {
     int axis, own_planes; // slab decomposition: axis (2 z, 1 y, -1 none) and owned planes along it
     uint32_t next_colour; // spin_halfsweep: colour expected next
     int vector_generic;  // n >= 2: force the one-thread-per-site kernel (test knob)
+    int variant;         // SPIN_OPT_KERNEL_VARIANT: 0 = the default kernel of each family, > 0 = a named alternative (A/B knob)
+    int l2_prefetch;     // SPIN_OPT_L2_PREFETCH: -1 each kernel's own distance (default), 0 off, > 0 that distance
     int grid_num, grid_den;
     uint32_t mblocks;    // CTAs (per replica) of the measurement kernels
     double table_beta;   // beta the cached table was built for (NaN = none)
@@ -191,6 +194,14 @@ static uint32_t tma_grid_x(uint64_t S, uint64_t R, uint64_t cap) {
     return (uint32_t)gx;
 }
 constexpr uint64_t TMA_MAX_CTAS = 512;
+constexpr uint32_t FINALIZE_BLOCKS = 128;   // first-level blocks of vector_partials_finalize
+
+// slots of the n = 1 accumulators: as many as 64, fewer when there are many replicas (8192 / R rounded down to a power of two)
+static uint32_t acc_slots_for(uint64_t R) {
+    uint32_t k = 64;
+    while (k > 1 && (uint64_t)k * R > 8192) k >>= 1;
+    return k;
+}
 
 static void make_layout(const spin_config *c, const Derived &dv, Layout *l, uint32_t *mblocks) {
     const uint64_t Nh = dv.N / 2, R = (uint64_t)c->n_replicas;
@@ -211,8 +222,14 @@ static void make_layout(const spin_config *c, const Derived &dv, Layout *l, uint
         const uint64_t gx = tma_grid_x(S, R, TMA_MAX_CTAS);
         if (gx > pblocks) pblocks = gx;
     }
-    l->bytes_acc = c->n == 1 ? (size_t)(R * 2 * sizeof(long long)) : (size_t)(R * pblocks * (1 + c->n) * sizeof(double));
-    l->off_acc = off; off += align_up(l->bytes_acc);
+    // n >= 2, rows of whole quads: the fused strip kernel leaves one partial per CTA (at least 32 quads each)
+    if (c->n > 1 && (dv.pad[0] / 2) % 4 == 0 && Nh / 128 + 4 > pblocks) pblocks = Nh / 128 + 4;   // CTAs of >= 32 quads
+    const size_t part_bytes = c->n == 1 ? (size_t)(acc_slots_for(R) * R * 2 * sizeof(long long)) : (size_t)(R * pblocks * (1 + c->n) * sizeof(double));
+    l->off_acc = off;
+    l->off_mid = off + align_up(part_bytes);
+    l->off_cnt = l->off_mid + (c->n == 1 ? 0 : align_up((size_t)(R * FINALIZE_BLOCKS * (1 + c->n) * sizeof(double))));
+    l->bytes_acc = (l->off_cnt - off) + (c->n == 1 ? 0 : align_up((size_t)(R * sizeof(unsigned))));
+    off += align_up(l->bytes_acc);
     l->bytes_res = (size_t)(R * (1 + c->n) * sizeof(double));
     l->off_res = off; off += align_up(l->bytes_res);
     l->total = off;
@@ -293,8 +310,10 @@ static IsingArgs ising_args(const spin_system *s) {
                    : (s->cfg.coupling_kind == SPIN_J_PER_DIRECTION ? (mu < s->d ? (int)s->cfg.J[mu] : 0) : 0);
     a.jneg = (s->cfg.coupling_kind == SPIN_J_UNIFORM && s->cfg.J[0] < 0.0) ? 1u : 0u;
     a.rule = s->cfg.update_rule == SPIN_UPDATE_HEATBATH ? 1u : 0u;
+    a.prefetch = s->l2_prefetch < 0 ? 0u : (uint32_t)s->l2_prefetch;   // +-J quad kernel: replicas ahead (no gain measured: off)
     a.hb = s->hb;
     a.acc = (long long *)(s->ws + s->lay.off_acc);
+    a.acc_slots = acc_slots_for(s->R);
     return a;
 }
 
@@ -309,6 +328,9 @@ static VectorArgs vector_args(const spin_system *s, double beta) {
         a.Jdir[mu] = s->cfg.coupling_kind == SPIN_J_UNIFORM ? (float)s->cfg.J[0] : (mu < s->d ? (float)s->cfg.J[mu] : 0.0f);
     a.beta = (float)beta;
     a.rule = s->cfg.update_rule == SPIN_UPDATE_HEATBATH ? 1u : 0u;
+    // strip kernel: CTAs ahead; default = one wave of resident CTAs (9 of 128 threads per SM at 52 registers)
+    a.prefetch = s->l2_prefetch < 0 ? (uint32_t)s->sm_count * 9u : (uint32_t)s->l2_prefetch;
+    a.part = (double *)(s->ws + s->lay.off_acc);
     return a;
 }
 
@@ -377,8 +399,18 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
         // Lx % 256 == 0: one thread per quad of four words, 128-bit accesses (ising_pmj_quad_halfsweep).
         // All replicas in one thread when the quads alone give every SM >= 256 threads (measured at 256^3, R = 16:
         // 35.2 / 37.1 / 35.2 / 47.4 / 78.1 us for 1 / 2 / 4 / 8 / 16 replica chunks), else chunks of >= 4 replicas
-        const int Bq = 128;
         const uint64_t quads = (uint64_t)s->g.NW / 4;
+        const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
+        if (s->variant == 1 && s->R >= 2) {
+            // cooperative kernel (A/B partner, same speed on B200: profiles/r02_pmj_diagnostics.md): a CTA of CH warps per 32 quads, warp c serves replica chunk c
+            int CH = s->block / 32;
+            while (CH > 1 && (uint32_t)CH > s->R) CH /= 2;
+            const dim3 G((unsigned)((quads + 31) / 32));
+            const int Bc = 32 * CH;
+            if (s->d == 2) { if (hb) ising_pmj_quad_coop_halfsweep<2, true><<<G, Bc, 0, st>>>(a); else ising_pmj_quad_coop_halfsweep<2, false><<<G, Bc, 0, st>>>(a); }
+            else { if (hb) ising_pmj_quad_coop_halfsweep<3, true><<<G, Bc, 0, st>>>(a); else ising_pmj_quad_coop_halfsweep<3, false><<<G, Bc, 0, st>>>(a); }
+        } else {
+        const int Bq = s->block < 128 ? s->block : 128;
         unsigned Gy = 1;
         if (quads < (uint64_t)s->sm_count * 256) {
             uint64_t want = ((uint64_t)s->sm_count * 256 + quads - 1) / quads;   // chunks that would fill the GPU
@@ -387,9 +419,15 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
             Gy = (unsigned)(want < 1 ? 1 : want);
         }
         const dim3 G((unsigned)((quads + Bq - 1) / Bq), Gy);
-        const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
+        if (fused && a.colour == 1u) {
+            // colour-1 half-sweep of a recorded sweep: E and M from the bond masks it forms anyway (row a7)
+            *fused = true;
+            if (s->d == 2) { if (hb) ising_pmj_quad_halfsweep<2, true, true><<<G, Bq, 0, st>>>(a); else ising_pmj_quad_halfsweep<2, false, true><<<G, Bq, 0, st>>>(a); }
+            else { if (hb) ising_pmj_quad_halfsweep<3, true, true><<<G, Bq, 0, st>>>(a); else ising_pmj_quad_halfsweep<3, false, true><<<G, Bq, 0, st>>>(a); }
+        } else
         if (s->d == 2) { if (hb) ising_pmj_quad_halfsweep<2, true><<<G, Bq, 0, st>>>(a); else ising_pmj_quad_halfsweep<2, false><<<G, Bq, 0, st>>>(a); }
         else { if (hb) ising_pmj_quad_halfsweep<3, true><<<G, Bq, 0, st>>>(a); else ising_pmj_quad_halfsweep<3, false><<<G, Bq, 0, st>>>(a); }
+        }
     } else {
         // shared update stream: chunks of >= 16 replicas per thread (the masks of a word are built once per chunk);
         // more chunks only when the lattice alone cannot fill the GPU (many realisations of a small lattice)
@@ -406,9 +444,12 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
             if (Gy > 65535) Gy = 65535;
         }
         const dim3 G(Gx, Gy);
+        const bool meas = fused && a.colour == 1u && s->cfg.update_rule != SPIN_UPDATE_HEATBATH;   // row a7, Metropolis kernels
+        if (meas) *fused = true;
 #define BP(D_, BONDS_, SH_)                                                                      \
     do {                                                                                         \
         if (s->cfg.update_rule == SPIN_UPDATE_HEATBATH) ising_bitpack_halfsweep_hb<D_, BONDS_, SH_><<<G, Bq, 0, st>>>(a); \
+        else if (meas) ising_bitpack_halfsweep<D_, BONDS_, SH_, true><<<G, Bq, 0, st>>>(a);     \
         else ising_bitpack_halfsweep<D_, BONDS_, SH_><<<G, Bq, 0, st>>>(a);                     \
     } while (0)
         if (s->d == 2) {
@@ -493,7 +534,7 @@ static uint32_t tma_ctas(const spin_system *s, bool hb, bool meas) {
 // one-thread-per-site kernel.  fused: NULL, or (colour 1) ask for E / M partials from the half-sweep itself (row a7);
 // *fused = number of per-replica partials written (0: this kernel cannot, run the measurement pass).
 static spin_status launch_halfsweep_vector(spin_system *s, const VectorArgs &a, cudaStream_t st, bool allow_tma = true,
-                                           uint32_t *fused = nullptr) {
+                                           uint32_t *fused = nullptr, bool *two_level = nullptr) {
     const Geometry &g = s->g;
     const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
     const bool strip_ok = g.RL % 4 == 0 && !s->vector_generic && s->R <= 65535;
@@ -501,6 +542,27 @@ static spin_status launch_halfsweep_vector(spin_system *s, const VectorArgs &a, 
     // the staged kernel serves (a) every half-sweep when SPIN_OPT_TMA_KERNELS is on, (b) by default only the colour-1 half-sweep
     // of a recorded sweep, whose fused E / M saves the measurement pass (the strip kernel is faster otherwise: profiles/)
     const bool want_fused = fused && a.colour == 1u;
+    if (two_level) *two_level = false;
+    if (want_fused && strip_ok && s->use_tma != 1 && two_level) {
+        // colour-1 half-sweep of a recorded sweep: the strip kernel (one row per thread) with E / M fused, one partial per warp
+        bool unitj = true;
+        for (int mu = 0; mu < s->d; ++mu) unitj = unitj && a.Jdir[mu] == 1.0f;
+        const int B = s->block > 128 ? 128 : s->block;
+        const uint64_t items = (uint64_t)(g.RL / 4) * g.Ly * g.Lz;
+        const dim3 G((unsigned)((items + B - 1) / B), s->R);
+#define VM4(NC_, D_, U_, HB_) vector_strip_halfsweep<NC_, D_, U_, 1, HB_, true><<<G, B, 0, st>>>(a)
+#define VM3(NC_, D_, HB_) do { if (unitj) VM4(NC_, D_, true, HB_); else VM4(NC_, D_, false, HB_); } while (0)
+        if (s->n == 2) { if (s->d == 2) VM3(2, 2, false); else VM3(2, 3, false); }
+        else if (hb) { if (s->d == 2) VM3(3, 2, true); else VM3(3, 3, true); }
+        else { if (s->d == 2) VM3(3, 2, false); else VM3(3, 3, false); }
+#undef VM3
+#undef VM4
+        CUDA_TRY(cudaGetLastError());
+        *fused = G.x;
+        *two_level = true;
+        s->launches += 1;
+        return SPIN_OK;
+    }
     if (allow_tma && s->tma_ok && (s->use_tma == 1 || (s->use_tma < 0 && want_fused)) && !s->vector_generic) {
         bool unitj = true;
         for (int mu = 0; mu < s->d; ++mu) unitj = unitj && a.Jdir[mu] == 1.0f;
@@ -690,16 +752,16 @@ static spin_status enqueue_measure(spin_system *s, double *dE, double *dM, cudaS
         long long *acc = (long long *)(s->ws + s->lay.off_acc);
         const bool bonds = s->cfg.coupling_kind == SPIN_J_BOND_PM1;
         if (s->path == PATH_ISING_BITPACK) {
-            if (s->d == 2) { if (bonds) ising_bitpack_measure<2, true><<<grid, 256, 0, st>>>(a, acc); else ising_bitpack_measure<2, false><<<grid, 256, 0, st>>>(a, acc); }
-            else { if (bonds) ising_bitpack_measure<3, true><<<grid, 256, 0, st>>>(a, acc); else ising_bitpack_measure<3, false><<<grid, 256, 0, st>>>(a, acc); }
+            if (s->d == 2) { if (bonds) ising_bitpack_measure<2, true><<<grid, 256, 0, st>>>(a); else ising_bitpack_measure<2, false><<<grid, 256, 0, st>>>(a); }
+            else { if (bonds) ising_bitpack_measure<3, true><<<grid, 256, 0, st>>>(a); else ising_bitpack_measure<3, false><<<grid, 256, 0, st>>>(a); }
         } else if (s->path == PATH_ISING_INT8) {
-            if (s->d == 2) ising_int8_measure<2><<<grid, 256, 0, st>>>(a, acc);
-            else ising_int8_measure<3><<<grid, 256, 0, st>>>(a, acc);
+            if (s->d == 2) ising_int8_measure<2><<<grid, 256, 0, st>>>(a);
+            else ising_int8_measure<3><<<grid, 256, 0, st>>>(a);
         } else {
-            ising_generic_measure<<<grid, 256, 0, st>>>(a, acc);
+            ising_generic_measure<<<grid, 256, 0, st>>>(a);
         }
         CUDA_TRY(cudaGetLastError());
-        ising_measure_finalize<<<(s->R + 63) / 64, 64, 0, st>>>(acc, s->R, dE, dM);
+        ising_measure_finalize<<<(s->R + 3) / 4, 128, 0, st>>>(acc, s->R, a.acc_slots, dE, dM);
     } else {
         VectorArgs a = vector_args(s, 0.0);
         double *part = (double *)(s->ws + s->lay.off_acc);
@@ -804,7 +866,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
     s->tma_ok = 0; s->use_tma = -1; s->tma_ty = 0;
     s->t = 0; s->launches = 0; s->staging = nullptr; s->staging_bytes = 0; s->gexec = nullptr; s->cap_stream = nullptr; s->gnodes = nullptr; s->n_gnodes = 0;
     // 128 threads per CTA for the Ising fast paths (measured: +-J R = 16 39.1 vs 40.4 us with 256)
-    s->block = (dv.path == PATH_ISING_INT8 || dv.path == PATH_ISING_BITPACK) ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0;
+    s->block = (dv.path == PATH_ISING_INT8 || dv.path == PATH_ISING_BITPACK) ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0; s->l2_prefetch = -1; s->variant = 0;
     s->table_beta = std::nan("");
     Geometry &g = s->g;
     g.Lx = dv.pad[0]; g.Ly = dv.pad[1]; g.Lz = dv.pad[2]; g.d = dv.d;
@@ -926,7 +988,7 @@ spin_status spin_sweep_record(spin_system *s, double beta, int64_t n_sweeps, dou
             if (rc != SPIN_OK) return rc;
             s->t += 1;
             if (fused) {
-                ising_measure_finalize<<<(s->R + 63) / 64, 64, 0, st>>>(a.acc, s->R, oE, oM);
+                ising_measure_finalize<<<(s->R + 3) / 4, 128, 0, st>>>(a.acc, s->R, a.acc_slots, oE, oM);
                 s->launches += 1;
                 CUDA_TRY(cudaGetLastError());
                 continue;
@@ -935,15 +997,22 @@ spin_status spin_sweep_record(spin_system *s, double beta, int64_t n_sweeps, dou
             // n >= 2: the TMA-staged colour-1 half-sweep leaves per-CTA partial sums of E and M (row a7)
             VectorArgs a = vector_args(s, beta);
             uint32_t parts = 0;
+            bool two_level = false;
             a.colour = 0;
             rc = launch_halfsweep_vector(s, a, st);
             if (rc != SPIN_OK) return rc;
             a.colour = 1;
-            rc = launch_halfsweep_vector(s, a, st, true, &parts);
+            rc = launch_halfsweep_vector(s, a, st, true, &parts, &two_level);
             if (rc != SPIN_OK) return rc;
             s->t += 1;
             if (parts) {
-                vector_measure_finalize<<<s->R, 256, 0, st>>>((const double *)(s->ws + s->lay.off_acc), parts, s->n, oE, oM);
+                const double *part = (const double *)(s->ws + s->lay.off_acc);
+                if (two_level) {
+                    const uint32_t F = parts / 256 + 1 < FINALIZE_BLOCKS ? parts / 256 + 1 : FINALIZE_BLOCKS;
+                    vector_partials_finalize<<<dim3(F, s->R), 256, 0, st>>>(part, parts, s->n, (double *)(s->ws + s->lay.off_mid),
+                                                                             (unsigned *)(s->ws + s->lay.off_cnt), oE, oM);
+                } else
+                vector_measure_finalize<<<s->R, 256, 0, st>>>(part, parts, s->n, oE, oM);
                 s->launches += 1;
                 CUDA_TRY(cudaGetLastError());
                 continue;
@@ -1176,6 +1245,18 @@ spin_status spin_set_option(spin_system *s, int32_t option, int64_t value) {
     if (option == SPIN_OPT_TMA_KERNELS) {
         if (value != 0 && value != 1 && value != -1) return fail(SPIN_ERR_INVALID_ARG, "SPIN_OPT_TMA_KERNELS takes 0, 1 or -1");
         s->use_tma = (int)value;
+        return SPIN_OK;
+    }
+    if (option == SPIN_OPT_KERNEL_VARIANT) {
+        if (value < 0 || value > 15) return fail(SPIN_ERR_INVALID_ARG, "SPIN_OPT_KERNEL_VARIANT takes 0 .. 15");
+        s->variant = (int)value;
+        graph_drop(s);
+        return SPIN_OK;
+    }
+    if (option == SPIN_OPT_L2_PREFETCH) {
+        if (value < -1 || value > (1 << 20)) return fail(SPIN_ERR_INVALID_ARG, "SPIN_OPT_L2_PREFETCH takes -1, 0 or a distance up to 2^20");
+        s->l2_prefetch = (int)value;
+        graph_drop(s);   // captured argument blocks hold the old distance
         return SPIN_OK;
     }
     return fail(SPIN_ERR_INVALID_ARG, "unknown option %d", (int)option);

@@ -19,6 +19,8 @@ struct VectorArgs {
     float Jdir[3];
     float beta;
     uint32_t rule;        // 0 Metropolis (Eq. (2)), 1 heat bath (n = 3 only)
+    uint32_t prefetch;    // strip kernel: L2 prefetch distance in CTAs (0 = off)
+    double *part;         // fused E / M of the strip kernel: [R][warps of the grid][1 + NC] partial sums
 };
 
 __device__ __forceinline__ float u24(uint32_t w) { return (float)(w >> 8) * 5.9604644775390625e-08f; }
@@ -286,9 +288,18 @@ __device__ __forceinline__ void vector_quad_field(float Jx, float Jy, float Jz, 
 }
 
 // phase 2: proposals, acceptance and the new spins res[c][i] of the four sites from their fields and old spins
-template <int NC, bool HB>
+// MEAS: *eq = sum over the four sites of s'_i . h_i (fp32, sites in order, each product and sum rounded separately)
+template <int NC, bool HB, bool MEAS = false>
 __device__ __forceinline__ void vector_quad_accept(const VectorArgs &a, const float2 hp[2][NC], const Quad<NC> &own,
-                                                   uint32_t ctr0, uint32_t rho, uint32_t tag, float res[NC][4]) {
+                                                   uint32_t ctr0, uint32_t rho, uint32_t tag, float res[NC][4], float *eq = nullptr) {
+    [[maybe_unused]] float esum = 0.0f;
+    // the two sites of pair pr: esum += s' . h, first site then second
+    [[maybe_unused]] const auto add_energy = [&](int pr) {
+        float2 dot = __fmul2_rn(f2(res[0][2 * pr], res[0][2 * pr + 1]), hp[pr][0]);
+#pragma unroll
+        for (int c = 1; c < NC; ++c) dot = __fadd2_rn(dot, __fmul2_rn(f2(res[c][2 * pr], res[c][2 * pr + 1]), hp[pr][c]));
+        esum = __fadd_rn(__fadd_rn(esum, dot.x), dot.y);
+    };
 #pragma unroll
     for (int pr = 0; pr < 2; ++pr) {
         uint32_t wa[4], wb[4];
@@ -301,6 +312,7 @@ __device__ __forceinline__ void vector_quad_accept(const VectorArgs &a, const fl
             heatbath3(a.beta, hb, wb[0], wb[1], sb);
 #pragma unroll
             for (int c = 0; c < NC; ++c) { res[c][2 * pr] = sa[c]; res[c][2 * pr + 1] = sb[c]; }
+            if (MEAS) add_energy(pr);
             continue;
         }
         float2 sn[NC], so[NC];
@@ -321,7 +333,9 @@ __device__ __forceinline__ void vector_quad_accept(const VectorArgs &a, const fl
             res[c][2 * pr] = acc_a ? sn[c].x : so[c].x;
             res[c][2 * pr + 1] = acc_b ? sn[c].y : so[c].y;
         }
+        if (MEAS) add_energy(pr);
     }
+    if (MEAS) *eq = esum;
 }
 
 template <int NC, int D, bool UNITJ, bool HB>
@@ -335,7 +349,12 @@ __device__ __forceinline__ void vector_quad_update(const VectorArgs &a, float Jx
     vector_quad_accept<NC, HB>(a, hp, own, ctr0, rho, tag, res);
 }
 
-template <int NC, int D, bool UNITJ, int K, bool HB = false>
+// MEAS (colour-1 half-sweep of spin_sweep_record): every bond joins the two colours, so
+// E = -sum_{i in colour 1} s'_i . h_i with the local field this half-sweep has formed anyway, and M = the new colour-1
+// spins plus the colour-0 spins at the same compressed indices (already loaded as o_cur).  Per-site terms in fp32 (each
+// product and sum rounded separately) summed in fp32 over the 128 sites of a warp (fixed shuffle tree), then in fp64 by
+// vector_partials_finalize in a fixed order: deterministic.
+template <int NC, int D, bool UNITJ, int K, bool HB = false, bool MEAS = false>
 __global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_constant__ VectorArgs a) {
     const Geometry &g = a.g;
     const uint32_t RL = g.RL, QX = RL >> 2, Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz, Nh = g.Nh;
@@ -344,8 +363,25 @@ __global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_const
     // the replica is blockIdx.y (host: gridDim.y = R), so the plane base pointers are warp-uniform and every access is
     // "uniform 64-bit base + 32-bit offset" (no per-thread 64-bit address arithmetic)
     const uint32_t it = blockIdx.x * blockDim.x + threadIdx.x;
-    if (it >= per_replica) return;
     const uint32_t r = blockIdx.y;
+    if (K == 1 && a.prefetch && threadIdx.x == 0u) {
+        // K = 1: quad `it` sits at float offset 4 it of every component plane, so the CTA `prefetch` places ahead reads two
+        // contiguous ranges per component (its own spins and the other colour at the same indices; the rows around them
+        // belong to CTAs that run at about the same time).  One thread asks for them now: bulk L2 prefetch, no registers.
+        const uint32_t it0 = (blockIdx.x + a.prefetch) * blockDim.x;
+        if (it0 < per_replica) {
+            const uint32_t bytes = 16u * min(blockDim.x, per_replica - it0);
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+                l2_prefetch_bulk(a.s[a.colour] + ((size_t)r * NC + c) * Nh + 4u * (size_t)it0, bytes);
+                l2_prefetch_bulk(a.s[1 - a.colour] + ((size_t)r * NC + c) * Nh + 4u * (size_t)it0, bytes);
+            }
+        }
+    }
+    float e_acc = 0.0f, m_acc[NC];
+#pragma unroll
+    for (int c = 0; c < NC; ++c) m_acc[c] = 0.0f;
+    if (it < per_replica) {
     const uint32_t sz = fdiv(it, g.divQX), q = it - sz * QX;       // sz = strip + nstrip * z
     const uint32_t z = sz / nstrip, y0 = (sz - z * nstrip) * K;
     const uint32_t kend = min((uint32_t)K, Ly - y0);
@@ -384,14 +420,55 @@ __global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_const
 #pragma unroll
             for (int c = 0; c < NC; ++c) side[c] = __ldg(other + (size_t)c * Nh + row + (p ? side_p1 : side_p0));
             float res[NC][4];
-            vector_quad_update<NC, D, UNITJ, HB>(a, Jx, Jy, Jz, p, o_cur, side, o_prev, o_next, o_zm, o_zp, own,
-                                                 off + g.j_off, rho, tag, res);
+            float2 hp[2][NC];
+            [[maybe_unused]] float osum[NC];   // MEAS: the colour-0 spins at the quad's indices, summed before they die
+            if (MEAS) {
+#pragma unroll
+                for (int c = 0; c < NC; ++c) osum[c] = __fadd_rn(__fadd_rn(o_cur.c[c].x, o_cur.c[c].y), __fadd_rn(o_cur.c[c].z, o_cur.c[c].w));
+            }
+            vector_quad_field<NC, D, UNITJ>(Jx, Jy, Jz, p, o_cur, side, o_prev, o_next, o_zm, o_zp, hp);
+            [[maybe_unused]] float eq = 0.0f;
+            vector_quad_accept<NC, HB, MEAS>(a, hp, own, off + g.j_off, rho, tag, res, &eq);
 #pragma unroll
             for (int c = 0; c < NC; ++c)
                 *(float4 *)(mine + (size_t)c * Nh + off) = make_float4(res[c][0], res[c][1], res[c][2], res[c][3]);
+            if (MEAS && off >= g.own_j0 && off < g.own_j1) {
+                e_acc = __fsub_rn(e_acc, eq);
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    const float mq = __fadd_rn(__fadd_rn(__fadd_rn(res[c][0], res[c][1]), __fadd_rn(res[c][2], res[c][3])), osum[c]);
+                    m_acc[c] = __fadd_rn(m_acc[c], mq);
+                }
+            }
             o_prev = o_cur;
             o_cur = o_next;
             p ^= 1u;
+        }
+    }
+    }
+    if (MEAS) {
+        // per warp: fp32 shuffle tree over the lanes' quad sums (128 sites: fixed order, dead lanes contribute 0); everything
+        // above the warp is summed in fp64: the CTA's warps here, the CTAs in vector_partials_finalize
+        float v[1 + NC];
+        v[0] = e_acc;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) v[1 + c] = m_acc[c];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+            for (int c = 0; c < 1 + NC; ++c) v[c] = __fadd_rn(v[c], __shfl_down_sync(0xFFFFFFFFu, v[c], o));
+        }
+        __shared__ float wsum[4][1 + NC];
+        if ((threadIdx.x & 31u) == 0u) {
+#pragma unroll
+            for (int c = 0; c < 1 + NC; ++c) wsum[threadIdx.x >> 5][c] = v[c];
+        }
+        __syncthreads();
+        if (threadIdx.x < 1 + NC) {
+            // the CTA's partial: its warps in order, in fp64
+            double t = 0.0;
+            for (uint32_t w = 0; w < (blockDim.x >> 5); ++w) t += (double)wsum[w][threadIdx.x];
+            a.part[((size_t)r * gridDim.x + blockIdx.x) * (1 + NC) + threadIdx.x] = t;
         }
     }
 }

@@ -506,6 +506,32 @@ def test_fused_measurement_in_recorded_sweeps(P, oracle, dims, storage, J, R, ru
     _assert_ising_equal(G, O, "after fused recorded sweeps")     # spin_measure (separate pass) agrees as well
 
 
+@pytest.mark.parametrize("dims,R,streams,rule", [((256, 12, 6), 5, 0, "metropolis"), ((512, 10, 1), 3, 0, "metropolis"),
+                                                 ((256, 6, 4), 4, 0, "heatbath"), ((64, 40, 6), 70, 0, "metropolis"),
+                                                 ((128, 36, 1), 40, 0, "metropolis"), ((64, 34, 20), 2, 1, "metropolis")])
+def test_fused_measurement_in_recorded_sweeps_pm_j(P, oracle, dims, R, streams, rule):
+    """The same for the +-J kernels (row a7 for per-bond couplings): the quad kernel (Lx % 256 == 0, both rules), the
+    one-thread-per-word kernel with a shared update stream (replica chunks over gridDim.y) and with own streams; E and M
+    of every sweep equal the oracle's, and no measurement pass is launched for the Metropolis kernels."""
+    import torch
+
+    beta = 1.0 / 1.1
+    G, O = _pair(P, oracle, dims, storage="bitpack", coupling="bond_pm1", replicas=R, replica_streams=streams, rule=rule)
+    if G.N * R // 64 <= 1024:
+        pytest.skip("resident kernel territory")
+    l0 = G.launch_count
+    dE, dM = G.sweep_record(beta, 5)
+    torch.cuda.synchronize()
+    if not _PLAIN and (rule == "metropolis" or dims[0] % 256 == 0):
+        assert G.launch_count - l0 == 3 * 5, "two half-sweeps and one finalize per recorded sweep"
+    Eg, Mg = dE.cpu().numpy(), dM.cpu().numpy()[:, :, 0]
+    for t in range(5):
+        O.sweep(beta, 1)
+        e, m = O.measure()
+        assert np.array_equal(Eg[t], e) and np.array_equal(Mg[t], m[:, 0]), (t, Eg[t], e, Mg[t], m[:, 0])
+    _assert_ising_equal(G, O, "after fused recorded sweeps (+-J)")
+
+
 @pytest.mark.parametrize("n", [2, 3])
 def test_direction_map_accuracy(P, oracle, n):
     """The kernels' own sincospi (exact integer range reduction + two polynomials) against the oracle's double-precision,
