@@ -158,7 +158,15 @@ enum { SPIN_OPT_PLAIN_KERNELS = 0,
        /* A/B knob: 0 (default) = the tuned kernel of each family; 1 = the alternative kept beside it
         * (+-J shared stream: the cooperative kernel, one CTA of replica-chunk warps per 32 quads, instead of one thread per quad and all replicas).  Results never
         * depend on it. */
-       SPIN_OPT_KERNEL_VARIANT = 3 };
+       SPIN_OPT_KERNEL_VARIANT = 3,
+       /* Exact temporal blocking ("k updates per tile load", made results-neutral): spin_sweep
+        * runs pairs of sweeps in one pass over the lattice (each row read once and written once per two sweeps), bit-identical
+        * to plain sweeps.  Offered for 2D Ising, INT8 or BITPACK storage, uniform J = +-1, Metropolis, 2048 <= Lx <= 32768,
+        * Lx % 2048 == 0, own random stream per replica; such handles ask for twice the spin storage (spin_workspace_bytes).
+        * -1 (default) = on for lattices too large for the CUDA-graph regime, 0 = off, 1 = on wherever offered. */
+       SPIN_OPT_TEMPORAL_BLOCKING = 4,
+       /* rows per stripe of the temporal-blocking kernel; 0 (default) = one wave of resident CTAs */
+       SPIN_OPT_TBLOCK_ROWS = 5 };
 spin_status spin_set_option(spin_system *s, int32_t option, int64_t value);
 
 /* Frees the handle only; never the workspace. */

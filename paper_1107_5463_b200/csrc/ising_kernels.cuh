@@ -24,6 +24,8 @@ struct IsingArgs {
     uint32_t acc_slots;     // power of two: a CTA adds into slot blockIdx.x & (acc_slots - 1), so that atomics on one address
                             // do not serialise (65 536 of them per launch on two addresses cost 18 us); the finalize sums the slots
     HeatBathTable hb;       // filled when rule = 1
+    void *alt[2];           // temporal blocking (ising_tblock_kernel.cuh): the second pair of colour arrays it writes to
+    uint32_t tb_rows;       // temporal blocking: rows per stripe
     uint32_t prefetch;      // L2 prefetch distance (0 = off): replicas ahead (+-J quad kernel) / CTAs ahead (strip kernels)
 };
 

@@ -1,0 +1,141 @@
+// ising_tblock_kernel.cuh -- exact temporal blocking for the 2D Ising models: TWO full sweeps (four
+// half-sweeps) per pass over the lattice, results bit-identical to four plain half-sweeps.  The results-neutral
+// counterpart of the paper's "k updates per tile load" (its k-fold multi-hit changes the dynamics, R-1).
+//
+// A CTA owns a stripe of H full rows and marches down it with a ring of 16 rows (both colours, bit-packed, one 32-site
+// word per thread and row) in shared memory.  Half-sweep s = 1 .. 4 (colour 0, colour 1 of sweep t, then of sweep t + 1)
+// of a row needs its three neighbour rows at half-sweep s - 1, so the four half-sweeps follow the load front at a
+// distance of 2 rows each: in iteration i the CTA loads row i, applies half-sweep 1 to row i - 2, half-sweep 2 to row
+// i - 4, 3 to row i - 6, 4 to row i - 8 and stores row i - 8.  With that skew everything an iteration reads was written in
+// an earlier one (ONE barrier per iteration; see the hazard table in DESIGN.md section 5) and the five pieces of work are
+// independent (four Philox chains per thread in flight).  Each row is read from HBM once and written once per TWO sweeps:
+// 1 byte per update (int8) instead of 3.  A stripe starts 4 rows above its first row and ends 4 below its last
+// (shrinking halo: 12 redundant row updates per stripe = 3 / H of the work), reading from one pair of colour arrays and
+// writing to the other (ping-pong: a neighbouring stripe may still need the old rows), which the host swaps afterwards.
+//
+// Random numbers: the same Philox unit (global row and word), sweep index and colour as the plain kernels, so the
+// update sequence is unchanged (north_star (b)).  Acceptance: the lazy digit comparison with the deferred tail of the strip
+// kernels -- two Philox calls per word unconditionally, words with undecided lanes queued per warp and finished one per
+// lane before the barrier.
+#pragma once
+#include "ising_int8_kernel.cuh"
+
+namespace spin {
+
+constexpr int TB_RING = 16;          // ring slots (rows) per colour; 10 are live
+constexpr int TB_QCAP = 64;          // deferred-tail queue entries per warp and iteration
+constexpr int TB_QFIELDS = 5;        // unit, sweep offset | colour, eq, m[0], index of the word in the ring
+
+__host__ __device__ constexpr size_t tblock_smem_bytes(uint32_t WX) {
+    return (size_t)(2u * TB_RING * WX + (WX / 32u) * (1u + TB_QFIELDS * TB_QCAP)) * 4u;
+}
+
+// INT8: global arrays in the int8 fast layout (32-byte units), else bit-packed words.  grid = (stripes, R),
+// block = WX threads (one per word of a row; 32 <= WX <= MAXT), dynamic shared memory = tblock_smem_bytes(WX).
+// Reads a.s[0], a.s[1]; writes a.alt[0], a.alt[1]; sweeps a.t and a.t + 1.
+template <bool INT8, int MAXT>
+__global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 1) ising_tblock2_sweeps(const __grid_constant__ IsingArgs a) {
+    extern __shared__ __align__(16) uint32_t tb_smem[];
+    const Geometry &g = a.g;
+    const uint32_t WX = g.WX, Ly = (uint32_t)g.Ly, w = threadIdx.x, r = blockIdx.y;
+    const uint32_t warp = w >> 5, lane = w & 31u;
+    uint32_t *const qn = tb_smem + 2u * TB_RING * WX + warp * (1u + TB_QFIELDS * TB_QCAP);   // this warp's queue: count, fields
+    uint32_t *const qf = qn + 1;
+    const uint32_t H = a.tb_rows, y0 = blockIdx.x * H;
+    if (y0 >= Ly) return;
+    const int Hs = (int)min(H, Ly - y0);
+    const uint32_t w_next = w + 1u == WX ? 0u : w + 1u, w_prev = w == 0u ? WX - 1u : w - 1u;
+    const uint32_t rho = a.replica_streams ? r : 0u;
+    const uint32_t jflip = a.jneg ? 0xFFFFFFFFu : 0u;
+    const size_t rep = INT8 ? (size_t)r * g.Nh : (size_t)r * g.NW * 4u;           // byte offset of the replica
+    const uint8_t *const src0 = (const uint8_t *)a.s[0] + rep, *const src1 = (const uint8_t *)a.s[1] + rep;
+    uint8_t *const dst0 = (uint8_t *)a.alt[0] + rep, *const dst1 = (uint8_t *)a.alt[1] + rep;
+    const uint32_t rowbytes = INT8 ? 32u * WX : 4u * WX, wbytes = INT8 ? 32u * w : 4u * w;
+    // global row of local row 0 (4 above the stripe, periodic); y_s = global row of the row half-sweep s works on
+    uint32_t y_in = (y0 + 4u * Ly - 4u) % Ly;
+    uint32_t y_st[4];
+#pragma unroll
+    for (int s = 0; s < 4; ++s) y_st[s] = (y_in + 8u * Ly - 2u * (uint32_t)(s + 1)) % Ly;
+    if (lane == 0u) *qn = 0u;
+    for (int i = 0; i <= Hs + 11; ++i) {
+        // ---- the loads of local row i, consumed at the end of the iteration
+        const bool loading = i <= Hs + 7;
+        Int8RawUnit ld0, ld1;
+        uint32_t lw0 = 0u, lw1 = 0u;
+        if (loading) {
+            const size_t off = (size_t)y_in * rowbytes + wbytes;
+            if (INT8) { ld0 = int8_load_unit(src0 + off); ld1 = int8_load_unit(src1 + off); }
+            else { lw0 = __ldg((const uint32_t *)(src0 + off)); lw1 = __ldg((const uint32_t *)(src1 + off)); }
+        }
+        // ---- half-sweeps 1 .. 4 on local rows i - 2, i - 4, i - 6, i - 8
+#pragma unroll
+        for (int s = 1; s <= 4; ++s) {
+            const int l = i - 2 * s;
+            if (l >= s && l <= Hs + 7 - s) {
+                const uint32_t c = (uint32_t)(s - 1) & 1u, tt = a.t + (uint32_t)(s > 2), y = y_st[s - 1];
+                uint32_t *const mine_r = tb_smem + c * (TB_RING * WX);
+                const uint32_t *const oth_r = tb_smem + (1u - c) * (TB_RING * WX);
+                const uint32_t slot = ((uint32_t)l & (TB_RING - 1u)) * WX;
+                const uint32_t raw = mine_r[slot + w], o_cur = oth_r[slot + w];
+                const uint32_t o_prev = oth_r[(((uint32_t)l - 1u) & (TB_RING - 1u)) * WX + w];
+                const uint32_t o_next = oth_r[(((uint32_t)l + 1u) & (TB_RING - 1u)) * WX + w];
+                const uint32_t p = (y + c) & 1u;
+                const uint32_t o_side = oth_r[slot + (p ? w_next : w_prev)];
+                const uint32_t side = p ? ((o_cur >> 1) | (o_side << 31)) : ((o_cur << 1) | (o_side >> 31));
+                const uint32_t sp = raw ^ jflip;
+                uint32_t av[6];
+                av[0] = sp ^ o_cur; av[1] = sp ^ side; av[2] = sp ^ o_prev; av[3] = sp ^ o_next; av[4] = 0u; av[5] = 0u;
+                const uint32_t unit = y * WX + w + g.unit_off;
+                uint32_t eq, mm[2];
+                uint32_t fresh = ising_new_word_head<2>(a, tt, c, unit, rho, raw, av, eq, mm);
+                if (eq != 0u) {
+                    const uint32_t pos = atomicAdd(qn, 1u);
+                    if (pos < (uint32_t)TB_QCAP) {
+                        qf[0 * TB_QCAP + pos] = unit; qf[1 * TB_QCAP + pos] = 2u * (uint32_t)(s > 2) + c; qf[2 * TB_QCAP + pos] = eq;
+                        qf[3 * TB_QCAP + pos] = mm[0]; qf[4 * TB_QCAP + pos] = c * (TB_RING * WX) + slot + w;
+                    } else {
+                        fresh ^= lt_mask_select_tail<2>(a, tt, c, unit, rho, mm, eq);
+                    }
+                }
+                mine_r[slot + w] = fresh;
+            }
+        }
+        // ---- deferred tails: one queued word per lane (two rounds if more than 32 are pending), patched in the ring
+        __syncwarp();
+        {
+            const uint32_t nq = min(*qn, (uint32_t)TB_QCAP);
+            for (uint32_t e = lane; e < nq; e += 32u) {
+                uint32_t mm[2];
+                mm[0] = qf[3 * TB_QCAP + e]; mm[1] = 0u;
+                const uint32_t tc = qf[1 * TB_QCAP + e];
+                const uint32_t lt = lt_mask_select_tail<2>(a, a.t + (tc >> 1), tc & 1u, qf[0 * TB_QCAP + e], rho, mm, qf[2 * TB_QCAP + e]);
+                tb_smem[qf[4 * TB_QCAP + e]] ^= lt;
+            }
+            __syncwarp();
+            if (lane == 0u) *qn = 0u;
+        }
+        // ---- store local row i - 8 (half-sweep 4 done: both colours final)
+        {
+            const int l = i - 8;
+            if (l >= 4 && l <= Hs + 3) {
+                const uint32_t slot = ((uint32_t)l & (TB_RING - 1u)) * WX;
+                const uint32_t f0 = tb_smem[slot + w], f1 = tb_smem[TB_RING * WX + slot + w];
+                const size_t off = (size_t)y_st[3] * rowbytes + wbytes;
+                if (INT8) { int8_store_unit(dst0 + off, f0); int8_store_unit(dst1 + off, f1); }
+                else { *(uint32_t *)(dst0 + off) = f0; *(uint32_t *)(dst1 + off) = f1; }
+            }
+        }
+        // ---- local row i into the ring
+        if (loading) {
+            const uint32_t slot = ((uint32_t)i & (TB_RING - 1u)) * WX;
+            tb_smem[slot + w] = INT8 ? int8_pack_raw(ld0) : lw0;
+            tb_smem[TB_RING * WX + slot + w] = INT8 ? int8_pack_raw(ld1) : lw1;
+        }
+        y_in = y_in + 1u == Ly ? 0u : y_in + 1u;
+#pragma unroll
+        for (int s = 0; s < 4; ++s) y_st[s] = y_st[s] + 1u == Ly ? 0u : y_st[s] + 1u;
+        __syncthreads();
+    }
+}
+
+}  // namespace spin

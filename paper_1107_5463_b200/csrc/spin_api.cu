@@ -12,6 +12,7 @@
 #include "ising_int8_kernel.cuh"
 #include "ising_kernels.cuh"
 #include "ising_resident_kernel.cuh"
+#include "ising_tblock_kernel.cuh"
 #include "measure_kernels.cuh"
 #include "setup_kernels.cuh"
 #include "vector_kernels.cuh"
@@ -41,6 +42,7 @@ enum Path { PATH_ISING_GENERIC, PATH_ISING_INT8, PATH_ISING_BITPACK, PATH_VECTOR
 
 struct Layout {
     size_t off_s[2], bytes_s;   // one colour array
+    size_t off_alt[2];          // temporal blocking: the second pair of colour arrays (bytes_s each), or off_s when not offered
     size_t off_bonds, bytes_bonds;
     size_t off_acc, bytes_acc;  // n = 1: int64 [R][2]; n >= 2: double [R][partials][1 + n], then the two below
     size_t off_mid, off_cnt;    // n >= 2: double [R][FINALIZE_BLOCKS][1 + n] and unsigned [R] of vector_partials_finalize
@@ -67,6 +69,9 @@ struct spin_system {
     int axis, own_planes; // slab decomposition: axis (2 z, 1 y, -1 none) and owned planes along it
     uint32_t next_colour; // spin_halfsweep: colour expected next
     int vector_generic;  // n >= 2: force the one-thread-per-site kernel (test knob)
+    int tblock;          // SPIN_OPT_TEMPORAL_BLOCKING: -1 auto (lattices beyond the CUDA-graph regime), 0 off, 1 wherever offered
+    int tblock_rows;     // SPIN_OPT_TBLOCK_ROWS: rows per stripe, 0 = one wave of resident CTAs
+    int tblock_ok;       // this handle has the second pair of arrays
     int variant;         // SPIN_OPT_KERNEL_VARIANT: 0 = the default kernel of each family, > 0 = a named alternative (A/B knob)
     int l2_prefetch;     // SPIN_OPT_L2_PREFETCH: -1 each kernel's own distance (default), 0 off, > 0 that distance
     int grid_num, grid_den;
@@ -196,6 +201,16 @@ static uint32_t tma_grid_x(uint64_t S, uint64_t R, uint64_t cap) {
 constexpr uint64_t TMA_MAX_CTAS = 512;
 constexpr uint32_t FINALIZE_BLOCKS = 128;   // first-level blocks of vector_partials_finalize
 
+// Exact temporal blocking (two sweeps per pass, ising_tblock_kernel.cuh) is offered for the 2D Ising fast layouts with uniform
+// couplings and the Metropolis rule when a row of one colour is 32 .. 512 words; it needs a second pair of colour arrays.
+static bool tblock_offered(const spin_config *c, const Derived &dv) {
+    if (c->n != 1 || dv.d != 2 || dv.axis >= 0 || c->update_rule != SPIN_UPDATE_METROPOLIS) return false;
+    if (!(dv.path == PATH_ISING_INT8 || dv.path == PATH_ISING_BITPACK) || c->coupling_kind != SPIN_J_UNIFORM) return false;
+    if (c->n_replicas > 1 && !c->replica_streams) return false;   // shared-stream replicas take the mask-reuse kernels
+    const int32_t WX = dv.pad[0] / 64;
+    return WX >= 32 && WX <= 512 && WX % 32 == 0;
+}
+
 // slots of the n = 1 accumulators: as many as 64, fewer when there are many replicas (8192 / R rounded down to a power of two)
 static uint32_t acc_slots_for(uint64_t R) {
     uint32_t k = 64;
@@ -210,6 +225,10 @@ static void make_layout(const spin_config *c, const Derived &dv, Layout *l, uint
     else if (dv.path == PATH_VECTOR) l->bytes_s = (size_t)(R * Nh * c->n * sizeof(float));
     else l->bytes_s = (size_t)(R * Nh);
     for (int k = 0; k < 2; ++k) { l->off_s[k] = off; off += align_up(l->bytes_s); }
+    for (int k = 0; k < 2; ++k) {
+        l->off_alt[k] = l->off_s[k];
+        if (tblock_offered(c, dv)) { l->off_alt[k] = off; off += align_up(l->bytes_s); }
+    }
     l->bytes_bonds = 0;
     if (c->coupling_kind == SPIN_J_BOND_PM1)
         l->bytes_bonds = dv.path == PATH_ISING_BITPACK ? (size_t)(2 * R * 3 * (Nh / 32) * 4) : (size_t)(R * dv.d * dv.N);
@@ -314,6 +333,9 @@ static IsingArgs ising_args(const spin_system *s) {
     a.hb = s->hb;
     a.acc = (long long *)(s->ws + s->lay.off_acc);
     a.acc_slots = acc_slots_for(s->R);
+    a.alt[0] = s->ws + s->lay.off_alt[0];
+    a.alt[1] = s->ws + s->lay.off_alt[1];
+    a.tb_rows = 0;
     return a;
 }
 
@@ -624,6 +646,63 @@ static spin_status launch_halfsweep_vector(spin_system *s, const VectorArgs &a, 
     return SPIN_OK;
 }
 
+// ------------------------------------------------------------------- temporal blocking -------
+static bool graph_ok(const spin_system *s, int64_t n_sweeps);
+static void graph_drop(spin_system *s);
+static bool tblock_use(const spin_system *s, int64_t n_sweeps) {
+    if (!s->tblock_ok || s->tblock == 0 || s->vector_generic || n_sweeps < 2) return false;
+    if (s->tblock == 1) return true;
+    return !graph_ok(s, 1 << 20);   // auto: only where a half-sweep outlasts its launch
+}
+
+template <bool INT8, int MAXT>
+static cudaError_t tblock_launch(const IsingArgs &a, dim3 G, int B, size_t smem, cudaStream_t st) {
+    static size_t configured = 0;
+    if (configured < smem) {
+        cudaError_t e = cudaFuncSetAttribute(ising_tblock2_sweeps<INT8, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = smem;
+    }
+    ising_tblock2_sweeps<INT8, MAXT><<<G, B, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+// pairs of sweeps through the temporal-blocking kernel; the colour arrays swap roles after every launch
+static spin_status tblock_sweeps(spin_system *s, int64_t pairs, cudaStream_t st) {
+    const int B = (int)s->g.WX;
+    const size_t smem = tblock_smem_bytes(s->g.WX);
+    const bool i8 = s->path == PATH_ISING_INT8;
+    // rows per stripe: one wave of resident CTAs (a stripe costs 3 / H redundant row updates; a second wave would idle)
+    uint32_t H = (uint32_t)s->tblock_rows;
+    if (H == 0) {
+        int per_sm = 1;
+        cudaError_t e;
+        if (B <= 256) e = i8 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_tblock2_sweeps<true, 256>, B, smem)
+                             : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_tblock2_sweeps<false, 256>, B, smem);
+        else e = i8 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_tblock2_sweeps<true, 512>, B, smem)
+                    : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_tblock2_sweeps<false, 512>, B, smem);
+        if (e != cudaSuccess || per_sm < 1) per_sm = 1;
+        uint64_t stripes = (uint64_t)s->sm_count * per_sm / s->R;
+        if (stripes < 1) stripes = 1;
+        H = (uint32_t)(((uint64_t)s->g.Ly + stripes - 1) / stripes);
+        if (H < 8) H = 8;
+    }
+    const dim3 G((unsigned)((s->g.Ly + H - 1) / H), s->R);
+    for (int64_t k = 0; k < pairs; ++k) {
+        IsingArgs a = ising_args(s);
+        a.tb_rows = H;
+        cudaError_t e;
+        if (B <= 256) e = i8 ? tblock_launch<true, 256>(a, G, B, smem, st) : tblock_launch<false, 256>(a, G, B, smem, st);
+        else e = i8 ? tblock_launch<true, 512>(a, G, B, smem, st) : tblock_launch<false, 512>(a, G, B, smem, st);
+        if (e != cudaSuccess) return fail(SPIN_ERR_CUDA, "temporal-blocking launch: %s", cudaGetErrorString(e));
+        for (int c = 0; c < 2; ++c) { const size_t t = s->lay.off_s[c]; s->lay.off_s[c] = s->lay.off_alt[c]; s->lay.off_alt[c] = t; }
+        s->t += 2;
+        s->launches += 1;
+    }
+    graph_drop(s);   // a captured graph holds the array pointers of before the swap
+    return SPIN_OK;
+}
+
 // One sweep at sweep index t_override (graph capture: the handle is not advanced) or at the handle's counter.
 static spin_status enqueue_sweep(spin_system *s, double beta, cudaStream_t st, bool capture = false, uint32_t t_override = 0) {
     if (s->n == 1) {
@@ -664,6 +743,7 @@ struct GraphNode {
     GraphNode() {}
 };
 
+static void graph_drop(spin_system *s);
 static bool graph_ok(const spin_system *s, int64_t n_sweeps) {
     if (s->vector_generic || s->axis >= 0 || n_sweeps < 2 * GRAPH_SWEEPS) return false;
     // threads of a half-sweep launch; beyond a few full waves the kernel outlasts its launch
@@ -866,7 +946,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
     s->tma_ok = 0; s->use_tma = -1; s->tma_ty = 0;
     s->t = 0; s->launches = 0; s->staging = nullptr; s->staging_bytes = 0; s->gexec = nullptr; s->cap_stream = nullptr; s->gnodes = nullptr; s->n_gnodes = 0;
     // 128 threads per CTA for the Ising fast paths (measured: +-J R = 16 39.1 vs 40.4 us with 256)
-    s->block = (dv.path == PATH_ISING_INT8 || dv.path == PATH_ISING_BITPACK) ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0; s->l2_prefetch = -1; s->variant = 0;
+    s->block = (dv.path == PATH_ISING_INT8 || dv.path == PATH_ISING_BITPACK) ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0; s->l2_prefetch = -1; s->variant = 0; s->tblock = -1; s->tblock_rows = 0; s->tblock_ok = tblock_offered(cfg, dv) ? 1 : 0;
     s->table_beta = std::nan("");
     Geometry &g = s->g;
     g.Lx = dv.pad[0]; g.Ly = dv.pad[1]; g.Lz = dv.pad[2]; g.d = dv.d;
@@ -952,7 +1032,12 @@ spin_status spin_sweep(spin_system *s, double beta, int64_t n_sweeps, void *stre
     if (rc != SPIN_OK) return rc;
     if (s->axis >= 0) return fail(SPIN_ERR_STATE, "slab handle: drive it with spin_halfsweep and the halo calls");
     if (s->next_colour != 0) return fail(SPIN_ERR_STATE, "a spin_halfsweep of colour 1 is pending");
-    if (resident_ok(s, false)) return enqueue_resident(s, n_sweeps, nullptr, nullptr, (cudaStream_t)stream);
+    if (tblock_use(s, n_sweeps)) {
+        // two sweeps per pass over the lattice; an odd last sweep goes through the plain kernels below
+        rc = tblock_sweeps(s, n_sweeps / 2, (cudaStream_t)stream);
+        if (rc != SPIN_OK) return rc;
+        n_sweeps &= 1;
+    } else if (resident_ok(s, false)) return enqueue_resident(s, n_sweeps, nullptr, nullptr, (cudaStream_t)stream);
     if (graph_ok(s, n_sweeps)) {
         int64_t done = 0;
         rc = graph_sweeps(s, beta, n_sweeps, (cudaStream_t)stream, &done);
@@ -1245,6 +1330,16 @@ spin_status spin_set_option(spin_system *s, int32_t option, int64_t value) {
     if (option == SPIN_OPT_TMA_KERNELS) {
         if (value != 0 && value != 1 && value != -1) return fail(SPIN_ERR_INVALID_ARG, "SPIN_OPT_TMA_KERNELS takes 0, 1 or -1");
         s->use_tma = (int)value;
+        return SPIN_OK;
+    }
+    if (option == SPIN_OPT_TEMPORAL_BLOCKING) {
+        if (value < -1 || value > 1) return fail(SPIN_ERR_INVALID_ARG, "SPIN_OPT_TEMPORAL_BLOCKING takes -1, 0 or 1");
+        s->tblock = (int)value;
+        return SPIN_OK;
+    }
+    if (option == SPIN_OPT_TBLOCK_ROWS) {
+        if (value < 0 || value > (1 << 24)) return fail(SPIN_ERR_INVALID_ARG, "SPIN_OPT_TBLOCK_ROWS takes 0 (automatic) or a number of rows");
+        s->tblock_rows = (int)value;
         return SPIN_OK;
     }
     if (option == SPIN_OPT_KERNEL_VARIANT) {
