@@ -35,8 +35,9 @@ UNIT = "flips/ns"
 DEFAULT_WORKLOAD = "ising2d_L16384_int8"
 # per-model legs of the default run: (workload, sweeps timed)
 PER_MODEL = [("ising2d_L64_int8", 200), ("ising2d_L16384_bitpack", 40), ("ising3d_L512_bitpack", 40),
-             ("ea3d_L256_R16_bitpack", 40), ("ea2d_L64_R4096_bitpack", 200), ("heisenberg3d_L256_fp32", 20),
-             ("xy3d_L256_fp32", 20)]
+             ("ea3d_L256_R16_bitpack", 40), ("ea3d_L256_R16_bitpack_ownstreams", 20), ("ea2d_L64_R4096_bitpack", 200),
+             ("heisenberg3d_L256_fp32", 20), ("xy3d_L256_fp32", 20)]
+RECORDED = ("ising2d_L16384_bitpack", "ea3d_L256_R16_bitpack", "heisenberg3d_L256_fp32", "xy3d_L256_fp32")
 DTYPE = {"int8": "u8", "bitpack": "u32 (bit-packed, 32 spins per word)", "fp32": "f32"}
 
 
@@ -99,19 +100,22 @@ class ClockSampler:
                 "samples": len(sm), "power_w_max": max(power) if power else None}
 
 
-def time_sweeps(S, beta, sweeps, warm=3):
-    """ms per half-sweep launch and flips/ns of `sweeps` sweeps of system S (state resident, CUDA events)."""
+def time_sweeps(S, beta, sweeps, warm=4, record=False):
+    """ms per half-sweep (time / 2 sweeps, whatever the number of launches), flips/ns and launches of `sweeps` sweeps of
+    system S (state resident, CUDA events on the launching stream)."""
     import torch
 
-    S.sweep(beta, warm)
+    run = S.sweep_record if record else S.sweep
+    run(beta, warm)
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = S.launch_count
     e0.record()
-    S.sweep(beta, sweeps)
+    run(beta, sweeps)
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1)
-    return ms / (2 * sweeps), S.N * S.R * sweeps / (ms * 1e6)
+    return ms / (2 * sweeps), S.N * S.R * sweeps / (ms * 1e6), S.launch_count - l0
 
 
 def run_per_model(P, peak):
@@ -119,8 +123,10 @@ def run_per_model(P, peak):
 
     out = {}
     for name, sweeps in PER_MODEL:
-        w = P.workloads.WORKLOADS[name]
-        S = P.from_workload(w, P.workloads.SEED)
+        # "<workload>_ownstreams": the same lattice with the replica index in the Philox counter (replica_streams = 1)
+        base = name[:-len("_ownstreams")] if name.endswith("_ownstreams") else name
+        w = P.workloads.WORKLOADS[base]
+        S = P.from_workload(w, P.workloads.SEED, **({"replica_streams": 1} if base != name else {}))
         if w["record"]:
             # config 1: E and M after every sweep (spin_sweep_record)
             S.sweep_record(w["beta"], 3)
@@ -135,20 +141,35 @@ def run_per_model(P, peak):
                          "note": "one launch of the shared-memory-resident kernel for all sweeps; E and M recorded "
                                  "every sweep; latency-bound (64 words per colour)"}
         else:
-            ms_launch, fpn = time_sweeps(S, w["beta"], sweeps)
-            bpu = P.workloads.BYTES_PER_UPDATE[name]
-            out[name] = {"flips_per_ns": fpn, "ms_per_halfsweep": ms_launch, "algorithmic_GBps": fpn * bpu,
-                         "hbm_frac": fpn * bpu / peak, "bytes_per_update": bpu}
-            if w["storage"] == "bitpack" and name in WARP_INSTR:
-                gwips = WARP_INSTR[name] / (ms_launch * 1e6)
-                out[name]["roofline"] = {"bound": "alu", "achieved": gwips, "peak": ISSUE_PEAK_GWIPS,
-                                         "unit": "Gwarp-instr/s", "frac": gwips / ISSUE_PEAK_GWIPS,
-                                         "traffic": TRAFFIC.get(name),
-                                         "note": "instructions per launch from the committed ncu capture; peak = issue rate"}
-                out[name]["note"] = "state is L2-resident or nearly so; bound by integer issue, not HBM"
+            ms_half, fpn, launches = time_sweeps(S, w["beta"], sweeps)
+            bpu = P.workloads.BYTES_PER_UPDATE[base]
+            cnt = COUNTERS.get(name, {})
+            out[name] = {"flips_per_ns": fpn, "ms_per_halfsweep": ms_half, "launches_per_sweep": launches / sweeps,
+                         "algorithmic_GBps": fpn * bpu, "hbm_frac": fpn * bpu / peak, "bytes_per_update": bpu,
+                         "kernel": cnt.get("kernel")}
+            if base != name:
+                out[name]["note"] = "16 replicas with their OWN update streams (replica_streams = 1): no mask reuse across replicas"
+            elif w["replicas"] > 1 and not w["replica_streams"]:
+                out[name]["note"] = "shared update stream (DESIGN.md R-17): the acceptance masks of a word serve every replica"
+            if cnt.get("bound") == "alu":
+                # executed warp-instructions per launch (committed ncu capture) / launch time, against the issue rate; the
+                # pipe that binds is the ALU pipe (LOP3 / IADD3 / SHF / ISETP at one warp-instruction per 2 clocks)
+                ms_launch = 2 * sweeps * ms_half / launches
+                gwips = cnt["warp_instr_per_launch"] / (ms_launch * 1e6)
+                out[name]["roofline"] = {"bound": "alu", "achieved": gwips, "peak": ISSUE_PEAK_GWIPS, "unit": "Gwarp-instr/s",
+                                         "frac": gwips / ISSUE_PEAK_GWIPS, "traffic": cnt.get("dram_bytes_per_launch"),
+                                         "alu_pipe_busy_pct_in_capture": cnt.get("alu_pipe_pct"),
+                                         "note": "instructions per launch from the committed ncu capture (%s); peak = issue "
+                                                 "rate; state L2-resident" % cnt.get("capture")}
             else:
                 out[name]["roofline"] = {"bound": "hbm", "achieved": fpn * bpu, "peak": peak, "unit": "GB/s",
-                                         "frac": fpn * bpu / peak, "traffic": TRAFFIC.get(name)}
+                                         "frac": fpn * bpu / peak, "frac_of_nominal_8000": fpn * bpu / 8000.0,
+                                         "traffic": cnt.get("dram_bytes_per_launch"), "capture": cnt.get("capture")}
+            if name in RECORDED:
+                # E and M after every sweep, fused into the colour-1 half-sweep
+                ms_rec, fpn_rec, l_rec = time_sweeps(S, w["beta"], max(4, sweeps // 2), record=True)
+                out[name]["recorded"] = {"flips_per_ns": fpn_rec, "ms_per_halfsweep": ms_rec, "launches_per_sweep": l_rec / max(4, sweeps // 2),
+                                         "cost_vs_unrecorded": ms_rec / ms_half}
         S.close()
         del S
         torch.cuda.empty_cache()
@@ -156,7 +177,7 @@ def run_per_model(P, peak):
     for name, sweeps in (("ising2d_L16384_int8", 20), ("ising3d_L512_bitpack", 20), ("heisenberg3d_L256_fp32", 10)):
         w = P.workloads.WORKLOADS[name]
         S = P.from_workload(w, P.workloads.SEED, rule="heatbath")
-        ms_launch, fpn = time_sweeps(S, w["beta"], sweeps)
+        ms_launch, fpn, _ = time_sweeps(S, w["beta"], sweeps)
         bpu = P.workloads.BYTES_PER_UPDATE[name]
         out[name + "_heatbath"] = {"flips_per_ns": fpn, "ms_per_halfsweep": ms_launch, "algorithmic_GBps": fpn * bpu,
                                    "hbm_frac": fpn * bpu / peak, "bytes_per_update": bpu, "update_rule": "heat bath"}
@@ -292,12 +313,15 @@ def run_graft(args):
     t_wall1 = time.time()
     clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
     launches = S.launch_count - launches0
+    cnt = COUNTERS.get(args.workload, {})
     ms_total = max_over_ranks(e0.elapsed_time(e1))
     ms_sweeps = sum(a.elapsed_time(b) for a, b in sweep_ev)
     value = world * updates_per_step * args.steps / (ms_total * 1e6)
-    ms_launch = ms_sweeps / (args.steps * SPS * 2)
+    sweep_launches = launches - 2 * args.steps                  # spin_measure: one pass + one finalize per step
+    ms_launch = ms_sweeps / sweep_launches
     bpu = P.workloads.BYTES_PER_UPDATE[args.workload]
-    bytes_per_launch = bpu * S.N * S.R / 2
+    updates_per_launch = S.N * S.R * SPS * args.steps / sweep_launches   # N R / 2 per half-sweep launch, 2 N R per two-sweep pass
+    bytes_per_launch = bpu * updates_per_launch
     achieved = bytes_per_launch / (ms_launch * 1e6)  # GB/s
 
     # ---- end-to-end arm: host buffers through the C ABI ------------------------------------------
@@ -341,11 +365,21 @@ def run_graft(args):
                    if w["storage"] != "bitpack" else "bit-packed state is L2-resident by design (33.5 MB); not flushed",
                    "parallelism": "independent lattice per GPU (weak scaling, no collective)" if world > 1 else "1 GPU"},
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": "half-sweep of %s" % args.workload, "achieved": achieved, "peak": peak,
-                     "unit": "GB/s", "frac": achieved / peak, "traffic": TRAFFIC.get(args.workload),
+        "roofline": {"bound": "hbm", "kernel": cnt.get("kernel", "half-sweep of %s" % args.workload), "achieved": achieved,
+                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": cnt.get("dram_bytes_per_launch"),
                      "peak_source": peak_src, "bytes_per_launch": bytes_per_launch, "ms_per_launch": ms_launch,
-                     "bytes_per_update": bpu, "frac_of_nominal_8000": achieved / 8000.0},
+                     "updates_per_launch": updates_per_launch, "bytes_per_update": bpu,
+                     "frac_of_nominal_8000": achieved / 8000.0, "capture": cnt.get("capture")},
     }
+    if cnt.get("dram_bytes_per_launch") and cnt.get("updates_per_launch"):
+        # what the kernel really moves: DRAM bytes of the committed ncu capture, per update and as a bandwidth at this run's time
+        tr = cnt["dram_bytes_per_launch"] * (updates_per_launch / cnt["updates_per_launch"])
+        line["roofline"].update({"dram_bytes_per_update": tr / updates_per_launch, "dram_GBps": tr / (ms_launch * 1e6),
+                                 "dram_frac": tr / (ms_launch * 1e6) / peak})
+    if cnt.get("warp_instr_per_launch") and cnt.get("updates_per_launch"):
+        wi = cnt["warp_instr_per_launch"] * (updates_per_launch / cnt["updates_per_launch"])
+        line["roofline"].update({"issue_frac": wi / (ms_launch * 1e6) / ISSUE_PEAK_GWIPS,
+                                 "alu_pipe_busy_pct_in_capture": cnt.get("alu_pipe_pct"), "note": cnt.get("note")})
     if not args.no_per_model and world == 1:
         line["per_model"] = run_per_model(P, peak)
     if not args.no_cpu_baseline:
@@ -356,21 +390,20 @@ def run_graft(args):
         dist.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
-TRAFFIC = {  # profiles/r01d_all_kernels.md
-    "ising2d_L16384_int8": 362360064,      # 268.50 MB read + 93.86 MB written
-    "ising2d_L16384_bitpack": 33593088,    # state L2-resident: one read pass, no write-back inside the launch
-    "ising3d_L512_bitpack": 16820224,
-    "ea3d_L256_R16_bitpack": 144403456,
-    "ea2d_L64_R4096_bitpack": 6305280,
-    "heisenberg3d_L256_fp32": 266009856,
-    "xy3d_L256_fp32": 166662144,
-}
-# Executed warp-instructions per half-sweep launch (smsp__inst_executed.sum of the same captures), for the kernels whose
-# bound is integer arithmetic rather than HBM; the peak they are set against is the issue rate
-# 148 SMs x 4 sub-cores x 1 warp-instruction per clock x 1.965 GHz.
-WARP_INSTR = {"ising2d_L16384_bitpack": 38098807, "ising3d_L512_bitpack": 21948915}
+# Counters of the dominant kernel of each workload, from the committed `ncu --set full` captures: profiles/counters.json is
+# written from the ncu exports (each entry names its kernel and its capture), so a replaced kernel cannot keep the numbers of
+# its predecessor -- an entry whose kernel no longer runs is dropped there and the fields here become null.
+#   dram_bytes_per_launch = dram__bytes_read.sum + dram__bytes_write.sum, warp_instr_per_launch = smsp__inst_executed.sum
+def load_counters():
+    try:
+        with open(os.path.join(ROOT, "profiles", "counters.json")) as f:
+            return json.load(f)
+    except Exception:
+        return {}
+
+
+COUNTERS = load_counters()
+# issue rate: 148 SMs x 4 sub-cores x 1 warp-instruction per clock x 1.965 GHz
 ISSUE_PEAK_GWIPS = 148 * 4 * 1.965
 
 

@@ -163,7 +163,7 @@ enum { SPIN_OPT_PLAIN_KERNELS = 0,
         * runs pairs of sweeps in one pass over the lattice (each row read once and written once per two sweeps), bit-identical
         * to plain sweeps.  Offered for 2D Ising, INT8 or BITPACK storage, uniform J = +-1, Metropolis, 2048 <= Lx <= 32768,
         * Lx % 2048 == 0, own random stream per replica; such handles ask for twice the spin storage (spin_workspace_bytes).
-        * -1 (default) = on for lattices too large for the CUDA-graph regime, 0 = off, 1 = on wherever offered. */
+        * -1 (default) = on for INT8 lattices too large for the CUDA-graph regime, 0 = off, 1 = on wherever offered. */
        SPIN_OPT_TEMPORAL_BLOCKING = 4,
        /* rows per stripe of the temporal-blocking kernel; 0 (default) = one wave of resident CTAs */
        SPIN_OPT_TBLOCK_ROWS = 5 };

@@ -23,7 +23,7 @@
 namespace spin {
 
 constexpr int TB_RING = 16;          // ring slots (rows) per colour; 10 are live
-constexpr int TB_QCAP = 64;          // deferred-tail queue entries per warp and iteration
+constexpr int TB_QCAP = 128;         // deferred-tail queue entries per warp and iteration: 4 half-sweeps x 32 lanes, it cannot overflow
 constexpr int TB_QFIELDS = 5;        // unit, sweep offset | colour, eq, m[0], index of the word in the ring
 
 __host__ __device__ constexpr size_t tblock_smem_bytes(uint32_t WX) {
@@ -67,43 +67,48 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 1) ising_tblock2_sweep
             if (INT8) { ld0 = int8_load_unit(src0 + off); ld1 = int8_load_unit(src1 + off); }
             else { lw0 = __ldg((const uint32_t *)(src0 + off)); lw1 = __ldg((const uint32_t *)(src1 + off)); }
         }
-        // ---- half-sweeps 1 .. 4 on local rows i - 2, i - 4, i - 6, i - 8
-#pragma unroll
-        for (int s = 1; s <= 4; ++s) {
+        // ---- half-sweeps 1 .. 4 on local rows i - 2, i - 4, i - 6, i - 8.  In the steady state (all four rows inside their
+        // ranges) the four updates are straight-line code, so that the scheduler can interleave their Philox chains
+        const auto half_sweep = [&](int s) {
             const int l = i - 2 * s;
-            if (l >= s && l <= Hs + 7 - s) {
-                const uint32_t c = (uint32_t)(s - 1) & 1u, tt = a.t + (uint32_t)(s > 2), y = y_st[s - 1];
-                uint32_t *const mine_r = tb_smem + c * (TB_RING * WX);
-                const uint32_t *const oth_r = tb_smem + (1u - c) * (TB_RING * WX);
-                const uint32_t slot = ((uint32_t)l & (TB_RING - 1u)) * WX;
-                const uint32_t raw = mine_r[slot + w], o_cur = oth_r[slot + w];
-                const uint32_t o_prev = oth_r[(((uint32_t)l - 1u) & (TB_RING - 1u)) * WX + w];
-                const uint32_t o_next = oth_r[(((uint32_t)l + 1u) & (TB_RING - 1u)) * WX + w];
-                const uint32_t p = (y + c) & 1u;
-                const uint32_t o_side = oth_r[slot + (p ? w_next : w_prev)];
-                const uint32_t side = p ? ((o_cur >> 1) | (o_side << 31)) : ((o_cur << 1) | (o_side >> 31));
-                const uint32_t sp = raw ^ jflip;
-                uint32_t av[6];
-                av[0] = sp ^ o_cur; av[1] = sp ^ side; av[2] = sp ^ o_prev; av[3] = sp ^ o_next; av[4] = 0u; av[5] = 0u;
-                const uint32_t unit = y * WX + w + g.unit_off;
-                uint32_t eq, mm[2];
-                uint32_t fresh = ising_new_word_head<2>(a, tt, c, unit, rho, raw, av, eq, mm);
-                if (eq != 0u) {
-                    const uint32_t pos = atomicAdd(qn, 1u);
-                    if (pos < (uint32_t)TB_QCAP) {
-                        qf[0 * TB_QCAP + pos] = unit; qf[1 * TB_QCAP + pos] = 2u * (uint32_t)(s > 2) + c; qf[2 * TB_QCAP + pos] = eq;
-                        qf[3 * TB_QCAP + pos] = mm[0]; qf[4 * TB_QCAP + pos] = c * (TB_RING * WX) + slot + w;
-                    } else {
-                        fresh ^= lt_mask_select_tail<2>(a, tt, c, unit, rho, mm, eq);
-                    }
+            const uint32_t c = (uint32_t)(s - 1) & 1u, tt = a.t + (uint32_t)(s > 2), y = y_st[s - 1];
+            uint32_t *const mine_r = tb_smem + c * (TB_RING * WX);
+            const uint32_t *const oth_r = tb_smem + (1u - c) * (TB_RING * WX);
+            const uint32_t slot = ((uint32_t)l & (TB_RING - 1u)) * WX;
+            const uint32_t raw = mine_r[slot + w], o_cur = oth_r[slot + w];
+            const uint32_t o_prev = oth_r[(((uint32_t)l - 1u) & (TB_RING - 1u)) * WX + w];
+            const uint32_t o_next = oth_r[(((uint32_t)l + 1u) & (TB_RING - 1u)) * WX + w];
+            const uint32_t p = (y + c) & 1u;
+            const uint32_t o_side = oth_r[slot + (p ? w_next : w_prev)];
+            const uint32_t side = p ? ((o_cur >> 1) | (o_side << 31)) : ((o_cur << 1) | (o_side >> 31));
+            const uint32_t sp = raw ^ jflip;
+            uint32_t av[6];
+            av[0] = sp ^ o_cur; av[1] = sp ^ side; av[2] = sp ^ o_prev; av[3] = sp ^ o_next; av[4] = 0u; av[5] = 0u;
+            const uint32_t unit = y * WX + w + g.unit_off;
+            uint32_t eq, mm[2];
+            const uint32_t fresh = ising_new_word_head<2>(a, tt, c, unit, rho, raw, av, eq, mm);
+            mine_r[slot + w] = fresh;
+            if (eq != 0u) {
+                const uint32_t pos = atomicAdd(qn, 1u);   // < TB_QCAP: at most 4 x 32 pushes per warp and iteration
+                qf[0 * TB_QCAP + pos] = unit; qf[1 * TB_QCAP + pos] = 2u * (uint32_t)(s > 2) + c; qf[2 * TB_QCAP + pos] = eq;
+                qf[3 * TB_QCAP + pos] = mm[0]; qf[4 * TB_QCAP + pos] = c * (TB_RING * WX) + slot + w;
+            }
+        };
+        if (i >= 12 && i <= Hs + 8) {
+            half_sweep(1); half_sweep(2); half_sweep(3); half_sweep(4);
+        } else {
+#pragma unroll 1
+            for (int s = 1; s <= 4; ++s) {
+                const int l = i - 2 * s;
+                if (l >= s && l <= Hs + 7 - s) {
+                    if (s == 1) half_sweep(1); else if (s == 2) half_sweep(2); else if (s == 3) half_sweep(3); else half_sweep(4);
                 }
-                mine_r[slot + w] = fresh;
             }
         }
         // ---- deferred tails: one queued word per lane (two rounds if more than 32 are pending), patched in the ring
         __syncwarp();
         {
-            const uint32_t nq = min(*qn, (uint32_t)TB_QCAP);
+            const uint32_t nq = *qn;
             for (uint32_t e = lane; e < nq; e += 32u) {
                 uint32_t mm[2];
                 mm[0] = qf[3 * TB_QCAP + e]; mm[1] = 0u;

@@ -652,7 +652,9 @@ static void graph_drop(spin_system *s);
 static bool tblock_use(const spin_system *s, int64_t n_sweeps) {
     if (!s->tblock_ok || s->tblock == 0 || s->vector_generic || n_sweeps < 2) return false;
     if (s->tblock == 1) return true;
-    return !graph_ok(s, 1 << 20);   // auto: only where a half-sweep outlasts its launch
+    // auto: int8 storage (where it cuts the HBM traffic to a third; the bit-packed lattices are L2-resident and gain nothing:
+    // 55.2 vs 55.6 us at L = 16384) and only where a half-sweep outlasts its launch
+    return s->path == PATH_ISING_INT8 && !graph_ok(s, 1 << 20);
 }
 
 template <bool INT8, int MAXT>

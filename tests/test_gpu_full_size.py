@@ -204,3 +204,30 @@ def test_full_size_vector_models(P, oracle, name):
     Eref = -sum(float((g * np.roll(g, -1, axis=ax)).sum()) for ax in (2, 1, 0))
     assert abs(E[0] - Eref) <= 1e-9 * abs(Eref) + 1e-6
     assert np.allclose(M[0], g.reshape(-1, n).sum(axis=0), rtol=0, atol=1e-6 * Lx * Ly * Lz * 1e-3 + 1e-3)
+
+
+@pytest.mark.parametrize("name", ["ising2d_L16384_int8", "ising2d_L16384_bitpack", "ising3d_L512_bitpack",
+                                  "ea3d_L256_R16_bitpack"])
+def test_whole_lattice_two_sweeps_against_the_oracle(P, name):
+    """SURVEY 8(c) protocol at full size: every byte of spin_get_spins equals the oracle's configuration after two full
+    sweeps of the BASELINE lattice (2.7e8 updates per sweep, about 9 s each for the single-threaded oracle), in the
+    launch configuration bench.py times -- for config 2 that is ONE launch of the temporal-blocking kernel (f3)."""
+    import oracle
+
+    w = P.workloads.WORKLOADS[name]
+    kinds = {"uniform": oracle.J_UNIFORM, "per_direction": oracle.J_PER_DIRECTION, "bond_pm1": oracle.J_BOND_PM1}
+    G = P.from_workload(w, P.workloads.SEED)
+    O = oracle.System(w["dims"], n=1, coupling_kind=kinds[w["coupling"]], J=w["J"], n_replicas=w["replicas"],
+                      replica_streams=w["replica_streams"], seed=P.workloads.SEED)
+    assert np.array_equal(G.get_spins(), O.get_spins()), "hot start"
+    l0 = G.launch_count
+    G.sweep(w["beta"], 2)
+    if name == "ising2d_L16384_int8":
+        assert G.launch_count - l0 == 1, "two sweeps in one pass (temporal blocking is the default for int8 at this size)"
+    O.sweep(w["beta"], 2)
+    gs, os_ = G.get_spins(), O.get_spins()
+    bad = int(np.count_nonzero(gs != os_))
+    assert bad == 0, "%d of %d spins differ after two sweeps" % (bad, gs.size)
+    Eg, Mg = G.measure()
+    Eo, Mo = O.measure()
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)

@@ -99,3 +99,18 @@ def test_temporal_blocking_not_offered(P):
     H.set_option(P.OPT_PLAIN_KERNELS, 1)
     H.sweep(BETA_C, 2)
     assert np.array_equal(G.get_spins(), H.get_spins())
+
+
+@pytest.mark.parametrize("storage", ["int8", "bitpack"])
+def test_full_size_pairs_equal_plain_sweeps(P, storage):
+    """BASELINE config 2 at full size, default knobs: five sweeps with temporal blocking (two passes + one plain sweep)
+    leave exactly the bytes of five plain sweeps."""
+    w = P.workloads.WORKLOADS["ising2d_L16384_" + storage]
+    A, B = P.from_workload(w, P.workloads.SEED), P.from_workload(w, P.workloads.SEED)
+    A.set_option(P.OPT_TEMPORAL_BLOCKING, 1 if storage == "bitpack" else -1)   # int8: the default; bit-packed: on request
+    B.set_option(P.OPT_TEMPORAL_BLOCKING, 0)
+    l0 = A.launch_count
+    A.sweep(w["beta"], 5)
+    B.sweep(w["beta"], 5)
+    assert A.launch_count - l0 == 2 + 2, "two passes of two sweeps and the two half-sweeps of the odd one"
+    assert np.array_equal(A.get_spins(), B.get_spins())
