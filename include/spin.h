@@ -51,7 +51,12 @@ typedef enum {
 enum { SPIN_STORE_INT8 = 0,   /* n = 1: one byte per spin                                             */
        SPIN_STORE_BITPACK = 1,/* n = 1: one bit per spin, 32 same-colour sites per word (multi-spin
                                  coding); needs Lx % 64 == 0 and |J| = 1                 */
-       SPIN_STORE_FP32 = 2 }; /* n = 2, 3: fp32 unit vectors, one plane per component and colour      */
+       SPIN_STORE_FP32 = 2,   /* n = 2, 3: fp32 unit vectors, one plane per component and colour      */
+       SPIN_STORE_MSC = 3 };  /* n = 1, SPIN_J_BOND_PM1, replica_streams = 0, n_replicas % 32 == 0,
+                                 N / 2 % 32 == 0: one bit per spin, the 32 realisations 32 k .. 32 k + 31
+                                 of ONE site per word ("asynchronous" multi-spin coding over disorder
+                                 realisations; Table 1 "Metro. multi-spin"): every
+                                 realisation of a site sees the same random number.  Takes L = 32.      */
 enum { SPIN_J_UNIFORM = 0,        /* J[0] on every bond                                               */
        SPIN_J_PER_DIRECTION = 1,  /* J[mu] on bonds in direction mu = x, y, z                         */
        SPIN_J_BOND_PM1 = 2 };     /* one +-1 per bond and replica (Edwards-Anderson); n = 1 */

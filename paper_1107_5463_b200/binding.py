@@ -11,7 +11,7 @@ import numpy as np
 
 from . import build as _build
 
-STORE_INT8, STORE_BITPACK, STORE_FP32 = 0, 1, 2
+STORE_INT8, STORE_BITPACK, STORE_FP32, STORE_MSC = 0, 1, 2, 3
 J_UNIFORM, J_PER_DIRECTION, J_BOND_PM1 = 0, 1, 2
 INIT_HOT, INIT_COLD = 0, 1
 OPT_PLAIN_KERNELS = 0
@@ -24,7 +24,7 @@ UPDATE_METROPOLIS, UPDATE_HEATBATH = 0, 1
 _RULE = {"metropolis": UPDATE_METROPOLIS, "heatbath": UPDATE_HEATBATH}
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE_TOO_SMALL, ERR_CUDA, ERR_STATE = range(6)
 
-_STORAGE = {"int8": STORE_INT8, "bitpack": STORE_BITPACK, "fp32": STORE_FP32}
+_STORAGE = {"int8": STORE_INT8, "bitpack": STORE_BITPACK, "fp32": STORE_FP32, "msc": STORE_MSC}
 _COUPLING = {"uniform": J_UNIFORM, "per_direction": J_PER_DIRECTION, "bond_pm1": J_BOND_PM1}
 
 # every symbol include/spin.h declares

@@ -11,6 +11,7 @@
 
 #include "ising_int8_kernel.cuh"
 #include "ising_kernels.cuh"
+#include "ising_msc_kernel.cuh"
 #include "ising_resident_kernel.cuh"
 #include "ising_tblock_kernel.cuh"
 #include "measure_kernels.cuh"
@@ -38,7 +39,7 @@ static spin_status fail(spin_status st, const char *fmt, ...) {
     } while (0)
 
 // ------------------------------------------------------------------------------- handle ------
-enum Path { PATH_ISING_GENERIC, PATH_ISING_INT8, PATH_ISING_BITPACK, PATH_VECTOR };
+enum Path { PATH_ISING_GENERIC, PATH_ISING_INT8, PATH_ISING_BITPACK, PATH_VECTOR, PATH_ISING_MSC };
 
 struct Layout {
     size_t off_s[2], bytes_s;   // one colour array
@@ -128,7 +129,8 @@ static spin_status derive(const spin_config *c, Derived *out) {
         return fail(SPIN_ERR_INVALID_ARG, "every lattice dimension must be even (checkerboard + periodic)");
     if (c->n < 1 || c->n > 3) return fail(SPIN_ERR_INVALID_ARG, "n must be 1, 2 or 3");
     if (c->n_replicas < 1) return fail(SPIN_ERR_INVALID_ARG, "n_replicas must be >= 1");
-    if (c->n_replicas > 65535) return fail(SPIN_ERR_UNSUPPORTED, "at most 65535 replicas per handle (replicas map to a grid dimension)");
+    if (c->storage == SPIN_STORE_MSC ? c->n_replicas > 32 * 65535 : c->n_replicas > 65535)
+        return fail(SPIN_ERR_UNSUPPORTED, "at most 65535 replicas (MSC: groups of 32 replicas) per handle (they map to a grid dimension)");
     if (c->coupling_kind < SPIN_J_UNIFORM || c->coupling_kind > SPIN_J_BOND_PM1)
         return fail(SPIN_ERR_INVALID_ARG, "bad coupling_kind");
     if (c->init != SPIN_INIT_HOT && c->init != SPIN_INIT_COLD) return fail(SPIN_ERR_INVALID_ARG, "bad init");
@@ -136,7 +138,7 @@ static spin_status derive(const spin_config *c, Derived *out) {
         return fail(SPIN_ERR_INVALID_ARG, "bad update_rule");
     if (c->update_rule == SPIN_UPDATE_HEATBATH && c->n == 2)
         return fail(SPIN_ERR_UNSUPPORTED, "heat bath is offered for n = 1 and n = 3 (no closed-form inverse for n = 2)");
-    if (c->storage < SPIN_STORE_INT8 || c->storage > SPIN_STORE_FP32) return fail(SPIN_ERR_INVALID_ARG, "bad storage");
+    if (c->storage < SPIN_STORE_INT8 || c->storage > SPIN_STORE_MSC) return fail(SPIN_ERR_INVALID_ARG, "bad storage");
     if (c->n == 1 && c->storage == SPIN_STORE_FP32) return fail(SPIN_ERR_INVALID_ARG, "n = 1 needs INT8 or BITPACK storage");
     if (c->n > 1 && c->storage != SPIN_STORE_FP32) return fail(SPIN_ERR_INVALID_ARG, "n >= 2 needs FP32 storage");
     out->d = L[2] == 1 ? 2 : 3;
@@ -168,7 +170,14 @@ static spin_status derive(const spin_config *c, Derived *out) {
             if (!(c->J[mu] == -1.0 || c->J[mu] == 0.0 || c->J[mu] == 1.0))
                 return fail(SPIN_ERR_UNSUPPORTED, "n = 1 supports couplings in {-1, 0, +1} only (integer table)");
         const bool unit_uniform = c->coupling_kind == SPIN_J_UNIFORM && c->J[0] != 0.0;
-        if (c->storage == SPIN_STORE_BITPACK) {
+        if (c->storage == SPIN_STORE_MSC) {
+            // replica-per-bit multi-spin coding: 32 realisations per word, one random number per site for all
+            if (c->coupling_kind != SPIN_J_BOND_PM1 || c->replica_streams != 0)
+                return fail(SPIN_ERR_UNSUPPORTED, "MSC storage is for per-bond +-1 couplings with a shared update stream (replica_streams = 0)");
+            if (c->n_replicas % 32) return fail(SPIN_ERR_UNSUPPORTED, "MSC storage needs n_replicas %% 32 == 0");
+            if ((out->N / 2) % 32) return fail(SPIN_ERR_UNSUPPORTED, "MSC storage needs N / 2 %% 32 == 0");
+            out->path = PATH_ISING_MSC;
+        } else if (c->storage == SPIN_STORE_BITPACK) {
             if (L[0] % 64) return fail(SPIN_ERR_UNSUPPORTED, "BITPACK storage needs Lx %% 64 == 0");
             if (!(unit_uniform || c->coupling_kind == SPIN_J_BOND_PM1))
                 return fail(SPIN_ERR_UNSUPPORTED, "BITPACK storage needs uniform J = +-1 or per-bond +-1 couplings");
@@ -221,7 +230,7 @@ static uint32_t acc_slots_for(uint64_t R) {
 static void make_layout(const spin_config *c, const Derived &dv, Layout *l, uint32_t *mblocks) {
     const uint64_t Nh = dv.N / 2, R = (uint64_t)c->n_replicas;
     size_t off = 0;
-    if (dv.path == PATH_ISING_BITPACK) l->bytes_s = (size_t)(R * Nh / 8);
+    if (dv.path == PATH_ISING_BITPACK || dv.path == PATH_ISING_MSC) l->bytes_s = (size_t)(R * Nh / 8);
     else if (dv.path == PATH_VECTOR) l->bytes_s = (size_t)(R * Nh * c->n * sizeof(float));
     else l->bytes_s = (size_t)(R * Nh);
     for (int k = 0; k < 2; ++k) { l->off_s[k] = off; off += align_up(l->bytes_s); }
@@ -231,7 +240,8 @@ static void make_layout(const spin_config *c, const Derived &dv, Layout *l, uint
     }
     l->bytes_bonds = 0;
     if (c->coupling_kind == SPIN_J_BOND_PM1)
-        l->bytes_bonds = dv.path == PATH_ISING_BITPACK ? (size_t)(2 * R * 3 * (Nh / 32) * 4) : (size_t)(R * dv.d * dv.N);
+        l->bytes_bonds = dv.path == PATH_ISING_BITPACK ? (size_t)(2 * R * 3 * (Nh / 32) * 4)
+                       : dv.path == PATH_ISING_MSC ? (size_t)(2 * (R / 32) * dv.d * Nh * 4) : (size_t)(R * dv.d * dv.N);
     l->off_bonds = off; off += align_up(l->bytes_bonds);
     *mblocks = measure_blocks(dv.path == PATH_ISING_BITPACK || dv.path == PATH_ISING_INT8 ? Nh / 32 : Nh);
     uint64_t pblocks = *mblocks;   // n >= 2: per-CTA partials of the measurement pass or of the fused TMA half-sweep
@@ -364,7 +374,20 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
     const bool shared = s->R > 1 && !s->cfg.replica_streams;
     const int B = s->path == PATH_ISING_INT8 && s->block > 128 ? 128 : s->block;   // the int8 kernel is built for <= 128 threads
     if (fused) *fused = false;
-    if (s->path == PATH_ISING_GENERIC) {
+    if (s->path == PATH_ISING_MSC) {
+        // replica-per-bit words: thread = site, lanes of a warp = the 32 sites of a Philox unit; the groups of 32 realisations
+        // are cut into chunks over gridDim.y so that the GPU is full, but not below 8 groups per thread (the site's uniform is
+        // assembled once per thread)
+        const uint32_t G = s->R / 32;
+        const int Bm = s->g.Nh < 128u ? (int)s->g.Nh : 128;
+        uint64_t Gy = (uint64_t)s->sm_count * 1024 * (uint64_t)s->grid_num / ((uint64_t)s->grid_den * s->g.Nh);
+        if (Gy > G / 8) Gy = G / 8;
+        if (Gy < 1) Gy = 1;
+        const dim3 Gm((s->g.Nh + Bm - 1) / Bm, (unsigned)Gy);
+        const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
+        if (s->d == 2) { if (hb) ising_msc_halfsweep<2, true><<<Gm, Bm, 0, st>>>(a); else ising_msc_halfsweep<2, false><<<Gm, Bm, 0, st>>>(a); }
+        else { if (hb) ising_msc_halfsweep<3, true><<<Gm, Bm, 0, st>>>(a); else ising_msc_halfsweep<3, false><<<Gm, Bm, 0, st>>>(a); }
+    } else if (s->path == PATH_ISING_GENERIC) {
         ising_generic_halfsweep<<<grid_for(s, (uint64_t)s->g.Nh * s->R), B, 0, st>>>(a);
     } else if (s->path == PATH_ISING_INT8) {
         // one thread per (replica, z, strip of K rows, unit column)
@@ -833,7 +856,11 @@ static spin_status enqueue_measure(spin_system *s, double *dE, double *dM, cudaS
         IsingArgs a = ising_args(s);
         long long *acc = (long long *)(s->ws + s->lay.off_acc);
         const bool bonds = s->cfg.coupling_kind == SPIN_J_BOND_PM1;
-        if (s->path == PATH_ISING_BITPACK) {
+        if (s->path == PATH_ISING_MSC) {
+            const uint32_t spt = 64;   // sites per thread (bit-sliced counters hold 4095)
+            const dim3 gm((unsigned)(((s->g.Nh + spt - 1) / spt + 127) / 128), s->R / 32);
+            if (s->d == 2) ising_msc_measure<2><<<gm, 128, 0, st>>>(a, spt); else ising_msc_measure<3><<<gm, 128, 0, st>>>(a, spt);
+        } else if (s->path == PATH_ISING_BITPACK) {
             if (s->d == 2) { if (bonds) ising_bitpack_measure<2, true><<<grid, 256, 0, st>>>(a); else ising_bitpack_measure<2, false><<<grid, 256, 0, st>>>(a); }
             else { if (bonds) ising_bitpack_measure<3, true><<<grid, 256, 0, st>>>(a); else ising_bitpack_measure<3, false><<<grid, 256, 0, st>>>(a); }
         } else if (s->path == PATH_ISING_INT8) {
@@ -948,7 +975,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
     s->tma_ok = 0; s->use_tma = -1; s->tma_ty = 0;
     s->t = 0; s->launches = 0; s->staging = nullptr; s->staging_bytes = 0; s->gexec = nullptr; s->cap_stream = nullptr; s->gnodes = nullptr; s->n_gnodes = 0;
     // 128 threads per CTA for the Ising fast paths (measured: +-J R = 16 39.1 vs 40.4 us with 256)
-    s->block = (dv.path == PATH_ISING_INT8 || dv.path == PATH_ISING_BITPACK) ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0; s->l2_prefetch = -1; s->variant = 0; s->tblock = -1; s->tblock_rows = 0; s->tblock_ok = tblock_offered(cfg, dv) ? 1 : 0;
+    s->block = (dv.path == PATH_ISING_INT8 || dv.path == PATH_ISING_BITPACK || dv.path == PATH_ISING_MSC) ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0; s->l2_prefetch = -1; s->variant = 0; s->tblock = -1; s->tblock_rows = 0; s->tblock_ok = tblock_offered(cfg, dv) ? 1 : 0;
     s->table_beta = std::nan("");
     Geometry &g = s->g;
     g.Lx = dv.pad[0]; g.Ly = dv.pad[1]; g.Lz = dv.pad[2]; g.d = dv.d;
@@ -996,7 +1023,13 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
     CREATE_TRY(cudaMemsetAsync(s->ws + s->lay.off_acc, 0, s->lay.bytes_acc, st));
     if (cfg->coupling_kind == SPIN_J_BOND_PM1) {
         const size_t nb = (size_t)s->R * s->d * s->N;
-        if (s->path == PATH_ISING_BITPACK) {
+        if (s->path == PATH_ISING_MSC) {
+            if (cfg->bonds) {
+                CREATE_TRY(cudaMalloc(&staging, nb));
+                CREATE_TRY(cudaMemcpyAsync(staging, cfg->bonds, nb, cudaMemcpyHostToDevice, st));
+            }
+            msc_bonds_pack<<<G, B, 0, st>>>(sa, (const int8_t *)staging, (uint32_t *)(s->ws + s->lay.off_bonds));
+        } else if (s->path == PATH_ISING_BITPACK) {
             if (cfg->bonds) {
                 CREATE_TRY(cudaMalloc(&staging, nb));
                 CREATE_TRY(cudaMemcpyAsync(staging, cfg->bonds, nb, cudaMemcpyHostToDevice, st));
@@ -1010,7 +1043,8 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
         CREATE_TRY(cudaGetLastError());
     }
     const int mode = cfg->init == SPIN_INIT_HOT ? 1 : 0;
-    if (s->n == 1) ising_fill<<<G, B, 0, st>>>(sa, mode, nullptr, s->ws + s->lay.off_s[0], s->ws + s->lay.off_s[1]);
+    if (s->path == PATH_ISING_MSC) msc_fill<<<G, B, 0, st>>>(sa, mode, nullptr, (uint32_t *)(s->ws + s->lay.off_s[0]), (uint32_t *)(s->ws + s->lay.off_s[1]));
+    else if (s->n == 1) ising_fill<<<G, B, 0, st>>>(sa, mode, nullptr, s->ws + s->lay.off_s[0], s->ws + s->lay.off_s[1]);
     else if (s->n == 2) vector_fill<2><<<G, B, 0, st>>>(sa, mode, nullptr, (float *)(s->ws + s->lay.off_s[0]), (float *)(s->ws + s->lay.off_s[1]));
     else vector_fill<3><<<G, B, 0, st>>>(sa, mode, nullptr, (float *)(s->ws + s->lay.off_s[0]), (float *)(s->ws + s->lay.off_s[1]));
     CREATE_TRY(cudaGetLastError());
@@ -1221,7 +1255,8 @@ spin_status spin_get_spins(spin_system *s, void *host, size_t bytes) {
     const SetupArgs sa = setup_args(s);
     const int G = grid_for(s, 2ull * s->R * s->g.Nh);
     void *s0 = s->ws + s->lay.off_s[0], *s1 = s->ws + s->lay.off_s[1];
-    if (s->n == 1) ising_to_canonical<<<G, 256>>>(sa, s0, s1, (int8_t *)staging);
+    if (s->path == PATH_ISING_MSC) msc_to_canonical<<<G, 256>>>(sa, (const uint32_t *)s0, (const uint32_t *)s1, (int8_t *)staging);
+    else if (s->n == 1) ising_to_canonical<<<G, 256>>>(sa, s0, s1, (int8_t *)staging);
     else if (s->n == 2) vector_to_canonical<2><<<G, 256>>>(sa, (const float *)s0, (const float *)s1, (float *)staging);
     else vector_to_canonical<3><<<G, 256>>>(sa, (const float *)s0, (const float *)s1, (float *)staging);
     cudaError_t e = cudaGetLastError();
@@ -1254,7 +1289,8 @@ spin_status spin_set_spins(spin_system *s, const void *host, size_t bytes) {
         const SetupArgs sa = setup_args(s);
         const int G = grid_for(s, 2ull * s->R * s->g.Nh);
         void *s0 = s->ws + s->lay.off_s[0], *s1 = s->ws + s->lay.off_s[1];
-        if (s->n == 1) ising_fill<<<G, 256>>>(sa, 2, (const int8_t *)staging, s0, s1);
+        if (s->path == PATH_ISING_MSC) msc_fill<<<G, 256>>>(sa, 2, (const int8_t *)staging, (uint32_t *)s0, (uint32_t *)s1);
+        else if (s->n == 1) ising_fill<<<G, 256>>>(sa, 2, (const int8_t *)staging, s0, s1);
         else if (s->n == 2) vector_fill<2><<<G, 256>>>(sa, 2, (const float *)staging, (float *)s0, (float *)s1);
         else vector_fill<3><<<G, 256>>>(sa, 2, (const float *)staging, (float *)s0, (float *)s1);
         e = cudaGetLastError();
@@ -1270,12 +1306,14 @@ spin_status spin_get_bonds(spin_system *s, int8_t *host, size_t bytes) {
     const size_t need = (size_t)s->R * s->d * s->N;
     if (bytes != need) return fail(SPIN_ERR_INVALID_ARG, "bonds need exactly %zu bytes, got %zu", need, bytes);
     CUDA_TRY(cudaDeviceSynchronize());
-    if (s->path != PATH_ISING_BITPACK) {
+    if (s->path != PATH_ISING_BITPACK && s->path != PATH_ISING_MSC) {
         CUDA_TRY(cudaMemcpy(host, s->ws + s->lay.off_bonds, need, cudaMemcpyDeviceToHost));
         return SPIN_OK;
     }
     CUDA_TRY(ensure_staging(s, need));
     void *staging = s->staging;
+    if (s->path == PATH_ISING_MSC) msc_bonds_unpack<<<grid_for(s, 2ull * s->R * s->g.Nh), 256>>>(setup_args(s), (const uint32_t *)(s->ws + s->lay.off_bonds), (int8_t *)staging);
+    else
     bonds_unpack<<<grid_for(s, 2ull * s->R * s->g.Nh), 256>>>(setup_args(s), (const uint32_t *)(s->ws + s->lay.off_bonds), (int8_t *)staging);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpy(host, staging, need, cudaMemcpyDeviceToHost);

@@ -35,6 +35,10 @@ WORKLOADS = {
     # lattice the bit-packed layout takes (the paper used L = 32)
     "ea2d_L64_R4096_bitpack": dict(dims=(64, 64, 1), n=1, storage="bitpack", coupling="bond_pm1", J=(1.0, 1.0, 1.0),
                                    beta=1.0, sweeps=1000, replicas=4096, replica_streams=0, record=False),
+    # SURVEY 8(f) f2 like for like: the paper's own lattice (2D +-J, L = 32, Table 1) in the paper's word layout
+    # (one site of 32 realisations per word, SPIN_STORE_MSC), with enough realisations to fill a B200
+    "ea2d_L32_R131072_msc": dict(dims=(32, 32, 1), n=1, storage="msc", coupling="bond_pm1", J=(1.0, 1.0, 1.0),
+                                 beta=1.0, sweeps=1000, replicas=131072, replica_streams=0, record=False),
 }
 
 # Algorithmic bytes moved per attempted update: read the target colour, read the
@@ -46,6 +50,7 @@ BYTES_PER_UPDATE = {
     "ising3d_L512_bitpack": 0.375,
     "ea3d_L256_R16_bitpack": 1.125,
     "ea2d_L64_R4096_bitpack": 0.875,   # 3 spin bits + 2 forward bonds from each end = 7 bits
+    "ea2d_L32_R131072_msc": 0.875,
     "heisenberg3d_L256_fp32": 36.0,
     "xy3d_L256_fp32": 24.0,
 }
