@@ -123,6 +123,26 @@ spin_status spin_halo_bytes(const spin_system *s, size_t *bytes);
 spin_status spin_halo_get(spin_system *s, int32_t colour, int32_t side, void *d_buf, void *stream);
 spin_status spin_halo_put(spin_system *s, int32_t colour, int32_t side, const void *d_buf, void *stream);
 
+/* The half-sweep of `colour` restricted to planes [plane0, plane0 + n_planes) of the planes this handle updates (slab
+ * handle: its owned planes, 0-based; whole lattice: planes along its slowest axis).  Sites of one colour do not
+ * interact, so a half-sweep may be issued in pieces, in any order: a slab updates its two boundary planes first, sends
+ * them, and updates the interior while the messages are in flight ("overlap by updating boundary planes
+ * first").  last != 0 on the piece that completes the colour (the handle then expects the other colour; after colour 1
+ * the sweep counter advances); the caller covers every plane exactly once.  n_planes = 0 with last != 0 only closes the
+ * colour.  Asynchronous. */
+spin_status spin_halfsweep_range(spin_system *s, double beta, int32_t colour, int32_t plane0, int32_t n_planes,
+                                 int32_t last, void *stream);
+
+/* Both faces of one colour with ONE kernel each way.  d_buf: device memory, 2 * spin_halo_bytes, 16-byte aligned.
+ * pack:   d_buf = [lowest owned plane][highest owned plane] (the messages for the slab below and the slab above).
+ * unpack: d_buf = [plane received from the slab below][plane received from the slab above] -> the two ghost planes.
+ * Asynchronous on `stream`. */
+spin_status spin_halo_pack(spin_system *s, int32_t colour, void *d_buf, void *stream);
+spin_status spin_halo_unpack(spin_system *s, int32_t colour, const void *d_buf, void *stream);
+/* A slab that is its own neighbour (one rank holds the whole extent, periodic): ghost below <- highest owned plane,
+ * ghost above <- lowest owned plane, one kernel.  Asynchronous. */
+spin_status spin_halo_wrap(spin_system *s, int32_t colour, void *stream);
+
 /* As spin_sweep, recording E and M after every sweep into DEVICE arrays d_E[n_sweeps][R] and
  * d_M[n_sweeps][R][n] (doubles).  Enqueues only. */
 spin_status spin_sweep_record(spin_system *s, double beta, int64_t n_sweeps, double *d_E, double *d_M, void *stream);

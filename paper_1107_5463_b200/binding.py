@@ -32,7 +32,7 @@ SYMBOLS = [
     "spin_workspace_bytes", "spin_create", "spin_sweep", "spin_measure", "spin_sweep_record", "spin_get_spins",
     "spin_set_spins", "spin_get_bonds", "spin_get_sweep_count", "spin_set_sweep_count", "spin_get_launch_count",
     "spin_set_launch_shape", "spin_set_strip_rows", "spin_set_option", "spin_halfsweep", "spin_halo_bytes",
-    "spin_halo_get", "spin_halo_put", "spin_destroy", "spin_last_error", "spin_version",
+    "spin_halo_get", "spin_halo_put", "spin_halfsweep_range", "spin_halo_pack", "spin_halo_unpack", "spin_halo_wrap", "spin_destroy", "spin_last_error", "spin_version",
 ]
 
 
@@ -89,6 +89,10 @@ def lib():
         L.spin_halo_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
         L.spin_halo_get.argtypes = [vp, C.c_int32, C.c_int32, vp, vp]
         L.spin_halo_put.argtypes = [vp, C.c_int32, C.c_int32, vp, vp]
+        L.spin_halfsweep_range.argtypes = [vp, C.c_double, C.c_int32, C.c_int32, C.c_int32, C.c_int32, vp]
+        L.spin_halo_pack.argtypes = [vp, C.c_int32, vp, vp]
+        L.spin_halo_unpack.argtypes = [vp, C.c_int32, vp, vp]
+        L.spin_halo_wrap.argtypes = [vp, C.c_int32, vp]
         L.spin_destroy.argtypes = [vp]
         for name in SYMBOLS:
             getattr(L, name).restype = C.c_int
@@ -190,6 +194,25 @@ class SpinSystem:
     def halfsweep(self, beta, colour):
         with self._torch.cuda.device(self.device):
             _check(lib().spin_halfsweep(self._h, float(beta), int(colour), self._stream()))
+
+    def halfsweep_range(self, beta, colour, plane0, n_planes, last):
+        with self._torch.cuda.device(self.device):
+            _check(lib().spin_halfsweep_range(self._h, float(beta), int(colour), int(plane0), int(n_planes), int(bool(last)), self._stream()))
+
+    def halo_pack(self, colour, buf):
+        """both owned boundary planes of colour `colour` -> buf (CUDA uint8 tensor of 2 * halo_bytes: [lowest][highest])"""
+        with self._torch.cuda.device(self.device):
+            _check(lib().spin_halo_pack(self._h, int(colour), C.c_void_p(buf.data_ptr()), self._stream()))
+
+    def halo_unpack(self, colour, buf):
+        """buf = [plane from the slab below][plane from the slab above] -> the two ghost planes"""
+        with self._torch.cuda.device(self.device):
+            _check(lib().spin_halo_unpack(self._h, int(colour), C.c_void_p(buf.data_ptr()), self._stream()))
+
+    def halo_wrap(self, colour):
+        """single slab, periodic: its own boundary planes become its ghost planes (one kernel)"""
+        with self._torch.cuda.device(self.device):
+            _check(lib().spin_halo_wrap(self._h, int(colour), self._stream()))
 
     def halo_bytes(self):
         out = C.c_size_t(0)

@@ -104,6 +104,11 @@ struct Geometry {
     uint32_t i_off;     // + local lexicographic idx -> global lexicographic index (mod 2^32)
     uint32_t own_j0, own_j1;   // owned compressed indices [own_j0, own_j1) of either colour
     uint32_t own_i0, own_in;   // owned lexicographic indices [own_i0, own_i0 + own_in)
+    // What a half-sweep launch updates: planes [sw_p0, sw_p0 + sw_pn) along the slowest axis (z for d = 3, rows y for
+    // d = 2) = compressed indices [sw_j0, sw_j0 + sw_jn).  Whole lattice: everything.  Slab handle: its owned planes (the
+    // ghost planes are only read), or a sub-range of them when the caller updates the boundary planes first and the
+    // interior while the halo exchange is in flight (spin_halfsweep_range).
+    uint32_t sw_p0, sw_pn, sw_j0, sw_jn;
 };
 
 }  // namespace spin

@@ -184,8 +184,10 @@ template <int D, int K, bool HB = false, bool MEAS = false>
 __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(const __grid_constant__ IsingArgs a) {
     const Geometry &g = a.g;
     const uint32_t WX = g.WX, Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz;
-    const uint32_t nstrip = (Ly + K - 1) / K;
-    const uint32_t per_replica = WX * nstrip * Lz;
+    // rows (d = 2) / planes (d = 3) this launch updates: [sw_p0, sw_p0 + sw_pn) along the slowest axis
+    const uint32_t ys0 = D == 2 ? g.sw_p0 : 0u, Lys = D == 2 ? g.sw_pn : Ly, zs0 = D == 3 ? g.sw_p0 : 0u, Lzs = D == 3 ? g.sw_pn : Lz;
+    const uint32_t nstrip = (Lys + K - 1) / K;
+    const uint32_t per_replica = WX * nstrip * Lzs;
     const uint32_t item = blockIdx.x * blockDim.x + threadIdx.x;
     // The deferred tail of the digit comparison (ising_bitpack_strip_halfsweep) is compiled out here: measured on B200 the
     // queue's live state pushes the d = 2 instance past its 72 registers (7 CTAs per SM): 87.7 us against 72.8 us without
@@ -196,8 +198,8 @@ __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(cons
     if (item < per_replica * a.R) {
     const uint32_t r = item / per_replica, it = item - r * per_replica;
     const uint32_t sz = fdiv(it, g.divWX), w = it - sz * WX;      // sz = strip + nstrip * z
-    const uint32_t z = sz / nstrip, y0 = (sz - z * nstrip) * K;
-    const uint32_t kend = min((uint32_t)K, Ly - y0);
+    const uint32_t zl = sz / nstrip, z = zs0 + zl, y0 = ys0 + (sz - zl * nstrip) * K;
+    const uint32_t kend = min((uint32_t)K, ys0 + Lys - y0);
     const uint8_t *__restrict__ other = (const uint8_t *)a.s[1 - a.colour] + (size_t)r * g.Nh;
     uint8_t *mine = (uint8_t *)a.s[a.colour] + (size_t)r * g.Nh;
     const uint32_t rho = a.replica_streams ? r : 0u;
@@ -280,8 +282,10 @@ template <int D, int K, bool HB = false, bool MEAS = false>
 __global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __grid_constant__ IsingArgs a) {
     const Geometry &g = a.g;
     const uint32_t WX = g.WX, Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz;
-    const uint32_t nstrip = (Ly + K - 1) / K;
-    const uint32_t per_replica = WX * nstrip * Lz;
+    // rows (d = 2) / planes (d = 3) this launch updates: [sw_p0, sw_p0 + sw_pn) along the slowest axis
+    const uint32_t ys0 = D == 2 ? g.sw_p0 : 0u, Lys = D == 2 ? g.sw_pn : Ly, zs0 = D == 3 ? g.sw_p0 : 0u, Lzs = D == 3 ? g.sw_pn : Lz;
+    const uint32_t nstrip = (Lys + K - 1) / K;
+    const uint32_t per_replica = WX * nstrip * Lzs;
     const uint32_t item = blockIdx.x * blockDim.x + threadIdx.x;
     constexpr bool DEFER = !HB && !MEAS;   // deferred tail of the digit comparison, as in ising_int8_halfsweep
     __shared__ DeferQueue dq;
@@ -290,8 +294,8 @@ __global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __gri
     if (item < per_replica * a.R) {
     const uint32_t r = item / per_replica, it = item - r * per_replica;
     const uint32_t sz = fdiv(it, g.divWX), w = it - sz * WX;      // sz = strip + nstrip * z
-    const uint32_t z = sz / nstrip, y0 = (sz - z * nstrip) * K;
-    const uint32_t kend = min((uint32_t)K, Ly - y0);
+    const uint32_t zl = sz / nstrip, z = zs0 + zl, y0 = ys0 + (sz - zl * nstrip) * K;
+    const uint32_t kend = min((uint32_t)K, ys0 + Lys - y0);
     const uint32_t *__restrict__ other = (const uint32_t *)a.s[1 - a.colour] + (size_t)r * g.NW;
     uint32_t *mine = (uint32_t *)a.s[a.colour] + (size_t)r * g.NW;
     const uint32_t rho = a.replica_streams ? r : 0u;

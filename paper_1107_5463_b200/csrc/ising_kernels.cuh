@@ -215,12 +215,12 @@ __device__ __forceinline__ void count_masks(const uint32_t b[6], uint32_t m[2 * 
 // neighbour coincide and both bonds count), zero couplings and per-bond couplings.
 __global__ void __launch_bounds__(256) ising_generic_halfsweep(const __grid_constant__ IsingArgs a) {
     const Geometry &g = a.g;
-    const uint32_t total = g.Nh * a.R;
+    const uint32_t total = g.sw_jn * a.R;
     const uint8_t *__restrict__ other_base = (const uint8_t *)a.s[1 - a.colour];
     uint8_t *mine_base = (uint8_t *)a.s[a.colour];
     const uint32_t N = 2u * g.Nh;
     for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
-        const uint32_t r = idx / g.Nh, j = idx - r * g.Nh;
+        const uint32_t r = idx / g.sw_jn, j = g.sw_j0 + idx - r * g.sw_jn;
         const uint32_t row = fdiv(j, g.divRL), xh = j - row * g.RL;
         const uint32_t z = fdiv(row, g.divLy), y = row - z * (uint32_t)g.Ly;
         const uint32_t p = (y + z + a.colour) & 1u;
@@ -374,9 +374,9 @@ __device__ __forceinline__ uint32_t bitpack_update_word(const IsingArgs &a, uint
 template <int D, bool BONDS, bool SHARED, bool MEAS = false>
 __global__ void __launch_bounds__(256) ising_bitpack_halfsweep(const __grid_constant__ IsingArgs a) {
     constexpr int NT = D;  // thresholds: dE = 4, 8 (2D) and 12 (3D)
-    const uint32_t NW = a.g.NW;
+    const uint32_t NW = a.g.NW, gi_end = (a.g.sw_j0 + a.g.sw_jn) >> 5;
     uint32_t *mine_base = (uint32_t *)a.s[a.colour];
-    for (uint32_t gi = blockIdx.x * blockDim.x + threadIdx.x; gi < NW; gi += gridDim.x * blockDim.x) {
+    for (uint32_t gi = (a.g.sw_j0 >> 5) + blockIdx.x * blockDim.x + threadIdx.x; gi < gi_end; gi += gridDim.x * blockDim.x) {
         const WordNbrs n = word_neighbours<D>(a.g, a.colour, gi);
         const bool owned = gi >= (a.g.own_j0 >> 5) && gi < (a.g.own_j1 >> 5);
         uint32_t ltf[NT];
@@ -406,9 +406,9 @@ __global__ void __launch_bounds__(256) ising_bitpack_halfsweep(const __grid_cons
 template <int D, bool BONDS, bool SHARED>
 __global__ void __launch_bounds__(256) ising_bitpack_halfsweep_hb(const __grid_constant__ IsingArgs a) {
     constexpr int NT = 2 * D + 1;
-    const uint32_t NW = a.g.NW;
+    const uint32_t NW = a.g.NW, gi_end = (a.g.sw_j0 + a.g.sw_jn) >> 5;
     uint32_t *mine_base = (uint32_t *)a.s[a.colour];
-    for (uint32_t gi = blockIdx.x * blockDim.x + threadIdx.x; gi < NW; gi += gridDim.x * blockDim.x) {
+    for (uint32_t gi = (a.g.sw_j0 >> 5) + blockIdx.x * blockDim.x + threadIdx.x; gi < gi_end; gi += gridDim.x * blockDim.x) {
         const WordNbrs n = word_neighbours<D>(a.g, a.colour, gi);
         uint32_t ltf[NT];
         if (SHARED) lt_masks_full<NT, true>(a, a.t, a.colour, gi + a.g.unit_off, 0u, ltf);

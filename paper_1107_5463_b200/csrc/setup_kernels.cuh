@@ -184,4 +184,30 @@ __global__ void __launch_bounds__(256) bonds_unpack(const __grid_constant__ Setu
     }
 }
 
+// Halo faces of a slab handle: `rows` pieces of `plane_elems` elements each, piece q of face f at
+// arr + plane[f] * plane_elems + q * stride_elems in the colour array and at buf + (f * rows + q) * plane_elems in the message
+// buffer.  pack = true: array -> buffer (the two owned boundary planes), false: buffer -> array (the two ghost planes).
+// One launch for both faces (four cudaMemcpy2DAsync per exchange before: 16 us of launch latency per half-sweep).
+template <typename T>
+__global__ void __launch_bounds__(256) halo_faces_copy(T *arr, T *buf, size_t plane_elems, size_t stride_elems, uint32_t rows,
+                                                       uint32_t plane_lo, uint32_t plane_hi, bool pack) {
+    const size_t per_face = plane_elems * rows, total = 2 * per_face;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t f = i / per_face, rem = i - f * per_face, q = rem / plane_elems, e = rem - q * plane_elems;
+        T *a = arr + (f ? plane_hi : plane_lo) * plane_elems + q * stride_elems + e;
+        if (pack) buf[i] = *a; else *a = buf[i];
+    }
+}
+
+// a single slab that is its own neighbour (one rank, periodic): ghost below <- highest owned plane, ghost above <- lowest
+template <typename T>
+__global__ void __launch_bounds__(256) halo_faces_wrap(T *arr, size_t plane_elems, size_t stride_elems, uint32_t rows, uint32_t own) {
+    const size_t per_face = plane_elems * rows, total = 2 * per_face;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t f = i / per_face, rem = i - f * per_face, q = rem / plane_elems, e = rem - q * plane_elems;
+        const size_t src = f ? 2u : own + 1u, dst = f ? own + 2u : 1u;
+        arr[dst * plane_elems + q * stride_elems + e] = arr[src * plane_elems + q * stride_elems + e];
+    }
+}
+
 }  // namespace spin

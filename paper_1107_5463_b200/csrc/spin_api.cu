@@ -366,6 +366,10 @@ static VectorArgs vector_args(const spin_system *s, double beta) {
     return a;
 }
 
+// rows and planes a launch with geometry g updates (Geometry::sw_*): the strips of the fast kernels are cut from these
+static uint32_t sweep_rows(const Geometry &g) { return g.d == 2 ? g.sw_pn : (uint32_t)g.Ly; }
+static uint32_t sweep_planes(const Geometry &g) { return g.d == 3 ? g.sw_pn : (uint32_t)g.Lz; }
+
 // ----------------------------------------------------------------------------- launches ------
 // fused: NULL, or (colour 1 only) ask for E / M to be accumulated into a.acc by the half-sweep itself;
 // *fused tells whether the kernel that ran could do it (the strip kernels with 1 or 4 rows per thread).
@@ -388,7 +392,7 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
         if (s->d == 2) { if (hb) ising_msc_halfsweep<2, true><<<Gm, Bm, 0, st>>>(a); else ising_msc_halfsweep<2, false><<<Gm, Bm, 0, st>>>(a); }
         else { if (hb) ising_msc_halfsweep<3, true><<<Gm, Bm, 0, st>>>(a); else ising_msc_halfsweep<3, false><<<Gm, Bm, 0, st>>>(a); }
     } else if (s->path == PATH_ISING_GENERIC) {
-        ising_generic_halfsweep<<<grid_for(s, (uint64_t)s->g.Nh * s->R), B, 0, st>>>(a);
+        ising_generic_halfsweep<<<grid_for(s, (uint64_t)a.g.sw_jn * s->R), B, 0, st>>>(a);
     } else if (s->path == PATH_ISING_INT8) {
         // one thread per (replica, z, strip of K rows, unit column)
         const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
@@ -397,11 +401,11 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
         // the heat-bath kernel is instantiated for K = 4 only
         int K = s->strip_rows;
         if (!s->strip_rows_set) {
-            const uint64_t threads4 = (uint64_t)s->g.WX * ((s->g.Ly + 3) / 4) * s->g.Lz * s->R;
+            const uint64_t threads4 = (uint64_t)s->g.WX * ((sweep_rows(a.g) + 3) / 4) * sweep_planes(a.g) * s->R;
             K = threads4 >= (uint64_t)s->sm_count * 2048 ? 4 : 1;
         }
         if (hb) K = 4;
-        const uint64_t items = (uint64_t)s->g.WX * ((s->g.Ly + K - 1) / K) * s->g.Lz * s->R;
+        const uint64_t items = (uint64_t)s->g.WX * ((sweep_rows(a.g) + K - 1) / K) * sweep_planes(a.g) * s->R;
         const int G = (int)((items + B - 1) / B);
         if (fused && (K == 1 || K == 4) && a.colour == 1u) {
             *fused = true;
@@ -421,12 +425,12 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
         // measured at L = 16384: 65.7 / 61.6 / 58.4 / 65.8 / 71.9 us for K = 1 / 2 / 4 / 8 / 16)
         int K = s->strip_rows_set ? s->strip_rows : 0;
         if (!K) {
-            const uint64_t threads4 = (uint64_t)s->g.WX * ((s->g.Ly + 3) / 4) * s->g.Lz * s->R;
+            const uint64_t threads4 = (uint64_t)s->g.WX * ((sweep_rows(a.g) + 3) / 4) * sweep_planes(a.g) * s->R;
             K = threads4 >= (uint64_t)s->sm_count * 2048 ? 4 : 1;
         }
         if (K > 4) K = 4;
         const int Bs = B > 128 ? 128 : B;
-        const uint64_t items = (uint64_t)s->g.WX * ((s->g.Ly + K - 1) / K) * s->g.Lz * s->R;
+        const uint64_t items = (uint64_t)s->g.WX * ((sweep_rows(a.g) + K - 1) / K) * sweep_planes(a.g) * s->R;
         const int G = (int)((items + Bs - 1) / Bs);
         const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
 #define BS3(D_, K_) do { if (hb) ising_bitpack_strip_halfsweep<D_, K_, true><<<G, Bs, 0, st>>>(a); else ising_bitpack_strip_halfsweep<D_, K_, false><<<G, Bs, 0, st>>>(a); } while (0)
@@ -477,8 +481,9 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
         // shared update stream: chunks of >= 16 replicas per thread (the masks of a word are built once per chunk);
         // more chunks only when the lattice alone cannot fill the GPU (many realisations of a small lattice)
         int Bq = B;
-        while (Bq > 32 && (uint32_t)(Bq / 2) >= s->g.NW) Bq /= 2;   // small lattices: no dead threads
-        const int Gx = (int)((s->g.NW + Bq - 1) / Bq) < grid_for(s, s->g.NW) ? (int)((s->g.NW + Bq - 1) / Bq) : grid_for(s, s->g.NW);
+        const uint32_t NWs = a.g.sw_jn >> 5;   // words this launch updates
+        while (Bq > 32 && (uint32_t)(Bq / 2) >= NWs) Bq /= 2;   // small lattices: no dead threads
+        const int Gx = (int)((NWs + Bq - 1) / Bq) < grid_for(s, NWs) ? (int)((NWs + Bq - 1) / Bq) : grid_for(s, NWs);
         int Gy = 1;
         if (shared && s->R > 16) {
             // replicas per thread: 16 when the lattice fills the GPU, down to 4 when it is the replicas that must
@@ -593,7 +598,7 @@ static spin_status launch_halfsweep_vector(spin_system *s, const VectorArgs &a, 
         bool unitj = true;
         for (int mu = 0; mu < s->d; ++mu) unitj = unitj && a.Jdir[mu] == 1.0f;
         const int B = s->block > 128 ? 128 : s->block;
-        const uint64_t items = (uint64_t)(g.RL / 4) * g.Ly * g.Lz;
+        const uint64_t items = (uint64_t)(g.RL / 4) * sweep_rows(a.g) * sweep_planes(a.g);
         const dim3 G((unsigned)((items + B - 1) / B), s->R);
 #define VM4(NC_, D_, U_, HB_) vector_strip_halfsweep<NC_, D_, U_, 1, HB_, true><<<G, B, 0, st>>>(a)
 #define VM3(NC_, D_, HB_) do { if (unitj) VM4(NC_, D_, true, HB_); else VM4(NC_, D_, false, HB_); } while (0)
@@ -640,7 +645,7 @@ static spin_status launch_halfsweep_vector(spin_system *s, const VectorArgs &a, 
         bool unitj = true;
         for (int mu = 0; mu < s->d; ++mu) unitj = unitj && a.Jdir[mu] == 1.0f;
         const int B = s->block > 128 ? 128 : s->block;
-        const uint64_t items = (uint64_t)(g.RL / 4) * g.Ly * g.Lz;
+        const uint64_t items = (uint64_t)(g.RL / 4) * sweep_rows(a.g) * sweep_planes(a.g);
         const dim3 G((unsigned)((items + B - 1) / B), s->R);
         if (s->d == 2) { if (unitj) vector_strip_halfsweep<3, 2, true, 1, true><<<G, B, 0, st>>>(a); else vector_strip_halfsweep<3, 2, false, 1, true><<<G, B, 0, st>>>(a); }
         else { if (unitj) vector_strip_halfsweep<3, 3, true, 1, true><<<G, B, 0, st>>>(a); else vector_strip_halfsweep<3, 3, false, 1, true><<<G, B, 0, st>>>(a); }
@@ -649,7 +654,7 @@ static spin_status launch_halfsweep_vector(spin_system *s, const VectorArgs &a, 
         for (int mu = 0; mu < s->d; ++mu) unitj = unitj && a.Jdir[mu] == 1.0f;
         const int K = s->strip_rows_set ? (s->strip_rows >= 4 ? 4 : s->strip_rows) : 1;  // default 1 (measured fastest)
         const int B = s->block > 128 ? 128 : s->block;
-        const uint64_t items = (uint64_t)(g.RL / 4) * ((g.Ly + K - 1) / K) * g.Lz;
+        const uint64_t items = (uint64_t)(g.RL / 4) * ((sweep_rows(a.g) + K - 1) / K) * sweep_planes(a.g);
         const dim3 G((unsigned)((items + B - 1) / B), s->R);
 #define VS4(NC_, D_, U_, K_) vector_strip_halfsweep<NC_, D_, U_, K_><<<G, B, 0, st>>>(a)
 #define VS3(NC_, D_, U_) do { if (K == 1) VS4(NC_, D_, U_, 1); else if (K == 2) VS4(NC_, D_, U_, 2); else VS4(NC_, D_, U_, 4); } while (0)
@@ -660,7 +665,7 @@ static spin_status launch_halfsweep_vector(spin_system *s, const VectorArgs &a, 
 #undef VS3
 #undef VS4
     } else {
-        const int G = grid_for(s, (uint64_t)g.Nh * s->R);
+        const int G = grid_for(s, (uint64_t)a.g.sw_jn * s->R);
         if (s->n == 2) vector_halfsweep<2><<<G, s->block, 0, st>>>(a);
         else vector_halfsweep<3><<<G, s->block, 0, st>>>(a);
     }
@@ -994,6 +999,13 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
         g.own_j0 = (uint32_t)(2 * plane_h); g.own_j1 = (uint32_t)((2 + cfg->dims[dv.axis]) * plane_h);
         g.own_i0 = (uint32_t)(2 * plane_sites); g.own_in = (uint32_t)dv.Nown;
     }
+    {
+        // what a half-sweep updates: everything, or the owned planes of a slab (the ghost planes are only read)
+        const uint32_t plane_h = g.d == 3 ? g.RL * (uint32_t)g.Ly : g.RL;
+        g.sw_p0 = dv.axis >= 0 ? 2u : 0u;
+        g.sw_pn = dv.axis >= 0 ? (uint32_t)cfg->dims[dv.axis] : (uint32_t)(g.d == 3 ? g.Lz : g.Ly);
+        g.sw_j0 = g.sw_p0 * plane_h; g.sw_jn = g.sw_pn * plane_h;
+    }
     for (int r = 0; r < 10; ++r) {
         s->keys.k0[r] = (uint32_t)(cfg->seed & 0xFFFFFFFFull) + (uint32_t)r * 0x9E3779B9u;
         s->keys.k1[r] = (uint32_t)(cfg->seed >> 32) + (uint32_t)r * 0xBB67AE85u;
@@ -1148,26 +1160,51 @@ spin_status spin_sweep_record(spin_system *s, double beta, int64_t n_sweeps, dou
     return SPIN_OK;
 }
 
-spin_status spin_halfsweep(spin_system *s, double beta, int32_t colour, void *stream) {
+// planes [plane0, plane0 + n_planes) of the swept range (whole lattice: along its slowest axis; slab: its owned planes)
+static void restrict_range(Geometry &g, int32_t plane0, int32_t n_planes) {
+    const uint32_t plane_h = g.d == 3 ? g.RL * (uint32_t)g.Ly : g.RL;
+    g.sw_p0 += (uint32_t)plane0;
+    g.sw_pn = (uint32_t)n_planes;
+    g.sw_j0 = g.sw_p0 * plane_h;
+    g.sw_jn = g.sw_pn * plane_h;
+}
+
+static spin_status halfsweep_impl(spin_system *s, double beta, int32_t colour, int32_t plane0, int32_t n_planes, bool ranged, bool last,
+                                  cudaStream_t st) {
     // either colour needs a sweep index below 2^32 (colour 0 at t = 2^32 would silently reuse the numbers of sweep 0)
     spin_status rc = check_sweep_args(s, beta, 1);
     if (rc != SPIN_OK) return rc;
     if (colour != 0 && colour != 1) return fail(SPIN_ERR_INVALID_ARG, "colour must be 0 or 1");
     if ((uint32_t)colour != s->next_colour) return fail(SPIN_ERR_STATE, "half-sweeps alternate: colour %u is next", s->next_colour);
-    cudaStream_t st = (cudaStream_t)stream;
-    if (s->n == 1) {
-        IsingArgs a = ising_args(s);
-        a.colour = (uint32_t)colour;
-        rc = launch_halfsweep_ising(s, a, st);
-    } else {
-        VectorArgs a = vector_args(s, beta);
-        a.colour = (uint32_t)colour;
-        rc = launch_halfsweep_vector(s, a, st);
+    if (ranged && (plane0 < 0 || n_planes < 0 || (uint32_t)plane0 + (uint32_t)n_planes > s->g.sw_pn))
+        return fail(SPIN_ERR_INVALID_ARG, "plane range [%d, %d) outside the %u planes this handle updates", plane0, plane0 + n_planes, s->g.sw_pn);
+    if (!ranged || n_planes > 0) {
+        if (s->n == 1) {
+            IsingArgs a = ising_args(s);
+            a.colour = (uint32_t)colour;
+            if (ranged) restrict_range(a.g, plane0, n_planes);
+            rc = launch_halfsweep_ising(s, a, st);
+        } else {
+            VectorArgs a = vector_args(s, beta);
+            a.colour = (uint32_t)colour;
+            if (ranged) restrict_range(a.g, plane0, n_planes);
+            rc = launch_halfsweep_vector(s, a, st, !ranged);
+        }
+        if (rc != SPIN_OK) return rc;
     }
-    if (rc != SPIN_OK) return rc;
-    s->next_colour = 1u - (uint32_t)colour;
-    if (colour == 1) s->t += 1;
+    if (last) {
+        s->next_colour = 1u - (uint32_t)colour;
+        if (colour == 1) s->t += 1;
+    }
     return SPIN_OK;
+}
+
+spin_status spin_halfsweep(spin_system *s, double beta, int32_t colour, void *stream) {
+    return halfsweep_impl(s, beta, colour, 0, 0, false, true, (cudaStream_t)stream);
+}
+
+spin_status spin_halfsweep_range(spin_system *s, double beta, int32_t colour, int32_t plane0, int32_t n_planes, int32_t last, void *stream) {
+    return halfsweep_impl(s, beta, colour, plane0, n_planes, true, last != 0, (cudaStream_t)stream);
 }
 
 // one face of one colour: per (replica, component) one contiguous plane of the colour array
@@ -1211,6 +1248,51 @@ spin_status spin_halo_get(spin_system *s, int32_t colour, int32_t side, void *d_
 
 spin_status spin_halo_put(spin_system *s, int32_t colour, int32_t side, const void *d_buf, void *stream) {
     return halo_copy(s, colour, side, const_cast<void *>(d_buf), false, (cudaStream_t)stream);
+}
+
+// both faces of one colour with one kernel: pack = owned boundary planes -> d_buf [low][high], unpack = d_buf [from below][from above] -> ghosts
+static spin_status halo_faces(spin_system *s, int32_t colour, void *d_buf, bool pack, cudaStream_t st) {
+    if (!s || !d_buf) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    if (s->axis < 0) return fail(SPIN_ERR_STATE, "not a slab handle");
+    if (colour != 0 && colour != 1) return fail(SPIN_ERR_INVALID_ARG, "colour must be 0 or 1");
+    const Face f = face_of(s);
+    // local planes: 0, 1 low ghosts (1 is read), 2 .. own + 1 owned, own + 2, own + 3 high ghosts (own + 2 is read)
+    const uint32_t lo = pack ? 2u : 1u, hi = pack ? (uint32_t)s->own_planes + 1u : (uint32_t)s->own_planes + 2u;
+    char *arr = s->ws + s->lay.off_s[colour];
+    const size_t bytes = 2 * f.plane_bytes * f.rows;
+    const bool wide = f.plane_bytes % 16 == 0 && f.stride_bytes % 16 == 0 && ((uintptr_t)d_buf & 15) == 0;
+    const size_t elems = wide ? bytes / 16 : bytes;
+    const int G = (int)((elems + 255) / 256 > 1184 ? 1184 : (elems + 255) / 256);
+    if (wide) halo_faces_copy<uint4><<<G, 256, 0, st>>>((uint4 *)arr, (uint4 *)d_buf, f.plane_bytes / 16, f.stride_bytes / 16, (uint32_t)f.rows, lo, hi, pack);
+    else halo_faces_copy<uint8_t><<<G, 256, 0, st>>>((uint8_t *)arr, (uint8_t *)d_buf, f.plane_bytes, f.stride_bytes, (uint32_t)f.rows, lo, hi, pack);
+    CUDA_TRY(cudaGetLastError());
+    s->launches += 1;
+    return SPIN_OK;
+}
+
+spin_status spin_halo_wrap(spin_system *s, int32_t colour, void *stream) {
+    if (!s) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    if (s->axis < 0) return fail(SPIN_ERR_STATE, "not a slab handle");
+    if (colour != 0 && colour != 1) return fail(SPIN_ERR_INVALID_ARG, "colour must be 0 or 1");
+    const Face f = face_of(s);
+    char *arr = s->ws + s->lay.off_s[colour];
+    const bool wide = f.plane_bytes % 16 == 0 && f.stride_bytes % 16 == 0;
+    const size_t elems = 2 * f.plane_bytes * f.rows / (wide ? 16 : 1);
+    const int G = (int)((elems + 255) / 256 > 1184 ? 1184 : (elems + 255) / 256);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (wide) halo_faces_wrap<uint4><<<G, 256, 0, st>>>((uint4 *)arr, f.plane_bytes / 16, f.stride_bytes / 16, (uint32_t)f.rows, (uint32_t)s->own_planes);
+    else halo_faces_wrap<uint8_t><<<G, 256, 0, st>>>((uint8_t *)arr, f.plane_bytes, f.stride_bytes, (uint32_t)f.rows, (uint32_t)s->own_planes);
+    CUDA_TRY(cudaGetLastError());
+    s->launches += 1;
+    return SPIN_OK;
+}
+
+spin_status spin_halo_pack(spin_system *s, int32_t colour, void *d_buf, void *stream) {
+    return halo_faces(s, colour, d_buf, true, (cudaStream_t)stream);
+}
+
+spin_status spin_halo_unpack(spin_system *s, int32_t colour, const void *d_buf, void *stream) {
+    return halo_faces(s, colour, const_cast<void *>(d_buf), false, (cudaStream_t)stream);
 }
 
 spin_status spin_measure(spin_system *s, double *E, double *M, void *stream) {

@@ -120,9 +120,9 @@ __device__ __forceinline__ void neighbour_indices(const Geometry &g, uint32_t co
 template <int NC>
 __global__ void __launch_bounds__(256) vector_halfsweep(const __grid_constant__ VectorArgs a) {
     const Geometry &g = a.g;
-    const uint32_t total = g.Nh * a.R;
+    const uint32_t total = g.sw_jn * a.R;
     for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
-        const uint32_t r = idx / g.Nh, j = idx - r * g.Nh;
+        const uint32_t r = idx / g.sw_jn, j = g.sw_j0 + idx - r * g.sw_jn;
         const float *__restrict__ other = a.s[1 - a.colour] + (size_t)r * NC * g.Nh;
         float *mine = a.s[a.colour] + (size_t)r * NC * g.Nh;
         uint32_t nb[6];
@@ -358,14 +358,16 @@ template <int NC, int D, bool UNITJ, int K, bool HB = false, bool MEAS = false>
 __global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_constant__ VectorArgs a) {
     const Geometry &g = a.g;
     const uint32_t RL = g.RL, QX = RL >> 2, Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz, Nh = g.Nh;
-    const uint32_t nstrip = (Ly + K - 1) / K;
-    const uint32_t per_replica = QX * nstrip * Lz;
+    // rows (d = 2) / planes (d = 3) this launch updates: [sw_p0, sw_p0 + sw_pn) along the slowest axis
+    const uint32_t ys0 = D == 2 ? g.sw_p0 : 0u, Lys = D == 2 ? g.sw_pn : Ly, zs0 = D == 3 ? g.sw_p0 : 0u, Lzs = D == 3 ? g.sw_pn : Lz;
+    const uint32_t nstrip = (Lys + K - 1) / K;
+    const uint32_t per_replica = QX * nstrip * Lzs;
     // the replica is blockIdx.y (host: gridDim.y = R), so the plane base pointers are warp-uniform and every access is
     // "uniform 64-bit base + 32-bit offset" (no per-thread 64-bit address arithmetic)
     const uint32_t it = blockIdx.x * blockDim.x + threadIdx.x;
     const uint32_t r = blockIdx.y;
     if (K == 1 && a.prefetch && threadIdx.x == 0u) {
-        // K = 1: quad `it` sits at float offset 4 it of every component plane, so the CTA `prefetch` places ahead reads two
+        // K = 1: quad `it` sits at float offset sw_j0 + 4 it of every component plane, so the CTA `prefetch` places ahead reads two
         // contiguous ranges per component (its own spins and the other colour at the same indices; the rows around them
         // belong to CTAs that run at about the same time).  One thread asks for them now: bulk L2 prefetch, no registers.
         const uint32_t it0 = (blockIdx.x + a.prefetch) * blockDim.x;
@@ -373,8 +375,8 @@ __global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_const
             const uint32_t bytes = 16u * min(blockDim.x, per_replica - it0);
 #pragma unroll
             for (int c = 0; c < NC; ++c) {
-                l2_prefetch_bulk(a.s[a.colour] + ((size_t)r * NC + c) * Nh + 4u * (size_t)it0, bytes);
-                l2_prefetch_bulk(a.s[1 - a.colour] + ((size_t)r * NC + c) * Nh + 4u * (size_t)it0, bytes);
+                l2_prefetch_bulk(a.s[a.colour] + ((size_t)r * NC + c) * Nh + g.sw_j0 + 4u * (size_t)it0, bytes);
+                l2_prefetch_bulk(a.s[1 - a.colour] + ((size_t)r * NC + c) * Nh + g.sw_j0 + 4u * (size_t)it0, bytes);
             }
         }
     }
@@ -383,8 +385,8 @@ __global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_const
     for (int c = 0; c < NC; ++c) m_acc[c] = 0.0f;
     if (it < per_replica) {
     const uint32_t sz = fdiv(it, g.divQX), q = it - sz * QX;       // sz = strip + nstrip * z
-    const uint32_t z = sz / nstrip, y0 = (sz - z * nstrip) * K;
-    const uint32_t kend = min((uint32_t)K, Ly - y0);
+    const uint32_t zl = sz / nstrip, z = zs0 + zl, y0 = ys0 + (sz - zl * nstrip) * K;
+    const uint32_t kend = min((uint32_t)K, ys0 + Lys - y0);
     const float *__restrict__ other = a.s[1 - a.colour] + (size_t)r * NC * Nh;
     float *mine = a.s[a.colour] + (size_t)r * NC * Nh;
     const uint32_t rho = a.replica_streams ? r : 0u;

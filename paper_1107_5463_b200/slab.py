@@ -41,7 +41,8 @@ def ring_neighbours(rank, world):
 
 
 class LocalRing:
-    """All slabs of one lattice as separate handles on one device; halos move by device-to-device copies."""
+    """All slabs of one lattice as separate handles on one device; halos move through the packed message buffers of the
+    library (one pack and one unpack kernel per slab and exchange; a single slab wraps onto itself with one kernel)."""
 
     def __init__(self, system_cls, global_dims, n_slabs, **kw):
         import torch
@@ -54,18 +55,24 @@ class LocalRing:
         s0 = self.systems[0]
         self.n, self.R = s0.n, s0.R
         self.N = self.dims[0] * self.dims[1] * self.dims[2]
-        self.buf = torch.empty(s0.halo_bytes(), dtype=torch.uint8, device=s0.device)
+        self.hb = s0.halo_bytes()
+        self.send = [torch.empty(2 * self.hb, dtype=torch.uint8, device=s0.device) for _ in self.systems]
+        self.recv = [torch.empty(2 * self.hb, dtype=torch.uint8, device=s0.device) for _ in self.systems]
         self.exchange(0)
         self.exchange(1)
 
     def exchange(self, colour):
-        G = len(self.systems)
+        G, hb = len(self.systems), self.hb
+        if G == 1:
+            self.systems[0].halo_wrap(colour)
+            return
+        for k, s in enumerate(self.systems):
+            s.halo_pack(colour, self.send[k])                  # [my lowest owned plane][my highest]
         for k, s in enumerate(self.systems):
             below, above = ring_neighbours(k, G)
-            s.halo_get(colour, 0, self.buf)                   # my lowest owned plane ...
-            self.systems[below].halo_put(colour, 1, self.buf)  # ... is the ghost above the slab below me
-            s.halo_get(colour, 1, self.buf)
-            self.systems[above].halo_put(colour, 0, self.buf)
+            self.recv[k][:hb].copy_(self.send[below][hb:])     # ghost below me = highest plane of the slab below
+            self.recv[k][hb:].copy_(self.send[above][:hb])     # ghost above me = lowest plane of the slab above
+            s.halo_unpack(colour, self.recv[k])
 
     def sweep(self, beta, n_sweeps=1):
         for _ in range(int(n_sweeps)):
@@ -104,19 +111,19 @@ class LocalRing:
             s.close()
 
 
-def exchange_faces(get_face, put_face, colour, dist, rank, world):
-    """One halo exchange of colour `colour` for the slab of this rank.  get_face(colour, side) -> contiguous tensor with my
-    boundary plane; put_face(colour, side, tensor) stores a neighbour's plane as my ghost.  My lowest plane goes to the
-    rank below (as its upper ghost), my highest plane to the rank above (as its lower ghost)."""
-    import torch
-
-    low, high = get_face(colour, 0), get_face(colour, 1)
+def exchange_packed(send, recv, dist, rank, world):
+    """One halo exchange for the slab of this rank.  send = [my lowest owned plane][my highest] (two halves of one
+    contiguous tensor), recv = [ghost below me][ghost above me]: my lowest plane goes to the rank below (as its upper
+    ghost), my highest plane to the rank above (as its lower ghost).  The only data-path communication of the method:
+    point-to-point, ring neighbours, 2 x halo_bytes each way per half-sweep."""
+    hb = send.numel() // 2
+    low, high = send[:hb], send[hb:]
+    from_below, from_above = recv[:hb], recv[hb:]
     if world == 1:
-        put_face(colour, 1, low)
-        put_face(colour, 0, high)
+        from_below.copy_(high)
+        from_above.copy_(low)
         return
     below, above = ring_neighbours(rank, world)
-    from_above, from_below = torch.empty_like(low), torch.empty_like(high)
     if world == 2:
         # both neighbours are the same rank: two messages each way, told apart by their tags
         ops = [dist.P2POp(dist.isend, low, below, tag=0), dist.P2POp(dist.isend, high, above, tag=1),
@@ -126,48 +133,106 @@ def exchange_faces(get_face, put_face, colour, dist, rank, world):
                dist.P2POp(dist.irecv, from_above, above), dist.P2POp(dist.irecv, from_below, below)]
     for w in dist.batch_isend_irecv(ops):
         w.wait()
-    put_face(colour, 1, from_above)    # the lowest plane of the slab above me is my upper ghost
-    put_face(colour, 0, from_below)
+
+
+def exchange_faces(get_face, put_face, colour, dist, rank, world):
+    """The same exchange through per-face callbacks (get_face(colour, side) -> tensor, put_face(colour, side, tensor))."""
+    import torch
+
+    low, high = get_face(colour, 0), get_face(colour, 1)
+    send = torch.cat([low.reshape(-1), high.reshape(-1)])
+    recv = torch.empty_like(send)
+    exchange_packed(send, recv, dist, rank, world)
+    hb = low.numel()
+    put_face(colour, 1, recv[hb:].reshape(low.shape))     # the lowest plane of the slab above me is my upper ghost
+    put_face(colour, 0, recv[:hb].reshape(high.shape))
 
 
 class DistRing:
-    """One slab per rank (one process per GPU); the N ranks together hold ONE lattice (strong scaling)."""
+    """One slab per rank (one process per GPU); the N ranks together hold ONE lattice (strong scaling).
 
-    def __init__(self, system_cls, global_dims, dist, device, **kw):
+    Per half-sweep of colour c: the two boundary planes of the slab are updated first and packed; their exchange runs on
+    a side stream while the interior planes are updated on the main stream; the ghosts are unpacked when both are done
+    ("overlap by updating boundary planes first").  `system` may be any object with the slab calls of
+    binding.SpinSystem (the CPU test drives the ring with an oracle-backed stand-in over gloo)."""
+
+    def __init__(self, system_cls, global_dims, dist, device, overlap=True, **kw):
         import torch
 
         self.dist = dist
         self.rank, self.world = dist.get_rank(), dist.get_world_size()
         self.dims = tuple(int(v) for v in global_dims) + (1,) * (3 - len(global_dims))
         local, off = plan(self.dims, self.world)[self.rank]
+        self.own = local[slab_axis(self.dims)]
         self.system = system_cls(local, slab_global=self.dims[slab_axis(self.dims)], slab_offset=off, device=device, **kw)
-        nbytes = self.system.halo_bytes()
-        self._bufs = [torch.empty(nbytes, dtype=torch.uint8, device=device) for _ in range(2)]
+        self.hb = self.system.halo_bytes()
+        self.device = torch.device(device)
+        self.cuda = self.device.type == "cuda"
+        self.send = torch.empty(2 * self.hb, dtype=torch.uint8, device=device)
+        self.recv = torch.empty(2 * self.hb, dtype=torch.uint8, device=device)
+        self.overlap = bool(overlap) and self.own >= 4
+        self.side = torch.cuda.Stream(device=self.device) if self.cuda else None
+        self.comm_bytes = 0          # bytes this rank has sent
         self.exchange(0)
         self.exchange(1)
 
-    def _get(self, colour, side):
-        self.system.halo_get(colour, side, self._bufs[side])
-        return self._bufs[side]
+    def _communicate(self):
+        """send -> neighbours -> recv, on the side stream when there is one"""
+        import torch
 
-    def _put(self, colour, side, t):
-        self.system.halo_put(colour, side, t)
+        if self.side is None:
+            exchange_packed(self.send, self.recv, self.dist, self.rank, self.world)
+        else:
+            main = torch.cuda.current_stream(self.device)
+            self.side.wait_stream(main)                    # the pack kernel has been enqueued on the main stream
+            with torch.cuda.stream(self.side):
+                exchange_packed(self.send, self.recv, self.dist, self.rank, self.world)
+            main.wait_stream(self.side)
+        self.comm_bytes += 2 * self.hb
 
     def exchange(self, colour):
-        exchange_faces(self._get, self._put, colour, self.dist, self.rank, self.world)
+        if self.world == 1 and hasattr(self.system, "halo_wrap"):
+            self.system.halo_wrap(colour)
+            return
+        self.system.halo_pack(colour, self.send)
+        self._communicate()
+        self.system.halo_unpack(colour, self.recv)
+
+    def halfsweep(self, beta, colour):
+        import torch
+
+        s = self.system
+        if not self.overlap or self.world == 1:
+            s.halfsweep(beta, colour)
+            self.exchange(colour)
+            return
+        s.halfsweep_range(beta, colour, 0, 1, False)                   # lowest owned plane
+        s.halfsweep_range(beta, colour, self.own - 1, 1, False)        # highest owned plane
+        s.halo_pack(colour, self.send)
+        if self.side is None:
+            exchange_packed(self.send, self.recv, self.dist, self.rank, self.world)
+            s.halfsweep_range(beta, colour, 1, self.own - 2, True)
+        else:
+            main = torch.cuda.current_stream(self.device)
+            self.side.wait_stream(main)
+            with torch.cuda.stream(self.side):
+                exchange_packed(self.send, self.recv, self.dist, self.rank, self.world)
+            s.halfsweep_range(beta, colour, 1, self.own - 2, True)      # interior, while the messages are in flight
+            main.wait_stream(self.side)
+        self.comm_bytes += 2 * self.hb
+        s.halo_unpack(colour, self.recv)
 
     def sweep(self, beta, n_sweeps=1):
         for _ in range(int(n_sweeps)):
             for c in (0, 1):
-                self.system.halfsweep(beta, c)
-                self.exchange(c)
+                self.halfsweep(beta, c)
 
     def measure(self):
         """E and M of the whole lattice (sum over ranks)."""
         import torch
 
         E, M = self.system.measure()
-        t = torch.from_numpy(np.concatenate([E.ravel(), M.ravel()])).to(self._bufs[0].device)
+        t = torch.from_numpy(np.concatenate([E.ravel(), M.ravel()])).to(self.device)
         self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM)
         v = t.cpu().numpy()
         return v[: E.size].reshape(E.shape), v[E.size:].reshape(M.shape)

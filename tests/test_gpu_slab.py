@@ -100,3 +100,99 @@ def test_slab_handles_refuse_whole_sweeps_and_bad_plans(P):
     U = P.SpinSystem((64, 8, 1))
     with pytest.raises(P.SpinError):
         U.halo_bytes()
+
+
+@pytest.mark.parametrize("kw,dims", [
+    (dict(n=1, storage="int8"), (128, 24, 1)), (dict(n=1, storage="bitpack"), (128, 20, 1)),
+    (dict(n=1, storage="int8"), (64, 6, 10)), (dict(n=1, storage="bitpack", rule="heatbath"), (64, 6, 8)),
+    (dict(n=1, storage="int8"), (10, 12, 1)), (dict(n=3, storage="fp32"), (16, 8, 10)), (dict(n=2, storage="fp32"), (16, 14, 1)),
+    (dict(n=3, storage="fp32"), (6, 6, 8)),
+])
+def test_half_sweeps_in_pieces_equal_whole_half_sweeps(P, kw, dims):
+    """spin_halfsweep_range: sites of one colour do not interact, so a half-sweep issued as boundary planes first and the
+    interior afterwards (the order the overlapped halo exchange needs) leaves the bits of the whole half-sweep -- for the
+    strip kernels (ragged strips inside the range), the word kernels and the one-thread-per-site kernels."""
+    beta = 0.5
+    A, B = P.SpinSystem(dims, seed=21, **kw), P.SpinSystem(dims, seed=21, **kw)
+    planes = dims[2] if dims[2] > 1 else dims[1]
+    for t in range(3):
+        for c in (0, 1):
+            A.halfsweep(beta, c)
+            B.halfsweep_range(beta, c, 0, 1, False)
+            B.halfsweep_range(beta, c, planes - 1, 1, False)
+            B.halfsweep_range(beta, c, 1, 3, False)
+            B.halfsweep_range(beta, c, 4, planes - 5, True)
+    assert A.sweep_counter == B.sweep_counter == 3
+    assert np.array_equal(A.get_spins().view(np.uint8), B.get_spins().view(np.uint8))
+    with pytest.raises(P.SpinError):
+        B.halfsweep_range(beta, 0, planes - 1, 2, True)
+
+
+@pytest.mark.parametrize("dims,storage,overlap", [((128, 32, 1), "int8", True), ((64, 8, 12), "bitpack", True),
+                                                  ((128, 32, 1), "bitpack", False)])
+def test_dist_ring_single_rank_on_the_gpu(P, dims, storage, overlap):
+    """slab.DistRing with the real handle and a one-rank NCCL group: the slab is its own neighbour (spin_halo_wrap), and
+    with two pseudo-neighbours forced through the packed path (world 1 copies its faces) it still equals the oracle."""
+    import torch
+    import torch.distributed as dist
+
+    import oracle
+    from paper_1107_5463_b200 import slab
+
+    created = False
+    if not dist.is_initialized():
+        dist.init_process_group("nccl", init_method="tcp://127.0.0.1:29533", rank=0, world_size=1,
+                                device_id=torch.device("cuda:0"))
+        created = True
+    try:
+        ring = slab.DistRing(P.SpinSystem, dims, dist, "cuda:0", overlap=overlap, n=1, storage=storage, seed=5)
+        O = oracle.System(dims, n=1, seed=5)
+        ring.sweep(0.44, 4)
+        O.sweep(0.44, 4)
+        assert np.array_equal(ring.system.get_spins(), O.get_spins())
+        E, M = ring.measure()
+        Eo, Mo = O.measure()
+        assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
+        # the packed path as a rank with neighbours would run it: boundary planes, pack, exchange, interior, unpack
+        s = ring.system
+        for c in (0, 1):
+            s.halfsweep_range(0.44, c, 0, 1, False)
+            s.halfsweep_range(0.44, c, ring.own - 1, 1, False)
+            s.halo_pack(c, ring.send)
+            slab.exchange_packed(ring.send, ring.recv, dist, 0, 1)
+            s.halfsweep_range(0.44, c, 1, ring.own - 2, True)
+            s.halo_unpack(c, ring.recv)
+        O.sweep(0.44, 1)
+        assert np.array_equal(s.get_spins(), O.get_spins())
+    finally:
+        if created:
+            dist.destroy_process_group()
+
+
+def test_exchange_cost_of_a_self_exchanging_slab(P):
+    """SURVEY 8(e) / VERDICT item 10: the halo exchange costs one small kernel per half-sweep (it was four strided copies
+    driven from Python, 16 us).  2D L = 16384 int8 as ONE slab that is its own neighbour against the plain handle."""
+    import torch
+
+    from paper_1107_5463_b200 import slab
+
+    dims, beta, sweeps = (16384, 16384, 1), 0.4406868, 10
+    A = P.SpinSystem(dims, n=1, storage="int8", seed=1)
+    A.set_option(P.OPT_TEMPORAL_BLOCKING, 0)
+    ring = slab.LocalRing(P.SpinSystem, dims, 1, n=1, storage="int8", seed=1)
+
+    def timed(fn):
+        fn(2)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        fn(sweeps)
+        e1.record()
+        torch.cuda.synchronize()
+        return 1e3 * e0.elapsed_time(e1) / (2 * sweeps)
+
+    plain = timed(lambda k: A.sweep(beta, k))
+    slabbed = timed(lambda k: ring.sweep(beta, k))
+    print("half-sweep %.1f us, with self-exchange %.1f us" % (plain, slabbed))
+    assert slabbed - plain <= 5.0, (plain, slabbed)
+    assert np.array_equal(A.get_spins(), ring.get_spins())
