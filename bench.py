@@ -260,6 +260,73 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def run_slab(args):
+    """--mode slab: ONE lattice cut into N slabs along its slowest axis, one per rank (strong scaling): per
+    half-sweep each rank updates its boundary planes, exchanges them with its two ring neighbours (point-to-point over
+    NCCL, on a side stream) while it updates the interior.  Prints the whole-lattice metric plus per-rank times and bytes."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_1107_5463_b200 import ranks, slab
+
+    rank, local_rank, world = ranks.env_rank()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = "cuda:%d" % local_rank
+    os.environ.setdefault("NCCL_DEBUG", "INFO")      # the ranks and their transports show in the log
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    else:
+        dist.init_process_group("nccl", init_method="tcp://127.0.0.1:29541", rank=0, world_size=1, device_id=torch.device(dev))
+    import paper_1107_5463_b200 as P
+
+    P.lib()
+    w = P.workloads.WORKLOADS[args.workload]
+    ring = slab.DistRing(P.SpinSystem, w["dims"], dist, dev, n=w["n"], storage=w["storage"], coupling=w["coupling"], J=w["J"],
+                         replicas=w["replicas"], replica_streams=w["replica_streams"], seed=P.workloads.SEED)
+    beta, SPS = w["beta"], args.sweeps_per_step
+    N = w["dims"][0] * w["dims"][1] * w["dims"][2] * w["replicas"]
+    for _ in range(args.warmup):
+        ring.sweep(beta, SPS)
+        ring.measure()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    bytes0 = ring.comm_bytes
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    dist.barrier()
+    torch.cuda.synchronize()
+    t0 = time.time()
+    e0.record()
+    for _ in range(args.steps):
+        ring.sweep(beta, SPS)
+        E, M = ring.measure()
+    e1.record()
+    dist.barrier()
+    torch.cuda.synchronize()
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1) if sampler else None
+    ms = e0.elapsed_time(e1)
+    per_rank = torch.tensor([ms, float(ring.comm_bytes - bytes0)], dtype=torch.float64, device=dev)
+    allr = [torch.zeros_like(per_rank) for _ in range(world)]
+    dist.all_gather(allr, per_rank)
+    ms_max = max(float(t[0]) for t in allr)
+    if rank == 0:
+        halfsweeps = 2 * SPS * args.steps
+        line = {"metric": METRIC, "value": N * SPS * args.steps / (ms_max * 1e6), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "strong",
+                "vs_baseline": None, "dtype": DTYPE[w["storage"]], "data": "synthetic", "mode": "slab",
+                "config": {"workload": args.workload, "dims": list(w["dims"]), "beta": beta, "sweeps_per_step": SPS,
+                           "parallelism": "%d slabs of %d planes along the slowest axis, ring halo exchange per half-sweep" % (world, ring.own),
+                           "overlap": ring.overlap},
+                "per_rank": [{"rank": r, "us_per_halfsweep": 1e3 * float(t[0]) / halfsweeps,
+                              "comm_bytes_per_halfsweep": float(t[1]) / halfsweeps} for r, t in enumerate(allr)],
+                "comm": {"kind": "point-to-point ring (torch.distributed batch_isend_irecv over NCCL)", "halo_bytes_per_face": ring.hb},
+                "E": float(E[0]), "clocks": clocks, "gpu_launches": int(ring.system.launch_count)}
+        print(json.dumps(line), flush=True)
+    dist.barrier()
+    dist.destroy_process_group()
+
+
 def run_graft(args):
     import numpy as np
     import torch
@@ -416,6 +483,9 @@ def main():
     ap.add_argument("--impl", default="graft", choices=["graft", "reference"])
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
     ap.add_argument("--sweeps-per-step", type=int, default=100)
+    ap.add_argument("--mode", default="replicas", choices=["replicas", "slab"],
+                    help="replicas: one independent lattice per GPU (weak scaling, the default and the driver's contract); "
+                         "slab: ONE lattice cut into one slab per GPU with a halo exchange per half-sweep (strong scaling)")
     ap.add_argument("--no-per-model", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -423,6 +493,8 @@ def main():
         args.warmup = 3
     if args.impl == "reference":
         run_reference(args)
+    elif args.mode == "slab":
+        run_slab(args)
     else:
         run_graft(args)
 
