@@ -143,6 +143,13 @@ spin_status spin_halo_unpack(spin_system *s, int32_t colour, const void *d_buf, 
  * ghost above <- lowest owned plane, one kernel.  Asynchronous. */
 spin_status spin_halo_wrap(spin_system *s, int32_t colour, void *stream);
 
+/* Temperature axis ("trivial parallelization"): n_sweeps sweeps with replica r at
+ * betas[r] (host array of n_replicas doubles, read before the call returns) -- many temperatures of one model side by
+ * side, the layout parallel tempering needs.  Needs replica_streams = 1 (or one replica); replica r then follows exactly
+ * the chain it would follow in a handle swept at betas[r].  Runs one launch per replica and half-sweep with the
+ * ordinary kernels.  SPIN_ERR_UNSUPPORTED for bit-packed per-bond couplings and MSC storage.  Asynchronous. */
+spin_status spin_sweep_betas(spin_system *s, const double *betas, int64_t n_sweeps, void *stream);
+
 /* As spin_sweep, recording E and M after every sweep into DEVICE arrays d_E[n_sweeps][R] and
  * d_M[n_sweeps][R][n] (doubles).  Enqueues only. */
 spin_status spin_sweep_record(spin_system *s, double beta, int64_t n_sweeps, double *d_E, double *d_M, void *stream);
@@ -186,7 +193,7 @@ enum { SPIN_OPT_PLAIN_KERNELS = 0,
        SPIN_OPT_KERNEL_VARIANT = 3,
        /* Exact temporal blocking ("k updates per tile load", made results-neutral): spin_sweep
         * runs pairs of sweeps in one pass over the lattice (each row read once and written once per two sweeps), bit-identical
-        * to plain sweeps.  Offered for 2D Ising, INT8 or BITPACK storage, uniform J = +-1, Metropolis, 2048 <= Lx <= 32768,
+        * to plain sweeps.  Offered for 2D Ising, INT8 storage, uniform J = +-1, Metropolis, 2048 <= Lx <= 32768,
         * Lx % 2048 == 0, own random stream per replica; such handles ask for twice the spin storage (spin_workspace_bytes).
         * -1 (default) = on for INT8 lattices too large for the CUDA-graph regime, 0 = off, 1 = on wherever offered. */
        SPIN_OPT_TEMPORAL_BLOCKING = 4,

@@ -29,7 +29,7 @@ _COUPLING = {"uniform": J_UNIFORM, "per_direction": J_PER_DIRECTION, "bond_pm1":
 
 # every symbol include/spin.h declares
 SYMBOLS = [
-    "spin_workspace_bytes", "spin_create", "spin_sweep", "spin_measure", "spin_sweep_record", "spin_get_spins",
+    "spin_workspace_bytes", "spin_create", "spin_sweep", "spin_measure", "spin_sweep_record", "spin_sweep_betas", "spin_get_spins",
     "spin_set_spins", "spin_get_bonds", "spin_get_sweep_count", "spin_set_sweep_count", "spin_get_launch_count",
     "spin_set_launch_shape", "spin_set_strip_rows", "spin_set_option", "spin_halfsweep", "spin_halo_bytes",
     "spin_halo_get", "spin_halo_put", "spin_halfsweep_range", "spin_halo_pack", "spin_halo_unpack", "spin_halo_wrap", "spin_destroy", "spin_last_error", "spin_version",
@@ -75,6 +75,7 @@ def lib():
         L.spin_create.argtypes = [cfgp, vp, C.c_size_t, vp, C.POINTER(vp)]
         L.spin_sweep.argtypes = [vp, C.c_double, C.c_int64, vp]
         L.spin_measure.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
+        L.spin_sweep_betas.argtypes = [vp, C.POINTER(C.c_double), C.c_int64, vp]
         L.spin_sweep_record.argtypes = [vp, C.c_double, C.c_int64, vp, vp, vp]
         L.spin_get_spins.argtypes = [vp, vp, C.c_size_t]
         L.spin_set_spins.argtypes = [vp, vp, C.c_size_t]
@@ -190,6 +191,14 @@ class SpinSystem:
     def sweep(self, beta, n_sweeps=1):
         with self._torch.cuda.device(self.device):
             _check(lib().spin_sweep(self._h, float(beta), int(n_sweeps), self._stream()))
+
+    def sweep_betas(self, betas, n_sweeps=1):
+        """temperature axis: replica r at betas[r]"""
+        b = np.ascontiguousarray(betas, dtype=np.float64)
+        if b.shape != (self.R,):
+            raise ValueError("betas must hold one value per replica")
+        with self._torch.cuda.device(self.device):
+            _check(lib().spin_sweep_betas(self._h, b.ctypes.data_as(C.POINTER(C.c_double)), int(n_sweeps), self._stream()))
 
     def halfsweep(self, beta, colour):
         with self._torch.cuda.device(self.device):

@@ -202,7 +202,7 @@ __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(cons
     const uint32_t kend = min((uint32_t)K, ys0 + Lys - y0);
     const uint8_t *__restrict__ other = (const uint8_t *)a.s[1 - a.colour] + (size_t)r * g.Nh;
     uint8_t *mine = (uint8_t *)a.s[a.colour] + (size_t)r * g.Nh;
-    const uint32_t rho = a.replica_streams ? r : 0u;
+    const uint32_t rho = a.replica_streams ? r + a.rho_off : 0u;
     const uint32_t jflip = a.jneg ? 0xFFFFFFFFu : 0u;
     const size_t rowbytes = g.RL, plane = rowbytes * Ly;
     const size_t zoff = (size_t)z * plane;
@@ -298,7 +298,7 @@ __global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __gri
     const uint32_t kend = min((uint32_t)K, ys0 + Lys - y0);
     const uint32_t *__restrict__ other = (const uint32_t *)a.s[1 - a.colour] + (size_t)r * g.NW;
     uint32_t *mine = (uint32_t *)a.s[a.colour] + (size_t)r * g.NW;
-    const uint32_t rho = a.replica_streams ? r : 0u;
+    const uint32_t rho = a.replica_streams ? r + a.rho_off : 0u;
     const uint32_t jflip = a.jneg ? 0xFFFFFFFFu : 0u;
     const uint32_t plane = WX * Ly, zoff = z * plane;
     const uint32_t zm_off = (D == 3) ? (z == 0 ? Lz - 1 : z - 1) * plane : 0u;

@@ -16,6 +16,7 @@ struct IsingArgs {
     void *s[2];          // per colour: int8 -> uint8_t [R][Nh] (0 = +1, 1 = -1); bitpack -> uint32_t [R][NW]
     const void *bonds;   // bitpack: uint32_t [2][R][3][NW] (bit = 1: J = -1); generic: int8 [R][d][N] of +-1
     uint32_t R, replica_streams, t, colour;
+    uint32_t rho_off;       // added to the replica index in the Philox counter (temperature axis: one launch per replica, R = 1)
     int32_t coupling_kind;  // 0 uniform, 1 per direction, 2 per bond
     int32_t Jdir[3];        // generic kernel: coupling per direction in {-1, 0, +1}
     uint32_t jneg;          // fast kernels: 1 iff the uniform coupling is -1
@@ -259,7 +260,7 @@ __global__ void __launch_bounds__(256) ising_generic_halfsweep(const __grid_cons
             const uint32_t T = hb ? a.hb.T[h + 6] : a.tab.T[dE];
             const uint32_t jg = j + g.j_off;   // global compressed index (slab decomposition)
             const uint32_t unit = jg >> 5, lane = jg & 31u;
-            const uint32_t rho = a.replica_streams ? r : 0u;
+            const uint32_t rho = a.replica_streams ? r + a.rho_off : 0u;
             bool decided = false;
             for (int call = 0; call < 8 && !decided; ++call) {
                 uint32_t w[4];
@@ -348,7 +349,7 @@ __device__ __forceinline__ uint32_t bitpack_update_word(const IsingArgs &a, uint
         if (SHARED) flip = ge2 | (ge1 & ltf[0]) | ltf[1];
         else {
             const uint32_t m[2] = {ge1 & ~ge2, ~ge1};
-            flip = ge2 | lt_mask_select<2>(a, a.t, a.colour, gi + a.g.unit_off, a.replica_streams ? r : 0u, m);
+            flip = ge2 | lt_mask_select<2>(a, a.t, a.colour, gi + a.g.unit_off, a.replica_streams ? r + a.rho_off : 0u, m);
         }
     } else {
         const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
@@ -359,7 +360,7 @@ __device__ __forceinline__ uint32_t bitpack_update_word(const IsingArgs &a, uint
         if (SHARED) flip = ge3 | ((b1 | b2) & ltf[0]) | ((b0 | b1 | b2) & ltf[1]) | ltf[2];
         else {
             const uint32_t m[3] = {b1 & ~b0 & ~b2, b0 & ~b1 & ~b2, ~(b0 | b1 | b2)};
-            flip = ge3 | lt_mask_select<3>(a, a.t, a.colour, gi + a.g.unit_off, a.replica_streams ? r : 0u, m);
+            flip = ge3 | lt_mask_select<3>(a, a.t, a.colour, gi + a.g.unit_off, a.replica_streams ? r + a.rho_off : 0u, m);
         }
     }
     return finish(flip);
@@ -426,7 +427,7 @@ __global__ void __launch_bounds__(256) ising_bitpack_halfsweep_hb(const __grid_c
 #pragma unroll
                 for (int k = 0; k < NT; ++k) up |= m[k] & ltf[k];
             } else {
-                up = lt_mask_select<NT, true>(a, a.t, a.colour, gi + a.g.unit_off, a.replica_streams ? r : 0u, m);
+                up = lt_mask_select<NT, true>(a, a.t, a.colour, gi + a.g.unit_off, a.replica_streams ? r + a.rho_off : 0u, m);
             }
             mine_base[(size_t)r * NW + gi] = ~up;
         }

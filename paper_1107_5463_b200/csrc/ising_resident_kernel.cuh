@@ -39,7 +39,7 @@ __global__ void __launch_bounds__(RESIDENT_MAX_WORDS) ising_resident_sweeps(cons
     const uint32_t i = threadIdx.x;
     const bool live = i < words;
     const uint32_t r = live ? i / NW : 0u, gi = live ? i - r * NW : 0u, rb = r * NW;
-    const uint32_t rho = a.replica_streams ? r : 0u;
+    const uint32_t rho = a.replica_streams ? r + a.rho_off : 0u;
     const uint32_t jflip = a.jneg ? 0xFFFFFFFFu : 0u;
     WordNbrs nb[2];
     nb[0] = word_neighbours<D>(a.g, 0u, gi);

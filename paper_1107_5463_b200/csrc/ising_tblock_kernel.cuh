@@ -45,7 +45,7 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 1) ising_tblock2_sweep
     if (y0 >= Ly) return;
     const int Hs = (int)min(H, Ly - y0);
     const uint32_t w_next = w + 1u == WX ? 0u : w + 1u, w_prev = w == 0u ? WX - 1u : w - 1u;
-    const uint32_t rho = a.replica_streams ? r : 0u;
+    const uint32_t rho = a.replica_streams ? r + a.rho_off : 0u;
     const uint32_t jflip = a.jneg ? 0xFFFFFFFFu : 0u;
     const size_t rep = INT8 ? (size_t)r * g.Nh : (size_t)r * g.NW * 4u;           // byte offset of the replica
     const uint8_t *const src0 = (const uint8_t *)a.s[0] + rep, *const src1 = (const uint8_t *)a.s[1] + rep;

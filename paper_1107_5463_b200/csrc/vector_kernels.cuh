@@ -16,6 +16,7 @@ struct VectorArgs {
     PhiloxKeys keys;
     float *s[2];          // per colour: float [R][NC][Nh]
     uint32_t R, replica_streams, t, colour;
+    uint32_t rho_off;     // added to the replica index in the Philox counter (temperature axis: one launch per replica, R = 1)
     float Jdir[3];
     float beta;
     uint32_t rule;        // 0 Metropolis (Eq. (2)), 1 heat bath (n = 3 only)
@@ -140,7 +141,7 @@ __global__ void __launch_bounds__(256) vector_halfsweep(const __grid_constant__ 
             }
         }
         uint32_t w[4];
-        philox4x32_10(j + g.j_off, a.replica_streams ? r : 0u, a.t, make_tag(a.colour, DOM_VECTOR_UPDATE, 0), a.keys, w);
+        philox4x32_10(j + g.j_off, a.replica_streams ? r + a.rho_off : 0u, a.t, make_tag(a.colour, DOM_VECTOR_UPDATE, 0), a.keys, w);
         float sn[NC];
         uint32_t wacc;
         if (NC == 3 && a.rule != 0u) {
@@ -389,7 +390,7 @@ __global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_const
     const uint32_t kend = min((uint32_t)K, ys0 + Lys - y0);
     const float *__restrict__ other = a.s[1 - a.colour] + (size_t)r * NC * Nh;
     float *mine = a.s[a.colour] + (size_t)r * NC * Nh;
-    const uint32_t rho = a.replica_streams ? r : 0u;
+    const uint32_t rho = a.replica_streams ? r + a.rho_off : 0u;
     const uint32_t tag = make_tag(a.colour, DOM_VECTOR_UPDATE, 0);
     const uint32_t plane = RL * Ly, zoff = z * plane;
     const uint32_t zm_off = (D == 3) ? (z == 0 ? Lz - 1 : z - 1) * plane : 0u;

@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(TMA_THREADS, tma_ctas_per_sm(HB, MEAS)) vector
         }
     } else if (sa < sb) {
         // ---- consumers
-        const uint32_t rho = a.replica_streams ? r : 0u;
+        const uint32_t rho = a.replica_streams ? r + a.rho_off : 0u;
         const uint32_t tag = make_tag(a.colour, DOM_VECTOR_UPDATE, 0);
         const float Jx = a.Jdir[0], Jy = a.Jdir[1], Jz = a.Jdir[2];
         const uint32_t cs_main = TY * TX;                           // component stride inside a main box (floats)

@@ -51,6 +51,8 @@ def test_workspace_bytes_and_validation_without_gpu(P):
     assert P.workspace_bytes(cfg) >= 4096
     cfg, _ = P.make_config((16384, 16384, 1), n=1, storage="bitpack")
     assert 33554432 <= P.workspace_bytes(cfg) < 34000000
+    cfg, _ = P.make_config((16384, 16384, 1), n=1, storage="int8")
+    assert 4 * 134217728 <= P.workspace_bytes(cfg) < 4 * 134217728 + 1000000   # two pairs of colour arrays (temporal blocking)
     cfg, _ = P.make_config((256, 256, 256), n=3, storage="fp32")
     assert P.workspace_bytes(cfg) >= 201326592
     cfg, _ = P.make_config((256, 256, 256), n=1, storage="bitpack", coupling="bond_pm1", replicas=16)

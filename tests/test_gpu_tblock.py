@@ -1,7 +1,7 @@
 """Exact temporal blocking ("k updates per tile load", made results-neutral): spin_sweep with
 SPIN_OPT_TEMPORAL_BLOCKING runs two sweeps per pass over the lattice and must leave EXACTLY the spins of plain sweeps.
 Bit-exact against the oracle after every pair of sweeps and after odd counts (the odd sweep goes through the plain
-kernel), for both storages, ragged and wrapping stripes, several replicas, the antiferromagnet, beta = 0 and a large beta."""
+kernel), for ragged and wrapping stripes, several replicas, the antiferromagnet, beta = 0 and a large beta."""
 import numpy as np
 import pytest
 
@@ -35,16 +35,15 @@ def _equal(G, O, tag):
 
 @pytest.mark.parametrize("dims,storage,rows,J,R,beta", [
     ((2048, 40, 1), "int8", 0, 1.0, 1, BETA_C),       # automatic stripe height
-    ((2048, 40, 1), "bitpack", 0, 1.0, 1, BETA_C),
     ((2048, 38, 1), "int8", 7, 1.0, 1, BETA_C),       # ragged last stripe
-    ((2048, 38, 1), "bitpack", 5, -1.0, 2, BETA_C),   # antiferromagnet, two replicas with their own streams
+    ((2048, 38, 1), "int8", 5, -1.0, 2, BETA_C),   # antiferromagnet, two replicas with their own streams
     ((2048, 6, 1), "int8", 2, 1.0, 1, BETA_C),        # halo wraps around the whole lattice
-    ((2048, 2, 1), "bitpack", 1, 1.0, 1, BETA_C),     # two rows: every neighbour row is the other row
+    ((2048, 2, 1), "int8", 1, 1.0, 1, BETA_C),     # two rows: every neighbour row is the other row
     ((4096, 24, 1), "int8", 9, 1.0, 3, 0.3),          # two warps per row
     ((2048, 30, 1), "int8", 30, 1.0, 1, 0.0),         # beta = 0: every spin flips twice per pair
-    ((2048, 30, 1), "bitpack", 11, 1.0, 1, 50.0),     # frozen
+    ((2048, 30, 1), "int8", 11, 1.0, 1, 50.0),     # frozen
     ((16384, 12, 1), "int8", 4, 1.0, 1, BETA_C),      # BASELINE row width (256 threads per CTA)
-    ((32768, 10, 1), "bitpack", 3, 1.0, 1, BETA_C),   # 512 threads per CTA
+    ((32768, 10, 1), "int8", 3, 1.0, 1, BETA_C),   # 512 threads per CTA
 ])
 def test_temporal_blocking_is_bit_exact(P, oracle, dims, storage, rows, J, R, beta):
     kw = dict(n=1, storage=storage, J=(J, J, J), replicas=R, replica_streams=1, seed=SEED)
@@ -101,13 +100,12 @@ def test_temporal_blocking_not_offered(P):
     assert np.array_equal(G.get_spins(), H.get_spins())
 
 
-@pytest.mark.parametrize("storage", ["int8", "bitpack"])
+@pytest.mark.parametrize("storage", ["int8"])
 def test_full_size_pairs_equal_plain_sweeps(P, storage):
     """BASELINE config 2 at full size, default knobs: five sweeps with temporal blocking (two passes + one plain sweep)
     leave exactly the bytes of five plain sweeps."""
     w = P.workloads.WORKLOADS["ising2d_L16384_" + storage]
     A, B = P.from_workload(w, P.workloads.SEED), P.from_workload(w, P.workloads.SEED)
-    A.set_option(P.OPT_TEMPORAL_BLOCKING, 1 if storage == "bitpack" else -1)   # int8: the default; bit-packed: on request
     B.set_option(P.OPT_TEMPORAL_BLOCKING, 0)
     l0 = A.launch_count
     A.sweep(w["beta"], 5)
