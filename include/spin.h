@@ -157,6 +157,19 @@ spin_status spin_sweep_record(spin_system *s, double beta, int64_t n_sweeps, dou
 /* Canonical HOST layouts.  n = 1: int8 [replica][i] of +-1; n >= 2: float [replica][i][n].  Blocking. */
 spin_status spin_get_spins(spin_system *s, void *host, size_t bytes);
 spin_status spin_set_spins(spin_system *s, const void *host, size_t bytes);
+
+/* The same two conversions without a device-wide synchronisation and without library-owned memory.
+ * spin_get_spins_device / spin_set_spins_device: the canonical array lives in DEVICE memory of the caller's (the same
+ *   layout and size as above); the conversion kernel is enqueued on `stream`.  For n = 1 the +-1 check needs d_flag, one
+ *   device int of the caller's: it is set nonzero if a value is not +-1, and the arrays are then left as they were.
+ * spin_set_spins_async: host array (pinned for a truly asynchronous upload) -> arrays on `stream`: chunked upload into the
+ *   handle's staging buffer, the +-1 check of each chunk under the remaining copies, one conversion kernel that the check
+ *   guards on the device.  Returns after enqueueing; spin_set_spins_status(stream) synchronises `stream` and reports the
+ *   check (SPIN_ERR_INVALID_ARG if it failed; the arrays are then unchanged).  The host array must stay valid until then. */
+spin_status spin_get_spins_device(spin_system *s, void *d_canon, size_t bytes, void *stream);
+spin_status spin_set_spins_device(spin_system *s, const void *d_canon, size_t bytes, int32_t *d_flag, void *stream);
+spin_status spin_set_spins_async(spin_system *s, const void *host, size_t bytes, void *stream);
+spin_status spin_set_spins_status(spin_system *s, void *stream);
 /* BOND_PM1 only: int8 [replica][mu][i] of +-1.  Blocking. */
 spin_status spin_get_bonds(spin_system *s, int8_t *host, size_t bytes);
 

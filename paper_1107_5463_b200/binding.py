@@ -30,7 +30,8 @@ _COUPLING = {"uniform": J_UNIFORM, "per_direction": J_PER_DIRECTION, "bond_pm1":
 # every symbol include/spin.h declares
 SYMBOLS = [
     "spin_workspace_bytes", "spin_create", "spin_sweep", "spin_measure", "spin_sweep_record", "spin_sweep_betas", "spin_get_spins",
-    "spin_set_spins", "spin_get_bonds", "spin_get_sweep_count", "spin_set_sweep_count", "spin_get_launch_count",
+    "spin_set_spins", "spin_get_spins_device", "spin_set_spins_device", "spin_set_spins_async", "spin_set_spins_status",
+    "spin_get_bonds", "spin_get_sweep_count", "spin_set_sweep_count", "spin_get_launch_count",
     "spin_set_launch_shape", "spin_set_strip_rows", "spin_set_option", "spin_halfsweep", "spin_halo_bytes",
     "spin_halo_get", "spin_halo_put", "spin_halfsweep_range", "spin_halo_pack", "spin_halo_unpack", "spin_halo_wrap", "spin_destroy", "spin_last_error", "spin_version",
 ]
@@ -79,6 +80,10 @@ def lib():
         L.spin_sweep_record.argtypes = [vp, C.c_double, C.c_int64, vp, vp, vp]
         L.spin_get_spins.argtypes = [vp, vp, C.c_size_t]
         L.spin_set_spins.argtypes = [vp, vp, C.c_size_t]
+        L.spin_get_spins_device.argtypes = [vp, vp, C.c_size_t, vp]
+        L.spin_set_spins_device.argtypes = [vp, vp, C.c_size_t, vp, vp]
+        L.spin_set_spins_async.argtypes = [vp, vp, C.c_size_t, vp]
+        L.spin_set_spins_status.argtypes = [vp, vp]
         L.spin_get_bonds.argtypes = [vp, vp, C.c_size_t]
         L.spin_get_sweep_count.argtypes = [vp, C.POINTER(C.c_uint64)]
         L.spin_set_sweep_count.argtypes = [vp, C.c_uint64]
@@ -269,6 +274,37 @@ class SpinSystem:
         a = np.ascontiguousarray(spins, dtype=np.int8 if self.n == 1 else np.float32)
         with self._torch.cuda.device(self.device):
             _check(lib().spin_set_spins(self._h, a.ctypes.data_as(C.c_void_p), a.nbytes))
+
+    def set_spins_async(self, spins):
+        """host array (pinned: truly asynchronous) -> arrays on the current stream; set_spins_status() reports the +-1 check"""
+        a = np.ascontiguousarray(spins, dtype=np.int8 if self.n == 1 else np.float32)
+        self._pending_host = a          # must stay valid until the stream has consumed it
+        with self._torch.cuda.device(self.device):
+            _check(lib().spin_set_spins_async(self._h, a.ctypes.data_as(C.c_void_p), a.nbytes, self._stream()))
+
+    def set_spins_status(self):
+        with self._torch.cuda.device(self.device):
+            _check(lib().spin_set_spins_status(self._h, self._stream()))
+        self._pending_host = None
+
+    def get_spins_device(self, out=None):
+        """canonical spins as a CUDA tensor (int8 [R, N] or float32 [R, N, n]), converted on the current stream"""
+        torch = self._torch
+        if out is None:
+            out = (torch.empty((self.R, self.N), dtype=torch.int8, device=self.device) if self.n == 1
+                   else torch.empty((self.R, self.N, self.n), dtype=torch.float32, device=self.device))
+        with torch.cuda.device(self.device):
+            _check(lib().spin_get_spins_device(self._h, C.c_void_p(out.data_ptr()), out.numel() * out.element_size(), self._stream()))
+        return out
+
+    def set_spins_device(self, canon):
+        """canonical spins from a contiguous CUDA tensor; returns the device flag tensor of the +-1 check (n = 1) or None"""
+        torch = self._torch
+        flag = torch.zeros(1, dtype=torch.int32, device=self.device) if self.n == 1 else None
+        with torch.cuda.device(self.device):
+            _check(lib().spin_set_spins_device(self._h, C.c_void_p(canon.data_ptr()), canon.numel() * canon.element_size(),
+                                               C.c_void_p(flag.data_ptr()) if flag is not None else None, self._stream()))
+        return flag
 
     def get_bonds(self):
         out = np.empty((self.R, self.d, self.N), dtype=np.int8)

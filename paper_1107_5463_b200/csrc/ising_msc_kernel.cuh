@@ -148,8 +148,10 @@ __global__ void __launch_bounds__(128) ising_msc_measure(const __grid_constant__
 
 // ------------------------------------------------------------------ setup / canonical conversion (not timed) ---------
 // mode 0: cold, 1: hot (seed contract: realisation r, site i as in ising_fill), 2: from canonical int8 [R][N]
-__global__ void __launch_bounds__(256) msc_fill(const __grid_constant__ SetupArgs a, int mode, const int8_t *canon, uint32_t *s0, uint32_t *s1) {
+__global__ void __launch_bounds__(256) msc_fill(const __grid_constant__ SetupArgs a, int mode, const int8_t *canon, uint32_t *s0, uint32_t *s1,
+                                                const int *d_bad = nullptr) {
     const Geometry &g = a.g;
+    if (d_bad && *d_bad) return;
     const uint32_t G = a.R >> 5, per_colour = G * g.Nh, total = 2u * per_colour, N = 2u * g.Nh;
     for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
         const uint32_t c = idx / per_colour, rem = idx - c * per_colour, k = rem / g.Nh, j = rem - k * g.Nh;

@@ -34,9 +34,11 @@ __device__ __forceinline__ uint32_t lex_index(const Geometry &g, uint32_t c, uin
 
 // mode 0: cold, 1: hot (from seed), 2: from canonical int8 [R][N] of +-1.
 // idx runs over (colour, replica, j); with bit-packing a warp covers exactly one word (Nh % 32 == 0).
+// d_bad (mode 2): nonzero = the canonical array failed its +-1 check: leave the arrays alone
 __global__ void __launch_bounds__(256) ising_fill(const __grid_constant__ SetupArgs a, int mode, const int8_t *canon,
-                                                  void *s0, void *s1) {
+                                                  void *s0, void *s1, const int *d_bad = nullptr) {
     const Geometry &g = a.g;
+    if (d_bad && *d_bad) return;
     const uint32_t per_colour = a.R * g.Nh, total = 2u * per_colour;
     for (uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += gridDim.x * blockDim.x) {
         const uint32_t c = idx / per_colour, rem = idx - c * per_colour;

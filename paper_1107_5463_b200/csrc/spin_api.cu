@@ -87,8 +87,10 @@ struct spin_system {
     cudaStream_t cap_stream;    // capture-only stream (nothing ever runs on it)
     double g_beta;
     int g_block, g_rows, g_rows_set, g_num, g_den;
+    int set_pending;     // a spin_set_spins_async whose +-1 check has not been read yet
     void *staging;       // device buffer for canonical arrays (get / set calls), kept until spin_destroy
     size_t staging_bytes;
+    void *h_res;         // pinned host doubles for spin_measure's result (made by the first call)
     // n >= 2, d = 3: TMA-staged kernel (vector_tma_kernel.cuh)
     int tma_ok;          // tensor maps encoded (rows of <= 256 sites per colour, driver entry point found)
     int use_tma;         // SPIN_OPT_TMA_KERNELS: 1 every half-sweep, 0 never, -1 (default) only where its fused E / M pays
@@ -983,7 +985,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
     }
     s->ws = (char *)d_workspace;
     s->tma_ok = 0; s->use_tma = -1; s->tma_ty = 0;
-    s->t = 0; s->launches = 0; s->staging = nullptr; s->staging_bytes = 0; s->gexec = nullptr; s->cap_stream = nullptr; s->gnodes = nullptr; s->n_gnodes = 0;
+    s->t = 0; s->launches = 0; s->staging = nullptr; s->staging_bytes = 0; s->set_pending = 0; s->h_res = nullptr; s->gexec = nullptr; s->cap_stream = nullptr; s->gnodes = nullptr; s->n_gnodes = 0;
     // 128 threads per CTA for the Ising fast paths (measured: +-J R = 16 39.1 vs 40.4 us with 256)
     s->block = (dv.path == PATH_ISING_INT8 || dv.path == PATH_ISING_BITPACK || dv.path == PATH_ISING_MSC) ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0; s->l2_prefetch = -1; s->variant = 0; s->tblock = -1; s->tblock_rows = 0; s->tblock_ok = tblock_offered(cfg, dv) ? 1 : 0;
     s->table_beta = std::nan("");
@@ -1074,6 +1076,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
 
 spin_status spin_destroy(spin_system *s) {
     if (s && s->staging) cudaFree(s->staging);
+    if (s && s->h_res) cudaFreeHost(s->h_res);
     if (s) graph_drop(s);
     if (s && s->cap_stream) cudaStreamDestroy(s->cap_stream);
     delete s;
@@ -1366,16 +1369,18 @@ spin_status spin_measure(spin_system *s, double *E, double *M, void *stream) {
     double *res = (double *)(s->ws + s->lay.off_res);
     spin_status rc = enqueue_measure(s, res, res + s->R, st);
     if (rc != SPIN_OK) return rc;
-    // small result: stage through a local buffer so outputs are written only on success
+    // small result: staged through the handle's pinned host buffer (made once) so outputs are written only on success
     const size_t nE = s->R, nM = (size_t)s->R * s->n;
-    double *tmp = new (std::nothrow) double[nE + nM];
-    if (!tmp) return fail(SPIN_ERR_INVALID_ARG, "out of host memory");
+    if (!s->h_res && cudaMallocHost(&s->h_res, (nE + nM) * sizeof(double)) != cudaSuccess) {
+        s->h_res = nullptr;
+        return fail(SPIN_ERR_CUDA, "measure: no pinned host memory");
+    }
+    double *tmp = (double *)s->h_res;
     cudaError_t e = cudaMemcpyAsync(tmp, res, (nE + nM) * sizeof(double), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) { delete[] tmp; return fail(SPIN_ERR_CUDA, "measure copy: %s", cudaGetErrorString(e)); }
+    if (e != cudaSuccess) return fail(SPIN_ERR_CUDA, "measure copy: %s", cudaGetErrorString(e));
     std::memcpy(E, tmp, nE * sizeof(double));
     std::memcpy(M, tmp + nE, nM * sizeof(double));
-    delete[] tmp;
     return SPIN_OK;
 }
 
@@ -1392,58 +1397,115 @@ static size_t canonical_spin_bytes(const spin_system *s) {
     return s->n == 1 ? (size_t)s->R * s->N : (size_t)s->R * s->N * s->n * sizeof(float);
 }
 
+// canonical spins <-> the colour arrays, everything on `st`; d_canon is device memory (the caller's or the staging buffer)
+static spin_status canonical_from_arrays(spin_system *s, void *d_canon, cudaStream_t st) {
+    const SetupArgs sa = setup_args(s);
+    const int G = grid_for(s, 2ull * s->R * s->g.Nh);
+    void *s0 = s->ws + s->lay.off_s[0], *s1 = s->ws + s->lay.off_s[1];
+    if (s->path == PATH_ISING_MSC) msc_to_canonical<<<G, 256, 0, st>>>(sa, (const uint32_t *)s0, (const uint32_t *)s1, (int8_t *)d_canon);
+    else if (s->n == 1) ising_to_canonical<<<G, 256, 0, st>>>(sa, s0, s1, (int8_t *)d_canon);
+    else if (s->n == 2) vector_to_canonical<2><<<G, 256, 0, st>>>(sa, (const float *)s0, (const float *)s1, (float *)d_canon);
+    else vector_to_canonical<3><<<G, 256, 0, st>>>(sa, (const float *)s0, (const float *)s1, (float *)d_canon);
+    CUDA_TRY(cudaGetLastError());
+    return SPIN_OK;
+}
+
+// d_bad: device int, nonzero = the canonical array holds a value that is not +-1; the fill kernels then leave the arrays alone
+static spin_status arrays_from_canonical(spin_system *s, const void *d_canon, const int *d_bad, cudaStream_t st) {
+    const SetupArgs sa = setup_args(s);
+    const int G = grid_for(s, 2ull * s->R * s->g.Nh);
+    void *s0 = s->ws + s->lay.off_s[0], *s1 = s->ws + s->lay.off_s[1];
+    if (s->path == PATH_ISING_MSC) msc_fill<<<G, 256, 0, st>>>(sa, 2, (const int8_t *)d_canon, (uint32_t *)s0, (uint32_t *)s1, d_bad);
+    else if (s->n == 1) ising_fill<<<G, 256, 0, st>>>(sa, 2, (const int8_t *)d_canon, s0, s1, d_bad);
+    else if (s->n == 2) vector_fill<2><<<G, 256, 0, st>>>(sa, 2, (const float *)d_canon, (float *)s0, (float *)s1);
+    else vector_fill<3><<<G, 256, 0, st>>>(sa, 2, (const float *)d_canon, (float *)s0, (float *)s1);
+    CUDA_TRY(cudaGetLastError());
+    return SPIN_OK;
+}
+
+spin_status spin_get_spins_device(spin_system *s, void *d_canon, size_t bytes, void *stream) {
+    if (!s || !d_canon) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    const size_t need = canonical_spin_bytes(s);
+    if (bytes != need) return fail(SPIN_ERR_INVALID_ARG, "spins need exactly %zu bytes, got %zu", need, bytes);
+    return canonical_from_arrays(s, d_canon, (cudaStream_t)stream);
+}
+
+// Ising spins are checked on the device (d_flag: one int of the caller's, set nonzero if a value is not +-1, in which case nothing
+// is overwritten); the caller reads the flag when it wants to know (spin_set_spins does, after synchronising)
+spin_status spin_set_spins_device(spin_system *s, const void *d_canon, size_t bytes, int32_t *d_flag, void *stream) {
+    if (!s || !d_canon) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    const size_t need = canonical_spin_bytes(s);
+    if (bytes != need) return fail(SPIN_ERR_INVALID_ARG, "spins need exactly %zu bytes, got %zu", need, bytes);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (s->n == 1) {
+        if (!d_flag) return fail(SPIN_ERR_INVALID_ARG, "n = 1 needs d_flag (device int that receives the +-1 check)");
+        CUDA_TRY(cudaMemsetAsync(d_flag, 0, sizeof(int), st));
+        ising_validate_canonical<<<grid_for(s, need / 16 + 1), 256, 0, st>>>((const int8_t *)d_canon, need, d_flag);
+        CUDA_TRY(cudaGetLastError());
+    }
+    return arrays_from_canonical(s, d_canon, s->n == 1 ? d_flag : nullptr, st);
+}
+
 spin_status spin_get_spins(spin_system *s, void *host, size_t bytes) {
     if (!s || !host) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
     const size_t need = canonical_spin_bytes(s);
     if (bytes != need) return fail(SPIN_ERR_INVALID_ARG, "spins need exactly %zu bytes, got %zu", need, bytes);
-    CUDA_TRY(cudaDeviceSynchronize());
+    CUDA_TRY(cudaDeviceSynchronize());   // work enqueued on any stream of the caller's has to be in the arrays
     CUDA_TRY(ensure_staging(s, need));
-    void *staging = s->staging;
-    const SetupArgs sa = setup_args(s);
-    const int G = grid_for(s, 2ull * s->R * s->g.Nh);
-    void *s0 = s->ws + s->lay.off_s[0], *s1 = s->ws + s->lay.off_s[1];
-    if (s->path == PATH_ISING_MSC) msc_to_canonical<<<G, 256>>>(sa, (const uint32_t *)s0, (const uint32_t *)s1, (int8_t *)staging);
-    else if (s->n == 1) ising_to_canonical<<<G, 256>>>(sa, s0, s1, (int8_t *)staging);
-    else if (s->n == 2) vector_to_canonical<2><<<G, 256>>>(sa, (const float *)s0, (const float *)s1, (float *)staging);
-    else vector_to_canonical<3><<<G, 256>>>(sa, (const float *)s0, (const float *)s1, (float *)staging);
-    cudaError_t e = cudaGetLastError();
-    if (e == cudaSuccess) e = cudaMemcpy(host, staging, need, cudaMemcpyDeviceToHost);
-    if (e != cudaSuccess) return fail(SPIN_ERR_CUDA, "get_spins: %s", cudaGetErrorString(e));
+    spin_status rc = canonical_from_arrays(s, s->staging, 0);
+    if (rc != SPIN_OK) return rc;
+    CUDA_TRY(cudaMemcpy(host, s->staging, need, cudaMemcpyDeviceToHost));
+    return SPIN_OK;
+}
+
+// Host array -> arrays on `stream`, without a device-wide synchronisation: the upload goes in chunks, each followed by the
+// +-1 check of that chunk (so the check runs under the remaining copies), then ONE fill kernel that reads the flag on the
+// device and leaves the arrays alone if the check failed.  Returns after enqueueing; a failed check is reported by the
+// next spin_set_spins_status (or by the blocking spin_set_spins).
+spin_status spin_set_spins_async(spin_system *s, const void *host, size_t bytes, void *stream) {
+    if (!s || !host) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    const size_t need = canonical_spin_bytes(s);
+    if (bytes != need) return fail(SPIN_ERR_INVALID_ARG, "spins need exactly %zu bytes, got %zu", need, bytes);
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(ensure_staging(s, need + 512));
+    char *staging = (char *)s->staging;
+    int *d_bad = (int *)(staging + need + (256 - need % 256) % 256);  // 4 aligned bytes after the spins
+    CUDA_TRY(cudaMemsetAsync(d_bad, 0, sizeof(int), st));
+    const size_t chunk = (size_t)32 << 20;
+    for (size_t o = 0; o < need; o += chunk) {
+        const size_t n = need - o < chunk ? need - o : chunk;
+        CUDA_TRY(cudaMemcpyAsync(staging + o, (const char *)host + o, n, cudaMemcpyHostToDevice, st));
+        if (s->n == 1) {
+            ising_validate_canonical<<<grid_for(s, n / 16 + 1), 256, 0, st>>>((const int8_t *)staging + o, n, d_bad);
+            CUDA_TRY(cudaGetLastError());
+        }
+    }
+    s->set_pending = s->n == 1;
+    return arrays_from_canonical(s, staging, s->n == 1 ? d_bad : nullptr, st);
+}
+
+// the +-1 check of the last spin_set_spins_async (synchronises `stream`)
+spin_status spin_set_spins_status(spin_system *s, void *stream) {
+    if (!s) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    if (!s->set_pending) return SPIN_OK;
+    const size_t need = canonical_spin_bytes(s);
+    const int *d_bad = (const int *)((char *)s->staging + need + (256 - need % 256) % 256);
+    int bad = 0;
+    CUDA_TRY(cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+    s->set_pending = 0;
+    if (bad) return fail(SPIN_ERR_INVALID_ARG, "Ising spins must be +-1 (the arrays were left as they were)");
     return SPIN_OK;
 }
 
 spin_status spin_set_spins(spin_system *s, const void *host, size_t bytes) {
     if (!s || !host) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
-    const size_t need = canonical_spin_bytes(s);
-    if (bytes != need) return fail(SPIN_ERR_INVALID_ARG, "spins need exactly %zu bytes, got %zu", need, bytes);
-    CUDA_TRY(cudaDeviceSynchronize());
-    CUDA_TRY(ensure_staging(s, need + 512));
-    char *staging = (char *)s->staging;
-    int *d_bad = (int *)(staging + need + (256 - need % 256) % 256);  // 4 aligned bytes after the spins
-    int bad = 0;
-    cudaError_t e = cudaMemcpy(staging, host, need, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess && s->n == 1) {
-        // Ising spins must be +-1: checked on the device before anything is overwritten
-        e = cudaMemset(d_bad, 0, sizeof(int));
-        if (e == cudaSuccess) {
-            ising_validate_canonical<<<grid_for(s, need / 16 + 1), 256>>>((const int8_t *)staging, need, d_bad);
-            e = cudaGetLastError();
-        }
-        if (e == cudaSuccess) e = cudaMemcpy(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost);
-    }
-    if (e == cudaSuccess && bad) return fail(SPIN_ERR_INVALID_ARG, "Ising spins must be +-1");
-    if (e == cudaSuccess) {
-        const SetupArgs sa = setup_args(s);
-        const int G = grid_for(s, 2ull * s->R * s->g.Nh);
-        void *s0 = s->ws + s->lay.off_s[0], *s1 = s->ws + s->lay.off_s[1];
-        if (s->path == PATH_ISING_MSC) msc_fill<<<G, 256>>>(sa, 2, (const int8_t *)staging, (uint32_t *)s0, (uint32_t *)s1);
-        else if (s->n == 1) ising_fill<<<G, 256>>>(sa, 2, (const int8_t *)staging, s0, s1);
-        else if (s->n == 2) vector_fill<2><<<G, 256>>>(sa, 2, (const float *)staging, (float *)s0, (float *)s1);
-        else vector_fill<3><<<G, 256>>>(sa, 2, (const float *)staging, (float *)s0, (float *)s1);
-        e = cudaGetLastError();
-        if (e == cudaSuccess) e = cudaDeviceSynchronize();
-    }
-    if (e != cudaSuccess) return fail(SPIN_ERR_CUDA, "set_spins: %s", cudaGetErrorString(e));
+    CUDA_TRY(cudaDeviceSynchronize());   // sweeps enqueued on any stream of the caller's come first
+    spin_status rc = spin_set_spins_async(s, host, bytes, nullptr);
+    if (rc != SPIN_OK) return rc;
+    rc = spin_set_spins_status(s, nullptr);
+    if (rc != SPIN_OK) return rc;
+    CUDA_TRY(cudaStreamSynchronize(0));
     return SPIN_OK;
 }
 

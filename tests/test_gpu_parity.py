@@ -543,3 +543,34 @@ def test_direction_map_accuracy(P, oracle, n):
     g, o = G.get_spins()[0].astype(np.float64), O.get_spins()[0].astype(np.float64)
     assert np.max(np.abs(g - o)) <= 2.4e-7, np.max(np.abs(g - o))
     assert np.max(np.abs(np.linalg.norm(g, axis=1) - 1.0)) <= 3e-7
+
+
+def test_stream_aware_get_set_spins(P, oracle):
+    """spin_set_spins_async / spin_set_spins_status and the device-canonical calls (caller-owned memory, no device-wide
+    synchronisation): same bytes as the blocking calls; a bad Ising value is reported and leaves the arrays untouched."""
+    import torch
+
+    for kw, dims in ((dict(n=1, storage="int8"), (128, 16, 1)), (dict(n=1, storage="bitpack"), (64, 6, 4)), (dict(n=3, storage="fp32"), (8, 6, 4))):
+        A, B = P.SpinSystem(dims, seed=3, **kw), P.SpinSystem(dims, seed=4, **kw)
+        ref = A.get_spins()
+        d = A.get_spins_device()
+        assert np.array_equal(d.cpu().numpy(), ref)
+        host = torch.from_numpy(ref).pin_memory()
+        B.set_spins_async(host.numpy())
+        B.set_spins_status()
+        assert np.array_equal(B.get_spins(), ref)
+        C2 = P.SpinSystem(dims, seed=5, **kw)
+        flag = C2.set_spins_device(d)
+        torch.cuda.synchronize()
+        assert (flag is None or int(flag.item()) == 0) and np.array_equal(C2.get_spins(), ref)
+        if kw["n"] == 1:
+            bad = ref.copy()
+            bad[0, 7] = 0
+            before = B.get_spins()
+            B.set_spins_async(bad)
+            with pytest.raises(P.SpinError):
+                B.set_spins_status()
+            assert np.array_equal(B.get_spins(), before)
+            flag = C2.set_spins_device(torch.from_numpy(bad).cuda())
+            torch.cuda.synchronize()
+            assert int(flag.item()) != 0 and np.array_equal(C2.get_spins(), ref)
