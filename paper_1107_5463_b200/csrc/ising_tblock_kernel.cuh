@@ -34,7 +34,7 @@ __host__ __device__ constexpr size_t tblock_smem_bytes(uint32_t WX) {
 // block = WX threads (one per word of a row; 32 <= WX <= MAXT), dynamic shared memory = tblock_smem_bytes(WX).
 // Reads a.s[0], a.s[1]; writes a.alt[0], a.alt[1]; sweeps a.t and a.t + 1.
 template <bool INT8, int MAXT>
-__global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 3 : 1) ising_tblock2_sweeps(const __grid_constant__ IsingArgs a) {
+__global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) ising_tblock2_sweeps(const __grid_constant__ IsingArgs a) {
     extern __shared__ __align__(16) uint32_t tb_smem[];
     const Geometry &g = a.g;
     const uint32_t WX = g.WX, Ly = (uint32_t)g.Ly, w = threadIdx.x, r = blockIdx.y;
