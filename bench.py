@@ -398,10 +398,14 @@ def run_graft(args):
     achieved = bytes_per_launch / (ms_launch * 1e6)  # GB/s
 
     # ---- end-to-end arm: host buffers through the C ABI ------------------------------------------
-    host = torch.from_numpy(S.get_spins()).pin_memory()
+    # Ising: the configuration travels as the canonical BIT array (one bit per spin; spin_set_spins_bits_async), continuous
+    # spins as the canonical fp32 array (spin_set_spins_async); both from pinned host memory on the timed stream
+    use_bits = S.n == 1 and w["storage"] in ("int8", "bitpack")
+    host = torch.from_numpy(S.get_spins_bits() if use_bits else S.get_spins()).pin_memory()
     host_np = host.numpy()
+    upload = S.set_spins_bits_async if use_bits else S.set_spins_async
     for _ in range(2):
-        S.set_spins_async(host_np)
+        upload(host_np)
         S.sweep(beta, SPS)
         S.measure()
     S.set_spins_status()
@@ -409,7 +413,7 @@ def run_graft(args):
     barrier()
     f0.record()
     for k in range(args.steps):
-        S.set_spins_async(host_np)       # pinned host array -> device on this stream (chunked upload, check, conversion)
+        upload(host_np)                  # pinned host array -> device on this stream, then the conversion kernel
         S.sweep(beta, SPS)
         E, M = S.measure()               # blocking: host doubles
     f1.record()
@@ -419,7 +423,8 @@ def run_graft(args):
     e2e = {"value": world * updates_per_step * args.steps / (ms_e2e * 1e6), "unit": UNIT,
            "h2d_bytes_per_step": int(host_np.nbytes), "d2h_bytes_per_step": int(8 * S.R * (1 + S.n)),
            "ms_per_step": ms_e2e / args.steps,
-           "what": "spin_set_spins_async(pinned host array, same stream) + spin_sweep + spin_measure(host E, M) per step"}
+           "what": ("spin_set_spins_bits_async(pinned host bit array, one bit per spin" if use_bits else "spin_set_spins_async(pinned host fp32 array")
+                   + ", same stream) + spin_sweep + spin_measure(host E, M) per step"}
     S_N_R = S.N * S.R
     S.close()
     del S, host, host_np

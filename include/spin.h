@@ -170,6 +170,14 @@ spin_status spin_get_spins_device(spin_system *s, void *d_canon, size_t bytes, v
 spin_status spin_set_spins_device(spin_system *s, const void *d_canon, size_t bytes, int32_t *d_flag, void *stream);
 spin_status spin_set_spins_async(spin_system *s, const void *host, size_t bytes, void *stream);
 spin_status spin_set_spins_status(spin_system *s, void *stream);
+
+/* Ising configurations as canonical BIT arrays (n = 1, INT8 or BITPACK storage, whole-lattice handles, Lx % 8 == 0):
+ * bit (i & 7) of byte (r N + i) >> 3 is 1 iff spin i of replica r is -1; n_replicas * N / 8 bytes -- an eighth of the int8
+ * array across PCIe, and every bit pattern is a valid configuration, so there is nothing to check.
+ * spin_set_spins_bits_async: host array (pinned for an asynchronous upload; it must stay valid until `stream` has consumed
+ * it) -> arrays, enqueued on `stream`.  spin_get_spins_bits: arrays -> host array; synchronises `stream`. */
+spin_status spin_set_spins_bits_async(spin_system *s, const void *host_bits, size_t bytes, void *stream);
+spin_status spin_get_spins_bits(spin_system *s, void *host_bits, size_t bytes, void *stream);
 /* BOND_PM1 only: int8 [replica][mu][i] of +-1.  Blocking. */
 spin_status spin_get_bonds(spin_system *s, int8_t *host, size_t bytes);
 

@@ -31,6 +31,7 @@ _COUPLING = {"uniform": J_UNIFORM, "per_direction": J_PER_DIRECTION, "bond_pm1":
 SYMBOLS = [
     "spin_workspace_bytes", "spin_create", "spin_sweep", "spin_measure", "spin_sweep_record", "spin_sweep_betas", "spin_get_spins",
     "spin_set_spins", "spin_get_spins_device", "spin_set_spins_device", "spin_set_spins_async", "spin_set_spins_status",
+    "spin_set_spins_bits_async", "spin_get_spins_bits",
     "spin_get_bonds", "spin_get_sweep_count", "spin_set_sweep_count", "spin_get_launch_count",
     "spin_set_launch_shape", "spin_set_strip_rows", "spin_set_option", "spin_halfsweep", "spin_halo_bytes",
     "spin_halo_get", "spin_halo_put", "spin_halfsweep_range", "spin_halo_pack", "spin_halo_unpack", "spin_halo_wrap", "spin_destroy", "spin_last_error", "spin_version",
@@ -84,6 +85,8 @@ def lib():
         L.spin_set_spins_device.argtypes = [vp, vp, C.c_size_t, vp, vp]
         L.spin_set_spins_async.argtypes = [vp, vp, C.c_size_t, vp]
         L.spin_set_spins_status.argtypes = [vp, vp]
+        L.spin_set_spins_bits_async.argtypes = [vp, vp, C.c_size_t, vp]
+        L.spin_get_spins_bits.argtypes = [vp, vp, C.c_size_t, vp]
         L.spin_get_bonds.argtypes = [vp, vp, C.c_size_t]
         L.spin_get_sweep_count.argtypes = [vp, C.POINTER(C.c_uint64)]
         L.spin_set_sweep_count.argtypes = [vp, C.c_uint64]
@@ -286,6 +289,20 @@ class SpinSystem:
         with self._torch.cuda.device(self.device):
             _check(lib().spin_set_spins_status(self._h, self._stream()))
         self._pending_host = None
+
+    def set_spins_bits_async(self, bits):
+        """canonical bit array (uint8 [R, N / 8], bit (i & 7) of byte i >> 3 set = spin -1; np.packbits(s < 0, bitorder="little"))
+        -> arrays on the current stream"""
+        a = np.ascontiguousarray(bits, dtype=np.uint8)
+        self._pending_host = a
+        with self._torch.cuda.device(self.device):
+            _check(lib().spin_set_spins_bits_async(self._h, a.ctypes.data_as(C.c_void_p), a.nbytes, self._stream()))
+
+    def get_spins_bits(self):
+        out = np.empty((self.R, self.N // 8), dtype=np.uint8)
+        with self._torch.cuda.device(self.device):
+            _check(lib().spin_get_spins_bits(self._h, out.ctypes.data_as(C.c_void_p), out.nbytes, self._stream()))
+        return out
 
     def get_spins_device(self, out=None):
         """canonical spins as a CUDA tensor (int8 [R, N] or float32 [R, N, n]), converted on the current stream"""

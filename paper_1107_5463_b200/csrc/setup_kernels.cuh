@@ -67,6 +67,34 @@ __global__ void __launch_bounds__(256) ising_fill(const __grid_constant__ SetupA
     }
 }
 
+// Canonical BIT arrays (n = 1; spin_set_spins_bits / spin_get_spins_bits): bit (i & 7) of byte (r N + i) >> 3 is 1 iff spin i of
+// replica r is -1 -- an eighth of the int8 canonical array over PCIe, and every bit pattern is a valid configuration (no check).
+// A thread converts 8 consecutive canonical sites (one byte): 4 of each colour.  Whole-lattice handles only (Lx % 8 == 0).
+__global__ void __launch_bounds__(256) ising_bits_convert(const __grid_constant__ SetupArgs a, uint8_t *bits, void *s0, void *s1, bool to_arrays) {
+    const Geometry &g = a.g;
+    const uint32_t N = 2u * g.Nh, nbytes = a.R * (N >> 3);
+    for (uint32_t b = blockIdx.x * blockDim.x + threadIdx.x; b < nbytes; b += gridDim.x * blockDim.x) {
+        const uint32_t r = b / (N >> 3), i0 = (b - r * (N >> 3)) << 3;       // 8 sites of one row: Lx % 8 == 0
+        const uint32_t row = i0 / (uint32_t)g.Lx, x0 = i0 - row * (uint32_t)g.Lx;
+        const uint32_t z = fdiv(row, g.divLy), y = row - z * (uint32_t)g.Ly;
+        uint32_t v = to_arrays ? bits[b] : 0u;
+#pragma unroll
+        for (uint32_t k = 0; k < 8u; ++k) {
+            const uint32_t x = x0 + k, c = (x + y + z) & 1u, j = (x >> 1) + g.RL * row;
+            void *arr = c ? s1 : s0;
+            if (a.bitpack) {
+                uint32_t *wp = (uint32_t *)arr + (size_t)r * g.NW + (j >> 5);
+                if (to_arrays) { if ((v >> k) & 1u) atomicOr(wp, 1u << (j & 31u)); }
+                else v |= ((*wp >> (j & 31u)) & 1u) << k;
+            } else {
+                uint8_t *bp = (uint8_t *)arr + (size_t)r * g.Nh + int8_byte_index(a, j);
+                if (to_arrays) *bp = (uint8_t)((v >> k) & 1u); else v |= (uint32_t)(*bp & 1u) << k;
+            }
+        }
+        if (!to_arrays) bits[b] = (uint8_t)v;
+    }
+}
+
 // *bad = 1 if any byte of canon[0 .. n) is not +1 or -1
 __global__ void __launch_bounds__(256) ising_validate_canonical(const int8_t *canon, size_t n, int *bad) {
     int local = 0;

@@ -945,7 +945,7 @@ static spin_status check_sweep_args(spin_system *s, double beta, int64_t n_sweep
 extern "C" {
 
 const char *spin_last_error(void) { return g_err; }
-const char *spin_version(void) { return "libspin 0.1 sm_100a"; }
+const char *spin_version(void) { return "libspin 0.2 sm_100a"; }
 
 spin_status spin_workspace_bytes(const spin_config *cfg, size_t *bytes) {
     if (!bytes) return fail(SPIN_ERR_INVALID_ARG, "bytes is NULL");
@@ -1444,6 +1444,46 @@ spin_status spin_set_spins_device(spin_system *s, const void *d_canon, size_t by
         CUDA_TRY(cudaGetLastError());
     }
     return arrays_from_canonical(s, d_canon, s->n == 1 ? d_flag : nullptr, st);
+}
+
+// canonical bit arrays (n = 1): an eighth of the bytes over PCIe, nothing to validate
+static spin_status bits_check(spin_system *s, const void *p, size_t bytes, size_t *need) {
+    if (!s || !p) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    if (s->n != 1 || s->path == PATH_ISING_MSC || s->axis >= 0 || s->g.Lx % 8)
+        return fail(SPIN_ERR_UNSUPPORTED, "bit arrays: n = 1, INT8 or BITPACK storage, whole-lattice handle, Lx %% 8 == 0");
+    *need = (size_t)s->R * s->N / 8;
+    if (bytes != *need) return fail(SPIN_ERR_INVALID_ARG, "spin bits need exactly %zu bytes, got %zu", *need, bytes);
+    return SPIN_OK;
+}
+
+spin_status spin_set_spins_bits_async(spin_system *s, const void *host_bits, size_t bytes, void *stream) {
+    size_t need = 0;
+    spin_status rc = bits_check(s, host_bits, bytes, &need);
+    if (rc != SPIN_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(ensure_staging(s, need));
+    CUDA_TRY(cudaMemcpyAsync(s->staging, host_bits, need, cudaMemcpyHostToDevice, st));
+    void *s0 = s->ws + s->lay.off_s[0], *s1 = s->ws + s->lay.off_s[1];
+    if (s->path == PATH_ISING_BITPACK) {   // bits are OR-ed in
+        CUDA_TRY(cudaMemsetAsync(s0, 0, s->lay.bytes_s, st));
+        CUDA_TRY(cudaMemsetAsync(s1, 0, s->lay.bytes_s, st));
+    }
+    ising_bits_convert<<<grid_for(s, need), 256, 0, st>>>(setup_args(s), (uint8_t *)s->staging, s0, s1, true);
+    CUDA_TRY(cudaGetLastError());
+    return SPIN_OK;
+}
+
+spin_status spin_get_spins_bits(spin_system *s, void *host_bits, size_t bytes, void *stream) {
+    size_t need = 0;
+    spin_status rc = bits_check(s, host_bits, bytes, &need);
+    if (rc != SPIN_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    CUDA_TRY(ensure_staging(s, need));
+    ising_bits_convert<<<grid_for(s, need), 256, 0, st>>>(setup_args(s), (uint8_t *)s->staging, s->ws + s->lay.off_s[0], s->ws + s->lay.off_s[1], false);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaMemcpyAsync(host_bits, s->staging, need, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return SPIN_OK;
 }
 
 spin_status spin_get_spins(spin_system *s, void *host, size_t bytes) {

@@ -574,3 +574,27 @@ def test_stream_aware_get_set_spins(P, oracle):
             flag = C2.set_spins_device(torch.from_numpy(bad).cuda())
             torch.cuda.synchronize()
             assert int(flag.item()) != 0 and np.array_equal(C2.get_spins(), ref)
+
+
+@pytest.mark.parametrize("dims,storage,R", [((128, 16, 1), "int8", 2), ((128, 12, 1), "bitpack", 3), ((64, 6, 4), "bitpack", 1),
+                                             ((16, 6, 1), "int8", 1), ((64, 6, 4), "int8", 2)])
+def test_canonical_bit_arrays(P, dims, storage, R):
+    """spin_set_spins_bits_async / spin_get_spins_bits: the canonical configuration as one bit per spin (an eighth of the
+    bytes across PCIe) is the same configuration as the int8 canonical array, for every n = 1 layout."""
+    import torch
+
+    A = P.SpinSystem(dims, n=1, storage=storage, replicas=R, replica_streams=1, seed=31)
+    A.sweep(0.4, 2)
+    ref = A.get_spins()
+    bits = A.get_spins_bits()
+    assert np.array_equal(bits, np.packbits(ref < 0, axis=1, bitorder="little"))
+    B = P.SpinSystem(dims, n=1, storage=storage, replicas=R, replica_streams=1, seed=31)
+    B.sweep(0.1, 1)                                    # some other configuration, overwritten by the upload
+    pinned = torch.from_numpy(bits).pin_memory()
+    B.set_spins_bits_async(pinned.numpy())
+    torch.cuda.synchronize()
+    assert np.array_equal(B.get_spins(), ref)
+    B.sweep_counter = A.sweep_counter
+    A.sweep(0.4, 3)
+    B.sweep(0.4, 3)
+    assert np.array_equal(A.get_spins(), B.get_spins())
