@@ -356,7 +356,7 @@ __device__ __forceinline__ void vector_quad_update(const VectorArgs &a, float Jx
 // product and sum rounded separately) summed in fp32 over the 128 sites of a warp (fixed shuffle tree), then in fp64 by
 // vector_partials_finalize in a fixed order: deterministic.
 template <int NC, int D, bool UNITJ, int K, bool HB = false, bool MEAS = false>
-__global__ void __launch_bounds__(128) vector_strip_halfsweep(const __grid_constant__ VectorArgs a) {
+__global__ void __launch_bounds__(128, (HB && !MEAS) ? 7 : 0) vector_strip_halfsweep(const __grid_constant__ VectorArgs a) {
     const Geometry &g = a.g;
     const uint32_t RL = g.RL, QX = RL >> 2, Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz, Nh = g.Nh;
     // rows (d = 2) / planes (d = 3) this launch updates: [sw_p0, sw_p0 + sw_pn) along the slowest axis
