@@ -372,6 +372,9 @@ static VectorArgs vector_args(const spin_system *s, double beta) {
 // rows and planes a launch with geometry g updates (Geometry::sw_*): the strips of the fast kernels are cut from these
 static uint32_t sweep_rows(const Geometry &g) { return g.d == 2 ? g.sw_pn : (uint32_t)g.Ly; }
 static uint32_t sweep_planes(const Geometry &g) { return g.d == 3 ? g.sw_pn : (uint32_t)g.Lz; }
+// does the launch update less than the whole local lattice (slab handle, half-sweep in pieces)?  Then the RANGED instances of
+// the strip kernels run (rows per thread 1 or 4 only); the whole-lattice instances carry no offsets (4 % faster at 512^3)
+static bool is_ranged(const Geometry &g) { return g.sw_p0 != 0u || g.sw_pn != (uint32_t)(g.d == 3 ? g.Lz : g.Ly); }
 
 // ----------------------------------------------------------------------------- launches ------
 // fused: NULL, or (colour 1 only) ask for E / M to be accumulated into a.acc by the half-sweep itself;
@@ -408,8 +411,17 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
             K = threads4 >= (uint64_t)s->sm_count * 2048 ? 4 : 1;
         }
         if (hb) K = 4;
+        const bool ranged = is_ranged(a.g);
+        if (ranged) K = K >= 4 ? 4 : 1;
         const uint64_t items = (uint64_t)s->g.WX * ((sweep_rows(a.g) + K - 1) / K) * sweep_planes(a.g) * s->R;
         const int G = (int)((items + B - 1) / B);
+        if (ranged) {
+#define I8R(D_, K_, HB_) ising_int8_halfsweep<D_, K_, HB_, false, true><<<G, B, 0, st>>>(a)
+            if (hb) { if (s->d == 2) I8R(2, 4, true); else I8R(3, 4, true); }
+            else if (s->d == 2) { if (K == 1) I8R(2, 1, false); else I8R(2, 4, false); }
+            else { if (K == 1) I8R(3, 1, false); else I8R(3, 4, false); }
+#undef I8R
+        } else
         if (fused && (K == 1 || K == 4) && a.colour == 1u) {
             *fused = true;
 #define I8M(D_, K_, HB_) ising_int8_halfsweep<D_, K_, HB_, true><<<G, B, 0, st>>>(a)
@@ -432,6 +444,8 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
             K = threads4 >= (uint64_t)s->sm_count * 2048 ? 4 : 1;
         }
         if (K > 4) K = 4;
+        const bool ranged = is_ranged(a.g);
+        if (ranged && K == 2) K = 1;
         const int Bs = B > 128 ? 128 : B;
         const uint64_t items = (uint64_t)s->g.WX * ((sweep_rows(a.g) + K - 1) / K) * sweep_planes(a.g) * s->R;
         const int G = (int)((items + Bs - 1) / Bs);
@@ -439,6 +453,11 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
 #define BS3(D_, K_) do { if (hb) ising_bitpack_strip_halfsweep<D_, K_, true><<<G, Bs, 0, st>>>(a); else ising_bitpack_strip_halfsweep<D_, K_, false><<<G, Bs, 0, st>>>(a); } while (0)
 #define BS2(D_) do { if (K == 1) BS3(D_, 1); else if (K == 2) BS3(D_, 2); else BS3(D_, 4); } while (0)
 #define BM3(D_, K_) do { if (hb) ising_bitpack_strip_halfsweep<D_, K_, true, true><<<G, Bs, 0, st>>>(a); else ising_bitpack_strip_halfsweep<D_, K_, false, true><<<G, Bs, 0, st>>>(a); } while (0)
+#define BR3(D_, K_) do { if (hb) ising_bitpack_strip_halfsweep<D_, K_, true, false, true><<<G, Bs, 0, st>>>(a); else ising_bitpack_strip_halfsweep<D_, K_, false, false, true><<<G, Bs, 0, st>>>(a); } while (0)
+        if (ranged) {
+            if (s->d == 2) { if (K == 1) BR3(2, 1); else BR3(2, 4); } else { if (K == 1) BR3(3, 1); else BR3(3, 4); }
+        } else
+#undef BR3
         if (fused && (K == 1 || K == 4) && a.colour == 1u) {
             *fused = true;
             if (s->d == 2) { if (K == 1) BM3(2, 1); else BM3(2, 4); } else { if (K == 1) BM3(3, 1); else BM3(3, 4); }
@@ -650,17 +669,22 @@ static spin_status launch_halfsweep_vector(spin_system *s, const VectorArgs &a, 
         const int B = s->block > 128 ? 128 : s->block;
         const uint64_t items = (uint64_t)(g.RL / 4) * sweep_rows(a.g) * sweep_planes(a.g);
         const dim3 G((unsigned)((items + B - 1) / B), s->R);
-        if (s->d == 2) { if (unitj) vector_strip_halfsweep<3, 2, true, 1, true><<<G, B, 0, st>>>(a); else vector_strip_halfsweep<3, 2, false, 1, true><<<G, B, 0, st>>>(a); }
-        else { if (unitj) vector_strip_halfsweep<3, 3, true, 1, true><<<G, B, 0, st>>>(a); else vector_strip_halfsweep<3, 3, false, 1, true><<<G, B, 0, st>>>(a); }
+#define VH(D_, U_) do { if (is_ranged(a.g)) vector_strip_halfsweep<3, D_, U_, 1, true, false, true><<<G, B, 0, st>>>(a); else vector_strip_halfsweep<3, D_, U_, 1, true><<<G, B, 0, st>>>(a); } while (0)
+        if (s->d == 2) { if (unitj) VH(2, true); else VH(2, false); }
+        else { if (unitj) VH(3, true); else VH(3, false); }
+#undef VH
     } else if (strip_ok) {
         bool unitj = true;
         for (int mu = 0; mu < s->d; ++mu) unitj = unitj && a.Jdir[mu] == 1.0f;
-        const int K = s->strip_rows_set ? (s->strip_rows >= 4 ? 4 : s->strip_rows) : 1;  // default 1 (measured fastest)
+        int K = s->strip_rows_set ? (s->strip_rows >= 4 ? 4 : s->strip_rows) : 1;  // default 1 (measured fastest)
+        const bool ranged = is_ranged(a.g);
+        if (ranged) K = 1;
         const int B = s->block > 128 ? 128 : s->block;
         const uint64_t items = (uint64_t)(g.RL / 4) * ((sweep_rows(a.g) + K - 1) / K) * sweep_planes(a.g);
         const dim3 G((unsigned)((items + B - 1) / B), s->R);
 #define VS4(NC_, D_, U_, K_) vector_strip_halfsweep<NC_, D_, U_, K_><<<G, B, 0, st>>>(a)
-#define VS3(NC_, D_, U_) do { if (K == 1) VS4(NC_, D_, U_, 1); else if (K == 2) VS4(NC_, D_, U_, 2); else VS4(NC_, D_, U_, 4); } while (0)
+#define VS3(NC_, D_, U_) do { if (ranged) vector_strip_halfsweep<NC_, D_, U_, 1, false, false, true><<<G, B, 0, st>>>(a); \
+                              else if (K == 1) VS4(NC_, D_, U_, 1); else if (K == 2) VS4(NC_, D_, U_, 2); else VS4(NC_, D_, U_, 4); } while (0)
 #define VS2(NC_, D_) do { if (unitj) VS3(NC_, D_, true); else VS3(NC_, D_, false); } while (0)
         if (s->n == 2) { if (s->d == 2) VS2(2, 2); else VS2(2, 3); }
         else { if (s->d == 2) VS2(3, 2); else VS2(3, 3); }

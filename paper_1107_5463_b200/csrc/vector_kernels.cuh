@@ -355,12 +355,14 @@ __device__ __forceinline__ void vector_quad_update(const VectorArgs &a, float Jx
 // spins plus the colour-0 spins at the same compressed indices (already loaded as o_cur).  Per-site terms in fp32 (each
 // product and sum rounded separately) summed in fp32 over the 128 sites of a warp (fixed shuffle tree), then in fp64 by
 // vector_partials_finalize in a fixed order: deterministic.
-template <int NC, int D, bool UNITJ, int K, bool HB = false, bool MEAS = false>
+template <int NC, int D, bool UNITJ, int K, bool HB = false, bool MEAS = false, bool RANGED = false>
 __global__ void __launch_bounds__(128, (HB && !MEAS) ? 7 : 0) vector_strip_halfsweep(const __grid_constant__ VectorArgs a) {
     const Geometry &g = a.g;
     const uint32_t RL = g.RL, QX = RL >> 2, Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz, Nh = g.Nh;
-    // rows (d = 2) / planes (d = 3) this launch updates: [sw_p0, sw_p0 + sw_pn) along the slowest axis
-    const uint32_t ys0 = D == 2 ? g.sw_p0 : 0u, Lys = D == 2 ? g.sw_pn : Ly, zs0 = D == 3 ? g.sw_p0 : 0u, Lzs = D == 3 ? g.sw_pn : Lz;
+    // RANGED: rows (d = 2) / planes (d = 3) [sw_p0, sw_p0 + sw_pn) of the slowest axis only (slab handles, half-sweeps in pieces)
+    const uint32_t ys0 = (RANGED && D == 2) ? g.sw_p0 : 0u, Lys = (RANGED && D == 2) ? g.sw_pn : Ly;
+    const uint32_t zs0 = (RANGED && D == 3) ? g.sw_p0 : 0u, Lzs = (RANGED && D == 3) ? g.sw_pn : Lz;
+    const uint32_t j_first = RANGED ? g.sw_j0 : 0u;
     const uint32_t nstrip = (Lys + K - 1) / K;
     const uint32_t per_replica = QX * nstrip * Lzs;
     // the replica is blockIdx.y (host: gridDim.y = R), so the plane base pointers are warp-uniform and every access is
@@ -376,8 +378,8 @@ __global__ void __launch_bounds__(128, (HB && !MEAS) ? 7 : 0) vector_strip_halfs
             const uint32_t bytes = 16u * min(blockDim.x, per_replica - it0);
 #pragma unroll
             for (int c = 0; c < NC; ++c) {
-                l2_prefetch_bulk(a.s[a.colour] + ((size_t)r * NC + c) * Nh + g.sw_j0 + 4u * (size_t)it0, bytes);
-                l2_prefetch_bulk(a.s[1 - a.colour] + ((size_t)r * NC + c) * Nh + g.sw_j0 + 4u * (size_t)it0, bytes);
+                l2_prefetch_bulk(a.s[a.colour] + ((size_t)r * NC + c) * Nh + j_first + 4u * (size_t)it0, bytes);
+                l2_prefetch_bulk(a.s[1 - a.colour] + ((size_t)r * NC + c) * Nh + j_first + 4u * (size_t)it0, bytes);
             }
         }
     }
