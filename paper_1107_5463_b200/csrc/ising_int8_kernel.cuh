@@ -321,6 +321,38 @@ __global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __gri
     }
     const uint32_t unit0 = (y0 + Ly * z) * WX + w + g.unit_off;
     int e_sum = 0, m_sum = 0;
+    if (DEFER && K > 1 && kend == (uint32_t)K) {
+        // whole strip (the steady state): every load first, then the K heads of the digit comparison as straight-line code --
+        // 2 K independent Philox chains in flight -- and only then the queue pushes and stores
+        uint32_t o_row[K + 2], raw_k[K], side_k[K], zm_k[K], zp_k[K];
+        o_row[0] = o_prev; o_row[1] = o_cur; o_row[2] = pf_next;
+        raw_k[0] = pf_mine; side_k[0] = pf_side; zm_k[0] = pf_zm; zp_k[0] = pf_zp;
+#pragma unroll
+        for (int k = 1; k < K; ++k) {
+            const uint32_t y1 = y0 + k, y2 = y1 + 1 == Ly ? 0u : y1 + 1, off1 = y1 * WX + w;
+            o_row[k + 2] = __ldg(other + zoff + y2 * WX + w);
+            raw_k[k] = mine[zoff + off1];
+            side_k[k] = __ldg(other + zoff + y1 * WX + (((p + k) & 1u) ? w_next : w_prev));
+            zm_k[k] = D == 3 ? __ldg(other + zm_off + off1) : 0u;
+            zp_k[k] = D == 3 ? __ldg(other + zp_off + off1) : 0u;
+        }
+        uint32_t fresh_k[K], eq_k[K], mm_k[K][D];
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const uint32_t pk = (p + k) & 1u, oc = o_row[k + 1];
+            const uint32_t side = pk ? ((oc >> 1) | (side_k[k] << 31)) : ((oc << 1) | (side_k[k] >> 31));
+            const uint32_t s = raw_k[k] ^ jflip;
+            uint32_t av[6];
+            av[0] = s ^ oc; av[1] = s ^ side; av[2] = s ^ o_row[k]; av[3] = s ^ o_row[k + 2];
+            av[4] = D == 3 ? s ^ zm_k[k] : 0u; av[5] = D == 3 ? s ^ zp_k[k] : 0u;
+            fresh_k[k] = ising_new_word_head<D>(a, a.t, a.colour, unit0 + (uint32_t)k * WX, rho, raw_k[k], av, eq_k[k], mm_k[k]);
+        }
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const uint32_t off = (y0 + k) * WX + w;
+            if (defer_or_finish<D>(a, dq, warp, unit0 + (uint32_t)k * WX, rho, eq_k[k], mm_k[k], fresh_k[k], r * g.NW + zoff + off)) mine[zoff + off] = fresh_k[k];
+        }
+    } else
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         if ((uint32_t)k < kend) {
