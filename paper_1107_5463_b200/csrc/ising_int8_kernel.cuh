@@ -321,7 +321,7 @@ __global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __gri
     }
     const uint32_t unit0 = (y0 + Ly * z) * WX + w + g.unit_off;
     int e_sum = 0, m_sum = 0;
-    if (DEFER && K > 1 && kend == (uint32_t)K) {
+    if ((DEFER || (MEAS && !HB)) && K > 1 && kend == (uint32_t)K) {
         // whole strip (the steady state): every load first, then the K heads of the digit comparison as straight-line code --
         // 2 K independent Philox chains in flight -- and only then the queue pushes and stores
         uint32_t o_row[K + 2], raw_k[K], side_k[K], zm_k[K], zp_k[K];
@@ -350,7 +350,20 @@ __global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __gri
 #pragma unroll
         for (int k = 0; k < K; ++k) {
             const uint32_t off = (y0 + k) * WX + w;
-            if (defer_or_finish<D>(a, dq, warp, unit0 + (uint32_t)k * WX, rho, eq_k[k], mm_k[k], fresh_k[k], r * g.NW + zoff + off)) mine[zoff + off] = fresh_k[k];
+            if constexpr (MEAS) {
+                // recorded sweep: the word is finished here (the few undecided lanes inline) so that E and M can be taken from it
+                if (eq_k[k] != 0u) fresh_k[k] ^= lt_mask_select_tail<D>(a, a.t, a.colour, unit0 + (uint32_t)k * WX, rho, mm_k[k], eq_k[k]);
+                mine[zoff + off] = fresh_k[k];
+                const uint32_t pk = (p + k) & 1u, oc = o_row[k + 1];
+                const uint32_t side = pk ? ((oc >> 1) | (side_k[k] << 31)) : ((oc << 1) | (side_k[k] >> 31));
+                const uint32_t s = raw_k[k] ^ jflip;
+                uint32_t av[6];
+                av[0] = s ^ oc; av[1] = s ^ side; av[2] = s ^ o_row[k]; av[3] = s ^ o_row[k + 2];
+                av[4] = D == 3 ? s ^ zm_k[k] : 0u; av[5] = D == 3 ? s ^ zp_k[k] : 0u;
+                fused_word_sums<D>(av, raw_k[k], fresh_k[k], oc, e_sum, m_sum);
+            } else {
+                if (defer_or_finish<D>(a, dq, warp, unit0 + (uint32_t)k * WX, rho, eq_k[k], mm_k[k], fresh_k[k], r * g.NW + zoff + off)) mine[zoff + off] = fresh_k[k];
+            }
         }
     } else
 #pragma unroll
