@@ -34,7 +34,7 @@ METRIC = "spin flips/ns (device-timed) and achieved HBM GB/s vs B200 peak, per m
 UNIT = "flips/ns"
 DEFAULT_WORKLOAD = "ising2d_L16384_int8"
 # per-model legs of the default run: (workload, sweeps timed)
-PER_MODEL = [("ising2d_L64_int8", 200), ("ising2d_L16384_bitpack", 40), ("ising3d_L512_bitpack", 40),
+PER_MODEL = [("ising2d_L64_int8", 1000), ("ising2d_L16384_bitpack", 40), ("ising3d_L512_bitpack", 40),
              ("ea3d_L256_R16_bitpack", 40), ("ea3d_L256_R16_bitpack_ownstreams", 20), ("ea2d_L64_R4096_bitpack", 200),
              ("ea2d_L32_R131072_msc", 100), ("heisenberg3d_L256_fp32", 20), ("xy3d_L256_fp32", 20)]
 RECORDED = ("ising2d_L16384_bitpack", "ea3d_L256_R16_bitpack", "heisenberg3d_L256_fp32", "xy3d_L256_fp32")
