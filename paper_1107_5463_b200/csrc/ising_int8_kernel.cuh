@@ -281,7 +281,7 @@ __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(cons
 // registers over the rows, the loads of row k + 1 are issued before row k is computed, and the index arithmetic is
 // paid once per strip instead of once per word.  Results are bit-identical to ising_bitpack_halfsweep.
 template <int D, int K, bool HB = false, bool MEAS = false, bool RANGED = false>
-__global__ void __launch_bounds__(128) ising_bitpack_strip_halfsweep(const __grid_constant__ IsingArgs a) {
+__global__ void __launch_bounds__(128, (D == 3 && K == 4 && !HB && !MEAS) ? 6 : 0) ising_bitpack_strip_halfsweep(const __grid_constant__ IsingArgs a) {
     const Geometry &g = a.g;
     const uint32_t WX = g.WX, Ly = (uint32_t)g.Ly, Lz = (uint32_t)g.Lz;
     // RANGED: the launch updates rows (d = 2) / planes (d = 3) [sw_p0, sw_p0 + sw_pn) of the slowest axis only (slab handles, half-sweeps
