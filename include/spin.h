@@ -214,9 +214,10 @@ enum { SPIN_OPT_PLAIN_KERNELS = 0,
        SPIN_OPT_KERNEL_VARIANT = 3,
        /* Exact temporal blocking ("k updates per tile load", made results-neutral): spin_sweep
         * runs pairs of sweeps in one pass over the lattice (each row read once and written once per two sweeps), bit-identical
-        * to plain sweeps.  Offered for 2D Ising, INT8 storage, uniform J = +-1, Metropolis, 2048 <= Lx <= 32768,
+        * to plain sweeps.  Offered for 2D Ising, INT8 storage, uniform J = +-1, both update rules, 2048 <= Lx <= 32768,
         * Lx % 2048 == 0, own random stream per replica; such handles ask for twice the spin storage (spin_workspace_bytes).
-        * -1 (default) = on for INT8 lattices too large for the CUDA-graph regime, 0 = off, 1 = on wherever offered. */
+        * -1 (default) = on for the Metropolis rule on INT8 lattices too large for the CUDA-graph regime, 0 = off,
+        * 1 = on wherever offered. */
        SPIN_OPT_TEMPORAL_BLOCKING = 4,
        /* rows per stripe of the temporal-blocking kernel; 0 (default) = one wave of resident CTAs */
        SPIN_OPT_TBLOCK_ROWS = 5 };

@@ -33,7 +33,8 @@ __host__ __device__ constexpr size_t tblock_smem_bytes(uint32_t WX) {
 // INT8: global arrays in the int8 fast layout (32-byte units), else bit-packed words.  grid = (stripes, R),
 // block = WX threads (one per word of a row; 32 <= WX <= MAXT), dynamic shared memory = tblock_smem_bytes(WX).
 // Reads a.s[0], a.s[1]; writes a.alt[0], a.alt[1]; sweeps a.t and a.t + 1.
-template <bool INT8, int MAXT>
+// HB: heat-bath rule: the new word comes from the lazy comparison against the 2 d + 1 heat-bath thresholds, no queue.
+template <bool INT8, int MAXT, bool HB = false>
 __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) ising_tblock2_sweeps(const __grid_constant__ IsingArgs a) {
     extern __shared__ __align__(16) uint32_t tb_smem[];
     const Geometry &g = a.g;
@@ -85,6 +86,10 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) ising_tblock2_sweep
             uint32_t av[6];
             av[0] = sp ^ o_cur; av[1] = sp ^ side; av[2] = sp ^ o_prev; av[3] = sp ^ o_next; av[4] = 0u; av[5] = 0u;
             const uint32_t unit = y * WX + w + g.unit_off;
+            if constexpr (HB) {
+                mine_r[slot + w] = ising_new_word<2, true>(a, tt, c, unit, rho, raw, av);
+                return;
+            }
             uint32_t eq, mm[2];
             const uint32_t fresh = ising_new_word_head<2>(a, tt, c, unit, rho, raw, av, eq, mm);
             mine_r[slot + w] = fresh;

@@ -215,7 +215,7 @@ constexpr uint32_t FINALIZE_BLOCKS = 128;   // first-level blocks of vector_part
 // Exact temporal blocking (two sweeps per pass, ising_tblock_kernel.cuh) is offered for the 2D Ising int8 fast layout with uniform
 // couplings and the Metropolis rule when a row of one colour is 32 .. 512 words; it needs a second pair of colour arrays.
 static bool tblock_offered(const spin_config *c, const Derived &dv) {
-    if (c->n != 1 || dv.d != 2 || dv.axis >= 0 || c->update_rule != SPIN_UPDATE_METROPOLIS) return false;
+    if (c->n != 1 || dv.d != 2 || dv.axis >= 0) return false;
     // int8 storage only: the bit-packed lattices are L2-resident and gain nothing (measured 55.2 vs 55.6 us at L = 16384)
     if (dv.path != PATH_ISING_INT8 || c->coupling_kind != SPIN_J_UNIFORM) return false;
     if (c->n_replicas > 1 && !c->replica_streams) return false;   // shared-stream replicas take the mask-reuse kernels
@@ -709,18 +709,19 @@ static bool tblock_use(const spin_system *s, int64_t n_sweeps) {
     if (s->tblock == 1) return true;
     // auto: int8 storage (where it cuts the HBM traffic to a third; the bit-packed lattices are L2-resident and gain nothing:
     // 55.2 vs 55.6 us at L = 16384) and only where a half-sweep outlasts its launch
-    return s->path == PATH_ISING_INT8 && !graph_ok(s, 1 << 20);
+    // (the heat-bath instance is ALU-bound either way: 84.3 vs 82.3 us for the strip kernel at L = 16384, so it runs on request only)
+    return s->path == PATH_ISING_INT8 && s->cfg.update_rule == SPIN_UPDATE_METROPOLIS && !graph_ok(s, 1 << 20);
 }
 
-template <bool INT8, int MAXT>
+template <bool INT8, int MAXT, bool HB>
 static cudaError_t tblock_launch(const IsingArgs &a, dim3 G, int B, size_t smem, cudaStream_t st) {
     static size_t configured = 0;
     if (configured < smem) {
-        cudaError_t e = cudaFuncSetAttribute(ising_tblock2_sweeps<INT8, MAXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(ising_tblock2_sweeps<INT8, MAXT, HB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    ising_tblock2_sweeps<INT8, MAXT><<<G, B, smem, st>>>(a);
+    ising_tblock2_sweeps<INT8, MAXT, HB><<<G, B, smem, st>>>(a);
     return cudaGetLastError();
 }
 
@@ -728,16 +729,16 @@ static cudaError_t tblock_launch(const IsingArgs &a, dim3 G, int B, size_t smem,
 static spin_status tblock_sweeps(spin_system *s, int64_t pairs, cudaStream_t st) {
     const int B = (int)s->g.WX;
     const size_t smem = tblock_smem_bytes(s->g.WX);
-    const bool i8 = s->path == PATH_ISING_INT8;
+    const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
     // rows per stripe: one wave of resident CTAs (a stripe costs 3 / H redundant row updates; a second wave would idle)
     uint32_t H = (uint32_t)s->tblock_rows;
     if (H == 0) {
         int per_sm = 1;
         cudaError_t e;
-        if (B <= 256) e = i8 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_tblock2_sweeps<true, 256>, B, smem)
-                             : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_tblock2_sweeps<false, 256>, B, smem);
-        else e = i8 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_tblock2_sweeps<true, 512>, B, smem)
-                    : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_tblock2_sweeps<false, 512>, B, smem);
+        if (B <= 256) e = hb ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_tblock2_sweeps<true, 256, true>, B, smem)
+                             : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_tblock2_sweeps<true, 256, false>, B, smem);
+        else e = hb ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_tblock2_sweeps<true, 512, true>, B, smem)
+                    : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ising_tblock2_sweeps<true, 512, false>, B, smem);
         if (e != cudaSuccess || per_sm < 1) per_sm = 1;
         uint64_t stripes = (uint64_t)s->sm_count * per_sm / s->R;
         if (stripes < 1) stripes = 1;
@@ -749,8 +750,8 @@ static spin_status tblock_sweeps(spin_system *s, int64_t pairs, cudaStream_t st)
         IsingArgs a = ising_args(s);
         a.tb_rows = H;
         cudaError_t e;
-        if (B <= 256) e = i8 ? tblock_launch<true, 256>(a, G, B, smem, st) : tblock_launch<false, 256>(a, G, B, smem, st);
-        else e = i8 ? tblock_launch<true, 512>(a, G, B, smem, st) : tblock_launch<false, 512>(a, G, B, smem, st);
+        if (B <= 256) e = hb ? tblock_launch<true, 256, true>(a, G, B, smem, st) : tblock_launch<true, 256, false>(a, G, B, smem, st);
+        else e = hb ? tblock_launch<true, 512, true>(a, G, B, smem, st) : tblock_launch<true, 512, false>(a, G, B, smem, st);
         if (e != cudaSuccess) return fail(SPIN_ERR_CUDA, "temporal-blocking launch: %s", cudaGetErrorString(e));
         for (int c = 0; c < 2; ++c) { const size_t t = s->lay.off_s[c]; s->lay.off_s[c] = s->lay.off_alt[c]; s->lay.off_alt[c] = t; }
         s->t += 2;

@@ -33,6 +33,21 @@ def _equal(G, O, tag):
     assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo), (tag, Eg, Eo)
 
 
+@pytest.mark.parametrize("dims,rows,R,beta", [((2048, 40, 1), 0, 1, BETA_C), ((2048, 26, 1), 5, 2, 0.3), ((4096, 12, 1), 3, 1, 0.0)])
+def test_temporal_blocking_heat_bath(P, oracle, dims, rows, R, beta):
+    """the same kernel with the heat-bath rule: bit-exact against the oracle after pairs and odd counts"""
+    G = P.SpinSystem(dims, n=1, storage="int8", replicas=R, replica_streams=1, seed=SEED, rule="heatbath")
+    G.set_option(P.OPT_TEMPORAL_BLOCKING, 1)
+    G.set_option(P.OPT_TBLOCK_ROWS, rows)
+    O = oracle.System(dims, n=1, n_replicas=R, replica_streams=1, seed=SEED, rule=oracle.RULE_HEATBATH)
+    for n in (2, 3, 4):
+        l0 = G.launch_count
+        G.sweep(beta, n)
+        assert G.launch_count - l0 == n // 2 + 2 * (n % 2)
+        O.sweep(beta, n)
+        _equal(G, O, "after %d sweeps" % n)
+
+
 @pytest.mark.parametrize("dims,storage,rows,J,R,beta", [
     ((2048, 40, 1), "int8", 0, 1.0, 1, BETA_C),       # automatic stripe height
     ((2048, 38, 1), "int8", 7, 1.0, 1, BETA_C),       # ragged last stripe
