@@ -209,7 +209,7 @@ enum { SPIN_OPT_PLAIN_KERNELS = 0,
         * performance hint: results never depend on it. */
        SPIN_OPT_L2_PREFETCH = 2,
        /* A/B knob: 0 (default) = the tuned kernel of each family; 1 = the alternative kept beside it
-        * (+-J shared stream: the cooperative kernel, one CTA of replica-chunk warps per 32 quads, instead of one thread per quad and all replicas).  Results never
+        * (+-J shared stream: one thread per quad and all replicas, instead of the cooperative kernel with one CTA of replica-chunk warps per 32 quads).  Results never
         * depend on it. */
        SPIN_OPT_KERNEL_VARIANT = 3,
        /* Exact temporal blocking ("k updates per tile load", made results-neutral): spin_sweep
@@ -220,7 +220,12 @@ enum { SPIN_OPT_PLAIN_KERNELS = 0,
         * 1 = on wherever offered. */
        SPIN_OPT_TEMPORAL_BLOCKING = 4,
        /* rows per stripe of the temporal-blocking kernel; 0 (default) = one wave of resident CTAs */
-       SPIN_OPT_TBLOCK_ROWS = 5 };
+       SPIN_OPT_TBLOCK_ROWS = 5,
+       /* L2 eviction priorities of the +-J quad kernel (createpolicy / ld.global.L2::cache_hint): the spins and the coupling
+        * words of `value` replicas are kept in L2 from half-sweep to half-sweep ("evict_last"), the other coupling words are
+        * streamed ("evict_first").  -1 (default) = as many replicas as fit in two thirds of L2 when the working set exceeds
+        * L2, -2 = no hints.  A pure performance hint. */
+       SPIN_OPT_L2_KEEP = 6 };
 spin_status spin_set_option(spin_system *s, int32_t option, int64_t value);
 
 /* Frees the handle only; never the workspace. */

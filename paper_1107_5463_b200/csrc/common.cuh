@@ -45,6 +45,37 @@ __device__ __forceinline__ void l2_prefetch_bulk(const void *p, uint32_t bytes) 
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
+// L2 eviction-priority hints (createpolicy + ld.global.L2::cache_hint): data that the next half-sweep reads again is loaded
+// "evict_last", data that is streamed once per half-sweep "evict_first", so that a working set a little larger than L2 keeps its
+// reusable part resident instead of thrashing the whole cache.
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint4 ldg_hint(const uint4 *ptr, uint64_t policy) {
+    uint4 v;
+    asm volatile("ld.global.nc.L2::cache_hint.v4.u32 {%0, %1, %2, %3}, [%4], %5;"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(ptr), "l"(policy));
+    return v;
+}
+
+__device__ __forceinline__ uint4 ld_hint(const uint4 *ptr, uint64_t policy) {   // coherent load (array written by the kernel)
+    uint4 v;
+    asm volatile("ld.global.L2::cache_hint.v4.u32 {%0, %1, %2, %3}, [%4], %5;"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(ptr), "l"(policy) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_hint(uint4 *ptr, const uint4 &v, uint64_t policy) {
+    asm volatile("st.global.L2::cache_hint.v4.u32 [%0], {%1, %2, %3, %4}, %5;"
+                 ::"l"(ptr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(policy) : "memory");
+}
+
 // ---------------------------------------------------------------------------------------------
 // Division by a run-time constant fixed at handle creation: q = (n * mul) >> (32 + shift) for
 // n < 2^31 (round-up method).  Two instructions instead of ~20.

@@ -27,6 +27,7 @@ struct IsingArgs {
     HeatBathTable hb;       // filled when rule = 1
     void *alt[2];           // temporal blocking (ising_tblock_kernel.cuh): the second pair of colour arrays it writes to
     uint32_t tb_rows;       // temporal blocking: rows per stripe
+    uint32_t l2_keep;       // +-J quad kernel: replicas whose coupling words are loaded "evict_last" (0xFFFFFFFF: no L2 hints)
     uint32_t prefetch;      // L2 prefetch distance (0 = off): replicas ahead (+-J quad kernel) / CTAs ahead (strip kernels)
 };
 
@@ -474,12 +475,31 @@ __device__ __forceinline__ void pmj_quad_replica(const IsingArgs &a, const QuadG
     uint4 *Sc = (uint4 *)a.s[a.colour] + (size_t)r * NW4;
     const uint4 *__restrict__ Bo = (const uint4 *)a.bonds + ((size_t)(a.colour * a.R + r) * 3) * NW4;   // own forward bonds
     const uint4 *__restrict__ Bt = (const uint4 *)a.bonds + ((size_t)(oc * a.R + r) * 3) * NW4;         // other colour's
-    const uint4 raw = Sc[me];   // plain load: this array is written by the kernel
-    const uint4 o = __ldg(So + me), ym = __ldg(So + k.q_ym), yp = __ldg(So + k.q_yp);
-    const uint4 zm = D == 3 ? __ldg(So + k.q_zm) : zero, zp = D == 3 ? __ldg(So + k.q_zp) : zero;
-    const uint4 bx_own = __ldg(Bo + me), bx_oth = __ldg(Bt + me);
-    const uint4 by_m = __ldg(Bt + NW4 + k.q_ym), by_own = __ldg(Bo + NW4 + me);
-    const uint4 bz_m = D == 3 ? __ldg(Bt + 2 * (size_t)NW4 + k.q_zm) : zero, bz_own = D == 3 ? __ldg(Bo + 2 * (size_t)NW4 + me) : zero;
+    uint4 raw, o, ym, yp, zm = zero, zp = zero, bx_own, bx_oth, by_m, by_own, bz_m = zero, bz_own = zero;
+    const bool hints = a.l2_keep != 0xFFFFFFFFu;
+    uint64_t keep = 0;
+    if (hints) {
+        // L2 eviction priorities: the working set (spins + coupling words of all replicas) is a little larger
+        // than L2, and a cyclic pass over it would evict every line before its reuse.  The spins and the coupling words of the
+        // first l2_keep replicas are loaded (and the spins stored) "evict_last", the other coupling words "evict_first": the
+        // first part stays resident from half-sweep to half-sweep, only the second streams from HBM.
+        keep = l2_policy_evict_last();
+        const uint64_t stream = l2_policy_evict_first();
+        const uint64_t pb = r < a.l2_keep ? keep : stream;
+        raw = ld_hint(Sc + me, keep);
+        o = ldg_hint(So + me, keep); ym = ldg_hint(So + k.q_ym, keep); yp = ldg_hint(So + k.q_yp, keep);
+        if (D == 3) { zm = ldg_hint(So + k.q_zm, keep); zp = ldg_hint(So + k.q_zp, keep); }
+        bx_own = ldg_hint(Bo + me, pb); bx_oth = ldg_hint(Bt + me, pb);
+        by_m = ldg_hint(Bt + NW4 + k.q_ym, pb); by_own = ldg_hint(Bo + NW4 + me, pb);
+        if (D == 3) { bz_m = ldg_hint(Bt + 2 * (size_t)NW4 + k.q_zm, pb); bz_own = ldg_hint(Bo + 2 * (size_t)NW4 + me, pb); }
+    } else {
+        raw = Sc[me];   // plain load: this array is written by the kernel
+        o = __ldg(So + me); ym = __ldg(So + k.q_ym); yp = __ldg(So + k.q_yp);
+        if (D == 3) { zm = __ldg(So + k.q_zm); zp = __ldg(So + k.q_zp); }
+        bx_own = __ldg(Bo + me); bx_oth = __ldg(Bt + me);
+        by_m = __ldg(Bt + NW4 + k.q_ym); by_own = __ldg(Bo + NW4 + me);
+        if (D == 3) { bz_m = __ldg(Bt + 2 * (size_t)NW4 + k.q_zm); bz_own = __ldg(Bo + 2 * (size_t)NW4 + me); }
+    }
     // the neighbour word outside the quad and (p = 0 only) its forward x coupling; inside the quad when QX == 1
     uint32_t o_edge, b_edge = 0u;
     if (k.QX == 1u) { o_edge = p ? o.x : o.w; b_edge = bx_oth.w; }
@@ -523,7 +543,8 @@ __device__ __forceinline__ void pmj_quad_replica(const IsingArgs &a, const QuadG
         }
         if (MEAS) fused_word_sums<D>(av, rw, out[i], oi, e_sum, m_sum);
     }
-    Sc[me] = make_uint4(out[0], out[1], out[2], out[3]);
+    if (hints) st_hint(Sc + me, make_uint4(out[0], out[1], out[2], out[3]), keep);
+    else Sc[me] = make_uint4(out[0], out[1], out[2], out[3]);
     if (MEAS) {
         // all live lanes of the warp are at replica r: one reduction, one atomic pair per warp
         const unsigned act = __activemask();
@@ -553,7 +574,7 @@ __device__ __forceinline__ void pmj_quad_prefetch(const IsingArgs &a, uint32_t r
 }
 
 // One thread per quad; the thread builds the masks of its four words and loops over the replicas of its chunk
-// (blockIdx.y).  Kept for rows of fewer than 32 quads per CTA column and as the A/B partner of the cooperative kernel.
+// (blockIdx.y).  The A/B partner of the cooperative kernel below (SPIN_OPT_KERNEL_VARIANT = 1).
 template <int D, bool HB, bool MEAS = false>
 __global__ void __launch_bounds__(128) ising_pmj_quad_halfsweep(const __grid_constant__ IsingArgs a) {
     constexpr int NT = HB ? 2 * D + 1 : D;
@@ -583,7 +604,7 @@ __global__ void __launch_bounds__(128) ising_pmj_quad_halfsweep(const __grid_con
 // quads (one per lane: coalesced 512-byte accesses) for the replicas of chunk c, reading the masks from shared memory.
 // Against the one-thread-per-quad kernel the Philox work per thread is 1 / 4 (the total is unchanged), the replica loop is
 // CH times shorter and CH times more warps keep loads in flight; CTAs in different phases overlap on an SM.
-template <int D, bool HB>
+template <int D, bool HB, bool MEAS = false>
 __global__ void __launch_bounds__(256) ising_pmj_quad_coop_halfsweep(const __grid_constant__ IsingArgs a) {
     constexpr int NT = HB ? 2 * D + 1 : D;
     __shared__ __align__(16) uint32_t sm_lt[NT][128];   // [threshold][word of the CTA's 32 quads]
@@ -616,7 +637,7 @@ __global__ void __launch_bounds__(256) ising_pmj_quad_coop_halfsweep(const __gri
     }
     for (uint32_t r = r0; r < r1; ++r) {
         if (a.prefetch && lane == 0u && r + a.prefetch < r1 && k.NW4 >= 32u) pmj_quad_prefetch<D>(a, r + a.prefetch, me0, pf_bytes, pf_ym, pf_zm, k.NW4);
-        pmj_quad_replica<D, HB, NT>(a, k, r, ltf);
+        pmj_quad_replica<D, HB, NT, MEAS>(a, k, r, ltf);
     }
 }
 

@@ -74,6 +74,8 @@ struct spin_system {
     int tblock_rows;     // SPIN_OPT_TBLOCK_ROWS: rows per stripe, 0 = one wave of resident CTAs
     int tblock_ok;       // this handle has the second pair of arrays
     int variant;         // SPIN_OPT_KERNEL_VARIANT: 0 = the default kernel of each family, > 0 = a named alternative (A/B knob)
+    int l2_keep;         // SPIN_OPT_L2_KEEP: -1 automatic, -2 no L2 eviction hints, >= 0 replicas whose coupling words are kept in L2
+    int l2_bytes;        // L2 size of the device
     int l2_prefetch;     // SPIN_OPT_L2_PREFETCH: -1 each kernel's own distance (default), 0 off, > 0 that distance
     int grid_num, grid_den;
     uint32_t mblocks;    // CTAs (per replica) of the measurement kernels
@@ -346,6 +348,17 @@ static IsingArgs ising_args(const spin_system *s) {
     a.hb = s->hb;
     a.acc = (long long *)(s->ws + s->lay.off_acc);
     a.acc_slots = acc_slots_for(s->R);
+    // +-J quad kernel: L2 eviction hints when spins + coupling words do not fit in L2 anyway: keep the spins and the coupling words
+    // of as many replicas as fit in two thirds of L2 (measured at 256^3 x 16: 4 .. 8 replicas 28.8 us, 0 30.8, 12 32.4, no hints 32.9)
+    a.l2_keep = 0xFFFFFFFFu;
+    if (s->l2_keep >= 0) a.l2_keep = (uint32_t)s->l2_keep;
+    else if (s->l2_keep == -1 && s->lay.bytes_bonds && s->l2_bytes > 0) {
+        const double budget = 0.66 * (double)s->l2_bytes, spins = 2.0 * (double)s->lay.bytes_s, per_rep = (double)s->lay.bytes_bonds / s->R;
+        if (spins + (double)s->lay.bytes_bonds > 0.6 * (double)s->l2_bytes && spins < budget) {
+            double k = (budget - spins) / per_rep;
+            a.l2_keep = k >= (double)s->R ? s->R : (uint32_t)k;
+        }
+    }
     a.alt[0] = s->ws + s->lay.off_alt[0];
     a.alt[1] = s->ws + s->lay.off_alt[1];
     a.tb_rows = 0;
@@ -472,14 +485,19 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
         // 35.2 / 37.1 / 35.2 / 47.4 / 78.1 us for 1 / 2 / 4 / 8 / 16 replica chunks), else chunks of >= 4 replicas
         const uint64_t quads = (uint64_t)s->g.NW / 4;
         const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
-        if (s->variant == 1 && s->R >= 2) {
-            // cooperative kernel (A/B partner, same speed on B200: profiles/r02_pmj_diagnostics.md): a CTA of CH warps per 32 quads, warp c serves replica chunk c
-            int CH = s->block / 32;
+        if (s->variant != 1 && s->R >= 2) {
+            // cooperative kernel (default; with the L2 eviction hints 26.8 vs 28.8 us at 256^3 x 16, and faster on small lattices):
+            // a CTA of CH warps per 32 quads, warp c serves replica chunk c
+            int CH = (s->block > 128 ? 128 : s->block) / 32;
             while (CH > 1 && (uint32_t)CH > s->R) CH /= 2;
             const dim3 G((unsigned)((quads + 31) / 32));
             const int Bc = 32 * CH;
-            if (s->d == 2) { if (hb) ising_pmj_quad_coop_halfsweep<2, true><<<G, Bc, 0, st>>>(a); else ising_pmj_quad_coop_halfsweep<2, false><<<G, Bc, 0, st>>>(a); }
-            else { if (hb) ising_pmj_quad_coop_halfsweep<3, true><<<G, Bc, 0, st>>>(a); else ising_pmj_quad_coop_halfsweep<3, false><<<G, Bc, 0, st>>>(a); }
+            const bool meas = fused && a.colour == 1u;   // row a7: E and M from the bond masks of the colour-1 half-sweep
+            if (meas) *fused = true;
+#define PC(D_, HB_) do { if (meas) ising_pmj_quad_coop_halfsweep<D_, HB_, true><<<G, Bc, 0, st>>>(a); else ising_pmj_quad_coop_halfsweep<D_, HB_, false><<<G, Bc, 0, st>>>(a); } while (0)
+            if (s->d == 2) { if (hb) PC(2, true); else PC(2, false); }
+            else { if (hb) PC(3, true); else PC(3, false); }
+#undef PC
         } else {
         const int Bq = s->block < 128 ? s->block : 128;
         unsigned Gy = 1;
@@ -1012,7 +1030,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
     s->tma_ok = 0; s->use_tma = -1; s->tma_ty = 0;
     s->t = 0; s->launches = 0; s->staging = nullptr; s->staging_bytes = 0; s->set_pending = 0; s->h_res = nullptr; s->gexec = nullptr; s->cap_stream = nullptr; s->gnodes = nullptr; s->n_gnodes = 0;
     // 128 threads per CTA for the Ising fast paths (measured: +-J R = 16 39.1 vs 40.4 us with 256)
-    s->block = (dv.path == PATH_ISING_INT8 || dv.path == PATH_ISING_BITPACK || dv.path == PATH_ISING_MSC) ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0; s->l2_prefetch = -1; s->variant = 0; s->tblock = -1; s->tblock_rows = 0; s->tblock_ok = tblock_offered(cfg, dv) ? 1 : 0;
+    s->block = (dv.path == PATH_ISING_INT8 || dv.path == PATH_ISING_BITPACK || dv.path == PATH_ISING_MSC) ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0; s->l2_prefetch = -1; s->l2_keep = -1; s->l2_bytes = 0; s->variant = 0; s->tblock = -1; s->tblock_rows = 0; s->tblock_ok = tblock_offered(cfg, dv) ? 1 : 0;
     s->table_beta = std::nan("");
     Geometry &g = s->g;
     g.Lx = dv.pad[0]; g.Ly = dv.pad[1]; g.Lz = dv.pad[2]; g.d = dv.d;
@@ -1046,7 +1064,8 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
     cudaError_t e;
     int dev = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess ||
-        (e = cudaDeviceGetAttribute(&s->sm_count, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) {
+        (e = cudaDeviceGetAttribute(&s->sm_count, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess ||
+        (e = cudaDeviceGetAttribute(&s->l2_bytes, cudaDevAttrL2CacheSize, dev)) != cudaSuccess) {
         delete s;
         return fail(SPIN_ERR_CUDA, "no usable CUDA device: %s", cudaGetErrorString(e));
     }
@@ -1654,6 +1673,12 @@ spin_status spin_set_option(spin_system *s, int32_t option, int64_t value) {
     if (option == SPIN_OPT_TBLOCK_ROWS) {
         if (value < 0 || value > (1 << 24)) return fail(SPIN_ERR_INVALID_ARG, "SPIN_OPT_TBLOCK_ROWS takes 0 (automatic) or a number of rows");
         s->tblock_rows = (int)value;
+        return SPIN_OK;
+    }
+    if (option == SPIN_OPT_L2_KEEP) {
+        if (value < -2 || value > 65535) return fail(SPIN_ERR_INVALID_ARG, "SPIN_OPT_L2_KEEP takes -2 (no hints), -1 (automatic) or a number of replicas");
+        s->l2_keep = (int)value;
+        graph_drop(s);
         return SPIN_OK;
     }
     if (option == SPIN_OPT_KERNEL_VARIANT) {
