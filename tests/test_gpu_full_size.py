@@ -207,14 +207,17 @@ def test_full_size_vector_models(P, oracle, name):
 
 
 @pytest.mark.parametrize("name", ["ising2d_L16384_int8", "ising2d_L16384_bitpack", "ising3d_L512_bitpack",
-                                  "ea3d_L256_R16_bitpack"])
+                                  "ea3d_L256_R16_bitpack", "ea3d_L256_R16_bitpack_ownstreams"])
 def test_whole_lattice_two_sweeps_against_the_oracle(P, name):
     """SURVEY 8(c) protocol at full size: every byte of spin_get_spins equals the oracle's configuration after two full
     sweeps of the BASELINE lattice (2.7e8 updates per sweep, about 9 s each for the single-threaded oracle), in the
     launch configuration bench.py times -- for config 2 that is ONE launch of the temporal-blocking kernel (f3)."""
     import oracle
 
-    w = P.workloads.WORKLOADS[name]
+    own = name.endswith("_ownstreams")       # config 4 with the replica index in the Philox counter (ADVICE round 1)
+    w = dict(P.workloads.WORKLOADS[name[:-len("_ownstreams")] if own else name])
+    if own:
+        w["replica_streams"] = 1
     kinds = {"uniform": oracle.J_UNIFORM, "per_direction": oracle.J_PER_DIRECTION, "bond_pm1": oracle.J_BOND_PM1}
     G = P.from_workload(w, P.workloads.SEED)
     O = oracle.System(w["dims"], n=1, coupling_kind=kinds[w["coupling"]], J=w["J"], n_replicas=w["replicas"],
