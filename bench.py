@@ -36,7 +36,7 @@ DEFAULT_WORKLOAD = "ising2d_L16384_int8"
 # per-model legs of the default run: (workload, sweeps timed)
 PER_MODEL = [("ising2d_L64_int8", 1000), ("ising2d_L16384_bitpack", 40), ("ising3d_L512_bitpack", 40),
              ("ea3d_L256_R16_bitpack", 40), ("ea3d_L256_R16_bitpack_ownstreams", 20), ("ea2d_L64_R4096_bitpack", 200),
-             ("ea2d_L32_R131072_msc", 100), ("heisenberg3d_L256_fp32", 20), ("xy3d_L256_fp32", 20)]
+             ("ea2d_L32_R131072_msc", 100), ("heisenberg3d_L256_fp32", 20), ("heisenberg2d_L4096_fp32", 20), ("xy3d_L256_fp32", 20)]
 RECORDED = ("ising2d_L16384_bitpack", "ea3d_L256_R16_bitpack", "heisenberg3d_L256_fp32", "xy3d_L256_fp32")
 DTYPE = {"int8": "u8", "bitpack": "u32 (bit-packed, 32 spins per word)", "fp32": "f32",
          "msc": "u32 (bit-packed, 32 realisations of one site per word)"}

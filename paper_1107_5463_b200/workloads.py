@@ -30,6 +30,9 @@ WORKLOADS = {
     # extra: 3D XY (named by north_star, absent from the configs)
     "xy3d_L256_fp32": dict(dims=(256, 256, 256), n=2, storage="fp32", coupling="uniform", J=(1.0, 1.0, 1.0),
                            beta=0.4542, sweeps=500, replicas=1, replica_streams=0, record=False),
+    # extra (SURVEY 8(d) 5''): the paper's own continuous-spin workload, 2D Heisenberg L = 4096 (Table 1)
+    "heisenberg2d_L4096_fp32": dict(dims=(4096, 4096, 1), n=3, storage="fp32", coupling="uniform", J=(1.0, 1.0, 1.0),
+                                    beta=0.693, sweeps=500, replicas=1, replica_streams=0, record=False),
     # extra: the shape of the paper's fastest Metropolis row (Table 1: 2D +-J, many
     # realisations, multi-spin coded, one random number per site for all realisations); L = 64 is the smallest
     # lattice the bit-packed layout takes (the paper used L = 32)
@@ -52,6 +55,7 @@ BYTES_PER_UPDATE = {
     "ea2d_L64_R4096_bitpack": 0.875,   # 3 spin bits + 2 forward bonds from each end = 7 bits
     "ea2d_L32_R131072_msc": 0.875,
     "heisenberg3d_L256_fp32": 36.0,
+    "heisenberg2d_L4096_fp32": 36.0,
     "xy3d_L256_fp32": 24.0,
 }
 
