@@ -24,10 +24,10 @@ namespace spin {
 
 constexpr int TB_RING = 16;          // ring slots (rows) per colour; 10 are live
 constexpr int TB_QCAP = 128;         // deferred-tail queue entries per warp and iteration: 4 half-sweeps x 32 lanes, it cannot overflow
-constexpr int TB_QFIELDS = 5;        // unit, sweep offset | colour, eq, m[0], index of the word in the ring
+constexpr int TB_QFIELDS = 4;        // one uint4 per entry: unit, eq, m[0], index of the word in the ring | (sweep offset, colour) << 30
 
 __host__ __device__ constexpr size_t tblock_smem_bytes(uint32_t WX) {
-    return (size_t)(2u * TB_RING * WX + (WX / 32u) * (1u + TB_QFIELDS * TB_QCAP)) * 4u;
+    return (size_t)(2u * TB_RING * WX + (WX / 32u) * (4u + TB_QFIELDS * TB_QCAP)) * 4u;
 }
 
 // INT8: global arrays in the int8 fast layout (32-byte units), else bit-packed words.  grid = (stripes, R),
@@ -40,8 +40,8 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) ising_tblock2_sweep
     const Geometry &g = a.g;
     const uint32_t WX = g.WX, Ly = (uint32_t)g.Ly, w = threadIdx.x, r = blockIdx.y;
     const uint32_t warp = w >> 5, lane = w & 31u;
-    uint32_t *const qn = tb_smem + 2u * TB_RING * WX + warp * (1u + TB_QFIELDS * TB_QCAP);   // this warp's queue: count, fields
-    uint32_t *const qf = qn + 1;
+    uint32_t *const qn = tb_smem + 2u * TB_RING * WX + warp * (4u + TB_QFIELDS * TB_QCAP);   // this warp's queue: count (16 bytes), entries
+    uint32_t *const qf = qn + 4;
     const uint32_t H = a.tb_rows, y0 = blockIdx.x * H;
     if (y0 >= Ly) return;
     const int Hs = (int)min(H, Ly - y0);
@@ -58,6 +58,9 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) ising_tblock2_sweep
 #pragma unroll
     for (int s = 0; s < 4; ++s) y_st[s] = (y_in + 8u * Ly - 2u * (uint32_t)(s + 1)) % Ly;
     if (lane == 0u) *qn = 0u;
+    // the other colour's words of rows l and l + 1 of each half-sweep, kept for the next iteration (where they are rows l - 1 and l):
+    // both were final when they were read, so in the steady state a half-sweep loads one new row instead of three
+    uint32_t roll_prev[4] = {0u, 0u, 0u, 0u}, roll_cur[4] = {0u, 0u, 0u, 0u};
     for (int i = 0; i <= Hs + 11; ++i) {
         // ---- the loads of local row i, consumed at the end of the iteration
         const bool loading = i <= Hs + 7;
@@ -70,15 +73,17 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) ising_tblock2_sweep
         }
         // ---- half-sweeps 1 .. 4 on local rows i - 2, i - 4, i - 6, i - 8.  In the steady state (all four rows inside their
         // ranges) the four updates are straight-line code, so that the scheduler can interleave their Philox chains
-        const auto half_sweep = [&](int s) {
+        const auto half_sweep = [&](int s, bool rolled) {
             const int l = i - 2 * s;
             const uint32_t c = (uint32_t)(s - 1) & 1u, tt = a.t + (uint32_t)(s > 2), y = y_st[s - 1];
             uint32_t *const mine_r = tb_smem + c * (TB_RING * WX);
             const uint32_t *const oth_r = tb_smem + (1u - c) * (TB_RING * WX);
             const uint32_t slot = ((uint32_t)l & (TB_RING - 1u)) * WX;
-            const uint32_t raw = mine_r[slot + w], o_cur = oth_r[slot + w];
-            const uint32_t o_prev = oth_r[(((uint32_t)l - 1u) & (TB_RING - 1u)) * WX + w];
+            const uint32_t raw = mine_r[slot + w];
+            const uint32_t o_cur = rolled ? roll_cur[s - 1] : oth_r[slot + w];
+            const uint32_t o_prev = rolled ? roll_prev[s - 1] : oth_r[(((uint32_t)l - 1u) & (TB_RING - 1u)) * WX + w];
             const uint32_t o_next = oth_r[(((uint32_t)l + 1u) & (TB_RING - 1u)) * WX + w];
+            roll_prev[s - 1] = o_cur; roll_cur[s - 1] = o_next;
             const uint32_t p = (y + c) & 1u;
             const uint32_t o_side = oth_r[slot + (p ? w_next : w_prev)];
             const uint32_t side = p ? ((o_cur >> 1) | (o_side << 31)) : ((o_cur << 1) | (o_side >> 31));
@@ -95,18 +100,18 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) ising_tblock2_sweep
             mine_r[slot + w] = fresh;
             if (eq != 0u) {
                 const uint32_t pos = atomicAdd(qn, 1u);   // < TB_QCAP: at most 4 x 32 pushes per warp and iteration
-                qf[0 * TB_QCAP + pos] = unit; qf[1 * TB_QCAP + pos] = 2u * (uint32_t)(s > 2) + c; qf[2 * TB_QCAP + pos] = eq;
-                qf[3 * TB_QCAP + pos] = mm[0]; qf[4 * TB_QCAP + pos] = c * (TB_RING * WX) + slot + w;
+                ((uint4 *)qf)[pos] = make_uint4(unit, eq, mm[0], (c * (TB_RING * WX) + slot + w) | ((2u * (uint32_t)(s > 2) + c) << 30));
             }
         };
         if (i >= 12 && i <= Hs + 8) {
-            half_sweep(1); half_sweep(2); half_sweep(3); half_sweep(4);
+            const bool rolled = i > 12;   // the iteration before ran all four half-sweeps as well
+            half_sweep(1, rolled); half_sweep(2, rolled); half_sweep(3, rolled); half_sweep(4, rolled);
         } else {
 #pragma unroll 1
             for (int s = 1; s <= 4; ++s) {
                 const int l = i - 2 * s;
                 if (l >= s && l <= Hs + 7 - s) {
-                    if (s == 1) half_sweep(1); else if (s == 2) half_sweep(2); else if (s == 3) half_sweep(3); else half_sweep(4);
+                    if (s == 1) half_sweep(1, false); else if (s == 2) half_sweep(2, false); else if (s == 3) half_sweep(3, false); else half_sweep(4, false);
                 }
             }
         }
@@ -115,11 +120,12 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) ising_tblock2_sweep
         {
             const uint32_t nq = *qn;
             for (uint32_t e = lane; e < nq; e += 32u) {
+                const uint4 q = ((const uint4 *)qf)[e];
                 uint32_t mm[2];
-                mm[0] = qf[3 * TB_QCAP + e]; mm[1] = 0u;
-                const uint32_t tc = qf[1 * TB_QCAP + e];
-                const uint32_t lt = lt_mask_select_tail<2>(a, a.t + (tc >> 1), tc & 1u, qf[0 * TB_QCAP + e], rho, mm, qf[2 * TB_QCAP + e]);
-                tb_smem[qf[4 * TB_QCAP + e]] ^= lt;
+                mm[0] = q.z; mm[1] = 0u;
+                const uint32_t tc = q.w >> 30;
+                const uint32_t lt = lt_mask_select_tail<2>(a, a.t + (tc >> 1), tc & 1u, q.x, rho, mm, q.y);
+                tb_smem[q.w & 0x3FFFFFFFu] ^= lt;
             }
             __syncwarp();
             if (lane == 0u) *qn = 0u;
