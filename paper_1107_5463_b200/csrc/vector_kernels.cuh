@@ -204,6 +204,11 @@ __device__ __forceinline__ float add_nb(float h, float J, float s) {
 __device__ __forceinline__ float2 f2(float a, float b) { return make_float2(a, b); }
 __device__ __forceinline__ float2 f2s(float a) { return make_float2(a, a); }
 __device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
+// A product that feeds a sum directly: ptxas contracts mul.rn.f32x2 + add.rn.f32x2 into one FFMA2 (measured: CUDA 12.9,
+// sm_100a; the scalar _rn intrinsics are never contracted), which would round once instead of twice.  Two scalar products
+// feeding a packed sum are not contracted, so where the contract (R-14) wants product and sum rounded separately
+// the product is taken with this helper.
+__device__ __forceinline__ float2 mul2s(float2 a, float2 b) { return make_float2(__fmul_rn(a.x, b.x), __fmul_rn(a.y, b.y)); }
 
 // sincospi_u24 for two sites at once: integer range reduction per site, the two polynomials packed
 __device__ __forceinline__ void sincospi_u24_x2(uint32_t wa, uint32_t wb, float2 *sn, float2 *cs) {
@@ -231,7 +236,7 @@ __device__ __forceinline__ void sincospi_u24_x2(uint32_t wa, uint32_t wb, float2
 __device__ __forceinline__ void direction3_x2(uint32_t w0a, uint32_t w1a, uint32_t w0b, uint32_t w1b, float2 out[3]) {
     // z = 2 u24(w) - 1 = k 2^-23 - 1 with k < 2^24: product and difference are exact, so one fma gives the same float
     const float2 z = __ffma2_rn(f2((float)(w0a >> 8), (float)(w0b >> 8)), f2s(1.1920928955078125e-07f), f2s(-1.0f));
-    const float2 om = __fadd2_rn(f2s(1.0f), neg2(__fmul2_rn(z, z)));
+    const float2 om = __fadd2_rn(f2s(1.0f), neg2(mul2s(z, z)));
     const float2 rho = f2(__fsqrt_rn(fmaxf(om.x, 0.0f)), __fsqrt_rn(fmaxf(om.y, 0.0f)));
     float2 sn, cs;
     sincospi_u24_x2(w1a, w1b, &sn, &cs);
@@ -246,9 +251,47 @@ __device__ __forceinline__ void direction2_x2(uint32_t w0a, uint32_t w0b, float2
     out[1] = sn;
 }
 
+// heatbath3 for two sites at once (site a in .x, site b in .y; h[c] = component c of both fields): the plain products and
+// sums are packed (each half is the scalar operation of heatbath3, in the same order: bit-identical), the square roots,
+// divisions, expf, logf stay scalar.  A zero field (H = 0) falls back to the uniform direction, per site.
+__device__ __forceinline__ void heatbath3_x2(float beta, const float2 h[3], uint32_t w0a, uint32_t w1a, uint32_t w0b, uint32_t w1b,
+                                             float2 out[3]) {
+    const float2 hh = __fadd2_rn(__fadd2_rn(mul2s(h[0], h[0]), mul2s(h[1], h[1])), mul2s(h[2], h[2]));
+    const float2 hn = f2(__fsqrt_rn(hh.x), __fsqrt_rn(hh.y));
+    const float2 H = __fmul2_rn(f2s(beta), hn);
+    const float2 u = __fmul2_rn(f2((float)(w0a >> 8), (float)(w0b >> 8)), f2s(5.9604644775390625e-08f));
+    const float2 m2H = __fmul2_rn(f2s(-2.0f), H);
+    const float2 e2H = f2(expf(m2H.x), expf(m2H.y));
+    const float2 arg = __fadd2_rn(f2s(1.0f), neg2(mul2s(u, __fadd2_rn(f2s(1.0f), neg2(e2H)))));
+    float2 c = __fadd2_rn(f2s(1.0f), f2(__fdiv_rn(logf(arg.x), H.x), __fdiv_rn(logf(arg.y), H.y)));
+    c = f2(fminf(fmaxf(c.x, -1.0f), 1.0f), fminf(fmaxf(c.y, -1.0f), 1.0f));
+    const float2 omc = __fadd2_rn(f2s(1.0f), neg2(mul2s(c, c)));
+    const float2 st = f2(__fsqrt_rn(fmaxf(omc.x, 0.0f)), __fsqrt_rn(fmaxf(omc.y, 0.0f)));
+    float2 sp, cp;
+    sincospi_u24_x2(w1a, w1b, &sp, &cp);
+    const float2 inv = f2(__fdiv_rn(1.0f, hn.x), __fdiv_rn(1.0f, hn.y));
+    const float2 x = __fmul2_rn(h[0], inv), y = __fmul2_rn(h[1], inv), z = __fmul2_rn(h[2], inv);
+    const float2 sg = f2(signbit(z.x) ? -1.0f : 1.0f, signbit(z.y) ? -1.0f : 1.0f);
+    const float2 sz = __fadd2_rn(sg, z);
+    const float2 a = f2(__fdiv_rn(-1.0f, sz.x), __fdiv_rn(-1.0f, sz.y));
+    const float2 b = __fmul2_rn(__fmul2_rn(x, y), a);
+    const float2 e1[3] = {__fadd2_rn(f2s(1.0f), mul2s(__fmul2_rn(sg, __fmul2_rn(x, x)), a)), __fmul2_rn(sg, b), __fmul2_rn(neg2(sg), x)};
+    const float2 e2[3] = {b, __fadd2_rn(sg, mul2s(__fmul2_rn(y, y), a)), neg2(y)};
+    const float2 fa = __fmul2_rn(st, cp), fb = __fmul2_rn(st, sp);
+    const float2 hk[3] = {x, y, z};
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+        out[k] = __fadd2_rn(__fadd2_rn(mul2s(fa, e1[k]), mul2s(fb, e2[k])), mul2s(c, hk[k]));
+    if (!(H.x > 0.0f) || !(H.y > 0.0f)) {
+        float d[3];
+        if (!(H.x > 0.0f)) { direction3(w0a, w1a, d); out[0].x = d[0]; out[1].x = d[1]; out[2].x = d[2]; }
+        if (!(H.y > 0.0f)) { direction3(w0b, w1b, d); out[0].y = d[0]; out[1].y = d[1]; out[2].y = d[2]; }
+    }
+}
+
 template <bool UNITJ>
 __device__ __forceinline__ float2 add_nb2(float2 h, float J, float sa, float sb) {
-    return UNITJ ? __fadd2_rn(h, f2(sa, sb)) : __fadd2_rn(h, __fmul2_rn(f2s(J), f2(sa, sb)));
+    return UNITJ ? __fadd2_rn(h, f2(sa, sb)) : __fadd2_rn(h, mul2s(f2s(J), f2(sa, sb)));
 }
 
 // The update of one quad of 4 consecutive same-colour sites of a row, shared by the strip kernel and the TMA-staged
@@ -270,9 +313,9 @@ __device__ __forceinline__ void vector_quad_field(float Jx, float Jy, float Jz, 
         const float4 o = o_cur.c[c];
         const float4 sh = p ? make_float4(o.y, o.z, o.w, side[c]) : make_float4(side[c], o.x, o.y, o.z);
         float2 v01 = UNITJ ? __fadd2_rn(f2(o.x, o.y), f2(sh.x, sh.y))
-                           : __fadd2_rn(__fmul2_rn(f2s(Jx), f2(o.x, o.y)), __fmul2_rn(f2s(Jx), f2(sh.x, sh.y)));
+                           : __fadd2_rn(mul2s(f2s(Jx), f2(o.x, o.y)), mul2s(f2s(Jx), f2(sh.x, sh.y)));
         float2 v23 = UNITJ ? __fadd2_rn(f2(o.z, o.w), f2(sh.z, sh.w))
-                           : __fadd2_rn(__fmul2_rn(f2s(Jx), f2(o.z, o.w)), __fmul2_rn(f2s(Jx), f2(sh.z, sh.w)));
+                           : __fadd2_rn(mul2s(f2s(Jx), f2(o.z, o.w)), mul2s(f2s(Jx), f2(sh.z, sh.w)));
         v01 = add_nb2<UNITJ>(v01, Jy, o_prev.c[c].x, o_prev.c[c].y);
         v23 = add_nb2<UNITJ>(v23, Jy, o_prev.c[c].z, o_prev.c[c].w);
         v01 = add_nb2<UNITJ>(v01, Jy, o_next.c[c].x, o_next.c[c].y);
@@ -298,7 +341,7 @@ __device__ __forceinline__ void vector_quad_accept(const VectorArgs &a, const fl
     [[maybe_unused]] const auto add_energy = [&](int pr) {
         float2 dot = __fmul2_rn(f2(res[0][2 * pr], res[0][2 * pr + 1]), hp[pr][0]);
 #pragma unroll
-        for (int c = 1; c < NC; ++c) dot = __fadd2_rn(dot, __fmul2_rn(f2(res[c][2 * pr], res[c][2 * pr + 1]), hp[pr][c]));
+        for (int c = 1; c < NC; ++c) dot = __fadd2_rn(dot, mul2s(f2(res[c][2 * pr], res[c][2 * pr + 1]), hp[pr][c]));
         esum = __fadd_rn(__fadd_rn(esum, dot.x), dot.y);
     };
 #pragma unroll
@@ -307,12 +350,11 @@ __device__ __forceinline__ void vector_quad_accept(const VectorArgs &a, const fl
         philox4x32_10(ctr0 + 2 * pr, rho, a.t, tag, a.keys, wa);
         philox4x32_10(ctr0 + 2 * pr + 1, rho, a.t, tag, a.keys, wb);
         if (HB && NC == 3) {
-            float ha[3] = {hp[pr][0].x, hp[pr][1].x, hp[pr][NC - 1].x}, hb[3] = {hp[pr][0].y, hp[pr][1].y, hp[pr][NC - 1].y};
-            float sa[3], sb[3];
-            heatbath3(a.beta, ha, wa[0], wa[1], sa);
-            heatbath3(a.beta, hb, wb[0], wb[1], sb);
+            const float2 h3[3] = {hp[pr][0], hp[pr][1], hp[pr][NC - 1]};
+            float2 s3[3];
+            heatbath3_x2(a.beta, h3, wa[0], wa[1], wb[0], wb[1], s3);
 #pragma unroll
-            for (int c = 0; c < NC; ++c) { res[c][2 * pr] = sa[c]; res[c][2 * pr + 1] = sb[c]; }
+            for (int c = 0; c < NC; ++c) { res[c][2 * pr] = s3[c].x; res[c][2 * pr + 1] = s3[c].y; }
             if (MEAS) add_energy(pr);
             continue;
         }
@@ -325,7 +367,7 @@ __device__ __forceinline__ void vector_quad_accept(const VectorArgs &a, const fl
         // acc = (s' - s) . h = -dE; accept iff dE <= 0 (acc >= 0) or u < exp(-beta dE) = exp(beta acc)
         float2 acc = __fmul2_rn(__fadd2_rn(sn[0], neg2(so[0])), hp[pr][0]);
 #pragma unroll
-        for (int c = 1; c < NC; ++c) acc = __fadd2_rn(acc, __fmul2_rn(__fadd2_rn(sn[c], neg2(so[c])), hp[pr][c]));
+        for (int c = 1; c < NC; ++c) acc = __fadd2_rn(acc, mul2s(__fadd2_rn(sn[c], neg2(so[c])), hp[pr][c]));
         const float2 arg = __fmul2_rn(f2s(a.beta), acc);
         const bool acc_a = acc.x >= 0.0f || u24(wacc_a) < expf(arg.x);
         const bool acc_b = acc.y >= 0.0f || u24(wacc_b) < expf(arg.y);
