@@ -307,7 +307,9 @@ def test_vector_models_within_tolerance(P, oracle, n, dims, beta):
 
 
 @pytest.mark.parametrize("n,dims,J", [(3, (16, 6, 4), (1.0, 1.0, 1.0)), (2, (24, 10, 1), (1.0, 1.0, 1.0)),
-                                      (3, (8, 4, 2), (1.0, -1.0, 0.5)), (2, (8, 2, 6), (-1.0, -1.0, -1.0))])
+                                      (3, (8, 4, 2), (1.0, -1.0, 0.5)), (2, (8, 2, 6), (-1.0, -1.0, -1.0)),
+                                      # couplings whose products J s are inexact: a contracted multiply-add (one rounding) would show
+                                      (3, (16, 8, 6), (0.3, 0.7, -1.3)), (2, (16, 12, 1), (1.1, -0.9, 1.0))])
 def test_vector_strip_rows_and_plain_kernel_agree_bitwise(P, n, dims, J):
     """n >= 2: the strip kernel (quads of 4 sites, K = 1, 2, 4 rows per thread, several block sizes) and the plain
     one-thread-per-site kernel perform the same fp32 operations in the same order: identical bits."""
