@@ -111,6 +111,19 @@ spin_status spin_sweep(spin_system *s, double beta, int64_t n_sweeps, void *stre
  * Runs on `stream` and blocks until the result is on the host. */
 spin_status spin_measure(spin_system *s, double *E, double *M, void *stream);
 
+/* The same measurement for callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): E and M go to DEVICE doubles d_E[R], d_M[R*n] of the caller's, the call only enqueues work on
+ * `stream` (no synchronisation) and calls no cudaMalloc, cudaFree or other allocating routine.  The kernels' scratch
+ * (per-CTA partial sums, accumulator slots) lives in ONE array built into the library, SPIN_NOALLOC_SCRATCH_BYTES per
+ * GPU (held by every GPU that loads the library until the process exits).  A system that needs more --
+ * n = 1: 16 * min(64, 8192 / R rounded down to a power of two) * R bytes; n >= 2: up to 592 * 8 * (1 + n) * R bytes,
+ * i.e. beyond about 55 Heisenberg replicas -- is refused with SPIN_ERR_UNSUPPORTED (use spin_measure).
+ * Every call, of every handle, shares that array: calls that overlap on the GPU (different streams without ordering)
+ * race; calls on one stream are safe, and the array is cleared where a kernel needs zeros.  Values are identical to
+ * spin_measure's. */
+#define SPIN_NOALLOC_SCRATCH_BYTES (1 << 20)
+spin_status spin_measure_noalloc(spin_system *s, double *d_E, double *d_M, void *stream);
+
 /* One half-sweep (colour 0, then colour 1, alternating; the sweep counter advances after colour 1), enqueued on
  * `stream`.  For slab handles the caller exchanges halos in between: before the half-sweep of colour c every handle
  * needs its neighbours' boundary planes of colour 1 - c (spin_halo_get on the owner, spin_halo_put here). */

@@ -30,7 +30,7 @@ _COUPLING = {"uniform": J_UNIFORM, "per_direction": J_PER_DIRECTION, "bond_pm1":
 
 # every symbol include/spin.h declares
 SYMBOLS = [
-    "spin_workspace_bytes", "spin_create", "spin_sweep", "spin_measure", "spin_sweep_record", "spin_sweep_betas", "spin_get_spins",
+    "spin_workspace_bytes", "spin_create", "spin_sweep", "spin_measure", "spin_sweep_record", "spin_sweep_betas", "spin_measure_noalloc", "spin_get_spins",
     "spin_set_spins", "spin_get_spins_device", "spin_set_spins_device", "spin_set_spins_async", "spin_set_spins_status",
     "spin_set_spins_bits_async", "spin_get_spins_bits",
     "spin_get_bonds", "spin_get_sweep_count", "spin_set_sweep_count", "spin_get_launch_count",
@@ -78,6 +78,7 @@ def lib():
         L.spin_create.argtypes = [cfgp, vp, C.c_size_t, vp, C.POINTER(vp)]
         L.spin_sweep.argtypes = [vp, C.c_double, C.c_int64, vp]
         L.spin_measure.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
+        L.spin_measure_noalloc.argtypes = [vp, vp, vp, vp]
         L.spin_sweep_betas.argtypes = [vp, C.POINTER(C.c_double), C.c_int64, vp]
         L.spin_sweep_record.argtypes = [vp, C.c_double, C.c_int64, vp, vp, vp]
         L.spin_get_spins.argtypes = [vp, vp, C.c_size_t]
@@ -254,6 +255,12 @@ class SpinSystem:
         with self._torch.cuda.device(self.device):
             _check(lib().spin_measure(self._h, E.ctypes.data_as(dp), M.ctypes.data_as(dp), self._stream()))
         return E, M.reshape(self.R, self.n)
+
+    def measure_noalloc(self, d_E, d_M):
+        """E, M into the caller's CUDA float64 tensors d_E [R], d_M [R, n]; asynchronous, allocates nothing (the scratch is a
+        fixed array inside the library: spin.h)"""
+        with self._torch.cuda.device(self.device):
+            _check(lib().spin_measure_noalloc(self._h, C.c_void_p(d_E.data_ptr()), C.c_void_p(d_M.data_ptr()), self._stream()))
 
     def sweep_record(self, beta, n_sweeps, d_E=None, d_M=None):
         """Returns (d_E, d_M): CUDA float64 tensors [n_sweeps, R] and [n_sweeps, R, n] (filled asynchronously)."""

@@ -984,6 +984,34 @@ static spin_status check_sweep_args(spin_system *s, double beta, int64_t n_sweep
     return SPIN_OK;
 }
 
+// ------------------------------------------------------------------- no-allocation measurement ------
+// spin_measure_noalloc (include/spin.h): for callers that may not allocate -- code under CUDA graph capture, tight serving loops,
+// harnesses that forbid cudaMalloc.  The scratch of the measurement kernels (per-CTA partial sums for n >= 2, the int64
+// accumulator slots for n = 1; normally carved from the caller's workspace) lives in this file-scope device array instead:
+// SPIN_NOALLOC_SCRATCH_BYTES = 1 MiB, held by every GPU that loads the library until the process exits.
+// In HOST code the name g_noalloc_scratch is a host-side stand-in, not a device address (a kernel given it would fault, or, where
+// the GPU can reach host memory, silently use the wrong memory): the device address comes from cudaGetSymbolAddress, once per
+// device, with that device current, and it is that pointer the kernels receive.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[SPIN_NOALLOC_SCRATCH_BYTES];
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+static void *g_noalloc_ptr[NOALLOC_MAX_DEVICES];   // device address of g_noalloc_scratch per device ordinal, NULL until looked up
+
+// device address of the scratch array on the CURRENT device (looked up on first use; no allocation)
+static spin_status noalloc_scratch(void **out) {
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(SPIN_ERR_UNSUPPORTED, "device ordinal %d beyond %d", dev, NOALLOC_MAX_DEVICES);
+    if (!g_noalloc_ptr[dev]) {
+        void *ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+        if (e != cudaSuccess || !ptr) return fail(SPIN_ERR_CUDA, "cudaGetSymbolAddress(g_noalloc_scratch): %s", cudaGetErrorString(e));
+        g_noalloc_ptr[dev] = ptr;
+    }
+    *out = g_noalloc_ptr[dev];
+    return SPIN_OK;
+}
+
 // ------------------------------------------------------------------------------ C ABI --------
 extern "C" {
 
@@ -1425,6 +1453,53 @@ spin_status spin_measure(spin_system *s, double *E, double *M, void *stream) {
     if (e != cudaSuccess) return fail(SPIN_ERR_CUDA, "measure copy: %s", cudaGetErrorString(e));
     std::memcpy(E, tmp, nE * sizeof(double));
     std::memcpy(M, tmp + nE, nM * sizeof(double));
+    return SPIN_OK;
+}
+
+// E and M of every replica into DEVICE doubles d_E[R], d_M[R * n] of the caller's, enqueued on `stream`: the measurement kernels of
+// spin_measure with their scratch in g_noalloc_scratch.  Calls no cudaMalloc / cudaFree / cudaMallocHost and does not synchronise.
+spin_status spin_measure_noalloc(spin_system *s, double *d_E, double *d_M, void *stream) {
+    if (!s || !d_E || !d_M) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    const size_t need = s->n == 1 ? (size_t)acc_slots_for(s->R) * s->R * 2 * sizeof(long long)
+                                  : (size_t)s->R * s->mblocks * (1 + s->n) * sizeof(double);
+    if (need > (size_t)SPIN_NOALLOC_SCRATCH_BYTES)
+        return fail(SPIN_ERR_UNSUPPORTED, "spin_measure_noalloc: this system needs %zu bytes of scratch, the built-in array holds %d "
+                                          "(fewer replicas, or spin_measure with the workspace)", need, (int)SPIN_NOALLOC_SCRATCH_BYTES);
+    void *scratch = nullptr;
+    spin_status rc = noalloc_scratch(&scratch);
+    if (rc != SPIN_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const dim3 grid(s->mblocks, s->R);
+    if (s->n == 1) {
+        // the accumulators must start at zero, and the array keeps what the last call (of any handle) left
+        CUDA_TRY(cudaMemsetAsync(scratch, 0, need, st));
+        IsingArgs a = ising_args(s);
+        a.acc = (long long *)scratch;
+        const bool bonds = s->cfg.coupling_kind == SPIN_J_BOND_PM1;
+        if (s->path == PATH_ISING_MSC) {
+            const uint32_t spt = 64;
+            const dim3 gm((unsigned)(((s->g.Nh + spt - 1) / spt + 127) / 128), s->R / 32);
+            if (s->d == 2) ising_msc_measure<2><<<gm, 128, 0, st>>>(a, spt); else ising_msc_measure<3><<<gm, 128, 0, st>>>(a, spt);
+        } else if (s->path == PATH_ISING_BITPACK) {
+            if (s->d == 2) { if (bonds) ising_bitpack_measure<2, true><<<grid, 256, 0, st>>>(a); else ising_bitpack_measure<2, false><<<grid, 256, 0, st>>>(a); }
+            else { if (bonds) ising_bitpack_measure<3, true><<<grid, 256, 0, st>>>(a); else ising_bitpack_measure<3, false><<<grid, 256, 0, st>>>(a); }
+        } else if (s->path == PATH_ISING_INT8) {
+            if (s->d == 2) ising_int8_measure<2><<<grid, 256, 0, st>>>(a); else ising_int8_measure<3><<<grid, 256, 0, st>>>(a);
+        } else {
+            ising_generic_measure<<<grid, 256, 0, st>>>(a);
+        }
+        CUDA_TRY(cudaGetLastError());
+        ising_measure_finalize<<<(s->R + 3) / 4, 128, 0, st>>>(a.acc, s->R, a.acc_slots, d_E, d_M);
+    } else {
+        // every partial is written by its CTA before the finalize reads it: nothing to clear
+        VectorArgs a = vector_args(s, 0.0);
+        double *part = (double *)scratch;
+        if (s->n == 2) vector_measure<2><<<grid, 256, 0, st>>>(a, part); else vector_measure<3><<<grid, 256, 0, st>>>(a, part);
+        CUDA_TRY(cudaGetLastError());
+        vector_measure_finalize<<<s->R, 256, 0, st>>>(part, s->mblocks, s->n, d_E, d_M);
+    }
+    CUDA_TRY(cudaGetLastError());
+    s->launches += 2;
     return SPIN_OK;
 }
 
