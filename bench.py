@@ -386,7 +386,10 @@ def run_graft(args):
     t_wall1 = time.time()
     clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
     launches = S.launch_count - launches0
-    cnt = COUNTERS.get(args.workload, {})
+    # counters of the kernel that ran: with --opt another kernel may serve the workload -- its capture if there is one
+    # (profiles/counters.json "<workload>#<variant>"), else none (null traffic rather than another kernel's numbers)
+    variant = {("4=0",): "#strip", ("1=1",): "#tma"}.get(tuple(args.opt)) if args.opt else ""
+    cnt = COUNTERS.get(args.workload + variant, {}) if variant is not None else {}
     ms_total = max_over_ranks(e0.elapsed_time(e1))
     ms_sweeps = sum(a.elapsed_time(b) for a, b in sweep_ev)
     value = world * updates_per_step * args.steps / (ms_total * 1e6)
