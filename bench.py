@@ -277,7 +277,9 @@ def run_slab(args):
     torch.cuda.set_device(local_rank)
     dev = "cuda:%d" % local_rank
     os.environ.setdefault("NCCL_DEBUG", "INFO")      # the ranks and their transports show in the log
-    if world > 1:
+    if "RANK" in os.environ and "MASTER_ADDR" in os.environ:
+        # under torchrun (any world size, 1 included): its rendezvous -- an explicit tcp:// address would be taken for the
+        # agent's store and wait for a server that is not there
         dist.init_process_group("nccl", device_id=torch.device(dev))
     else:
         dist.init_process_group("nccl", init_method="tcp://127.0.0.1:29541", rank=0, world_size=1, device_id=torch.device(dev))
