@@ -430,7 +430,8 @@ __global__ void __launch_bounds__(128, (HB && !MEAS) ? 7 : 0) vector_strip_halfs
     for (int c = 0; c < NC; ++c) m_acc[c] = 0.0f;
     if (it < per_replica) {
     const uint32_t sz = fdiv(it, g.divQX), q = it - sz * QX;       // sz = strip + nstrip * z
-    const uint32_t zl = sz / nstrip, z = zs0 + zl, y0 = ys0 + (sz - zl * nstrip) * K;
+    // one row per thread on the whole lattice: nstrip = Ly, whose host-prepared reciprocal replaces the ~20-instruction division
+    const uint32_t zl = (K == 1 && !RANGED) ? fdiv(sz, g.divLy) : sz / nstrip, z = zs0 + zl, y0 = ys0 + (sz - zl * nstrip) * K;
     const uint32_t kend = min((uint32_t)K, ys0 + Lys - y0);
     const float *__restrict__ other = a.s[1 - a.colour] + (size_t)r * NC * Nh;
     float *mine = a.s[a.colour] + (size_t)r * NC * Nh;
