@@ -183,16 +183,20 @@ def test_exchange_cost_of_a_self_exchanging_slab(P):
 
     def timed(fn):
         fn(2)
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        fn(sweeps)
-        e1.record()
-        torch.cuda.synchronize()
-        return 1e3 * e0.elapsed_time(e1) / (2 * sweeps)
+        best = 1e30
+        for _ in range(3):                       # best of three: the assertion below is about cost, not about noise
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn(sweeps)
+            e1.record()
+            torch.cuda.synchronize()
+            best = min(best, 1e3 * e0.elapsed_time(e1) / (2 * sweeps))
+        return best
 
     plain = timed(lambda k: A.sweep(beta, k))
     slabbed = timed(lambda k: ring.sweep(beta, k))
     print("half-sweep %.1f us, with self-exchange %.1f us" % (plain, slabbed))
     assert slabbed - plain <= 5.0, (plain, slabbed)
+    assert A.sweep_counter == ring.systems[0].sweep_counter
     assert np.array_equal(A.get_spins(), ring.get_spins())
