@@ -225,18 +225,15 @@ __global__ void __launch_bounds__(1024) ising_resident_ahead_sweeps(const __grid
                         }
                     }
                     if (c == 1 && record) {
-                        int minus = __popc(w[0]) + __popc(w[1]);
+                        // both sums in one word (unsatisfied bonds of the CTA <= 256 words x 192 < 2^16, minus spins <= 2^14): one
+                        // warp reduction instruction (REDUX) and one shared-memory atomic per warp instead of two shuffle trees
+                        const int both = unsat + ((__popc(w[0]) + __popc(w[1])) << 16);
                         const uint32_t par = k & 1u;
                         if (warp_one_replica) {
-#pragma unroll
-                            for (int o = 16; o > 0; o >>= 1) {
-                                unsat += __shfl_down_sync(0xFFFFFFFFu, unsat, o);
-                                minus += __shfl_down_sync(0xFFFFFFFFu, minus, o);
-                            }
-                            if ((i & 31u) == 0u && live) { atomicAdd(&acc[par][0][r], unsat); atomicAdd(&acc[par][1][r], minus); }
+                            const int tot = __reduce_add_sync(0xFFFFFFFFu, live ? both : 0);
+                            if ((i & 31u) == 0u && live) atomicAdd(&acc[par][0][r], tot);
                         } else if (live) {
-                            atomicAdd(&acc[par][0][r], unsat);
-                            atomicAdd(&acc[par][1][r], minus);
+                            atomicAdd(&acc[par][0][r], both);
                         }
                     }
                     asm volatile("bar.sync 1, %0;" ::"r"(cthreads) : "memory");   // the consumer warps only
@@ -244,10 +241,10 @@ __global__ void __launch_bounds__(1024) ising_resident_ahead_sweeps(const __grid
                 if (record && i < a.R) {
                     const uint32_t par = k & 1u;
                     const long long nbonds = (long long)D * 64ll * NW;
-                    d_E[(size_t)k * a.R + i] = (double)(2ll * acc[par][0][i] - nbonds);
-                    d_M[(size_t)k * a.R + i] = (double)(64ll * NW - 2ll * acc[par][1][i]);
+                    const int tot = acc[par][0][i];
+                    d_E[(size_t)k * a.R + i] = (double)(2ll * (tot & 0xFFFF) - nbonds);
+                    d_M[(size_t)k * a.R + i] = (double)(64ll * NW - 2ll * (tot >> 16));
                     acc[par][0][i] = 0;
-                    acc[par][1][i] = 0;
                 }
             }
         }
