@@ -128,8 +128,10 @@ namespace spin {
 constexpr int AHEAD_MAX_WORDS = 256;          // consumer warps: at most 8
 constexpr int AHEAD_SMEM_WORDS = 10240;       // 40 KB for the two mask buffers
 
-template <int D, bool INT8, bool HB>
-__global__ void __launch_bounds__(1024) ising_resident_ahead_sweeps(const __grid_constant__ IsingArgs a, uint32_t n_sweeps,
+// MAXT = threads per CTA: 1024 (64 registers per thread, up to 256 words) or 512 (128 registers: no spills in the consumers'
+// chain; up to 128 words: config 1 has 64)
+template <int D, bool INT8, bool HB, int MAXT = 1024>
+__global__ void __launch_bounds__(MAXT) ising_resident_ahead_sweeps(const __grid_constant__ IsingArgs a, uint32_t n_sweeps,
                                                                      double *d_E, double *d_M) {
     constexpr int NT = HB ? 2 * D + 1 : D;
     __shared__ uint32_t sp[2][AHEAD_MAX_WORDS];
@@ -137,7 +139,7 @@ __global__ void __launch_bounds__(1024) ising_resident_ahead_sweeps(const __grid
     __shared__ int acc[2][2][32];
     const uint32_t NW = a.g.NW, words = NW * a.R;
     // Roles.  Warp w issues from sub-core w % 4: the consumer warps are the warps of sub-core 0 (warps 0, 4, 8, ...: word
-    // i = 32 (w / 4) + lane), the producers all warps of sub-cores 1 .. 3 (768 threads), so that the consumers' short
+    // i = 32 (w / 4) + lane), the producers all warps of sub-cores 1 .. 3 (three quarters of the CTA), so that the consumers' short
     // dependent chain never queues behind the Philox chains (measured at 64 x 64, recorded sweeps: 0.64 us with the roles
     // mixed over the sub-cores).
     const uint32_t tid = threadIdx.x, T = blockDim.x, warp = tid >> 5, sub = warp & 3u;
@@ -145,7 +147,7 @@ __global__ void __launch_bounds__(1024) ising_resident_ahead_sweeps(const __grid
     const uint32_t i = sub == 0u ? ((warp >> 2) << 5) + (tid & 31u) : 0xFFFFFFFFu;   // consumer: the word it owns
     const bool consumer = i < cthreads, live = i < words;
     const bool producer = sub != 0u;
-    const uint32_t P = 768u, pidx = (((warp >> 2) * 3u + (sub - 1u)) << 5) + (tid & 31u);
+    const uint32_t P = (uint32_t)(MAXT / 128) * 96u, pidx = (((warp >> 2) * 3u + (sub - 1u)) << 5) + (tid & 31u);
     const uint32_t per_sweep = 2u * NT * words;
     const uint32_t DEPTH = min(32u, (uint32_t)AHEAD_SMEM_WORDS / (2u * per_sweep));   // sweeps per round
     const uint32_t r = live ? i / NW : 0u, gi = live ? i - r * NW : 0u, rb = r * NW;
