@@ -369,8 +369,10 @@ __device__ __forceinline__ void vector_quad_accept(const VectorArgs &a, const fl
 #pragma unroll
         for (int c = 1; c < NC; ++c) acc = __fadd2_rn(acc, mul2s(__fadd2_rn(sn[c], neg2(so[c])), hp[pr][c]));
         const float2 arg = __fmul2_rn(f2s(a.beta), acc);
-        const bool acc_a = acc.x >= 0.0f || u24(wacc_a) < expf(arg.x);
-        const bool acc_b = acc.y >= 0.0f || u24(wacc_b) < expf(arg.y);
+        // branch-free (`|`, not `||`): a short-circuit branch around the exponential diverges inside the warp anyway and its
+        // reconvergence barriers keep the two sites' chains from interleaving
+        const bool acc_a = (acc.x >= 0.0f) | (u24(wacc_a) < expf(arg.x));
+        const bool acc_b = (acc.y >= 0.0f) | (u24(wacc_b) < expf(arg.y));
 #pragma unroll
         for (int c = 0; c < NC; ++c) {
             res[c][2 * pr] = acc_a ? sn[c].x : so[c].x;
