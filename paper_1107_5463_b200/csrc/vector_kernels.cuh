@@ -207,7 +207,8 @@ __device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y
 // A product that feeds a sum directly: ptxas contracts mul.rn.f32x2 + add.rn.f32x2 into one FFMA2 (measured: CUDA 12.9,
 // sm_100a; the scalar _rn intrinsics are never contracted), which would round once instead of twice.  Two scalar products
 // feeding a packed sum are not contracted, so where the contract (R-14) wants product and sum rounded separately
-// the product is taken with this helper.
+// the product is taken with this helper -- every product of such a sum, the first one included: ptxas contracts whichever packed
+// product has the sum as its only use (found by reading the SASS: an FFMA2 in the acceptance sum of the XY kernel).
 __device__ __forceinline__ float2 mul2s(float2 a, float2 b) { return make_float2(__fmul_rn(a.x, b.x), __fmul_rn(a.y, b.y)); }
 
 // sincospi_u24 for two sites at once: integer range reduction per site, the two polynomials packed
@@ -240,8 +241,8 @@ __device__ __forceinline__ void direction3_x2(uint32_t w0a, uint32_t w1a, uint32
     const float2 rho = f2(__fsqrt_rn(fmaxf(om.x, 0.0f)), __fsqrt_rn(fmaxf(om.y, 0.0f)));
     float2 sn, cs;
     sincospi_u24_x2(w1a, w1b, &sn, &cs);
-    out[0] = __fmul2_rn(rho, cs);
-    out[1] = __fmul2_rn(rho, sn);
+    out[0] = mul2s(rho, cs);   // the proposal feeds the difference s' - s: it must not be contracted into it
+    out[1] = mul2s(rho, sn);
     out[2] = z;
 }
 __device__ __forceinline__ void direction2_x2(uint32_t w0a, uint32_t w0b, float2 out[2]) {
@@ -270,7 +271,7 @@ __device__ __forceinline__ void heatbath3_x2(float beta, const float2 h[3], uint
     float2 sp, cp;
     sincospi_u24_x2(w1a, w1b, &sp, &cp);
     const float2 inv = f2(__fdiv_rn(1.0f, hn.x), __fdiv_rn(1.0f, hn.y));
-    const float2 x = __fmul2_rn(h[0], inv), y = __fmul2_rn(h[1], inv), z = __fmul2_rn(h[2], inv);
+    const float2 x = __fmul2_rn(h[0], inv), y = __fmul2_rn(h[1], inv), z = mul2s(h[2], inv);   // z feeds the sum sg + z
     const float2 sg = f2(signbit(z.x) ? -1.0f : 1.0f, signbit(z.y) ? -1.0f : 1.0f);
     const float2 sz = __fadd2_rn(sg, z);
     const float2 a = f2(__fdiv_rn(-1.0f, sz.x), __fdiv_rn(-1.0f, sz.y));
@@ -339,7 +340,7 @@ __device__ __forceinline__ void vector_quad_accept(const VectorArgs &a, const fl
     [[maybe_unused]] float esum = 0.0f;
     // the two sites of pair pr: esum += s' . h, first site then second
     [[maybe_unused]] const auto add_energy = [&](int pr) {
-        float2 dot = __fmul2_rn(f2(res[0][2 * pr], res[0][2 * pr + 1]), hp[pr][0]);
+        float2 dot = mul2s(f2(res[0][2 * pr], res[0][2 * pr + 1]), hp[pr][0]);
 #pragma unroll
         for (int c = 1; c < NC; ++c) dot = __fadd2_rn(dot, mul2s(f2(res[c][2 * pr], res[c][2 * pr + 1]), hp[pr][c]));
         esum = __fadd_rn(__fadd_rn(esum, dot.x), dot.y);
@@ -365,7 +366,7 @@ __device__ __forceinline__ void vector_quad_accept(const VectorArgs &a, const fl
 #pragma unroll
         for (int c = 0; c < NC; ++c) so[c] = pr == 0 ? f2(own.c[c].x, own.c[c].y) : f2(own.c[c].z, own.c[c].w);
         // acc = (s' - s) . h = -dE; accept iff dE <= 0 (acc >= 0) or u < exp(-beta dE) = exp(beta acc)
-        float2 acc = __fmul2_rn(__fadd2_rn(sn[0], neg2(so[0])), hp[pr][0]);
+        float2 acc = mul2s(__fadd2_rn(sn[0], neg2(so[0])), hp[pr][0]);   // every product of the sum, the first one too (mul2s)
 #pragma unroll
         for (int c = 1; c < NC; ++c) acc = __fadd2_rn(acc, mul2s(__fadd2_rn(sn[c], neg2(so[c])), hp[pr][c]));
         const float2 arg = __fmul2_rn(f2s(a.beta), acc);
