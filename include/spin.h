@@ -18,11 +18,15 @@
  *   - Every call returns a spin_status; nothing throws or aborts across the ABI; outputs are
  *     written only on SPIN_OK.  spin_last_error() gives a thread-local message.
  *   - The CALLER owns device memory: spin_create() carves everything it needs out of the
- *     device workspace passed in (size from spin_workspace_bytes()).  The only device memory the
- *     library allocates itself is one staging buffer for canonical arrays, created by the first
- *     get/set call, reused by later ones and freed by spin_destroy().
+ *     device workspace passed in (size from spin_workspace_bytes()).  The only memory the library
+ *     allocates itself: one device staging buffer for canonical arrays, created by the first HOST-array
+ *     get/set call, reused by later ones and freed by spin_destroy() (the *_device variants take the
+ *     caller's device arrays instead and allocate nothing); a few pinned host doubles for
+ *     spin_measure's result (first call; spin_measure_noalloc has none); and the fixed 1 MiB device
+ *     array of spin_measure_noalloc, part of the library image.
  *   - "stream" arguments are cudaStream_t passed as void* (NULL = the legacy default stream).
- *   - spin_sweep / spin_sweep_record only enqueue work; spin_measure and the get/set calls block.
+ *   - spin_sweep / spin_sweep_record / spin_sweep_betas / spin_halfsweep* / spin_halo_* / spin_measure_noalloc and the
+ *     *_async / *_device conversions only enqueue work; spin_measure and the host-array get/set calls block.
  *   - A handle is not thread-safe; different handles are independent.
  *   - Sites: (x, y, z), lexicographic index i = x + Lx (y + Ly z); colour = (x + y + z) mod 2;
  *     colour 0 is updated first.  Periodic boundaries in every direction.
