@@ -159,6 +159,15 @@ spin_status spin_halo_unpack(spin_system *s, int32_t colour, const void *d_buf, 
 /* A slab that is its own neighbour (one rank holds the whole extent, periodic): ghost below <- highest owned plane,
  * ghost above <- lowest owned plane, one kernel.  Asynchronous. */
 spin_status spin_halo_wrap(spin_system *s, int32_t colour, void *stream);
+/* Peer stores instead of messages ("direct peer stores over NVLink 5 / NVSwitch"): spin_colour_array gives
+ * the device address (and size) of a handle's colour array, which the owner of a neighbouring slab may map on its own GPU
+ * (same process: cudaDeviceEnablePeerAccess; another process: CUDA IPC); spin_halo_push then writes this handle's two
+ * owned boundary planes of `colour` straight into the ghost planes of the slab below (d_peer_below = THAT handle's colour
+ * array) and of the slab above, with one kernel and no message buffer.  Both neighbours must have this handle's slab
+ * thickness and layout.  The push is ordered on `stream` only: the caller makes sure (event, barrier) that a neighbour
+ * does not start the half-sweep that reads the ghosts before the push has completed.  Asynchronous. */
+spin_status spin_colour_array(spin_system *s, int32_t colour, void **d_ptr, size_t *bytes);
+spin_status spin_halo_push(spin_system *s, int32_t colour, void *d_peer_below, void *d_peer_above, void *stream);
 
 /* Temperature axis ("trivial parallelization"): n_sweeps sweeps with replica r at
  * betas[r] (host array of n_replicas doubles, read before the call returns) -- many temperatures of one model side by

@@ -35,7 +35,7 @@ SYMBOLS = [
     "spin_set_spins_bits_async", "spin_get_spins_bits",
     "spin_get_bonds", "spin_get_sweep_count", "spin_set_sweep_count", "spin_get_launch_count",
     "spin_set_launch_shape", "spin_set_strip_rows", "spin_set_option", "spin_halfsweep", "spin_halo_bytes",
-    "spin_halo_get", "spin_halo_put", "spin_halfsweep_range", "spin_halo_pack", "spin_halo_unpack", "spin_halo_wrap", "spin_destroy", "spin_last_error", "spin_version",
+    "spin_halo_get", "spin_halo_put", "spin_halfsweep_range", "spin_halo_pack", "spin_halo_unpack", "spin_halo_wrap", "spin_colour_array", "spin_halo_push", "spin_destroy", "spin_last_error", "spin_version",
 ]
 
 
@@ -104,6 +104,8 @@ def lib():
         L.spin_halo_pack.argtypes = [vp, C.c_int32, vp, vp]
         L.spin_halo_unpack.argtypes = [vp, C.c_int32, vp, vp]
         L.spin_halo_wrap.argtypes = [vp, C.c_int32, vp]
+        L.spin_colour_array.argtypes = [vp, C.c_int32, C.POINTER(vp), C.POINTER(C.c_size_t)]
+        L.spin_halo_push.argtypes = [vp, C.c_int32, vp, vp, vp]
         L.spin_destroy.argtypes = [vp]
         for name in SYMBOLS:
             getattr(L, name).restype = C.c_int
@@ -227,6 +229,17 @@ class SpinSystem:
         """buf = [plane from the slab below][plane from the slab above] -> the two ghost planes"""
         with self._torch.cuda.device(self.device):
             _check(lib().spin_halo_unpack(self._h, int(colour), C.c_void_p(buf.data_ptr()), self._stream()))
+
+    def colour_array(self, colour):
+        """(device address, bytes) of the colour array: what a neighbouring slab's owner maps for peer stores"""
+        ptr, n = C.c_void_p(), C.c_size_t(0)
+        _check(lib().spin_colour_array(self._h, int(colour), C.byref(ptr), C.byref(n)))
+        return int(ptr.value), int(n.value)
+
+    def halo_push(self, colour, peer_below_ptr, peer_above_ptr):
+        """my two owned boundary planes -> the ghost planes of the slabs below and above (peer stores, one kernel)"""
+        with self._torch.cuda.device(self.device):
+            _check(lib().spin_halo_push(self._h, int(colour), C.c_void_p(peer_below_ptr), C.c_void_p(peer_above_ptr), self._stream()))
 
     def halo_wrap(self, colour):
         """single slab, periodic: its own boundary planes become its ghost planes (one kernel)"""

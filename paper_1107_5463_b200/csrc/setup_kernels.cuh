@@ -229,6 +229,22 @@ __global__ void __launch_bounds__(256) halo_faces_copy(T *arr, T *buf, size_t pl
     }
 }
 
+// Peer stores ("direct peer stores over NVLink 5 / NVSwitch"): my two owned boundary planes go straight into the ghost
+// planes of the two neighbour slabs' colour arrays -- below: its ghost above its owned planes (plane own + 2), above: its ghost
+// below (plane 1).  dst_below / dst_above are device pointers to the neighbours' colour arrays of the same layout and slab
+// thickness, valid on this device (the same device, or peer-mapped memory of another GPU).  One kernel, no message buffer.
+template <typename T>
+__global__ void __launch_bounds__(256) halo_faces_push(const T *src, T *dst_below, T *dst_above, size_t plane_elems, size_t stride_elems,
+                                                       uint32_t rows, uint32_t own) {
+    const size_t per_face = plane_elems * rows, total = 2 * per_face;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t f = i / per_face, rem = i - f * per_face, q = rem / plane_elems, e = rem - q * plane_elems;
+        const size_t off = q * stride_elems + e;
+        if (f == 0) dst_below[(own + 2u) * plane_elems + off] = src[2u * plane_elems + off];      // my lowest plane -> its upper ghost
+        else dst_above[1u * plane_elems + off] = src[(own + 1u) * plane_elems + off];             // my highest plane -> its lower ghost
+    }
+}
+
 // a single slab that is its own neighbour (one rank, periodic): ghost below <- highest owned plane, ghost above <- lowest
 template <typename T>
 __global__ void __launch_bounds__(256) halo_faces_wrap(T *arr, size_t plane_elems, size_t stride_elems, uint32_t rows, uint32_t own) {

@@ -1430,6 +1430,31 @@ spin_status spin_halo_wrap(spin_system *s, int32_t colour, void *stream) {
     return SPIN_OK;
 }
 
+spin_status spin_colour_array(spin_system *s, int32_t colour, void **d_ptr, size_t *bytes) {
+    if (!s || !d_ptr) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    if (colour != 0 && colour != 1) return fail(SPIN_ERR_INVALID_ARG, "colour must be 0 or 1");
+    *d_ptr = s->ws + s->lay.off_s[colour];
+    if (bytes) *bytes = s->lay.bytes_s;
+    return SPIN_OK;
+}
+
+spin_status spin_halo_push(spin_system *s, int32_t colour, void *d_peer_below, void *d_peer_above, void *stream) {
+    if (!s || !d_peer_below || !d_peer_above) return fail(SPIN_ERR_INVALID_ARG, "NULL argument");
+    if (s->axis < 0) return fail(SPIN_ERR_STATE, "not a slab handle");
+    if (colour != 0 && colour != 1) return fail(SPIN_ERR_INVALID_ARG, "colour must be 0 or 1");
+    const Face f = face_of(s);
+    const char *arr = s->ws + s->lay.off_s[colour];
+    const bool wide = f.plane_bytes % 16 == 0 && f.stride_bytes % 16 == 0 && (((uintptr_t)d_peer_below | (uintptr_t)d_peer_above) & 15) == 0;
+    const size_t elems = 2 * f.plane_bytes * f.rows / (wide ? 16 : 1);
+    const int G = (int)((elems + 255) / 256 > 1184 ? 1184 : (elems + 255) / 256);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (wide) halo_faces_push<uint4><<<G, 256, 0, st>>>((const uint4 *)arr, (uint4 *)d_peer_below, (uint4 *)d_peer_above, f.plane_bytes / 16, f.stride_bytes / 16, (uint32_t)f.rows, (uint32_t)s->own_planes);
+    else halo_faces_push<uint8_t><<<G, 256, 0, st>>>((const uint8_t *)arr, (uint8_t *)d_peer_below, (uint8_t *)d_peer_above, f.plane_bytes, f.stride_bytes, (uint32_t)f.rows, (uint32_t)s->own_planes);
+    CUDA_TRY(cudaGetLastError());
+    s->launches += 1;
+    return SPIN_OK;
+}
+
 spin_status spin_halo_pack(spin_system *s, int32_t colour, void *d_buf, void *stream) {
     return halo_faces(s, colour, d_buf, true, (cudaStream_t)stream);
 }

@@ -41,10 +41,12 @@ def ring_neighbours(rank, world):
 
 
 class LocalRing:
-    """All slabs of one lattice as separate handles on one device; halos move through the packed message buffers of the
-    library (one pack and one unpack kernel per slab and exchange; a single slab wraps onto itself with one kernel)."""
+    """All slabs of one lattice as separate handles on one device; halos move by peer stores (spin_halo_push: every slab
+    writes its boundary planes straight into its neighbours' ghost planes, one kernel per slab) or, with
+    peer_stores=False, through the packed message buffers DistRing sends (one pack and one unpack kernel per slab and
+    exchange); a single slab wraps onto itself with one kernel."""
 
-    def __init__(self, system_cls, global_dims, n_slabs, **kw):
+    def __init__(self, system_cls, global_dims, n_slabs, peer_stores=True, **kw):
         import torch
 
         self.dims = tuple(int(v) for v in global_dims) + (1,) * (3 - len(global_dims))
@@ -53,6 +55,7 @@ class LocalRing:
         self.systems = [system_cls(local, slab_global=self.dims[self.axis], slab_offset=off, **kw)
                         for local, off in self.parts]
         s0 = self.systems[0]
+        self.peer_stores = bool(peer_stores) and hasattr(s0, "halo_push")
         self.n, self.R = s0.n, s0.R
         self.N = self.dims[0] * self.dims[1] * self.dims[2]
         self.hb = s0.halo_bytes()
@@ -65,6 +68,14 @@ class LocalRing:
         G, hb = len(self.systems), self.hb
         if G == 1:
             self.systems[0].halo_wrap(colour)
+            return
+        if self.peer_stores:
+            # every slab stores its boundary planes straight into its neighbours' ghost planes (one kernel per slab; all
+            # slabs share the stream here, which orders the pushes before the half-sweeps that read the ghosts)
+            ptrs = [s.colour_array(colour)[0] for s in self.systems]
+            for k, s in enumerate(self.systems):
+                below, above = ring_neighbours(k, G)
+                s.halo_push(colour, ptrs[below], ptrs[above])
             return
         for k, s in enumerate(self.systems):
             s.halo_pack(colour, self.send[k])                  # [my lowest owned plane][my highest]

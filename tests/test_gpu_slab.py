@@ -200,3 +200,23 @@ def test_exchange_cost_of_a_self_exchanging_slab(P):
     assert slabbed - plain <= 5.0, (plain, slabbed)
     assert A.sweep_counter == ring.systems[0].sweep_counter
     assert np.array_equal(A.get_spins(), ring.get_spins())
+
+
+@pytest.mark.parametrize("dims,kw,G", [((128, 24, 1), dict(n=1, storage="int8"), 3), ((64, 6, 12), dict(n=1, storage="bitpack", replicas=2, replica_streams=1), 2),
+                                       ((16, 8, 12), dict(n=3, storage="fp32"), 3), ((10, 12, 1), dict(n=1, storage="int8"), 2)])
+def test_peer_stores_and_packed_messages_agree(P, dims, kw, G):
+    """The two halo paths -- spin_halo_push (boundary planes stored straight into the neighbours' ghost planes) and the packed
+    messages DistRing sends (spin_halo_pack / copy / spin_halo_unpack) -- leave identical slabs, equal to the single handle."""
+    from paper_1107_5463_b200 import slab
+
+    beta = 0.5
+    A = slab.LocalRing(P.SpinSystem, dims, G, peer_stores=True, seed=8, **kw)
+    B = slab.LocalRing(P.SpinSystem, dims, G, peer_stores=False, seed=8, **kw)
+    W = P.SpinSystem(dims, seed=8, **kw)
+    assert A.peer_stores and not B.peer_stores
+    for S in (A, B, W):
+        S.sweep(beta, 5)
+    a, b, w = A.get_spins(), B.get_spins(), W.get_spins()
+    assert np.array_equal(a.view(np.uint8), w.view(np.uint8)) and np.array_equal(b.view(np.uint8), w.view(np.uint8))
+    A.close()
+    B.close()
