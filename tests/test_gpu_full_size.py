@@ -253,3 +253,62 @@ def test_full_size_vector_kernels_agree_bitwise(P, name):
     Ea, Ma = A.measure()
     Eb, Mb = B.measure()
     assert Ea[0] == Eb[0] and np.array_equal(Ma, Mb)
+
+
+@pytest.mark.parametrize("dims,storage", [((32768, 32768, 1), "int8"), ((32768, 65534, 1), "bitpack"), ((1024, 1024, 1022), "bitpack")])
+def test_maximum_sizes(P, oracle, dims, storage):
+    """The largest lattices the library takes (N R < 2^31; 32768 is also the widest row of the temporal-blocking kernel):
+    2^30 int8 sites (the default path at this size is one temporal-blocking launch per two sweeps), 2^31 - 65536 bit-packed
+    sites in 2D and 2^30 - 2^21 in 3D.  Index arithmetic near 2^31 is what this covers: the hot start, two sweeps on
+    sampled sites against the oracle's decision functions (edges and wrap-around included), E and M against numpy."""
+    seed, beta = 5, 0.4406868 if dims[2] == 1 else 0.2216546
+    N = dims[0] * dims[1] * dims[2]
+    assert N < 2 ** 31
+    rng = np.random.default_rng(2)
+    idx = _sample_sites(dims, rng, 6000)
+    G = P.SpinSystem(dims, n=1, storage=storage, seed=seed)
+    s0 = G.get_spins()[0]
+    _check_hot_start(oracle, s0, seed, 0, idx)
+    G.sweep(beta, 1)                         # one plain sweep ...
+    s1 = G.get_spins()[0]
+    _check_ising_sweep(oracle, dims, seed, beta, 0, 0, 0, s0, s1, idx)
+    del s0
+    l0 = G.launch_count
+    G.sweep(beta, 2)                         # ... then a pair (int8: the temporal-blocking kernel), checked through its second sweep
+    if storage == "int8":
+        assert G.launch_count - l0 == 1
+    H = P.SpinSystem(dims, n=1, storage=storage, seed=seed)
+    H.set_option(P.OPT_TEMPORAL_BLOCKING, 0)
+    H.sweep(beta, 2)
+    s2 = H.get_spins()[0]
+    del H
+    s3 = G.get_spins()[0]
+    _check_ising_sweep(oracle, dims, seed, beta, 2, 0, 0, s2, s3, idx)
+    del s2
+    E, M = G.measure()
+    assert M[0, 0] == int(s3.sum(dtype=np.int64))
+    assert E[0] == _full_energy_ising(s3, dims)
+    G.close()
+
+
+@pytest.mark.parametrize("dims,storage,coupling,R", [((4, 4, 1), "int8", "uniform", 65535), ((64, 2, 1), "bitpack", "bond_pm1", 65535),
+                                                     ((8, 8, 1), "msc", "bond_pm1", 32 * 2048)])
+def test_maximum_replica_counts(P, dims, storage, coupling, R):
+    """The most replicas a handle takes (65535: they map to a grid dimension; MSC storage counts groups of 32), each a tiny
+    lattice: bit-exact against the oracle after every sweep, E and M of every replica."""
+    import oracle
+
+    streams = 1 if coupling == "uniform" else 0
+    G = P.SpinSystem(dims, n=1, storage=storage, coupling=coupling, replicas=R, replica_streams=streams, seed=9)
+    O = oracle.System(dims, n=1, coupling_kind=oracle.J_BOND_PM1 if coupling == "bond_pm1" else oracle.J_UNIFORM, n_replicas=R,
+                      replica_streams=streams, seed=9)
+    for t in range(3):
+        G.sweep(0.6, 1)
+        O.sweep(0.6, 1)
+        assert np.array_equal(G.get_spins(), O.get_spins()), t
+    Eg, Mg = G.measure()
+    Eo, Mo = O.measure()
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    with pytest.raises(P.SpinError):
+        P.SpinSystem(dims, n=1, storage=storage, coupling=coupling, replicas=(R + 32 if storage == "msc" else R + 1) * (33 if storage == "msc" else 1),
+                     replica_streams=streams, seed=9)
