@@ -12,6 +12,7 @@
 #include "ising_int8_kernel.cuh"
 #include "ising_kernels.cuh"
 #include "ising_msc_kernel.cuh"
+#include "ising_pmj_own_kernel.cuh"
 #include "ising_resident_kernel.cuh"
 #include "ising_tblock_kernel.cuh"
 #include "measure_kernels.cuh"
@@ -479,6 +480,19 @@ static spin_status launch_halfsweep_ising(spin_system *s, const IsingArgs &a, cu
 #undef BM3
 #undef BS2
 #undef BS3
+    } else if (bonds && !shared && s->g.WX % 4 == 0 && !s->vector_generic && s->variant != 1 && s->cfg.update_rule != SPIN_UPDATE_HEATBATH &&
+               !(fused && a.colour == 1u)) {
+        // per-bond couplings, own update stream per replica (or one replica), Lx % 256 == 0: one thread per quad, deferred digit tails
+        const int Bq = 128;
+        const uint64_t quads = (uint64_t)s->g.NW / 4;
+        unsigned Gy = 1;
+        if (quads < (uint64_t)s->sm_count * 512) {
+            uint64_t want = ((uint64_t)s->sm_count * 512 + quads - 1) / quads;   // replica chunks that fill the GPU
+            if (want > s->R) want = s->R;
+            Gy = (unsigned)(want < 1 ? 1 : want);
+        }
+        const dim3 G((unsigned)((quads + Bq - 1) / Bq), Gy);
+        if (s->d == 2) ising_pmj_quad_own_halfsweep<2><<<G, Bq, 0, st>>>(a); else ising_pmj_quad_own_halfsweep<3><<<G, Bq, 0, st>>>(a);
     } else if (bonds && shared && s->g.WX % 4 == 0 && !s->vector_generic) {
         // Lx % 256 == 0: one thread per quad of four words, 128-bit accesses (ising_pmj_quad_halfsweep).
         // All replicas in one thread when the quads alone give every SM >= 256 threads (measured at 256^3, R = 16:

@@ -600,3 +600,31 @@ def test_canonical_bit_arrays(P, dims, storage, R):
     A.sweep(0.4, 3)
     B.sweep(0.4, 3)
     assert np.array_equal(A.get_spins(), B.get_spins())
+
+
+@pytest.mark.parametrize("dims,R,beta", [((256, 6, 4), 3, 1.0 / 1.1), ((512, 10, 1), 2, 0.7), ((256, 4, 2), 1, 0.9), ((768, 2, 6), 5, 0.0),
+                                         ((256, 34, 1), 40, 50.0)])
+def test_pm_j_own_streams_quad_kernel(P, oracle, dims, R, beta):
+    """+-J couplings with an OWN update stream per replica on rows of whole quads (ising_pmj_quad_own_halfsweep: one thread per
+    quad, deferred digit tails finished through the per-warp queue, replica chunks over gridDim.y): bit-exact against the
+    oracle after every sweep, also through recorded sweeps (whose colour-1 half runs the fused word kernel) and with the
+    one-thread-per-word kernel as A/B partner."""
+    import torch
+
+    G, O = _pair(P, oracle, dims, storage="bitpack", coupling="bond_pm1", replicas=R, replica_streams=1)
+    H = _system(P, dims, storage="bitpack", coupling="bond_pm1", replicas=R, replica_streams=1, seed=SEED)
+    H.set_option(P.OPT_KERNEL_VARIANT, 1)
+    for t in range(4):
+        G.sweep(beta, 1)
+        H.sweep(beta, 1)
+        O.sweep(beta, 1)
+        _assert_ising_equal(G, O, "sweep %d" % t)
+    assert np.array_equal(G.get_spins(), H.get_spins())
+    dE, dM = G.sweep_record(beta, 3)
+    torch.cuda.synchronize()
+    O.sweep(beta, 3)
+    Eo, Mo = O.measure()
+    assert np.array_equal(dE[-1].cpu().numpy(), Eo) and np.array_equal(dM[-1, :, 0].cpu().numpy(), Mo[:, 0])
+    G.sweep(beta, 40)          # CUDA-graph replay for the small ones
+    O.sweep(beta, 40)
+    _assert_ising_equal(G, O, "after 47 sweeps")
