@@ -127,9 +127,9 @@ def run_per_model(P, peak):
     out = {}
     for name, sweeps in PER_MODEL:
         # "<workload>_ownstreams": the same lattice with the replica index in the Philox counter (replica_streams = 1)
-        base = name[:-len("_ownstreams")] if name.endswith("_ownstreams") else name
-        w = P.workloads.WORKLOADS[base]
-        S = P.from_workload(w, P.workloads.SEED, **({"replica_streams": 1} if base != name else {}))
+        base = name
+        w = P.workloads.WORKLOADS[name]
+        S = P.from_workload(w, P.workloads.SEED)
         if w["record"]:
             # config 1: E and M after every sweep (spin_sweep_record)
             S.sweep_record(w["beta"], 3)
@@ -150,7 +150,7 @@ def run_per_model(P, peak):
             out[name] = {"flips_per_ns": fpn, "ms_per_halfsweep": ms_half, "launches_per_sweep": launches / sweeps,
                          "algorithmic_GBps": fpn * bpu, "hbm_frac": fpn * bpu / peak, "bytes_per_update": bpu,
                          "kernel": cnt.get("kernel")}
-            if base != name:
+            if name.endswith("_ownstreams"):
                 out[name]["note"] = "16 replicas with their OWN update streams (replica_streams = 1): no mask reuse across replicas"
             elif w["replicas"] > 1 and not w["replica_streams"]:
                 out[name]["note"] = "shared update stream (DESIGN.md R-17): the acceptance masks of a word serve every replica"

@@ -24,6 +24,10 @@ WORKLOADS = {
     "ea3d_L256_R16_bitpack": dict(dims=(256, 256, 256), n=1, storage="bitpack", coupling="bond_pm1",
                                   J=(1.0, 1.0, 1.0), beta=1.0 / 1.1, sweeps=1000, replicas=16, replica_streams=0,
                                   record=False),
+    # config 4 read literally ("16 independent replicas"): the same lattices with the replica index in the Philox counter
+    "ea3d_L256_R16_bitpack_ownstreams": dict(dims=(256, 256, 256), n=1, storage="bitpack", coupling="bond_pm1",
+                                             J=(1.0, 1.0, 1.0), beta=1.0 / 1.1, sweeps=1000, replicas=16, replica_streams=1,
+                                             record=False),
     # config 5: 3D Heisenberg L = 256, 500 sweeps
     "heisenberg3d_L256_fp32": dict(dims=(256, 256, 256), n=3, storage="fp32", coupling="uniform", J=(1.0, 1.0, 1.0),
                                    beta=0.693, sweeps=500, replicas=1, replica_streams=0, record=False),
@@ -52,6 +56,7 @@ BYTES_PER_UPDATE = {
     "ising2d_L16384_bitpack": 0.375,
     "ising3d_L512_bitpack": 0.375,
     "ea3d_L256_R16_bitpack": 1.125,
+    "ea3d_L256_R16_bitpack_ownstreams": 1.125,
     "ea2d_L64_R4096_bitpack": 0.875,   # 3 spin bits + 2 forward bonds from each end = 7 bits
     "ea2d_L32_R131072_msc": 0.875,
     "heisenberg3d_L256_fp32": 36.0,

@@ -214,10 +214,7 @@ def test_whole_lattice_two_sweeps_against_the_oracle(P, name):
     launch configuration bench.py times -- for config 2 that is ONE launch of the temporal-blocking kernel (f3)."""
     import oracle
 
-    own = name.endswith("_ownstreams")       # config 4 with the replica index in the Philox counter (ADVICE round 1)
-    w = dict(P.workloads.WORKLOADS[name[:-len("_ownstreams")] if own else name])
-    if own:
-        w["replica_streams"] = 1
+    w = P.workloads.WORKLOADS[name]          # "_ownstreams": config 4 with the replica index in the Philox counter (ADVICE round 1)
     kinds = {"uniform": oracle.J_UNIFORM, "per_direction": oracle.J_PER_DIRECTION, "bond_pm1": oracle.J_BOND_PM1}
     G = P.from_workload(w, P.workloads.SEED)
     O = oracle.System(w["dims"], n=1, coupling_kind=kinds[w["coupling"]], J=w["J"], n_replicas=w["replicas"],
