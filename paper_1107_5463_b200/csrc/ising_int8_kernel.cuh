@@ -11,6 +11,8 @@
 // Work decomposition: one thread owns unit column w over K consecutive rows (a "strip") and rolls the other
 // colour's rows through registers, so each neighbour row is loaded and packed (K + 2) / K times instead of 3.
 #pragma once
+#include <type_traits>
+
 #include "ising_kernels.cuh"
 
 namespace spin {
@@ -137,6 +139,46 @@ __device__ __forceinline__ void defer_drain(const IsingArgs &a, DeferQueue &q, u
         m[D - 1] = 0u;   // the last mask never enters select_digit (its lanes take the default digit)
         const uint32_t lt = lt_mask_select_tail<D>(a, a.t, a.colour, q.f[warp][0][lane], q.f[warp][1][lane], m, q.f[warp][2][lane]);
         store(q.f[warp][6][lane], q.f[warp][5][lane] ^ lt);
+    }
+}
+
+// Heat-bath counterparts of the three helpers above (bit-packed strip kernel): head = two unconditional calls against the
+// 2 D + 1 heat-bath thresholds, the new word is ~(U < T_hb); a queued word is patched by XOR with its tail, as for Metropolis
+// (the tail's lanes are undecided lanes, whose provisional bit is 1).
+template <int D>
+__device__ __forceinline__ uint32_t ising_new_word_head_hb(const IsingArgs &a, uint32_t t, uint32_t colour, uint32_t unit, uint32_t rho,
+                                                           uint32_t raw, const uint32_t av[6], uint32_t &eq, uint32_t m[2 * D + 1]) {
+    uint32_t b[6];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) b[k] = k < 2 * D ? av[k] ^ raw : 0u;
+    count_masks<D>(b, m);
+    return ~lt_mask_select_head<2 * D + 1, true>(a, t, colour, unit, rho, m, eq);
+}
+template <int D>
+__device__ __forceinline__ bool defer_or_finish_hb(const IsingArgs &a, DeferQueueHB<D> &q, uint32_t warp, uint32_t unit, uint32_t rho,
+                                                   uint32_t eq, const uint32_t m[2 * D + 1], uint32_t &word, uint32_t index) {
+    if (eq == 0u) return true;
+    const uint32_t pos = atomicAdd(&q.n[warp], 1u);
+    if (pos >= (uint32_t)DEFER_CAP) {
+        word ^= lt_mask_select_tail<2 * D + 1, true>(a, a.t, a.colour, unit, rho, m, eq);
+        return true;
+    }
+    q.f[warp][0][pos] = unit; q.f[warp][1][pos] = rho; q.f[warp][2][pos] = eq; q.f[warp][3][pos] = word; q.f[warp][4][pos] = index;
+#pragma unroll
+    for (int k = 0; k < 2 * D; ++k) q.f[warp][5 + k][pos] = m[k];
+    return false;
+}
+template <int D, typename Store>
+__device__ __forceinline__ void defer_drain_hb(const IsingArgs &a, DeferQueueHB<D> &q, uint32_t warp, uint32_t lane, Store store) {
+    __syncwarp();
+    const uint32_t n = min(q.n[warp], (uint32_t)DEFER_CAP);
+    if (lane < n) {
+        uint32_t m[2 * D + 1];
+#pragma unroll
+        for (int k = 0; k < 2 * D; ++k) m[k] = q.f[warp][5 + k][lane];
+        m[2 * D] = 0u;   // the last class takes the default digit
+        const uint32_t lt = lt_mask_select_tail<2 * D + 1, true>(a, a.t, a.colour, q.f[warp][0][lane], q.f[warp][1][lane], m, q.f[warp][2][lane]);
+        store(q.f[warp][4][lane], q.f[warp][3][lane] ^ lt);
     }
 }
 
@@ -291,8 +333,8 @@ __global__ void __launch_bounds__(128, (D == 3 && K == 4 && !HB && !MEAS) ? 6 : 
     const uint32_t nstrip = (Lys + K - 1) / K;
     const uint32_t per_replica = WX * nstrip * Lzs;
     const uint32_t item = blockIdx.x * blockDim.x + threadIdx.x;
-    constexpr bool DEFER = !HB && !MEAS;   // deferred tail of the digit comparison, as in ising_int8_halfsweep
-    __shared__ DeferQueue dq;
+    constexpr bool DEFER = !MEAS;          // deferred tail of the digit comparison (both rules; recorded sweeps finish their words inline)
+    __shared__ typename std::conditional<HB, DeferQueueHB<D>, DeferQueue>::type dq;
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
     if (DEFER) { if (lane == 0u) dq.n[warp] = 0u; __syncwarp(); }
     if (item < per_replica * a.R) {
@@ -321,7 +363,9 @@ __global__ void __launch_bounds__(128, (D == 3 && K == 4 && !HB && !MEAS) ? 6 : 
     }
     const uint32_t unit0 = (y0 + Ly * z) * WX + w + g.unit_off;
     int e_sum = 0, m_sum = 0;
-    if ((DEFER || (MEAS && !HB)) && K > 1 && kend == (uint32_t)K) {
+    bool whole_strip = false;
+    if constexpr (!HB) if (K > 1 && kend == (uint32_t)K) {   // Metropolis (DEFER or MEAS)
+        whole_strip = true;
         // whole strip (the steady state): every load first, then the K heads of the digit comparison as straight-line code --
         // 2 K independent Philox chains in flight -- and only then the queue pushes and stores
         uint32_t o_row[K + 2], raw_k[K], side_k[K], zm_k[K], zp_k[K];
@@ -365,7 +409,8 @@ __global__ void __launch_bounds__(128, (D == 3 && K == 4 && !HB && !MEAS) ? 6 : 
                 if (defer_or_finish<D>(a, dq, warp, unit0 + (uint32_t)k * WX, rho, eq_k[k], mm_k[k], fresh_k[k], r * g.NW + zoff + off)) mine[zoff + off] = fresh_k[k];
             }
         }
-    } else
+    }
+    if (!whole_strip)
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         if ((uint32_t)k < kend) {
@@ -383,7 +428,12 @@ __global__ void __launch_bounds__(128, (D == 3 && K == 4 && !HB && !MEAS) ? 6 : 
             uint32_t av[6];
             av[0] = s ^ o_cur; av[1] = s ^ side; av[2] = s ^ o_prev; av[3] = s ^ o_next;
             av[4] = D == 3 ? s ^ o_zm : 0u; av[5] = D == 3 ? s ^ o_zp : 0u;
-            if constexpr (DEFER) {
+            if constexpr (DEFER && HB) {
+                uint32_t eq, mm[2 * D + 1];
+                const uint32_t unit = unit0 + (uint32_t)k * WX;
+                uint32_t fresh = ising_new_word_head_hb<D>(a, a.t, a.colour, unit, rho, raw, av, eq, mm);
+                if (defer_or_finish_hb<D>(a, dq, warp, unit, rho, eq, mm, fresh, r * g.NW + zoff + off)) mine[zoff + off] = fresh;
+            } else if constexpr (DEFER) {
                 uint32_t eq, mm[D];
                 const uint32_t unit = unit0 + (uint32_t)k * WX;
                 uint32_t fresh = ising_new_word_head<D>(a, a.t, a.colour, unit, rho, raw, av, eq, mm);
@@ -400,7 +450,10 @@ __global__ void __launch_bounds__(128, (D == 3 && K == 4 && !HB && !MEAS) ? 6 : 
     }
     if (MEAS) fused_commit(a, r, e_sum, m_sum);
     }
-    if constexpr (DEFER) {
+    if constexpr (DEFER && HB) {
+        uint32_t *base = (uint32_t *)a.s[a.colour];
+        defer_drain_hb<D>(a, dq, warp, lane, [&](uint32_t widx, uint32_t word) { base[widx] = word; });
+    } else if constexpr (DEFER) {
         uint32_t *base = (uint32_t *)a.s[a.colour];
         defer_drain<D>(a, dq, warp, lane, [&](uint32_t widx, uint32_t word) { base[widx] = word; });
     }

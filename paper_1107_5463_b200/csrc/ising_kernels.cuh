@@ -113,30 +113,37 @@ struct DeferQueue {
     uint32_t n[4];
     uint32_t f[4][DEFER_FIELDS + 1][DEFER_CAP];
 };
+// the same for the heat-bath rule: 2 D masks (the last of the 2 D + 1 classes is the default), unit, rho, eq, word, index
+template <int D>
+struct DeferQueueHB {
+    uint32_t n[4];
+    uint32_t f[4][2 * D + 5][DEFER_CAP];
+};
 
 // digit k of the threshold each lane compares against: lanes of m[th] use T(4 (th + 1)), the rest the last one
-template <int NT>
+// (HB: the heat-bath table, NT = 2 D + 1 masks by the number of neighbour terms equal to -1)
+template <int NT, bool HB = false>
 __device__ __forceinline__ uint32_t select_digit(const IsingArgs &a, const uint32_t m[NT], int dg) {
-    uint32_t tk = tab_digit<false>(a, NT - 1, dg);
+    uint32_t tk = tab_digit<HB>(a, NT - 1, dg);
 #pragma unroll
-    for (int th = NT - 2; th >= 0; --th) tk = (m[th] & tab_digit<false>(a, th, dg)) | (~m[th] & tk);
+    for (int th = NT - 2; th >= 0; --th) tk = (m[th] & tab_digit<HB>(a, th, dg)) | (~m[th] & tk);
     return tk;
 }
 
 // calls [0, DEFER_CALLS) of the comparison, unconditionally; returns lt, leaves the undecided lanes in eq
-template <int NT>
+template <int NT, bool HB = false>
 __device__ __forceinline__ uint32_t lt_mask_select_head(const IsingArgs &a, uint32_t t, uint32_t colour, uint32_t unit, uint32_t rho,
                                                         const uint32_t m[NT], uint32_t &eq_out) {
     uint32_t lt = 0u, eq = 0u;
 #pragma unroll
-    for (int th = 0; th < NT; ++th) { lt |= m[th] & tab_always<false>(a, th); eq |= m[th] & ~tab_always<false>(a, th); }
+    for (int th = 0; th < NT; ++th) { lt |= m[th] & tab_always<HB>(a, th); eq |= m[th] & ~tab_always<HB>(a, th); }
 #pragma unroll
     for (int call = 0; call < DEFER_CALLS; ++call) {
         uint32_t w[4];
         philox4x32_10(unit, rho, t, make_tag(colour, DOM_ISING_UPDATE, call), a.keys, w);
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-            const uint32_t tk = select_digit<NT>(a, m, 4 * call + k);
+            const uint32_t tk = select_digit<NT, HB>(a, m, 4 * call + k);
             lt |= eq & ~w[k] & tk;
             eq &= ~(w[k] ^ tk);
         }
@@ -146,7 +153,7 @@ __device__ __forceinline__ uint32_t lt_mask_select_head(const IsingArgs &a, uint
 }
 
 // calls [DEFER_CALLS, 8) for the lanes still in eq, lazily; returns the lanes that turn out to have U < T
-template <int NT>
+template <int NT, bool HB = false>
 __device__ __forceinline__ uint32_t lt_mask_select_tail(const IsingArgs &a, uint32_t t, uint32_t colour, uint32_t unit, uint32_t rho,
                                                         const uint32_t m[NT], uint32_t eq) {
     uint32_t lt = 0u;
@@ -156,7 +163,7 @@ __device__ __forceinline__ uint32_t lt_mask_select_tail(const IsingArgs &a, uint
         philox4x32_10(unit, rho, t, make_tag(colour, DOM_ISING_UPDATE, call), a.keys, w);
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
-            const uint32_t tk = select_digit<NT>(a, m, 4 * call + k);
+            const uint32_t tk = select_digit<NT, HB>(a, m, 4 * call + k);
             lt |= eq & ~w[k] & tk;
             eq &= ~(w[k] ^ tk);
         }
