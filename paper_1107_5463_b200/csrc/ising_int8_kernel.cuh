@@ -233,10 +233,11 @@ __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(cons
     const uint32_t nstrip = (Lys + K - 1) / K;
     const uint32_t per_replica = WX * nstrip * Lzs;
     const uint32_t item = blockIdx.x * blockDim.x + threadIdx.x;
-    // The deferred tail of the digit comparison (ising_bitpack_strip_halfsweep) is compiled out here: measured on B200 the
-    // queue's live state pushes the d = 2 instance past its 72 registers (7 CTAs per SM): 87.7 us against 72.8 us without
-    constexpr bool DEFER = false;
-    __shared__ DeferQueue dq;
+    // The deferred tail of the digit comparison (ising_bitpack_strip_halfsweep) is compiled out for Metropolis: measured on B200
+    // the queue's live state pushes the d = 2 instance past its 72 registers (7 CTAs per SM): 87.7 us against 72.8 us without.
+    // The heat-bath rule, whose inline tail is longer, gains from it: 2D L = 16384 83.5 -> 78.1 us, 3D L = 512 47.4 us (= Metropolis)
+    constexpr bool DEFER = HB && !MEAS;
+    __shared__ typename std::conditional<HB, DeferQueueHB<D>, DeferQueue>::type dq;
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31u;
     if (DEFER) { if (lane == 0u) dq.n[warp] = 0u; __syncwarp(); }
     if (item < per_replica * a.R) {
@@ -294,10 +295,15 @@ __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(cons
             if (D == 3) { av[4] = s ^ o_zm; av[5] = s ^ o_zp; }
             const uint32_t unit = unit0 + (uint32_t)k * WX;
             if (D == 2) { av[4] = 0u; av[5] = 0u; }
-            if constexpr (DEFER) {
+            if constexpr (DEFER && HB) {
+                uint32_t eq, mm[2 * D + 1];
+                uint32_t fresh = ising_new_word_head_hb<D>(a, a.t, a.colour, unit, rho, raw, av, eq, mm);
+                // index of the unit in the whole colour array (32-byte units)
+                const uint32_t uidx = (uint32_t)(((size_t)r * g.Nh + zoff + off) >> 5);
+                if (defer_or_finish_hb<D>(a, dq, warp, unit, rho, eq, mm, fresh, uidx)) int8_store_unit(mine + zoff + off, fresh);
+            } else if constexpr (DEFER) {
                 uint32_t eq, mm[D];
                 uint32_t fresh = ising_new_word_head<D>(a, a.t, a.colour, unit, rho, raw, av, eq, mm);
-                // index of the unit in the whole colour array (32-byte units)
                 const uint32_t uidx = (uint32_t)(((size_t)r * g.Nh + zoff + off) >> 5);
                 if (defer_or_finish<D>(a, dq, warp, unit, rho, eq, mm, fresh, uidx)) int8_store_unit(mine + zoff + off, fresh);
             } else {
@@ -312,7 +318,10 @@ __global__ void __launch_bounds__(128, D == 2 ? 7 : 4) ising_int8_halfsweep(cons
     }
     if (MEAS) fused_commit(a, r, e_sum, m_sum);
     }
-    if constexpr (DEFER) {
+    if constexpr (DEFER && HB) {
+        uint8_t *base = (uint8_t *)a.s[a.colour];
+        defer_drain_hb<D>(a, dq, warp, lane, [&](uint32_t uidx, uint32_t word) { int8_store_unit(base + 32u * (size_t)uidx, word); });
+    } else if constexpr (DEFER) {
         uint8_t *base = (uint8_t *)a.s[a.colour];
         defer_drain<D>(a, dq, warp, lane, [&](uint32_t uidx, uint32_t word) { int8_store_unit(base + 32u * (size_t)uidx, word); });
     }
