@@ -251,7 +251,12 @@ enum { SPIN_OPT_PLAIN_KERNELS = 0,
         * words of `value` replicas are kept in L2 from half-sweep to half-sweep ("evict_last"), the other coupling words are
         * streamed ("evict_first").  -1 (default) = as many replicas as fit in two thirds of L2 when the working set exceeds
         * L2, -2 = no hints.  A pure performance hint. */
-       SPIN_OPT_L2_KEEP = 6 };
+       SPIN_OPT_L2_KEEP = 6,
+       /* Capacity (0 .. 32, default 32) of the per-warp queue of the deferred digit comparison (bit-packed / int8 strip
+        * kernels, own-stream +-J kernel): a thread that finds the queue full finishes its word itself.  Results do not
+        * depend on it (the same digits decide either way); 0 finishes every word inline.  Exists so that the overflow
+        * path, which a full queue takes about once in 10^6 warps, can be exercised by tests. */
+       SPIN_OPT_DEFER_CAP = 7 };
 spin_status spin_set_option(spin_system *s, int32_t option, int64_t value);
 
 /* Frees the handle only; never the workspace. */

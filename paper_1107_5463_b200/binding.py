@@ -21,6 +21,7 @@ OPT_KERNEL_VARIANT = 3
 OPT_TEMPORAL_BLOCKING = 4
 OPT_TBLOCK_ROWS = 5
 OPT_L2_KEEP = 6
+OPT_DEFER_CAP = 7
 UPDATE_METROPOLIS, UPDATE_HEATBATH = 0, 1
 _RULE = {"metropolis": UPDATE_METROPOLIS, "heatbath": UPDATE_HEATBATH}
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_WORKSPACE_TOO_SMALL, ERR_CUDA, ERR_STATE = range(6)

@@ -116,7 +116,7 @@ __device__ __forceinline__ bool defer_or_finish(const IsingArgs &a, DeferQueue &
                                                 uint32_t eq, const uint32_t m[D], uint32_t &word, uint32_t index) {
     if (eq == 0u) return true;
     const uint32_t pos = atomicAdd(&q.n[warp], 1u);
-    if (pos >= (uint32_t)DEFER_CAP) {
+    if (pos >= a.defer_cap) {
         word ^= lt_mask_select_tail<D>(a, a.t, a.colour, unit, rho, m, eq);
         return true;
     }
@@ -131,7 +131,7 @@ __device__ __forceinline__ bool defer_or_finish(const IsingArgs &a, DeferQueue &
 template <int D, typename Store>
 __device__ __forceinline__ void defer_drain(const IsingArgs &a, DeferQueue &q, uint32_t warp, uint32_t lane, Store store) {
     __syncwarp();
-    const uint32_t n = min(q.n[warp], (uint32_t)DEFER_CAP);
+    const uint32_t n = min(q.n[warp], a.defer_cap);
     if (lane < n) {
         uint32_t m[D];
         m[0] = q.f[warp][3][lane];
@@ -159,7 +159,7 @@ __device__ __forceinline__ bool defer_or_finish_hb(const IsingArgs &a, DeferQueu
                                                    uint32_t eq, const uint32_t m[2 * D + 1], uint32_t &word, uint32_t index) {
     if (eq == 0u) return true;
     const uint32_t pos = atomicAdd(&q.n[warp], 1u);
-    if (pos >= (uint32_t)DEFER_CAP) {
+    if (pos >= a.defer_cap) {
         word ^= lt_mask_select_tail<2 * D + 1, true>(a, a.t, a.colour, unit, rho, m, eq);
         return true;
     }
@@ -171,7 +171,7 @@ __device__ __forceinline__ bool defer_or_finish_hb(const IsingArgs &a, DeferQueu
 template <int D, typename Store>
 __device__ __forceinline__ void defer_drain_hb(const IsingArgs &a, DeferQueueHB<D> &q, uint32_t warp, uint32_t lane, Store store) {
     __syncwarp();
-    const uint32_t n = min(q.n[warp], (uint32_t)DEFER_CAP);
+    const uint32_t n = min(q.n[warp], a.defer_cap);
     if (lane < n) {
         uint32_t m[2 * D + 1];
 #pragma unroll

@@ -28,6 +28,7 @@ struct IsingArgs {
     void *alt[2];           // temporal blocking (ising_tblock_kernel.cuh): the second pair of colour arrays it writes to
     uint32_t tb_rows;       // temporal blocking: rows per stripe
     uint32_t l2_keep;       // +-J quad kernel: replicas whose coupling words are loaded "evict_last" (0xFFFFFFFF: no L2 hints)
+    uint32_t defer_cap;     // deferred digit comparison: queue entries per warp in use (<= DEFER_CAP; SPIN_OPT_DEFER_CAP)
     uint32_t prefetch;      // L2 prefetch distance (0 = off): replicas ahead (+-J quad kernel) / CTAs ahead (strip kernels)
 };
 

@@ -75,6 +75,7 @@ struct spin_system {
     int tblock_rows;     // SPIN_OPT_TBLOCK_ROWS: rows per stripe, 0 = one wave of resident CTAs
     int tblock_ok;       // this handle has the second pair of arrays
     int variant;         // SPIN_OPT_KERNEL_VARIANT: 0 = the default kernel of each family, > 0 = a named alternative (A/B knob)
+    int defer_cap;       // SPIN_OPT_DEFER_CAP: queue entries per warp of the deferred digit comparison (default DEFER_CAP)
     int l2_keep;         // SPIN_OPT_L2_KEEP: -1 automatic, -2 no L2 eviction hints, >= 0 replicas whose coupling words are kept in L2
     int l2_bytes;        // L2 size of the device
     int l2_prefetch;     // SPIN_OPT_L2_PREFETCH: -1 each kernel's own distance (default), 0 off, > 0 that distance
@@ -351,6 +352,7 @@ static IsingArgs ising_args(const spin_system *s) {
     a.acc_slots = acc_slots_for(s->R);
     // +-J quad kernel: L2 eviction hints when spins + coupling words do not fit in L2 anyway: keep the spins and the coupling words
     // of as many replicas as fit in two thirds of L2 (measured at 256^3 x 16: 4 .. 8 replicas 28.8 us, 0 30.8, 12 32.4, no hints 32.9)
+    a.defer_cap = (uint32_t)s->defer_cap;
     a.l2_keep = 0xFFFFFFFFu;
     if (s->l2_keep >= 0) a.l2_keep = (uint32_t)s->l2_keep;
     else if (s->l2_keep == -1 && s->lay.bytes_bonds && s->l2_bytes > 0) {
@@ -1075,7 +1077,7 @@ spin_status spin_create(const spin_config *cfg, void *d_workspace, size_t bytes,
     s->tma_ok = 0; s->use_tma = -1; s->tma_ty = 0;
     s->t = 0; s->launches = 0; s->staging = nullptr; s->staging_bytes = 0; s->set_pending = 0; s->h_res = nullptr; s->gexec = nullptr; s->cap_stream = nullptr; s->gnodes = nullptr; s->n_gnodes = 0;
     // 128 threads per CTA for the Ising fast paths (measured: +-J R = 16 39.1 vs 40.4 us with 256)
-    s->block = (dv.path == PATH_ISING_INT8 || dv.path == PATH_ISING_BITPACK || dv.path == PATH_ISING_MSC) ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0; s->l2_prefetch = -1; s->l2_keep = -1; s->l2_bytes = 0; s->variant = 0; s->tblock = -1; s->tblock_rows = 0; s->tblock_ok = tblock_offered(cfg, dv) ? 1 : 0;
+    s->block = (dv.path == PATH_ISING_INT8 || dv.path == PATH_ISING_BITPACK || dv.path == PATH_ISING_MSC) ? 128 : 256; s->grid_num = 1; s->grid_den = 1; s->strip_rows = 4; s->strip_rows_set = 0; s->vector_generic = 0; s->l2_prefetch = -1; s->l2_keep = -1; s->defer_cap = DEFER_CAP; s->l2_bytes = 0; s->variant = 0; s->tblock = -1; s->tblock_rows = 0; s->tblock_ok = tblock_offered(cfg, dv) ? 1 : 0;
     s->table_beta = std::nan("");
     Geometry &g = s->g;
     g.Lx = dv.pad[0]; g.Ly = dv.pad[1]; g.Lz = dv.pad[2]; g.d = dv.d;
@@ -1795,6 +1797,12 @@ spin_status spin_set_option(spin_system *s, int32_t option, int64_t value) {
     if (option == SPIN_OPT_L2_KEEP) {
         if (value < -2 || value > 65535) return fail(SPIN_ERR_INVALID_ARG, "SPIN_OPT_L2_KEEP takes -2 (no hints), -1 (automatic) or a number of replicas");
         s->l2_keep = (int)value;
+        graph_drop(s);
+        return SPIN_OK;
+    }
+    if (option == SPIN_OPT_DEFER_CAP) {
+        if (value < 0 || value > DEFER_CAP) return fail(SPIN_ERR_INVALID_ARG, "SPIN_OPT_DEFER_CAP takes 0 .. %d", DEFER_CAP);
+        s->defer_cap = (int)value;
         graph_drop(s);
         return SPIN_OK;
     }
