@@ -63,6 +63,21 @@ void rand4(uint64_t seed, uint32_t unit, uint32_t rho, uint32_t t, uint32_t tag,
 
 uint32_t make_tag(int colour, int domain, int call) { return (uint32_t)colour + 16u * (uint32_t)domain + 256u * (uint32_t)call; }
 
+/* Words of the n >= 2 update of the site with compressed same-colour index j (R-16b):
+ * n = 3 takes three words, so every site has its own call rand(j, ...);
+ * n = 2 takes two (angle, acceptance), so sites 2k and 2k + 1 of a colour share the call rand(k, ...):
+ * the even one takes words 0 and 1, the odd one words 2 and 3 (returned as w[0], w[1]). */
+void vector_site_words(uint64_t seed, int n, uint64_t j, uint32_t rho, uint32_t t, int colour, uint32_t w[4]) {
+    if (n == 2) {
+        uint32_t c[4];
+        rand4(seed, (uint32_t)(j >> 1), rho, t, make_tag(colour, DOMAIN_VECTOR_UPDATE, 0), c);
+        const int o = (int)(j & 1u) * 2;
+        w[0] = c[o]; w[1] = c[o + 1]; w[2] = 0u; w[3] = 0u;
+    } else {
+        rand4(seed, (uint32_t)j, rho, t, make_tag(colour, DOMAIN_VECTOR_UPDATE, 0), w);
+    }
+}
+
 /* Bit-plane contract (R-16): the 32-bit acceptance uniform of lane `lane` of a
  * unit has digit k (k = 0 is the most significant) equal to bit `lane` of word
  * (k & 3) of Philox call (k >> 2). */
@@ -316,7 +331,7 @@ int64_t sweep_vector(oracle_system &S, double beta) {
                         const int64_t i = S.site(x, y, z);
                         const int64_t j = S.compressed(x, y, z);
                         uint32_t w[4];
-                        rand4(S.seed, (uint32_t)j, rho, t32, make_tag(colour, DOMAIN_VECTOR_UPDATE, 0), w);
+                        vector_site_words(S.seed, n, (uint64_t)j, rho, t32, colour, w);
                         float snew[3] = {0.0f, 0.0f, 0.0f};
                         uint32_t w_accept;
                         if (n == 3) { direction3(w[0], w[1], snew); w_accept = w[2]; }
@@ -366,6 +381,10 @@ void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t
 
 void oracle_rand(uint64_t seed, uint32_t unit, uint32_t rho, uint32_t t, uint32_t tag, uint32_t out[4]) {
     rand4(seed, unit, rho, t, tag, out);
+}
+
+void oracle_vector_site_words(uint64_t seed, int n, uint64_t j, uint32_t rho, uint32_t t, int colour, uint32_t out[4]) {
+    vector_site_words(seed, n, j, rho, t, colour, out);
 }
 
 uint32_t oracle_ising_uniform(uint64_t seed, uint64_t j, uint32_t rho, uint32_t t, int colour) {

@@ -141,7 +141,12 @@ __global__ void __launch_bounds__(256) vector_halfsweep(const __grid_constant__ 
             }
         }
         uint32_t w[4];
-        philox4x32_10(j + g.j_off, a.replica_streams ? r + a.rho_off : 0u, a.t, make_tag(a.colour, DOM_VECTOR_UPDATE, 0), a.keys, w);
+        {
+            // n = 3: a call per site; n = 2: sites 2k, 2k + 1 of a colour share the call of unit k (words 0, 1 / 2, 3; R-16b)
+            const uint32_t jg = j + g.j_off;
+            philox4x32_10(NC == 2 ? jg >> 1 : jg, a.replica_streams ? r + a.rho_off : 0u, a.t, make_tag(a.colour, DOM_VECTOR_UPDATE, 0), a.keys, w);
+            if (NC == 2 && (jg & 1u)) { w[0] = w[2]; w[1] = w[3]; }
+        }
         float sn[NC];
         uint32_t wacc;
         if (NC == 3 && a.rule != 0u) {
@@ -348,8 +353,14 @@ __device__ __forceinline__ void vector_quad_accept(const VectorArgs &a, const fl
 #pragma unroll
     for (int pr = 0; pr < 2; ++pr) {
         uint32_t wa[4], wb[4];
-        philox4x32_10(ctr0 + 2 * pr, rho, a.t, tag, a.keys, wa);
-        philox4x32_10(ctr0 + 2 * pr + 1, rho, a.t, tag, a.keys, wb);
+        if (NC == 2) {
+            // the two sites of a pair share one call (R-16b; ctr0 is a multiple of 4): words 0, 1 -> first site, 2, 3 -> second
+            philox4x32_10((ctr0 >> 1) + pr, rho, a.t, tag, a.keys, wa);
+            wb[0] = wa[2]; wb[1] = wa[3];
+        } else {
+            philox4x32_10(ctr0 + 2 * pr, rho, a.t, tag, a.keys, wa);
+            philox4x32_10(ctr0 + 2 * pr + 1, rho, a.t, tag, a.keys, wb);
+        }
         if (HB && NC == 3) {
             const float2 h3[3] = {hp[pr][0], hp[pr][1], hp[pr][NC - 1]};
             float2 s3[3];

@@ -180,7 +180,7 @@ def test_full_size_vector_models(P, oracle, name):
         h = (h + np.float32(1.0) * s_nb).astype(np.float32)      # J = 1: every product and sum rounded to fp32
     mismatched = 0
     for k in range(idx.size):
-        wds = oracle.rand(seed, int(j[k]), 0, 0, int(colour[k]) + 16 * 3)
+        wds = oracle.vector_site_words(seed, n, int(j[k]), 0, 0, int(colour[k]))
         if n == 3:
             snew, wacc = oracle.direction3(wds[0], wds[1]), wds[2]
         else:
