@@ -28,7 +28,7 @@ def lib():
         L.oracle_philox4x32_10.restype = None
         L.oracle_rand.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, u32p]
         L.oracle_rand.restype = None
-        L.oracle_vector_site_words.argtypes = [C.c_uint64, C.c_int, C.c_uint64, C.c_uint32, C.c_uint32, C.c_int, u32p]
+        L.oracle_vector_site_words.argtypes = [C.c_uint64, C.c_int, C.c_int, C.c_uint64, C.c_uint32, C.c_uint32, C.c_int, u32p]
         L.oracle_vector_site_words.restype = None
         L.oracle_ising_uniform.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, C.c_int]
         L.oracle_ising_uniform.restype = C.c_uint32
@@ -91,10 +91,10 @@ def rand(seed, unit, rho, t, tag):
     return [int(v) for v in o]
 
 
-def vector_site_words(seed, n, j, rho, t, colour):
-    """words of the n >= 2 update of the site with compressed index j (n = 2: pairs of sites share a call, R-16b)"""
+def vector_site_words(seed, n, j, rho, t, colour, rule=0):
+    """words of the n >= 2 update of the site with compressed index j (n = 2 and heat bath: pairs of sites share a call, R-16b)"""
     o = (C.c_uint32 * 4)()
-    lib().oracle_vector_site_words(seed, n, j, rho, t, colour, o)
+    lib().oracle_vector_site_words(seed, n, rule, j, rho, t, colour, o)
     return [int(v) for v in o]
 
 

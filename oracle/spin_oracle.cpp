@@ -64,11 +64,11 @@ void rand4(uint64_t seed, uint32_t unit, uint32_t rho, uint32_t t, uint32_t tag,
 uint32_t make_tag(int colour, int domain, int call) { return (uint32_t)colour + 16u * (uint32_t)domain + 256u * (uint32_t)call; }
 
 /* Words of the n >= 2 update of the site with compressed same-colour index j (R-16b):
- * n = 3 takes three words, so every site has its own call rand(j, ...);
- * n = 2 takes two (angle, acceptance), so sites 2k and 2k + 1 of a colour share the call rand(k, ...):
- * the even one takes words 0 and 1, the odd one words 2 and 3 (returned as w[0], w[1]). */
-void vector_site_words(uint64_t seed, int n, uint64_t j, uint32_t rho, uint32_t t, int colour, uint32_t w[4]) {
-    if (n == 2) {
+ * the Metropolis update of n = 3 takes three words, so every site has its own call rand(j, ...);
+ * n = 2 (angle, acceptance) and the heat bath of n = 3 (polar cosine, azimuth) take two, so sites 2k and 2k + 1 of a
+ * colour share the call rand(k, ...): the even one takes words 0 and 1, the odd one words 2 and 3 (returned as w[0], w[1]). */
+void vector_site_words(uint64_t seed, int n, int rule, uint64_t j, uint32_t rho, uint32_t t, int colour, uint32_t w[4]) {
+    if (n == 2 || rule == ORACLE_RULE_HEATBATH) {
         uint32_t c[4];
         rand4(seed, (uint32_t)(j >> 1), rho, t, make_tag(colour, DOMAIN_VECTOR_UPDATE, 0), c);
         const int o = (int)(j & 1u) * 2;
@@ -331,7 +331,7 @@ int64_t sweep_vector(oracle_system &S, double beta) {
                         const int64_t i = S.site(x, y, z);
                         const int64_t j = S.compressed(x, y, z);
                         uint32_t w[4];
-                        vector_site_words(S.seed, n, (uint64_t)j, rho, t32, colour, w);
+                        vector_site_words(S.seed, n, S.rule, (uint64_t)j, rho, t32, colour, w);
                         float snew[3] = {0.0f, 0.0f, 0.0f};
                         uint32_t w_accept;
                         if (n == 3) { direction3(w[0], w[1], snew); w_accept = w[2]; }
@@ -383,8 +383,8 @@ void oracle_rand(uint64_t seed, uint32_t unit, uint32_t rho, uint32_t t, uint32_
     rand4(seed, unit, rho, t, tag, out);
 }
 
-void oracle_vector_site_words(uint64_t seed, int n, uint64_t j, uint32_t rho, uint32_t t, int colour, uint32_t out[4]) {
-    vector_site_words(seed, n, j, rho, t, colour, out);
+void oracle_vector_site_words(uint64_t seed, int n, int rule, uint64_t j, uint32_t rho, uint32_t t, int colour, uint32_t out[4]) {
+    vector_site_words(seed, n, rule, j, rho, t, colour, out);
 }
 
 uint32_t oracle_ising_uniform(uint64_t seed, uint64_t j, uint32_t rho, uint32_t t, int colour) {

@@ -54,9 +54,10 @@ void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t
  * key = (seed & 0xffffffff, seed >> 32). */
 void oracle_rand(uint64_t seed, uint32_t unit, uint32_t rho, uint32_t t, uint32_t tag, uint32_t out[4]);
 /* The random words of the n >= 2 update of one site (compressed same-colour index j): out[0], out[1] feed the proposal
- * (n = 2: out[0] the angle, out[1] the acceptance word; n = 3: out[2] the acceptance word).  n = 2: sites 2k, 2k + 1 share
- * the call of unit k (R-16b). */
-void oracle_vector_site_words(uint64_t seed, int n, uint64_t j, uint32_t rho, uint32_t t, int colour, uint32_t out[4]);
+ * (n = 2: out[0] the angle, out[1] the acceptance word; n = 3 Metropolis: out[2] the acceptance word; n = 3 heat bath:
+ * out[0] the polar cosine, out[1] the azimuth).  Updates that take two words (n = 2; heat bath) share the call of unit
+ * k between sites 2k, 2k + 1 (R-16b).  rule: ORACLE_RULE_METROPOLIS / ORACLE_RULE_HEATBATH. */
+void oracle_vector_site_words(uint64_t seed, int n, int rule, uint64_t j, uint32_t rho, uint32_t t, int colour, uint32_t out[4]);
 
 /* n = 1 acceptance uniform of the colour-`colour` site with compressed index j
  * (bit-plane contract, R-16): a 32-bit integer, MSB first digit. */

@@ -142,10 +142,12 @@ __global__ void __launch_bounds__(256) vector_halfsweep(const __grid_constant__ 
         }
         uint32_t w[4];
         {
-            // n = 3: a call per site; n = 2: sites 2k, 2k + 1 of a colour share the call of unit k (words 0, 1 / 2, 3; R-16b)
+            // n = 3 Metropolis: a call per site; updates that take two words (n = 2; heat bath): sites 2k, 2k + 1 of a colour
+            // share the call of unit k (words 0, 1 / 2, 3; R-16b)
             const uint32_t jg = j + g.j_off;
-            philox4x32_10(NC == 2 ? jg >> 1 : jg, a.replica_streams ? r + a.rho_off : 0u, a.t, make_tag(a.colour, DOM_VECTOR_UPDATE, 0), a.keys, w);
-            if (NC == 2 && (jg & 1u)) { w[0] = w[2]; w[1] = w[3]; }
+            const bool pair = NC == 2 || a.rule != 0u;
+            philox4x32_10(pair ? jg >> 1 : jg, a.replica_streams ? r + a.rho_off : 0u, a.t, make_tag(a.colour, DOM_VECTOR_UPDATE, 0), a.keys, w);
+            if (pair && (jg & 1u)) { w[0] = w[2]; w[1] = w[3]; }
         }
         float sn[NC];
         uint32_t wacc;
@@ -353,7 +355,7 @@ __device__ __forceinline__ void vector_quad_accept(const VectorArgs &a, const fl
 #pragma unroll
     for (int pr = 0; pr < 2; ++pr) {
         uint32_t wa[4], wb[4];
-        if (NC == 2) {
+        if (NC == 2 || HB) {
             // the two sites of a pair share one call (R-16b; ctr0 is a multiple of 4): words 0, 1 -> first site, 2, 3 -> second
             philox4x32_10((ctr0 >> 1) + pr, rho, a.t, tag, a.keys, wa);
             wb[0] = wa[2]; wb[1] = wa[3];
