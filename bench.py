@@ -182,8 +182,11 @@ def run_per_model(P, peak):
         S = P.from_workload(w, P.workloads.SEED, rule="heatbath")
         ms_launch, fpn, _ = time_sweeps(S, w["beta"], sweeps)
         bpu = P.workloads.BYTES_PER_UPDATE[name]
+        cnt = COUNTERS.get(name + "#heatbath", {})
         out[name + "_heatbath"] = {"flips_per_ns": fpn, "ms_per_halfsweep": ms_launch, "algorithmic_GBps": fpn * bpu,
-                                   "hbm_frac": fpn * bpu / peak, "bytes_per_update": bpu, "update_rule": "heat bath"}
+                                   "hbm_frac": fpn * bpu / peak, "bytes_per_update": bpu, "update_rule": "heat bath",
+                                   "kernel": cnt.get("kernel"), "traffic": cnt.get("dram_bytes_per_launch"),
+                                   "capture": cnt.get("capture")}
         S.close()
         del S
         torch.cuda.empty_cache()
@@ -352,7 +355,8 @@ def run_graft(args):
     P.lib()
     peak, peak_src = measured_peaks()
     w = P.workloads.WORKLOADS[args.workload]
-    S = P.from_workload(w, ranks.rank_seed(P.workloads.SEED, rank), device=dev)  # every rank: its own independent lattice
+    rule_kw = {"rule": "heatbath"} if args.rule == "heatbath" else {}
+    S = P.from_workload(w, ranks.rank_seed(P.workloads.SEED, rank), device=dev, **rule_kw)  # every rank: its own independent lattice
     for kv in args.opt:
         k, v = kv.split("=")
         S.set_option(int(k), int(v))
@@ -391,6 +395,8 @@ def run_graft(args):
     # counters of the kernel that ran: with --opt another kernel may serve the workload -- its capture if there is one
     # (profiles/counters.json "<workload>#<variant>"), else none (null traffic rather than another kernel's numbers)
     variant = {("4=0",): "#strip", ("1=1",): "#tma"}.get(tuple(args.opt)) if args.opt else ""
+    if args.rule == "heatbath":
+        variant = "#heatbath" if not args.opt else None
     cnt = COUNTERS.get(args.workload + variant, {}) if variant is not None else {}
     ms_total = max_over_ranks(e0.elapsed_time(e1))
     ms_sweeps = sum(a.elapsed_time(b) for a, b in sweep_ev)
@@ -450,7 +456,7 @@ def run_graft(args):
                    "l2": "state (%.0f MB) larger than L2 (126 MB); no flush needed" % (w["dims"][0] * w["dims"][1] * w["dims"][2] * w["replicas"] / 1e6)
                    if w["storage"] != "bitpack" else "bit-packed state is L2-resident by design (33.5 MB); not flushed",
                    "parallelism": "independent lattice per GPU (weak scaling, no collective)" if world > 1 else "1 GPU",
-                   "options": args.opt},
+                   "options": args.opt, "update_rule": args.rule},
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "roofline": {"bound": "hbm", "kernel": cnt.get("kernel", "half-sweep of %s" % args.workload), "achieved": achieved,
                      "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": cnt.get("dram_bytes_per_launch"),
@@ -512,6 +518,8 @@ def main():
     ap.add_argument("--opt", action="append", default=[], metavar="ID=VALUE",
                     help="spin_set_option(ID, VALUE) on the timed handle (A/B of kernel variants, e.g. 1=1: TMA-staged kernel, "
                          "4=0: no temporal blocking); repeatable")
+    ap.add_argument("--rule", default="metropolis", choices=["metropolis", "heatbath"],
+                    help="update rule of the timed handle (heat bath: SURVEY f1; the per-model legs time it on three lattices)")
     ap.add_argument("--no-per-model", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
