@@ -158,7 +158,9 @@ def run_per_model(P, peak):
                 # executed warp-instructions per launch (committed ncu capture) / launch time, against the issue rate; the
                 # pipe that binds is the ALU pipe (LOP3 / IADD3 / SHF / ISETP at one warp-instruction per 2 clocks)
                 ms_launch = 2 * sweeps * ms_half / launches
-                gwips = cnt["warp_instr_per_launch"] / (ms_launch * 1e6)
+                # the capture's instruction count, scaled if a launch here serves more updates (resident kernels: a launch per call)
+                scale = (S.N * S.R * sweeps / launches) / cnt["updates_per_launch"] if cnt.get("updates_per_launch") else 1.0
+                gwips = cnt["warp_instr_per_launch"] * scale / (ms_launch * 1e6)
                 out[name]["roofline"] = {"bound": "alu", "achieved": gwips, "peak": ISSUE_PEAK_GWIPS, "unit": "Gwarp-instr/s",
                                          "frac": gwips / ISSUE_PEAK_GWIPS, "traffic": cnt.get("dram_bytes_per_launch"),
                                          "alu_pipe_busy_pct_in_capture": cnt.get("alu_pipe_pct"),
@@ -473,7 +475,10 @@ def run_graft(args):
         wi = cnt["warp_instr_per_launch"] * (updates_per_launch / cnt["updates_per_launch"])
         line["roofline"].update({"issue_frac": wi / (ms_launch * 1e6) / ISSUE_PEAK_GWIPS,
                                  "alu_pipe_busy_pct_in_capture": cnt.get("alu_pipe_pct")})
-    if updates_per_launch > S_N_R:
+    if updates_per_launch > S_N_R and "tblock" not in str(cnt.get("kernel", "tblock")):
+        line["roofline"]["note"] = ("one launch = all sweeps of the call with the state resident in shared memory: the HBM fraction on "
+                                    "algorithmic bytes is nominal (frac > 1 is possible); the kernel is bound by instruction issue")
+    elif updates_per_launch > S_N_R:
         line["roofline"]["note"] = ("exact temporal blocking (SURVEY f3): one launch = two full sweeps, each row read once and written "
                                     "once, so the DRAM traffic is a third of the algorithmic 3 B per update the fraction is quoted on "
                                     "(frac > 1 is that saving, not idle work); the kernel is bound by the integer ALU pipe")

@@ -14,6 +14,7 @@
 #include "ising_msc_kernel.cuh"
 #include "ising_pmj_own_kernel.cuh"
 #include "ising_resident_kernel.cuh"
+#include "ising_resident_pmj_kernel.cuh"
 #include "ising_tblock_kernel.cuh"
 #include "measure_kernels.cuh"
 #include "setup_kernels.cuh"
@@ -1174,6 +1175,46 @@ spin_status spin_destroy(spin_system *s) {
     return SPIN_OK;
 }
 
+// Many +-J realisations of a small lattice with a shared update stream (bit-packed, Metropolis): groups of realisations stay in
+// shared memory for all n_sweeps sweeps of the call (ising_resident_pmj_kernel.cuh).  G = realisations per CTA: a multiple of the
+// RG threads per word position, about two CTAs per SM, within RPMJ_SMEM_MAX bytes of shared memory (two CTAs per SM).
+constexpr size_t RPMJ_SMEM_MAX = 100 * 1024;
+static uint32_t resident_pmj_group(const spin_system *s) {
+    const uint32_t NW = (uint32_t)s->g.NW;
+    if (NW == 0 || NW > (uint32_t)RPMJ_THREADS || RPMJ_THREADS % NW != 0) return 0;
+    const uint32_t RG = RPMJ_THREADS / NW;
+    uint64_t G = RG * ((s->R + (uint64_t)RG * 2 * s->sm_count - 1) / ((uint64_t)RG * 2 * s->sm_count));
+    while (G > RG && 4 * rpmj_smem_words((uint32_t)G, NW, s->d) > RPMJ_SMEM_MAX) G -= RG;
+    while (G > 1 && 4 * rpmj_smem_words((uint32_t)G, NW, s->d) > RPMJ_SMEM_MAX) G -= 1;
+    if (4 * rpmj_smem_words((uint32_t)G, NW, s->d) > RPMJ_SMEM_MAX) return 0;
+    return (uint32_t)G;
+}
+static bool resident_pmj_ok(const spin_system *s) {
+    if (s->variant == 1) return false;   // A/B: one launch per half-sweep (ising_bitpack_halfsweep / the quad kernels)
+    if (s->vector_generic || s->n != 1 || s->axis >= 0 || s->path != PATH_ISING_BITPACK) return false;
+    if (s->cfg.coupling_kind != SPIN_J_BOND_PM1 || s->cfg.update_rule != SPIN_UPDATE_METROPOLIS) return false;
+    if (!(s->R > 1 && !s->cfg.replica_streams)) return false;
+    return resident_pmj_group(s) != 0;
+}
+static spin_status enqueue_resident_pmj(spin_system *s, int64_t n_sweeps, cudaStream_t st) {
+    const uint32_t G = resident_pmj_group(s);
+    const size_t smem = 4 * rpmj_smem_words(G, (uint32_t)s->g.NW, s->d);
+    const unsigned grid = (unsigned)((s->R + G - 1) / G);
+    if (s->d == 2) CUDA_TRY(cudaFuncSetAttribute(ising_resident_pmj_sweeps<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    else CUDA_TRY(cudaFuncSetAttribute(ising_resident_pmj_sweeps<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    while (n_sweeps > 0) {
+        const uint32_t chunk = (uint32_t)(n_sweeps > (1 << 20) ? (1 << 20) : n_sweeps);
+        const IsingArgs a = ising_args(s);
+        if (s->d == 2) ising_resident_pmj_sweeps<2><<<grid, RPMJ_THREADS, smem, st>>>(a, chunk, G);
+        else ising_resident_pmj_sweeps<3><<<grid, RPMJ_THREADS, smem, st>>>(a, chunk, G);
+        CUDA_TRY(cudaGetLastError());
+        s->launches += 1;
+        s->t += chunk;
+        n_sweeps -= chunk;
+    }
+    return SPIN_OK;
+}
+
 spin_status spin_sweep(spin_system *s, double beta, int64_t n_sweeps, void *stream) {
     spin_status rc = check_sweep_args(s, beta, n_sweeps);
     if (rc != SPIN_OK) return rc;
@@ -1185,6 +1226,7 @@ spin_status spin_sweep(spin_system *s, double beta, int64_t n_sweeps, void *stre
         if (rc != SPIN_OK) return rc;
         n_sweeps &= 1;
     } else if (resident_ok(s, false)) return enqueue_resident(s, n_sweeps, nullptr, nullptr, (cudaStream_t)stream);
+    else if (resident_pmj_ok(s)) return enqueue_resident_pmj(s, n_sweeps, (cudaStream_t)stream);
     if (graph_ok(s, n_sweeps)) {
         int64_t done = 0;
         rc = graph_sweeps(s, beta, n_sweeps, (cudaStream_t)stream, &done);
