@@ -23,6 +23,54 @@ __host__ __device__ inline size_t rpmj_smem_words(uint32_t G, uint32_t NW, int D
     return (size_t)2 * G * NW * (1 + D) + (size_t)RPMJ_THREADS * D;
 }
 
+// one half-sweep of colour C over the replicas rg, rg + RG, ... of the group: word position gi, masks m[NT] of this half-sweep.
+// The colour is a template parameter so that the four array bases are fixed offsets and only rr NW moves in the loop.
+template <int D, int C>
+__device__ __forceinline__ void rpmj_half(uint32_t *sp, const uint32_t *bd, const uint32_t *m, const WordNbrs &n, uint32_t jneg,
+                                          uint32_t G, uint32_t Gc, uint32_t NW, uint32_t RG, uint32_t gi, uint32_t rg) {
+    constexpr int NT = D;
+    uint32_t ltf[NT];
+#pragma unroll
+    for (int th = 0; th < NT; ++th) ltf[th] = m[th];
+    const uint32_t *other = sp + ((1 - C) * G + rg) * NW;
+    uint32_t *mine = sp + (C * G + rg) * NW;
+    const uint32_t *bo = bd + ((C * G + rg) * D) * NW;           // own forward bonds
+    const uint32_t *bt = bd + (((1 - C) * G + rg) * D) * NW;     // the other colour's
+    const uint32_t step = RG * NW, bstep = step * D;
+    for (uint32_t rr = rg; rr < Gc; rr += RG, other += step, mine += step, bo += bstep, bt += bstep) {
+        // unsatisfied-bond masks exactly as unsatisfied_bonds<D, true> forms them
+        const uint32_t raw = mine[gi];
+        const uint32_t s = jneg ? ~raw : raw;
+        const uint32_t o = other[gi], os = other[n.g_side];
+        const uint32_t side = n.p ? ((o >> 1) | (os << 31)) : ((o << 1) | (os >> 31));
+        uint32_t av[6];
+        av[0] = s ^ o; av[1] = s ^ side; av[2] = s ^ other[n.g_ym]; av[3] = s ^ other[n.g_yp];
+        av[4] = 0u; av[5] = 0u;
+        if (D == 3) { av[4] = s ^ other[n.g_zm]; av[5] = s ^ other[n.g_zp]; }
+        const uint32_t bx_own = bo[gi], bx_oth = bt[gi];
+        if (n.p) { av[0] ^= bx_oth; av[1] ^= bx_own; }
+        else { av[0] ^= bx_own; av[1] ^= (bx_oth << 1) | (bt[n.g_side] >> 31); }
+        av[2] ^= bt[NW + n.g_ym];
+        av[3] ^= bo[NW + gi];
+        if (D == 3) { av[4] ^= bt[2 * NW + n.g_zm]; av[5] ^= bo[2 * NW + gi]; }
+        // the flip mask of bitpack_update_word<D, true, true>
+        uint32_t flip;
+        if (D == 2) {
+            const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
+            const uint32_t ge2 = c1 | (s1 & av[3]), ge1 = av[0] | av[1] | av[2] | av[3];
+            flip = ge2 | (ge1 & ltf[0]) | ltf[1];
+        } else {
+            const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
+            const uint32_t s2 = av[3] ^ av[4] ^ av[5], c2 = maj3(av[3], av[4], av[5]);
+            const uint32_t b0 = s1 ^ s2, c3 = s1 & s2;
+            const uint32_t b1 = c1 ^ c2 ^ c3, b2 = maj3(c1, c2, c3);
+            const uint32_t ge3 = b2 | (b1 & b0);
+            flip = ge3 | ((b1 | b2) & ltf[0]) | ((b0 | b1 | b2) & ltf[1]) | ltf[2];
+        }
+        mine[gi] = raw ^ flip;
+    }
+}
+
 template <int D>
 __global__ void __launch_bounds__(RPMJ_THREADS) ising_resident_pmj_sweeps(const __grid_constant__ IsingArgs a, uint32_t n_sweeps,
                                                                             uint32_t G) {
@@ -61,47 +109,9 @@ __global__ void __launch_bounds__(RPMJ_THREADS) ising_resident_pmj_sweeps(const 
         __syncthreads();
         const uint32_t hn = min(RG, HS - h0);
         for (uint32_t hh = 0; hh < hn; ++hh) {
-            const uint32_t c = (h0 + hh) & 1u;
-            const WordNbrs n = c ? nb1 : nb0;
-            uint32_t ltf[NT];
-#pragma unroll
-            for (int th = 0; th < NT; ++th) ltf[th] = mk[(hh * NW + gi) * NT + th];
-            for (uint32_t rr = rg; rr < Gc; rr += RG) {
-                const uint32_t *other = sp + ((1u - c) * G + rr) * NW;
-                uint32_t *mine = sp + (c * G + rr) * NW;
-                const uint32_t *bo = bd + ((c * G + rr) * D) * NW;           // own forward bonds
-                const uint32_t *bt = bd + (((1u - c) * G + rr) * D) * NW;    // the other colour's
-                // unsatisfied-bond masks exactly as unsatisfied_bonds<D, true> forms them
-                const uint32_t raw = mine[gi];
-                const uint32_t s = a.jneg ? ~raw : raw;
-                const uint32_t o = other[gi], os = other[n.g_side];
-                const uint32_t side = n.p ? ((o >> 1) | (os << 31)) : ((o << 1) | (os >> 31));
-                uint32_t av[6];
-                av[0] = s ^ o; av[1] = s ^ side; av[2] = s ^ other[n.g_ym]; av[3] = s ^ other[n.g_yp];
-                av[4] = 0u; av[5] = 0u;
-                if (D == 3) { av[4] = s ^ other[n.g_zm]; av[5] = s ^ other[n.g_zp]; }
-                const uint32_t bx_own = bo[gi], bx_oth = bt[gi];
-                if (n.p) { av[0] ^= bx_oth; av[1] ^= bx_own; }
-                else { av[0] ^= bx_own; av[1] ^= (bx_oth << 1) | (bt[n.g_side] >> 31); }
-                av[2] ^= bt[NW + n.g_ym];
-                av[3] ^= bo[NW + gi];
-                if (D == 3) { av[4] ^= bt[2 * NW + n.g_zm]; av[5] ^= bo[2 * NW + gi]; }
-                // the flip mask of bitpack_update_word<D, true, true>
-                uint32_t flip;
-                if (D == 2) {
-                    const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
-                    const uint32_t ge2 = c1 | (s1 & av[3]), ge1 = av[0] | av[1] | av[2] | av[3];
-                    flip = ge2 | (ge1 & ltf[0]) | ltf[1];
-                } else {
-                    const uint32_t s1 = av[0] ^ av[1] ^ av[2], c1 = maj3(av[0], av[1], av[2]);
-                    const uint32_t s2 = av[3] ^ av[4] ^ av[5], c2 = maj3(av[3], av[4], av[5]);
-                    const uint32_t b0 = s1 ^ s2, c3 = s1 & s2;
-                    const uint32_t b1 = c1 ^ c2 ^ c3, b2 = maj3(c1, c2, c3);
-                    const uint32_t ge3 = b2 | (b1 & b0);
-                    flip = ge3 | ((b1 | b2) & ltf[0]) | ((b0 | b1 | b2) & ltf[1]) | ltf[2];
-                }
-                mine[gi] = raw ^ flip;
-            }
+            const uint32_t *m = mk + (hh * NW + gi) * NT;
+            if ((h0 + hh) & 1u) rpmj_half<D, 1>(sp, bd, m, nb1, a.jneg, G, Gc, NW, RG, gi, rg);
+            else rpmj_half<D, 0>(sp, bd, m, nb0, a.jneg, G, Gc, NW, RG, gi, rg);
             __syncthreads();
         }
     }
