@@ -236,7 +236,7 @@ enum { SPIN_OPT_PLAIN_KERNELS = 0,
        SPIN_OPT_L2_PREFETCH = 2,
        /* A/B knob: 0 (default) = the tuned kernel of each family; 1 = the alternative kept beside it
         * (+-J shared stream: one thread per quad and all replicas, instead of the cooperative kernel with one CTA of replica-chunk warps per 32 quads;
-        * many +-J realisations of a lattice of at most 512 words per colour, shared stream, Metropolis: one launch per half-sweep instead of the
+        * many +-J realisations of a lattice of at most 512 words per colour, shared stream: one launch per half-sweep instead of the
         * kernel that keeps groups of realisations in shared memory for all sweeps of a spin_sweep call).  Results never
         * depend on it. */
        SPIN_OPT_KERNEL_VARIANT = 3,

@@ -3,7 +3,7 @@
 // a CTA keeps a group of G realisations -- spins of both colours and all coupling words -- in shared memory and runs
 // ALL n_sweeps sweeps of a spin_sweep call in one launch (the tile stays on chip for k updates; here
 // the tile is the whole lattice of each realisation, so the dynamics is the plain checkerboard sweep, bit for bit
-// that of ising_bitpack_halfsweep<D, true, true>).  One launch per half-sweep leaves such systems launch- and
+// that of ising_bitpack_halfsweep<D, true, true>, or of ising_bitpack_halfsweep_hb<D, true, true> under the heat-bath rule).  One launch per half-sweep leaves such systems launch- and
 // latency-bound (4.6 us per half-sweep of 4096 x 64^2 in a CUDA graph, 0.24 of HBM).
 //
 // Work decomposition: blockDim = NW * RG threads; thread (gi, rg) serves word position gi of the replicas rg,
@@ -18,17 +18,18 @@ namespace spin {
 
 constexpr int RPMJ_THREADS = 512;
 
-// shared-memory words of a CTA: spins [2][G][NW], coupling words [2][G][D][NW], masks [RG][NW][D] (RG NW = RPMJ_THREADS)
-__host__ __device__ inline size_t rpmj_smem_words(uint32_t G, uint32_t NW, int D) {
-    return (size_t)2 * G * NW * (1 + D) + (size_t)RPMJ_THREADS * D;
+// shared-memory words of a CTA: spins [2][G][NW], coupling words [2][G][D][NW], masks [RG][NW][NT] (RG NW = RPMJ_THREADS);
+// NT = D thresholds (Metropolis: dE = 4, 8, 12) or 2 D + 1 probabilities (heat bath: 0 .. 2 D neighbour terms equal to -1)
+__host__ __device__ inline size_t rpmj_smem_words(uint32_t G, uint32_t NW, int D, bool hb) {
+    return (size_t)2 * G * NW * (1 + D) + (size_t)RPMJ_THREADS * (hb ? 2 * D + 1 : D);
 }
 
 // one half-sweep of colour C over the replicas rg, rg + RG, ... of the group: word position gi, masks m[NT] of this half-sweep.
 // The colour is a template parameter so that the four array bases are fixed offsets and only rr NW moves in the loop.
-template <int D, int C>
+template <int D, int C, bool HB>
 __device__ __forceinline__ void rpmj_half(uint32_t *sp, const uint32_t *bd, const uint32_t *m, const WordNbrs &n, uint32_t jneg,
                                           uint32_t G, uint32_t Gc, uint32_t NW, uint32_t RG, uint32_t gi, uint32_t rg) {
-    constexpr int NT = D;
+    constexpr int NT = HB ? 2 * D + 1 : D;
     uint32_t ltf[NT];
 #pragma unroll
     for (int th = 0; th < NT; ++th) ltf[th] = m[th];
@@ -53,6 +54,18 @@ __device__ __forceinline__ void rpmj_half(uint32_t *sp, const uint32_t *bd, cons
         av[2] ^= bt[NW + n.g_ym];
         av[3] ^= bo[NW + gi];
         if (D == 3) { av[4] ^= bt[2 * NW + n.g_zm]; av[5] ^= bo[2 * NW + gi]; }
+        if (HB) {
+            // ising_bitpack_halfsweep_hb<D, true, true>: cnt[k] = lanes with k neighbour terms J s_j equal to -1, new spin +1 iff U < T_hb
+            uint32_t b[6], cnt[2 * D + 1];
+#pragma unroll
+            for (int k = 0; k < 6; ++k) b[k] = k < 2 * D ? av[k] ^ raw : 0u;
+            count_masks<D>(b, cnt);
+            uint32_t up = 0u;
+#pragma unroll
+            for (int k = 0; k < 2 * D + 1; ++k) up |= cnt[k] & ltf[k];
+            mine[gi] = ~up;
+            continue;
+        }
         // the flip mask of bitpack_update_word<D, true, true>
         uint32_t flip;
         if (D == 2) {
@@ -71,11 +84,11 @@ __device__ __forceinline__ void rpmj_half(uint32_t *sp, const uint32_t *bd, cons
     }
 }
 
-template <int D>
+template <int D, bool HB = false>
 __global__ void __launch_bounds__(RPMJ_THREADS) ising_resident_pmj_sweeps(const __grid_constant__ IsingArgs a, uint32_t n_sweeps,
                                                                             uint32_t G) {
     extern __shared__ uint32_t rpmj_smem[];
-    constexpr int NT = D;   // thresholds: dE = 4, 8 (2D) and 12 (3D)
+    constexpr int NT = HB ? 2 * D + 1 : D;
     const uint32_t NW = a.g.NW, RG = blockDim.x / NW;
     const uint32_t gi = threadIdx.x % NW, rg = threadIdx.x / NW;
     const uint32_t r0 = blockIdx.x * G, Gc = min(G, a.R - r0);
@@ -101,7 +114,7 @@ __global__ void __launch_bounds__(RPMJ_THREADS) ising_resident_pmj_sweeps(const 
             const uint32_t h = h0 + rg;
             if (h < HS) {
                 uint32_t ltf[NT];
-                lt_masks_full<NT>(a, a.t + (h >> 1), h & 1u, gi + a.g.unit_off, 0u, ltf);
+                lt_masks_full<NT, HB>(a, a.t + (h >> 1), h & 1u, gi + a.g.unit_off, 0u, ltf);
 #pragma unroll
                 for (int th = 0; th < NT; ++th) mk[(rg * NW + gi) * NT + th] = ltf[th];
             }
@@ -110,8 +123,8 @@ __global__ void __launch_bounds__(RPMJ_THREADS) ising_resident_pmj_sweeps(const 
         const uint32_t hn = min(RG, HS - h0);
         for (uint32_t hh = 0; hh < hn; ++hh) {
             const uint32_t *m = mk + (hh * NW + gi) * NT;
-            if ((h0 + hh) & 1u) rpmj_half<D, 1>(sp, bd, m, nb1, a.jneg, G, Gc, NW, RG, gi, rg);
-            else rpmj_half<D, 0>(sp, bd, m, nb0, a.jneg, G, Gc, NW, RG, gi, rg);
+            if ((h0 + hh) & 1u) rpmj_half<D, 1, HB>(sp, bd, m, nb1, a.jneg, G, Gc, NW, RG, gi, rg);
+            else rpmj_half<D, 0, HB>(sp, bd, m, nb0, a.jneg, G, Gc, NW, RG, gi, rg);
             __syncthreads();
         }
     }

@@ -1175,7 +1175,7 @@ spin_status spin_destroy(spin_system *s) {
     return SPIN_OK;
 }
 
-// Many +-J realisations of a small lattice with a shared update stream (bit-packed, Metropolis): groups of realisations stay in
+// Many +-J realisations of a small lattice with a shared update stream (bit-packed, both update rules): groups of realisations stay in
 // shared memory for all n_sweeps sweeps of the call (ising_resident_pmj_kernel.cuh).  G = realisations per CTA: two CTAs per SM, within
 // RPMJ_SMEM_MAX bytes of shared memory each.
 constexpr size_t RPMJ_SMEM_MAX = 100 * 1024;
@@ -1185,33 +1185,35 @@ static uint32_t resident_pmj_group(const spin_system *s) {
     // an even share of the replicas for each of the 2 sm_count CTAs that are resident at once (measured at 4096 x 64^2: groups of 14,
     // 293 CTAs, against groups of 16 = a multiple of RG, 256 CTAs of which 108 SMs hold two and 40 one)
     uint64_t G = (s->R + 2 * (uint64_t)s->sm_count - 1) / (2 * (uint64_t)s->sm_count);
-    while (G > 1 && 4 * rpmj_smem_words((uint32_t)G, NW, s->d) > RPMJ_SMEM_MAX) G -= 1;
-    if (4 * rpmj_smem_words((uint32_t)G, NW, s->d) > RPMJ_SMEM_MAX) return 0;
+    while (G > 1 && 4 * rpmj_smem_words((uint32_t)G, NW, s->d, s->cfg.update_rule == SPIN_UPDATE_HEATBATH) > RPMJ_SMEM_MAX) G -= 1;
+    if (4 * rpmj_smem_words((uint32_t)G, NW, s->d, s->cfg.update_rule == SPIN_UPDATE_HEATBATH) > RPMJ_SMEM_MAX) return 0;
     return (uint32_t)G;
 }
 static bool resident_pmj_ok(const spin_system *s) {
     if (s->variant == 1) return false;   // A/B: one launch per half-sweep (ising_bitpack_halfsweep / the quad kernels)
     if (s->vector_generic || s->n != 1 || s->axis >= 0 || s->path != PATH_ISING_BITPACK) return false;
-    if (s->cfg.coupling_kind != SPIN_J_BOND_PM1 || s->cfg.update_rule != SPIN_UPDATE_METROPOLIS) return false;
+    if (s->cfg.coupling_kind != SPIN_J_BOND_PM1) return false;
     if (!(s->R > 1 && !s->cfg.replica_streams)) return false;
     return resident_pmj_group(s) != 0;
 }
 static spin_status enqueue_resident_pmj(spin_system *s, int64_t n_sweeps, cudaStream_t st) {
     const uint32_t G = resident_pmj_group(s);
-    const size_t smem = 4 * rpmj_smem_words(G, (uint32_t)s->g.NW, s->d);
+    const bool hb = s->cfg.update_rule == SPIN_UPDATE_HEATBATH;
+    const size_t smem = 4 * rpmj_smem_words(G, (uint32_t)s->g.NW, s->d, hb);
     const unsigned grid = (unsigned)((s->R + G - 1) / G);
-    if (s->d == 2) CUDA_TRY(cudaFuncSetAttribute(ising_resident_pmj_sweeps<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    else CUDA_TRY(cudaFuncSetAttribute(ising_resident_pmj_sweeps<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+#define RPMJ(D_, HB_) do { CUDA_TRY(cudaFuncSetAttribute(ising_resident_pmj_sweeps<D_, HB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+                           ising_resident_pmj_sweeps<D_, HB_><<<grid, RPMJ_THREADS, smem, st>>>(a, chunk, G); } while (0)
     while (n_sweeps > 0) {
         const uint32_t chunk = (uint32_t)(n_sweeps > (1 << 20) ? (1 << 20) : n_sweeps);
         const IsingArgs a = ising_args(s);
-        if (s->d == 2) ising_resident_pmj_sweeps<2><<<grid, RPMJ_THREADS, smem, st>>>(a, chunk, G);
-        else ising_resident_pmj_sweeps<3><<<grid, RPMJ_THREADS, smem, st>>>(a, chunk, G);
+        if (s->d == 2) { if (hb) RPMJ(2, true); else RPMJ(2, false); }
+        else { if (hb) RPMJ(3, true); else RPMJ(3, false); }
         CUDA_TRY(cudaGetLastError());
         s->launches += 1;
         s->t += chunk;
         n_sweeps -= chunk;
     }
+#undef RPMJ
     return SPIN_OK;
 }
 

@@ -33,6 +33,7 @@ def _equal(G, O, tag):
     assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo), (tag, Eg[:4], Eo[:4], Mg[:4], Mo[:4])
 
 
+@pytest.mark.parametrize("rule", ["metropolis", "heatbath"])
 @pytest.mark.parametrize("dims,R,beta", [
     ((64, 64, 1), 19, 1.0),          # the bench lattice: 64 words per colour, 8 threads per word position
     ((64, 2, 1), 5, 0.4406868),      # 2 words per colour: a round builds the masks of 256 half-sweeps
@@ -44,9 +45,10 @@ def _equal(G, O, tag):
     ((64, 8, 2), 33, 0.0),           # a size-2 dimension; beta = 0
     ((64, 8, 1), 2, 50.0),           # frozen
 ])
-def test_resident_pmj_bit_exact_against_the_oracle(P, oracle, dims, R, beta):
-    G = P.SpinSystem(dims, n=1, storage="bitpack", coupling="bond_pm1", replicas=R, replica_streams=0, seed=SEED)
-    O = oracle.System(dims, n=1, coupling_kind=oracle.J_BOND_PM1, n_replicas=R, replica_streams=0, seed=SEED)
+def test_resident_pmj_bit_exact_against_the_oracle(P, oracle, dims, R, beta, rule):
+    G = P.SpinSystem(dims, n=1, storage="bitpack", coupling="bond_pm1", replicas=R, replica_streams=0, seed=SEED, rule=rule)
+    O = oracle.System(dims, n=1, coupling_kind=oracle.J_BOND_PM1, n_replicas=R, replica_streams=0, seed=SEED,
+                      rule=oracle.RULE_HEATBATH if rule == "heatbath" else oracle.RULE_METROPOLIS)
     assert np.array_equal(G.get_bonds(), O.get_bonds())
     _equal(G, O, "hot start")
     done = 0
@@ -61,10 +63,11 @@ def test_resident_pmj_bit_exact_against_the_oracle(P, oracle, dims, R, beta):
     G.close()
 
 
+@pytest.mark.parametrize("rule", ["metropolis", "heatbath"])
 @pytest.mark.parametrize("dims,R,sweeps", [((64, 64, 1), 4096, 37), ((64, 64, 1), 1000, 130), ((64, 16, 8), 777, 21)])
-def test_resident_pmj_agrees_with_the_per_half_sweep_kernels(P, dims, R, sweeps):
-    A = P.SpinSystem(dims, n=1, storage="bitpack", coupling="bond_pm1", replicas=R, replica_streams=0, seed=SEED)
-    B = P.SpinSystem(dims, n=1, storage="bitpack", coupling="bond_pm1", replicas=R, replica_streams=0, seed=SEED)
+def test_resident_pmj_agrees_with_the_per_half_sweep_kernels(P, dims, R, sweeps, rule):
+    A = P.SpinSystem(dims, n=1, storage="bitpack", coupling="bond_pm1", replicas=R, replica_streams=0, seed=SEED, rule=rule)
+    B = P.SpinSystem(dims, n=1, storage="bitpack", coupling="bond_pm1", replicas=R, replica_streams=0, seed=SEED, rule=rule)
     B.set_option(P.OPT_KERNEL_VARIANT, 1)
     la, lb = A.launch_count, B.launch_count
     A.sweep(1.0, sweeps)
